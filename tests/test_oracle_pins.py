@@ -1,0 +1,362 @@
+"""Pins for the CPU oracle (oracle/enuf_oracle.c) against things other than itself:
+closed forms, values fixed by the paper / task statement (tests/golden/paper_values.txt),
+invariants, finite differences, quadrature, numpy.fft and brute force.  CPU only.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+from enuf_inputs import make_workload, random_neutral_gas
+
+GOLDEN = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")) as fh:
+    for line in fh:
+        line = line.split("#")[0].strip()
+        if "=" in line:
+            k, v = line.split("=")
+            GOLDEN[k.strip()] = float(v)
+
+
+# ----------------------------------------------------------------- Oracle A: energy
+
+def _total_ewald(O, r, q, L, alpha, k_cut, r_cut, shells):
+    e_rec, _ = O.direct(r, q, L, alpha, k_cut, forces=False)
+    return O.real_energy(r, q, L, alpha, r_cut, shells) + e_rec - O.self_energy(q, alpha)
+
+
+@pytest.mark.parametrize("name,tol", [("cfg2_perfect", 1e-6), ("cfg2_perfect_k16", 1e-9)])
+def test_madelung_rock_salt(oracle, name, tol):
+    """Full Ewald energy (real + reciprocal - self, Eq. 25) of rock salt
+    reproduces the Madelung constant (BASELINE north_star: 1.747565 to 1e-6)."""
+    w = make_workload(name)
+    e = _total_ewald(oracle, w.r, w.q, w.L, w.alpha, w.k_cut, r_cut=w.L / 2, shells=1)
+    madelung = -e * w.meta["r0"] / (w.N / 2)
+    assert abs(madelung - GOLDEN["madelung_nacl"]) < 1e-6
+    assert abs(madelung - 1.7475645946331822) < tol   # more digits of the same constant
+
+
+@pytest.mark.parametrize("alpha", [2.0, 3.0, 5.0])
+def test_wigner_single_charge(oracle, alpha):
+    """One charge in a unit cube with neutralising background: E = -xi/(2L)."""
+    L = 1.0
+    r = np.array([[0.3, 0.55, 0.8]]); q = np.array([1.0])
+    k_cut = 14
+    e_rec, _ = oracle.direct(r, q, L, alpha, k_cut, forces=False)
+    e = (e_rec + oracle.real_energy(r, q, L, alpha, 6.0, 6) - oracle.self_energy(q, alpha)
+         - math.pi / (2 * alpha ** 2 * L ** 3))
+    assert abs(e + GOLDEN["wigner_cubic"] / (2 * L)) < 2e-9
+
+
+def test_total_energy_independent_of_alpha(oracle):
+    """PAPER.md:467 'the electrostatic energy is invariant to alpha'."""
+    r, q = random_neutral_gas(24, 3.0, seed=77)
+    L = 3.0
+    es = [_total_ewald(oracle, r, q, L, a, k_cut=kc, r_cut=3 * L, shells=3)
+          for a, kc in ((1.4, 10), (2.0, 14), (2.6, 18))]
+    assert max(es) - min(es) < 1e-9 * abs(es[0])
+
+
+def test_parameter_rule(oracle):
+    """Eq. 31-32: literals of the configs and the paper's alpha >= 0.12."""
+    for name in ("cfg3", "cfg4", "cfg5"):
+        w = make_workload(name) if name != "cfg5" else None
+        if name == "cfg5":
+            a = oracle.alpha_from_rc(10.0, 1e-4)
+            assert abs(a - 0.30348542587702925) < 1e-15
+            assert oracle.ncut(a, 215.0, 1e-4) == 64
+        else:
+            assert oracle.ncut(w.alpha, w.L, w.meta["delta"]) == w.k_cut
+    r_c = GOLDEN["dpd_rc_over_Rc"] * GOLDEN["dpd_beta"] * GOLDEN["dpd_lambda_e"]
+    a = oracle.alpha_from_rc(r_c, GOLDEN["dpd_delta"])
+    assert GOLDEN["dpd_alpha_min"] <= a < GOLDEN["dpd_alpha_min"] + 0.01   # prints "0.12"
+
+
+# ----------------------------------------------------------------- Oracle A: forces
+
+def test_direct_forces_are_minus_gradient(oracle):
+    r, q = random_neutral_gas(12, 4.0, seed=5)
+    L, alpha, kc = 4.0, 1.1, 6
+    _, F = oracle.direct(r, q, L, alpha, kc)
+    h = 1e-5
+    for i in (0, 5, 11):
+        for d in range(3):
+            rp = r.copy(); rp[i, d] += h
+            rm = r.copy(); rm[i, d] -= h
+            ep, _ = oracle.direct(rp, q, L, alpha, kc, forces=False)
+            em, _ = oracle.direct(rm, q, L, alpha, kc, forces=False)
+            assert abs(F[i, d] + (ep - em) / (2 * h)) < 2e-9 * np.abs(F).max()
+
+
+def test_direct_momentum_and_antisymmetry(oracle):
+    r, q = random_neutral_gas(64, 5.0, seed=9)
+    _, F = oracle.direct(r, q, 5.0, 1.0, 7)
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).max()          # 'momentum conserved' :79
+    r2 = np.array([[0.1, 0.2, 0.3], [1.7, 2.9, 0.4]]); q2 = np.array([1.0, -1.0])
+    _, F2 = oracle.direct(r2, q2, 5.0, 1.0, 7)
+    assert np.abs(F2[0] + F2[1]).max() < 1e-13 * np.abs(F2).max()
+
+
+def test_direct_sampled_forces_match_full(oracle):
+    r, q = random_neutral_gas(32, 5.0, seed=10)
+    _, F = oracle.direct(r, q, 5.0, 1.0, 6)
+    _, Fs = oracle.direct(r, q, 5.0, 1.0, 6, sample=[3, 30, 7])
+    assert np.array_equal(Fs, F[[3, 30, 7]])
+
+
+def test_direct_S_single_particle_closed_form(oracle):
+    """S(n) of one charge is exp(-2 pi i n.x) (Eq. 37)."""
+    r = np.array([[1.0, 2.5, 7.0]]); q = np.array([2.0]); L = 10.0
+    S = oracle.direct_S(r, q, L, [[1, 0, 0], [0, 1, 0], [0, 0, 1], [1, -2, 3]])
+    x = r[0] / L
+    exp = [2 * np.exp(-2j * np.pi * np.dot(n, x)) for n in ([1, 0, 0], [0, 1, 0], [0, 0, 1], [1, -2, 3])]
+    assert np.allclose(S, exp, rtol=0, atol=1e-14)
+
+
+# ----------------------------------------------------------------- windows
+
+@pytest.mark.parametrize("window,m,tol", [("kaiser_bessel", 4, 1e-8), ("kaiser_bessel", 6, 1e-11),
+                                          ("kaiser_bessel", 2, 1e-4), ("gaussian", 4, 1e-11),
+                                          ("gaussian", 6, 1e-11)])
+def test_window_transform_by_quadrature(oracle, window, m, tol):
+    """Phi(k) is the continuous Fourier transform of phi (R6), checked by quadrature."""
+    n, sigma = 64, 2.0
+    lim = m if window == "kaiser_bessel" else 30.0
+    for k in (0, 1, 5, 16):
+        f = lambda d: oracle.phi(window, m, sigma, d) * math.cos(2 * math.pi * k * d / n)
+        val, _ = integrate.quad(f, -lim, lim, limit=400, epsabs=1e-13, epsrel=1e-13)
+        ref = oracle.Phi(window, m, sigma, n, k)
+        assert abs(val - ref) < tol * abs(oracle.Phi(window, m, sigma, n, 0)), (k, val, ref)
+
+
+@pytest.mark.parametrize("window,m", [("kaiser_bessel", 4), ("kaiser_bessel", 6), ("gaussian", 4)])
+def test_window_normalisation_symmetry_support(oracle, window, m):
+    assert abs(oracle.phi(window, m, 2.0, 0.0) - 1.0) < 1e-15           # R7
+    for d in (0.3, 1.7, m - 0.01):
+        assert oracle.phi(window, m, 2.0, d) == oracle.phi(window, m, 2.0, -d)
+        assert oracle.dphi(window, m, 2.0, d) == -oracle.dphi(window, m, 2.0, -d)
+    if window == "kaiser_bessel":
+        assert oracle.phi(window, m, 2.0, m + 0.25) == 0.0             # support radius m (R8)
+        assert oracle.dphi(window, m, 2.0, m + 0.25) == 0.0
+
+
+@pytest.mark.parametrize("window,m", [("kaiser_bessel", 4), ("kaiser_bessel", 6), ("gaussian", 4),
+                                      ("gaussian", 6)])
+def test_window_derivative_by_differences(oracle, window, m):
+    h = 1e-5
+    pts = [-m + 0.3, -2.2, -0.4, 0.0, 0.37, 1.0, m - 0.6, m - 1e-3, m - 1e-6]
+    for d in pts:
+        if window == "kaiser_bessel" and abs(d) + h >= m:
+            hh = (m - abs(d)) / 4
+        else:
+            hh = h
+        fd = (oracle.phi(window, m, 2.0, d + hh) - oracle.phi(window, m, 2.0, d - hh)) / (2 * hh)
+        an = oracle.dphi(window, m, 2.0, d)
+        assert abs(fd - an) < 1e-8 * max(1.0, abs(an)) + 1e-3 * abs(an) * (hh < h), (d, fd, an)
+
+
+def test_kb_derivative_series_branch_is_continuous(oracle):
+    """The small-s series of phi' must join the closed form (x = b s = 0.25 switch)."""
+    m, b = 6, math.pi * 1.5
+    s = 0.25 / b
+    for eps in (1e-9, 1e-7):
+        d_lo = math.sqrt(m * m - (s * (1 - eps)) ** 2)
+        d_hi = math.sqrt(m * m - (s * (1 + eps)) ** 2)
+        a, c = oracle.dphi("kaiser_bessel", m, 2.0, d_lo), oracle.dphi("kaiser_bessel", m, 2.0, d_hi)
+        assert abs(a - c) < 1e-6 * abs(a)
+
+
+def test_slater_form_factor_by_radial_quadrature(oracle):
+    """R19: f(k) is the Fourier transform of Eq. 51, whose integral is q."""
+    lam, L = 0.25, 20.0
+    rho = lambda r: math.exp(-2 * r / lam) / (math.pi * lam ** 3)
+    total, _ = integrate.quad(lambda r: 4 * math.pi * r * r * rho(r), 0, 40 * lam)
+    assert abs(total - 1.0) < 1e-10
+    for n2 in (1, 9, 100, 324):
+        k = 2 * math.pi * math.sqrt(n2) / L
+        f, _ = integrate.quad(lambda r: 4 * math.pi * r * r * rho(r) * math.sin(k * r) / (k * r),
+                              1e-300, 40 * lam, epsabs=1e-14)
+        assert abs(f * f - oracle.slater_f2(n2, lam, L)) < 1e-10
+    assert oracle.slater_f2(50, 0.0, L) == 1.0
+    assert abs(oracle.slater_f2(50, 1e-9, L) - 1.0) < 1e-12
+
+
+# ----------------------------------------------------------------- Oracle B: FFT
+
+@pytest.mark.parametrize("n", [8, 32, 64])
+def test_dft_fft_numpy_agree_on_lines(oracle, n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    for sign, ref in ((-1, np.fft.fft(x)), (+1, np.fft.ifft(x) * n)):
+        a = oracle.fft_line(x, sign, use_dft=True)
+        b = oracle.fft_line(x, sign, use_dft=False)
+        scale = np.abs(ref).max()
+        assert np.abs(a - ref).max() < 1e-13 * scale
+        assert np.abs(b - ref).max() < 1e-13 * scale
+
+
+def test_fft_line_256_vs_numpy(oracle):
+    rng = np.random.default_rng(256)
+    x = rng.standard_normal(256) + 1j * rng.standard_normal(256)
+    assert np.abs(oracle.fft_line(x, -1, False) - np.fft.fft(x)).max() < 1e-12 * np.abs(x).sum()
+
+
+def test_fft3d_vs_numpy_and_axis_order(oracle):
+    rng = np.random.default_rng(3)
+    n = 16
+    a = rng.standard_normal((n, n, n)) + 1j * rng.standard_normal((n, n, n))
+    ref = np.fft.fftn(a)
+    for use_dft in (True, False):
+        assert np.abs(oracle.fft3d(a, -1, use_dft) - ref).max() < 1e-12 * np.abs(ref).max()
+    assert np.abs(oracle.fft3d(a, +1) - np.fft.ifftn(a) * n ** 3).max() < 1e-12 * np.abs(ref).max()
+
+
+# ----------------------------------------------------------------- Oracle B: spreading / S~
+
+def test_spread_additivity_eq61(oracle):
+    """Eq. 61: S (hence the spread grid) is additive over subsets."""
+    w = make_workload("cfg1")
+    half = w.N // 2
+    g = oracle.spread(w.r, w.q, w.L, w.n, w.m, w.window)
+    ga = oracle.spread(w.r[:half], w.q[:half], w.L, w.n, w.m, w.window)
+    gb = oracle.spread(w.r[half:], w.q[half:], w.L, w.n, w.m, w.window)
+    assert np.abs(g - (ga + gb)).max() < 1e-13 * np.abs(g).max()
+
+
+def test_spread_total_mass_and_periodic_wrap(oracle):
+    """sum_l g[l] = q * (sum_k phi)^3 for one particle, also when the stencil wraps."""
+    for pos in ([5.2, 5.7, 5.1], [0.05, 9.99, 0.4]):
+        r = np.array([pos]); q = np.array([1.5])
+        n, m, L = 32, 4, 10.0
+        g = oracle.spread(r, q, L, n, m, "kaiser_bessel")
+        tot = 1.5
+        for t in range(3):
+            u = n * (pos[t] / L % 1.0)
+            c = math.floor(u + 0.5)
+            tot *= sum(oracle.phi("kaiser_bessel", m, 2.0, u - (c - m + k)) for k in range(2 * m + 1))
+        assert abs(g.sum() - tot) < 1e-13 * abs(tot)
+        assert np.count_nonzero(g) <= (2 * m + 1) ** 3
+
+
+def test_spread_layout_x_fastest(oracle):
+    """A particle displaced along x only moves weight along the last grid axis [z,y,x]."""
+    n, m, L = 32, 4, 32.0
+    g = oracle.spread(np.array([[10.0, 16.0, 20.0]]), np.array([1.0]), L, n, m, "gaussian")
+    z, y, x = np.unravel_index(np.argmax(g), g.shape)
+    assert (x, y, z) == (10, 16, 20)
+
+
+@pytest.mark.parametrize("window,m,tol", [("kaiser_bessel", 6, 5e-11), ("kaiser_bessel", 4, 5e-7),
+                                          ("gaussian", 4, 5e-4)])
+def test_Stilde_matches_direct_S_mode_by_mode(oracle, window, m, tol):
+    w = make_workload("cfg1")
+    out = oracle.enuf(w.r, w.q, w.L, w.alpha, w.k_cut, w.n, m, window, forces=False, want_S=True)
+    ml = oracle.modes(w.k_cut)
+    S = oracle.direct_S(w.r, w.q, w.L, ml)
+    assert np.abs(out["S"] - S).max() < tol * np.abs(S).max()
+
+
+def test_dft_and_fft_paths_agree(oracle):
+    w = make_workload("cfg1")
+    a = oracle.enuf_workload(w, use_dft=True)
+    b = oracle.enuf_workload(w, use_dft=False)
+    assert abs(a["E"] - b["E"]) < 1e-13 * abs(a["E"])
+    assert np.abs(a["F"] - b["F"]).max() < 1e-12 * np.abs(a["F"]).max()
+
+
+# ----------------------------------------------------------------- Oracle B: accuracy
+
+def _rel_rms(a, b):
+    return math.sqrt(((a - b) ** 2).sum() / (b ** 2).sum())
+
+
+def test_error_falls_with_m(oracle):
+    """for fixed sigma_s > 1 the error decays rapidly with m."""
+    w = make_workload("cfg1")
+    Ea, Fa = oracle.direct(w.r, w.q, w.L, w.alpha, w.k_cut)
+    for window, bounds in (("gaussian", (5e-3, 2e-5, 2e-7)), ("kaiser_bessel", (3e-3, 3e-7, 1e-10))):
+        errs = []
+        for m in (2, 4, 6):
+            out = oracle.enuf(w.r, w.q, w.L, w.alpha, w.k_cut, w.n, m, window, variant="ik")
+            errs.append(_rel_rms(out["F"], Fa))
+            assert abs(out["E"] - Ea) / abs(Ea) < bounds[(m - 2) // 2]
+        assert errs[0] > 20 * errs[1] > 400 * errs[2]
+        assert all(e < b for e, b in zip(errs, bounds))
+
+
+CASES = [("gaussian", 4, "ik", 3e-5), ("gaussian", 4, "analytic", 3e-4),
+         ("gaussian", 6, "ik", 3e-7), ("gaussian", 6, "analytic", 3e-6),
+         ("kaiser_bessel", 4, "ik", 5e-7), ("kaiser_bessel", 4, "analytic", 3e-5),
+         ("kaiser_bessel", 6, "ik", 1e-10), ("kaiser_bessel", 6, "analytic", 5e-9)]
+
+
+@pytest.mark.parametrize("window,m,variant,tol", CASES)
+def test_brute_force_small_N(oracle, window, m, variant, tol):
+    """N = 64: every window / force variant against the direct Ewald sum (BASELINE)."""
+    L, alpha, kc, n = 6.0, 2.0 * math.pi / 6.0, 8, 32
+    r, q = random_neutral_gas(64, L, seed=123)
+    Ea, Fa = oracle.direct(r, q, L, alpha, kc)
+    out = oracle.enuf(r, q, L, alpha, kc, n, m, window, variant=variant)
+    assert abs(out["E"] - Ea) < tol * abs(Ea)
+    assert _rel_rms(out["F"], Fa) < tol
+
+
+def test_analytic_variant_is_exact_gradient_of_enuf_energy(oracle):
+    """the analytic-derivative force is -grad of E~ (step 5) itself."""
+    L, alpha, kc, n, m = 6.0, 1.0, 8, 32, 4
+    r, q = random_neutral_gas(10, L, seed=321)
+    for window in ("gaussian", "kaiser_bessel"):
+        F = oracle.enuf(r, q, L, alpha, kc, n, m, window, variant="analytic")["F"]
+        h = 1e-5
+        for i, d in ((0, 0), (3, 1), (9, 2)):
+            rp = r.copy(); rp[i, d] += h
+            rm = r.copy(); rm[i, d] -= h
+            ep = oracle.enuf(rp, q, L, alpha, kc, n, m, window, forces=False)["E"]
+            em = oracle.enuf(rm, q, L, alpha, kc, n, m, window, forces=False)["E"]
+            assert abs(F[i, d] + (ep - em) / (2 * h)) < 5e-9 * np.abs(F).max(), (window, i, d)
+
+
+def test_ik_variant_conserves_momentum(oracle):
+    """R16: sum_i F_i = 0 to round-off for the ik variant (and not for the analytic one)."""
+    w = make_workload("cfg1")
+    F = oracle.enuf_workload(w, variant="ik")["F"]
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).max()
+
+
+def test_enuf_invariances(oracle):
+    """Translation by a lattice vector, charge scaling (E, F ~ q^2), q = 0 particles inert."""
+    L, alpha, kc, n, m = 6.0, 1.0, 8, 32, 4
+    r, q = random_neutral_gas(20, L, seed=4)
+    a = oracle.enuf(r, q, L, alpha, kc, n, m, "kaiser_bessel")
+    b = oracle.enuf(r + np.array([L, -2 * L, 3 * L]), q, L, alpha, kc, n, m, "kaiser_bessel")
+    assert abs(a["E"] - b["E"]) < 1e-12 * abs(a["E"])
+    assert np.abs(a["F"] - b["F"]).max() < 1e-11 * np.abs(a["F"]).max()
+    c = oracle.enuf(r, 3 * q, L, alpha, kc, n, m, "kaiser_bessel")
+    assert abs(c["E"] - 9 * a["E"]) < 1e-13 * abs(c["E"])
+    assert np.abs(c["F"] - 9 * a["F"]).max() < 1e-12 * np.abs(c["F"]).max()
+    r2 = np.vstack([r, [[1.0, 2.0, 3.0]]]); q2 = np.append(q, 0.0)
+    d = oracle.enuf(r2, q2, L, alpha, kc, n, m, "kaiser_bessel")
+    assert d["E"] == a["E"] and np.array_equal(d["F"][:-1], a["F"]) and not d["F"][-1].any()
+
+
+def test_slater_factor_against_direct_and_limit(oracle):
+    """R19 (unpinned against the paper): Oracle B with the factor vs Oracle A with the factor."""
+    L, alpha, kc, n, m, lam = 6.0, 1.0, 8, 32, 6, 0.4
+    r, q = random_neutral_gas(30, L, seed=8)
+    Ea, Fa = oracle.direct(r, q, L, alpha, kc, slater_lambda=lam)
+    out = oracle.enuf(r, q, L, alpha, kc, n, m, "kaiser_bessel", variant="ik", slater_lambda=lam)
+    assert abs(out["E"] - Ea) < 1e-10 * abs(Ea) and _rel_rms(out["F"], Fa) < 1e-9
+    E0, _ = oracle.direct(r, q, L, alpha, kc, forces=False)
+    assert Ea < E0    # smearing lowers every |k| > 0 weight
+
+
+def test_predicted_error_cfg2(oracle):
+    """cfg2 (KB m=6) ENUF vs direct, both variants."""
+    w = make_workload("cfg2")
+    Ea, Fa = oracle.direct(w.r, w.q, w.L, w.alpha, w.k_cut)
+    for variant, tol in (("ik", 5e-10), ("analytic", 5e-9)):
+        out = oracle.enuf_workload(w, variant=variant)
+        assert abs(out["E"] - Ea) < 1e-10 * abs(Ea)
+        assert _rel_rms(out["F"], Fa) < tol
