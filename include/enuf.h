@@ -1,0 +1,160 @@
+/*
+ * enuf.h -- C ABI of the B200-native ENUF reciprocal-space library (libenuf_b200.so).
+ *
+ * ENUF = Ewald summation based on the non-uniform FFT (arxiv 2004.12484).  Citations
+ * are PAPER.md:<line> of the paper text; R-numbers are the readings listed in DESIGN.md.
+ *
+ * What one evaluation computes (section II.C, and :487-507, section III.A):
+ *   a1  wrap x = r/L (:301), bin particles by grid tile (counting sort)
+ *   a2  spreading  g[l] = sum_j q_j phi(u_jx-l_x) phi(u_jy-l_y) phi(u_jz-l_z)      (:491)
+ *   a3  forward 3D FFT of g on the oversampled n^3 grid, n = sigma*M              (:491)
+ *   a4  scaling: S~(n) = g^[n]/D(n) for 0<|n|<=k_cut; E = (1/(2 pi L)) sum f^2 w |S~|^2
+ *       with w(n) = exp(-(pi n)^2/(alpha L)^2)/n^2 (Eq. 38, :310); subdividing (:493)
+ *   a5  inverse 3D FFT of the scaled spectrum (one field, or three for the ik variant)
+ *   a6  interpolating back onto the particles as forces (Eq. 41-42, :332-340)
+ *   a7  energy reduction to one fp64 scalar
+ * Units: 1/(4 pi eps0) = 1 and eps_r = 1 (R1).  E is the reciprocal-space energy only
+ * (includes i = j terms, no self / real-space / background term, R12-R13).
+ *
+ * Conventions for every entry point
+ *   - returns ENUF_OK (0) or a negative enuf_status; enuf_last_error() then holds a
+ *     thread-local message (for ENUF_ECUDA the CUDA error string).  No exception and no
+ *     CPU fallback: without a CUDA device every compute call fails with ENUF_ECUDA.
+ *   - "device pointer" = CUDA device memory of the plan's precision (float or double);
+ *     "host pointer" = ordinary (preferably pinned) host memory.
+ *   - the plan owns all workspace; nothing is allocated inside an evaluation.
+ *   - a plan is not thread-safe; different plans may be used from different threads.
+ */
+#ifndef ENUF_H
+#define ENUF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct enuf_plan enuf_plan; /* opaque */
+
+enum enuf_status {
+    ENUF_OK = 0,
+    ENUF_EINVAL = -1, /* bad argument (message says which)            */
+    ENUF_ENOMEM = -2, /* host or device allocation failed              */
+    ENUF_ECUDA = -3,  /* a CUDA runtime call or kernel launch failed   */
+    ENUF_ESTATE = -4  /* call not allowed in the plan's current state  */
+};
+
+/* keys of enuf_plan_set(); values are passed as double */
+enum enuf_option {
+    ENUF_OPT_PRECISION = 1,      /* ENUF_F32 (default) | ENUF_F64; only before the first evaluation */
+    ENUF_OPT_WINDOW = 2,         /* ENUF_WINDOW_KAISER_BESSEL (default) | ENUF_WINDOW_GAUSSIAN (R6) */
+    ENUF_OPT_FORCE_VARIANT = 3,  /* ENUF_FORCE_ANALYTIC (default) | ENUF_FORCE_IK (paper, Eq. 41)   */
+    ENUF_OPT_SLATER_LAMBDA = 4,  /* decay length of the Slater density Eq. 51 (:407); 0 = point (R19) */
+    ENUF_OPT_NUM_PARTICLES = 5,  /* lower N for the next calls, 0 <= N <= planned capacity          */
+    ENUF_OPT_PROFILE = 6,        /* 1: record per-stage CUDA-event times (enuf_plan_stage_ms)        */
+    ENUF_OPT_KEEP_SPECTRUM = 7   /* 1: also store S~(n) so enuf_plan_structure_factor() can read it  */
+};
+
+enum { ENUF_F32 = 0, ENUF_F64 = 1 };
+enum { ENUF_WINDOW_GAUSSIAN = 0, ENUF_WINDOW_KAISER_BESSEL = 1 };
+enum { ENUF_FORCE_ANALYTIC = 0, ENUF_FORCE_IK = 1 };
+
+/* stage indices of enuf_plan_stage_ms() */
+enum enuf_stage {
+    ENUF_STAGE_BIN = 0,     /* a1 */
+    ENUF_STAGE_SPREAD = 1,  /* a2 (includes clearing the grid) */
+    ENUF_STAGE_FFT = 2,     /* a3 + a4 + a5 */
+    ENUF_STAGE_GATHER = 3,  /* a6 */
+    ENUF_STAGE_ENERGY = 4,  /* a7 */
+    ENUF_NUM_STAGES = 5
+};
+
+/*
+ * Create a plan (step a0: tables of the window transform Phi(k), the influence function
+ * f^2 w(|n|^2), FFT twiddles, workspace).
+ *   N      particle capacity, >= 0
+ *   L      cubic box edge (> 0); positions are wrapped into [0, L) internally (R10)
+ *   alpha  Ewald convergence parameter (> 0)
+ *   k_cut  reciprocal cutoff n_c in integer wavevectors: modes 0 < |n|^2 <= k_cut^2 (R4);
+ *          1 <= k_cut <= M/2 (R5)
+ *   M      NFFT bandwidth per dimension (Eq. 33, :272)
+ *   sigma  oversampling factor; n = sigma*M must be 32, 64, 128 or 256
+ *   m      window cut-off: stencil of 2m+1 grid points per dimension (:268, R8), 1 <= m <= 6
+ * Defaults: fp32, Kaiser-Bessel window, analytic-derivative forces, point charges,
+ * the legacy default stream.  *out is set to NULL on failure.
+ */
+int enuf_plan_create(enuf_plan **out, int64_t N, double L, double alpha, int k_cut, int M,
+                     double sigma, int m);
+
+/* Change an option (see enuf_option).  Tables are rebuilt lazily at the next evaluation. */
+int enuf_plan_set(enuf_plan *plan, int key, double value);
+
+/* CUDA stream all work of the plan is issued to (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream); NULL = legacy default stream. */
+int enuf_plan_set_stream(enuf_plan *plan, void *cuda_stream);
+
+/*
+ * One evaluation of the whole path a1..a7.
+ *   r  device pointer, N x 3 row-major (x, y, z per particle), any real value
+ *   q  device pointer, N charges; particles with q == 0 get F = 0 and are skipped
+ *   F  device pointer, N x 3, OVERWRITTEN (not accumulated), caller's particle order
+ *   E  host pointer to one double, or NULL.  If non-NULL the plan's stream is
+ *      synchronised and *E receives E_rec; if NULL the call is fully asynchronous and
+ *      the energy can be fetched later with enuf_plan_energy().
+ * Caller owns r, q, F; they must stay valid until the stream has finished the call.
+ */
+int enuf_energy_forces(enuf_plan *plan, const void *r, const void *q, void *F, double *E);
+
+/* Same, with HOST buffers: copies r, q to plan-owned device staging, evaluates, copies F
+ * back, synchronises.  E may be NULL.  (The end-to-end path bench.py times.) */
+int enuf_energy_forces_host(enuf_plan *plan, const void *r_host, const void *q_host,
+                            void *F_host, double *E);
+
+/* Synchronise the plan's stream and return the energy of the last evaluation. */
+int enuf_plan_energy(enuf_plan *plan, double *E);
+
+/* Per-stage device times (milliseconds) of the last evaluation; needs ENUF_OPT_PROFILE.
+ * Writes min(count, ENUF_NUM_STAGES) floats.  Synchronises the stream. */
+int enuf_plan_stage_ms(enuf_plan *plan, float *ms, int count);
+
+/* Number of kernel launches (this library's kernels, excluding memsets/copies) the last
+ * evaluation issued. */
+int enuf_plan_launch_count(const enuf_plan *plan);
+
+/* Test / multi-GPU taps (valid after an evaluation; each synchronises the stream).
+ *   enuf_plan_copy_grid: spread grid g (after a2) is NOT kept -- this returns the real-space
+ *     field Psi (analytic variant) or B_x (ik) that the gather read, n^3 values [z][y][x],
+ *     to a HOST buffer of the plan's precision.
+ *   enuf_plan_structure_factor: S~(n) for `count` modes (nx, ny, nz triples, each within
+ *     the cutoff sphere) into out[2*count] (re, im) as fp64; needs ENUF_OPT_KEEP_SPECTRUM. */
+int enuf_plan_copy_field(enuf_plan *plan, void *host_out);
+int enuf_plan_structure_factor(enuf_plan *plan, int64_t count, const int *modes, double *out);
+
+/* Spread only (a1 + a2) into a HOST buffer n^3 [z][y][x] of the plan's precision.
+ * Used by the grid-vs-grid parity tests. */
+int enuf_spread_only(enuf_plan *plan, const void *r, const void *q, void *grid_host);
+
+/* Bytes of device workspace the plan holds. */
+size_t enuf_plan_workspace_bytes(const enuf_plan *plan);
+
+void enuf_plan_destroy(enuf_plan *plan);
+
+/* Thread-local message of the last failing call ("" if none). */
+const char *enuf_last_error(void);
+
+/*
+ * Parameter rule, Eq. 31-32, host only:
+ *   enuf_ncut            smallest integer n_c >= (alpha L/pi) sqrt(-ln delta)      (R14)
+ *   enuf_alpha_from_rc   alpha with exp(-alpha^2 r_c^2) = delta                    (R15)
+ *   enuf_rc_from_ncut    r_c = pi n_c / (alpha^2 L)                                (Eq. 32)
+ * Return a negative value / NaN on bad arguments.
+ */
+int enuf_ncut(double alpha, double L, double delta);
+double enuf_alpha_from_rc(double r_c, double delta);
+double enuf_rc_from_ncut(int n_c, double alpha, double L);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ENUF_H */

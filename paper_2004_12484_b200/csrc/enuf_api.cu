@@ -1,0 +1,502 @@
+// C ABI of libenuf_b200.so (see include/enuf.h): plan life cycle, host-side tables
+// (step a0) and the orchestration of one evaluation a1..a7 on the plan's stream.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "enuf_plan.h"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int fail_cuda(cudaError_t e, const char* what) {
+    snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return ENUF_ECUDA;
+}
+
+#define CU(call)                                                   \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return fail_cuda(e__, #call);      \
+    } while (0)
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+
+// modified Bessel function of the first kind, order 0 (power series; x <= ~60 here)
+double bessel_i0_series(double x) {
+    const double q = 0.25 * x * x;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 1000; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term <= 1e-18 * sum) break;
+    }
+    return sum;
+}
+
+// Window transform Phi(k) = int phi(d) exp(-2 pi i k d/n) dd for the phi(0)=1 windows (R6, R7)
+double window_transform(const enuf_plan* p, int k) {
+    const double m = p->m, sg = p->sigma, n = p->n;
+    if (p->window == ENUF_WINDOW_GAUSSIAN) {
+        const double b = 2.0 * sg * m / ((2.0 * sg - 1.0) * kPi);
+        const double t = kPi * k / n;
+        return std::sqrt(kPi * b) * std::exp(-b * t * t);
+    }
+    const double b = kPi * (2.0 - 1.0 / sg);
+    const double om = 2.0 * kPi * k / n;
+    const double arg2 = b * b - om * om;   // > 0 for |k| <= M/2 = n/(2 sigma), sigma > 1
+    return kPi * m / std::sinh(b * m) * bessel_i0_series(m * std::sqrt(arg2 > 0 ? arg2 : 0.0));
+}
+
+void fill_window_params(enuf_plan* p) {
+    enuf::WindowParams& w = p->wp;
+    w.kind = p->window;
+    w.m = p->m;
+    if (p->window == ENUF_WINDOW_GAUSSIAN) {
+        w.b = 2.0 * p->sigma * p->m / ((2.0 * p->sigma - 1.0) * kPi);
+        w.inv_b = 1.0 / w.b;
+        w.bm = w.b * p->m;
+        w.inv1m = 1.0;
+        w.A = 0.0;
+    } else {
+        w.b = kPi * (2.0 - 1.0 / p->sigma);
+        w.inv_b = 1.0 / w.b;
+        w.bm = w.b * p->m;
+        w.inv1m = 1.0 / (1.0 - std::exp(-2.0 * w.bm));
+        w.A = p->m / std::sinh(w.bm);
+    }
+}
+
+template <typename T>
+int upload(void* dst, const std::vector<double>& src, cudaStream_t s) {
+    std::vector<T> tmp(src.size());
+    for (size_t i = 0; i < src.size(); ++i) tmp[i] = (T)src[i];
+    CU(cudaMemcpyAsync(dst, tmp.data(), sizeof(T) * tmp.size(), cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s));
+    return ENUF_OK;
+}
+
+// Step a0: twiddles, 1/Phi(k), f^2 w(|n|^2) in fp64 on the host, rounded once to T.
+int build_tables(enuf_plan* p) {
+    fill_window_params(p);
+    const int n = p->n, kc = p->k_cut;
+    std::vector<double> tw(2 * (size_t)n), iphi((size_t)kc + 1), wf((size_t)kc * kc + 1);
+    for (int j = 0; j < n; ++j) {
+        tw[2 * j] = std::cos(2.0 * kPi * j / n);
+        tw[2 * j + 1] = -std::sin(2.0 * kPi * j / n);
+    }
+    for (int k = 0; k <= kc; ++k) iphi[k] = 1.0 / window_transform(p, k);
+    wf[0] = 0.0;
+    const double a = kPi / (p->alpha * p->L), tl = kPi * p->lambda / p->L;
+    for (int s = 1; s <= kc * kc; ++s) {
+        double w = std::exp(-a * a * s) / s;                    // Eq. 38
+        if (p->lambda != 0.0) {                                 // R19: (1 + (pi lambda |n|/L)^2)^-4
+            const double g = 1.0 + tl * tl * s;
+            w /= (g * g) * (g * g);
+        }
+        wf[s] = w;
+    }
+    int rc;
+    if (p->precision == ENUF_F32) {
+        if ((rc = upload<float>(p->tw, tw, p->stream))) return rc;
+        if ((rc = upload<float>(p->iphi, iphi, p->stream))) return rc;
+        if ((rc = upload<float>(p->wf, wf, p->stream))) return rc;
+    } else {
+        if ((rc = upload<double>(p->tw, tw, p->stream))) return rc;
+        if ((rc = upload<double>(p->iphi, iphi, p->stream))) return rc;
+        if ((rc = upload<double>(p->wf, wf, p->stream))) return rc;
+    }
+    p->tables_dirty = false;
+    return ENUF_OK;
+}
+
+int dev_alloc(enuf_plan* p, void** ptr, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(ptr, bytes);
+    if (e != cudaSuccess) {
+        *ptr = nullptr;
+        (void)cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? fail(ENUF_ENOMEM, "cudaMalloc(%zu) failed: out of device memory", bytes)
+                                              : fail_cuda(e, "cudaMalloc");
+    }
+    p->workspace_bytes += bytes;
+    return ENUF_OK;
+}
+
+void free_workspace(enuf_plan* p) {
+    auto fr = [](void* q) { if (q) cudaFree(q); };
+    fr(p->rec); fr(p->cell); fr(p->idx); fr(p->tile_count); fr(p->tile_offset); fr(p->tile_cursor);
+    for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
+    fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev);
+    fr(p->r_stage); fr(p->q_stage); fr(p->F_stage);
+    if (p->e_pinned) cudaFreeHost(p->e_pinned);
+    if (p->events_valid) for (int i = 0; i <= ENUF_NUM_STAGES; ++i) cudaEventDestroy(p->ev[i]);
+    p->rec = p->spectrum = p->tw = p->iphi = p->wf = p->r_stage = p->q_stage = p->F_stage = nullptr;
+    p->cell = p->idx = p->tile_count = p->tile_offset = p->tile_cursor = nullptr;
+    p->e_partial = p->e_dev = p->e_pinned = nullptr;
+    p->events_valid = false;
+    p->allocated = false;
+    p->workspace_bytes = 0;
+    (void)cudaGetLastError();
+}
+
+// Allocate everything that depends on precision / variant (lazily, at the first evaluation).
+int ensure_allocated(enuf_plan* p) {
+    if (p->allocated) return ENUF_OK;
+    int dev_count = 0;
+    cudaError_t e = cudaGetDeviceCount(&dev_count);
+    if (e != cudaSuccess || dev_count == 0) {
+        (void)cudaGetLastError();
+        return fail(ENUF_ECUDA, "no CUDA device available (%s); this library has no CPU fallback",
+                    e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    }
+    p->esize = p->precision == ENUF_F32 ? 4 : 8;
+    const size_t es = p->esize, n = p->n, n3 = n * n * n, cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1);
+    const int nfield = p->variant == ENUF_FORCE_IK ? 3 : 1;
+    int rc;
+#define ALLOC(ptr, bytes) if ((rc = dev_alloc(p, (void**)&(ptr), (bytes)))) { free_workspace(p); return rc; }
+    ALLOC(p->rec, 4 * es * cap);
+    ALLOC(p->cell, 4 * cap);
+    ALLOC(p->idx, 4 * cap);
+    ALLOC(p->tile_count, 4 * (size_t)p->tg.ntiles);
+    ALLOC(p->tile_offset, 4 * ((size_t)p->tg.ntiles + 1));
+    ALLOC(p->tile_cursor, 4 * (size_t)p->tg.ntiles);
+    for (int d = 0; d < nfield; ++d) {
+        ALLOC(p->grid[d], es * n3);
+        ALLOC(p->A1[d], 2 * es * n * n * p->Kxp);
+        ALLOC(p->A2[d], 2 * es * n * p->Ky * p->Kxp);
+    }
+    if (p->keep_spectrum) ALLOC(p->spectrum, 2 * es * (size_t)p->Ky * p->Ky * p->Kxp);
+    ALLOC(p->tw, 2 * es * n);
+    ALLOC(p->iphi, es * ((size_t)p->k_cut + 1));
+    ALLOC(p->wf, es * ((size_t)p->k_cut * p->k_cut + 1));
+    const int lpc = 256 / (p->n / 16);
+    p->n_partial = (int)(((size_t)p->Ky * p->Kxp + lpc - 1) / lpc);
+    ALLOC(p->e_partial, 8 * (size_t)p->n_partial);
+    ALLOC(p->e_dev, 8);
+#undef ALLOC
+    if (cudaMallocHost((void**)&p->e_pinned, 8) != cudaSuccess) {
+        (void)cudaGetLastError();
+        free_workspace(p);
+        return fail(ENUF_ENOMEM, "cudaMallocHost failed");
+    }
+    for (int i = 0; i <= ENUF_NUM_STAGES; ++i) {
+        if (cudaEventCreate(&p->ev[i]) != cudaSuccess) { free_workspace(p); return fail(ENUF_ECUDA, "cudaEventCreate failed"); }
+    }
+    p->events_valid = true;
+    // pad columns of A1/A2 (kx in (k_cut, Kxp)) must hold finite values
+    for (int d = 0; d < nfield; ++d) {
+        cudaMemsetAsync(p->A1[d], 0, 2 * es * n * n * p->Kxp, p->stream);
+        cudaMemsetAsync(p->A2[d], 0, 2 * es * n * p->Ky * p->Kxp, p->stream);
+    }
+    if (p->spectrum) cudaMemsetAsync(p->spectrum, 0, 2 * es * (size_t)p->Ky * p->Ky * p->Kxp, p->stream);
+    cudaMemsetAsync(p->e_dev, 0, 8, p->stream);
+    rc = p->precision == ENUF_F32 ? enuf::configure_kernels<float>(p) : enuf::configure_kernels<double>(p);
+    if (rc) {
+        cudaError_t le = cudaGetLastError();
+        free_workspace(p);
+        return fail_cuda(le, "cudaFuncSetAttribute(max dynamic shared memory)");
+    }
+    p->allocated = true;
+    p->tables_dirty = true;
+    return ENUF_OK;
+}
+
+int prepare(enuf_plan* p) {
+    int rc = ensure_allocated(p);
+    if (rc) return rc;
+    if (p->tables_dirty && (rc = build_tables(p))) return rc;
+    return ENUF_OK;
+}
+
+template <typename T>
+int run_bin_spread(enuf_plan* p, const void* r, const void* q, void* F) {
+    int l = enuf::launch_bin<T>(p, r, q, F);
+    if (l < 0) return -1;
+    p->launches += l;
+    if (p->profile) cudaEventRecord(p->ev[1], p->stream);
+    l = enuf::launch_spread<T>(p);
+    if (l < 0) return -1;
+    p->launches += l;
+    if (p->profile) cudaEventRecord(p->ev[2], p->stream);
+    return 0;
+}
+
+template <typename T>
+int run_all(enuf_plan* p, const void* r, const void* q, void* F) {
+    if (p->profile) cudaEventRecord(p->ev[0], p->stream);
+    if (run_bin_spread<T>(p, r, q, F)) return -1;
+    int l = enuf::launch_fft<T>(p);
+    if (l < 0) return -1;
+    p->launches += l;
+    if (p->profile) cudaEventRecord(p->ev[3], p->stream);
+    l = enuf::launch_gather<T>(p, F);
+    if (l < 0) return -1;
+    p->launches += l;
+    if (p->profile) { cudaEventRecord(p->ev[4], p->stream); cudaEventRecord(p->ev[5], p->stream); }
+    return 0;
+}
+
+int evaluate_device(enuf_plan* p, const void* r, const void* q, void* F, double* E) {
+    p->launches = 0;
+    if (p->N == 0) {
+        CU(cudaMemsetAsync(p->e_dev, 0, 8, p->stream));
+        if (p->profile) for (int i = 0; i <= ENUF_NUM_STAGES; ++i) cudaEventRecord(p->ev[i], p->stream);
+    } else {
+        int rc = p->precision == ENUF_F32 ? run_all<float>(p, r, q, F) : run_all<double>(p, r, q, F);
+        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+    }
+    p->evaluated = true;
+    if (E) {
+        CU(cudaMemcpyAsync(p->e_pinned, p->e_dev, 8, cudaMemcpyDeviceToHost, p->stream));
+        CU(cudaStreamSynchronize(p->stream));
+        *E = *p->e_pinned;
+    }
+    return ENUF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* enuf_last_error(void) { return g_err; }
+
+int enuf_plan_create(enuf_plan** out, int64_t N, double L, double alpha, int k_cut, int M, double sigma, int m) {
+    g_err[0] = 0;
+    if (!out) return fail(ENUF_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (N < 0 || N > 0xFFFFFFFFll) return fail(ENUF_EINVAL, "N = %lld out of range [0, 2^32)", (long long)N);
+    if (!(L > 0) || !std::isfinite(L)) return fail(ENUF_EINVAL, "L must be positive and finite");
+    if (!(alpha > 0) || !std::isfinite(alpha)) return fail(ENUF_EINVAL, "alpha must be positive and finite");
+    if (M < 2) return fail(ENUF_EINVAL, "M must be >= 2");
+    if (!(sigma > 1.0) || !std::isfinite(sigma)) return fail(ENUF_EINVAL, "sigma must be > 1");
+    const double nd = sigma * M;
+    const int n = (int)std::lround(nd);
+    if (std::fabs(nd - n) > 1e-9 || (n != 32 && n != 64 && n != 128 && n != 256))
+        return fail(ENUF_EINVAL, "sigma*M = %g must be one of 32, 64, 128, 256", nd);
+    if (k_cut < 1 || 2 * k_cut > M) return fail(ENUF_EINVAL, "k_cut = %d must satisfy 1 <= k_cut <= M/2 = %d", k_cut, M / 2);
+    if (m < 1 || m > enuf::kMaxM) return fail(ENUF_EINVAL, "m = %d must satisfy 1 <= m <= %d", m, enuf::kMaxM);
+    enuf_plan* p = new (std::nothrow) enuf_plan();
+    if (!p) return fail(ENUF_ENOMEM, "out of host memory");
+    p->N_cap = p->N = N;
+    p->L = L; p->alpha = alpha; p->sigma = sigma; p->k_cut = k_cut; p->M = M; p->n = n; p->m = m;
+    p->tg.n = n;
+    p->tg.T = n >= 128 ? 16 : 8;
+    p->tg.nt = n / p->tg.T;
+    p->tg.ntiles = p->tg.nt * p->tg.nt * p->tg.nt;
+    p->Kxp = ((k_cut + 1 + enuf::kLinesPerGroup - 1) / enuf::kLinesPerGroup) * enuf::kLinesPerGroup;
+    p->Ky = 2 * k_cut + 1;
+    fill_window_params(p);
+    *out = p;
+    return ENUF_OK;
+}
+
+int enuf_plan_set(enuf_plan* p, int key, double value) {
+    g_err[0] = 0;
+    if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    const int iv = (int)value;
+    switch (key) {
+        case ENUF_OPT_PRECISION:
+            if (iv != ENUF_F32 && iv != ENUF_F64) return fail(ENUF_EINVAL, "precision must be ENUF_F32 or ENUF_F64");
+            if (p->allocated && iv != p->precision) return fail(ENUF_ESTATE, "precision is fixed after the first evaluation");
+            p->precision = iv;
+            return ENUF_OK;
+        case ENUF_OPT_WINDOW:
+            if (iv != ENUF_WINDOW_GAUSSIAN && iv != ENUF_WINDOW_KAISER_BESSEL) return fail(ENUF_EINVAL, "unknown window");
+            p->window = iv; p->tables_dirty = true; fill_window_params(p);
+            return ENUF_OK;
+        case ENUF_OPT_FORCE_VARIANT:
+            if (iv != ENUF_FORCE_ANALYTIC && iv != ENUF_FORCE_IK) return fail(ENUF_EINVAL, "unknown force variant");
+            if (p->allocated && iv != p->variant) { cudaStreamSynchronize(p->stream); free_workspace(p); }
+            p->variant = iv;
+            return ENUF_OK;
+        case ENUF_OPT_SLATER_LAMBDA:
+            if (!(value >= 0) || !std::isfinite(value)) return fail(ENUF_EINVAL, "lambda must be >= 0");
+            p->lambda = value; p->tables_dirty = true;
+            return ENUF_OK;
+        case ENUF_OPT_NUM_PARTICLES:
+            if (value < 0 || value > (double)p->N_cap || value != std::floor(value))
+                return fail(ENUF_EINVAL, "N must be an integer in [0, %lld]", (long long)p->N_cap);
+            p->N = (int64_t)value;
+            return ENUF_OK;
+        case ENUF_OPT_PROFILE:
+            p->profile = iv != 0;
+            return ENUF_OK;
+        case ENUF_OPT_KEEP_SPECTRUM:
+            if (p->allocated && (iv != 0) != p->keep_spectrum) { cudaStreamSynchronize(p->stream); free_workspace(p); }
+            p->keep_spectrum = iv != 0;
+            return ENUF_OK;
+        default:
+            return fail(ENUF_EINVAL, "unknown option key %d", key);
+    }
+}
+
+int enuf_plan_set_stream(enuf_plan* p, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    p->stream = static_cast<cudaStream_t>(cuda_stream);
+    return ENUF_OK;
+}
+
+int enuf_energy_forces(enuf_plan* p, const void* r, const void* q, void* F, double* E) {
+    g_err[0] = 0;
+    if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    if (p->N > 0 && (!r || !q || !F)) return fail(ENUF_EINVAL, "r, q and F must be non-NULL when N > 0");
+    int rc = prepare(p);
+    if (rc) return rc;
+    return evaluate_device(p, r, q, F, E);
+}
+
+int enuf_energy_forces_host(enuf_plan* p, const void* r_host, const void* q_host, void* F_host, double* E) {
+    g_err[0] = 0;
+    if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    if (p->N > 0 && (!r_host || !q_host || !F_host)) return fail(ENUF_EINVAL, "r, q and F must be non-NULL when N > 0");
+    int rc = prepare(p);
+    if (rc) return rc;
+    const size_t es = p->esize, cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1);
+    if (!p->r_stage) {
+        if ((rc = dev_alloc(p, &p->r_stage, 3 * es * cap))) return rc;
+        if ((rc = dev_alloc(p, &p->q_stage, es * cap))) return rc;
+        if ((rc = dev_alloc(p, &p->F_stage, 3 * es * cap))) return rc;
+    }
+    const size_t N = (size_t)p->N;
+    if (N > 0) {
+        CU(cudaMemcpyAsync(p->r_stage, r_host, 3 * es * N, cudaMemcpyHostToDevice, p->stream));
+        CU(cudaMemcpyAsync(p->q_stage, q_host, es * N, cudaMemcpyHostToDevice, p->stream));
+    }
+    rc = evaluate_device(p, p->r_stage, p->q_stage, p->F_stage, nullptr);
+    if (rc) return rc;
+    if (N > 0) CU(cudaMemcpyAsync(F_host, p->F_stage, 3 * es * N, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaMemcpyAsync(p->e_pinned, p->e_dev, 8, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    if (E) *E = *p->e_pinned;
+    return ENUF_OK;
+}
+
+int enuf_plan_energy(enuf_plan* p, double* E) {
+    g_err[0] = 0;
+    if (!p || !E) return fail(ENUF_EINVAL, "plan or E is NULL");
+    if (!p->evaluated) return fail(ENUF_ESTATE, "no evaluation has been run");
+    CU(cudaMemcpyAsync(p->e_pinned, p->e_dev, 8, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    *E = *p->e_pinned;
+    return ENUF_OK;
+}
+
+int enuf_plan_stage_ms(enuf_plan* p, float* ms, int count) {
+    g_err[0] = 0;
+    if (!p || !ms) return fail(ENUF_EINVAL, "plan or ms is NULL");
+    if (!p->profile || !p->evaluated) return fail(ENUF_ESTATE, "needs ENUF_OPT_PROFILE = 1 and one evaluation");
+    CU(cudaStreamSynchronize(p->stream));
+    // events: 0 start, 1 after bin, 2 after spread, 3 after fft(+energy), 4 after gather, 5 end
+    for (int i = 0; i < count && i < ENUF_NUM_STAGES; ++i) {
+        float t = 0.f;
+        CU(cudaEventElapsedTime(&t, p->ev[i], p->ev[i + 1]));
+        ms[i] = t;
+    }
+    return ENUF_OK;
+}
+
+int enuf_plan_launch_count(const enuf_plan* p) { return p ? p->launches : 0; }
+
+size_t enuf_plan_workspace_bytes(const enuf_plan* p) { return p ? p->workspace_bytes : 0; }
+
+int enuf_plan_copy_field(enuf_plan* p, void* host_out) {
+    g_err[0] = 0;
+    if (!p || !host_out) return fail(ENUF_EINVAL, "plan or host_out is NULL");
+    if (!p->evaluated || !p->allocated) return fail(ENUF_ESTATE, "no evaluation has been run");
+    const size_t n = p->n;
+    CU(cudaMemcpyAsync(host_out, p->grid[0], p->esize * n * n * n, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    return ENUF_OK;
+}
+
+int enuf_plan_structure_factor(enuf_plan* p, int64_t count, const int* modes, double* out) {
+    g_err[0] = 0;
+    if (!p || !modes || !out || count < 0) return fail(ENUF_EINVAL, "bad argument");
+    if (!p->keep_spectrum || !p->evaluated || !p->allocated || !p->spectrum)
+        return fail(ENUF_ESTATE, "needs ENUF_OPT_KEEP_SPECTRUM = 1 before the evaluation");
+    const size_t cnt = (size_t)p->Ky * p->Ky * p->Kxp, es = p->esize;
+    std::vector<unsigned char> host(2 * es * cnt);
+    CU(cudaMemcpyAsync(host.data(), p->spectrum, host.size(), cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    const int kc = p->k_cut;
+    for (int64_t i = 0; i < count; ++i) {
+        int nx = modes[3 * i], ny = modes[3 * i + 1], nz = modes[3 * i + 2];
+        const int s = nx * nx + ny * ny + nz * nz;
+        if (s == 0 || s > kc * kc) return fail(ENUF_EINVAL, "mode %lld is outside 0 < |n|^2 <= k_cut^2", (long long)i);
+        const bool conj = nx < 0;            // S~(-n) = conj S~(n): only kx >= 0 is stored
+        if (conj) { nx = -nx; ny = -ny; nz = -nz; }
+        const int kyp = ny >= 0 ? ny : ny + p->Ky, kzp = nz >= 0 ? nz : nz + p->Ky;
+        const size_t o = ((size_t)kzp * p->Ky + kyp) * p->Kxp + nx;
+        double re, im;
+        if (es == 4) { const float* h = reinterpret_cast<const float*>(host.data()); re = h[2 * o]; im = h[2 * o + 1]; }
+        else { const double* h = reinterpret_cast<const double*>(host.data()); re = h[2 * o]; im = h[2 * o + 1]; }
+        out[2 * i] = re;
+        out[2 * i + 1] = conj ? -im : im;
+    }
+    return ENUF_OK;
+}
+
+int enuf_spread_only(enuf_plan* p, const void* r, const void* q, void* grid_host) {
+    g_err[0] = 0;
+    if (!p || !grid_host) return fail(ENUF_EINVAL, "plan or grid_host is NULL");
+    if (p->N > 0 && (!r || !q)) return fail(ENUF_EINVAL, "r and q must be non-NULL when N > 0");
+    int rc = prepare(p);
+    if (rc) return rc;
+    const size_t n = p->n, bytes = p->esize * n * n * n;
+    p->launches = 0;
+    if (p->N == 0) {
+        CU(cudaMemsetAsync(p->grid[0], 0, bytes, p->stream));
+    } else {
+        // F of neutral particles is written by the bin kernel: use the staging-free scratch A1
+        void* scratch = p->A1[0];
+        if ((size_t)p->N * 3 * p->esize > 2 * p->esize * n * n * p->Kxp)
+            return fail(ENUF_EINVAL, "enuf_spread_only: N too large for the scratch buffer");
+        rc = p->precision == ENUF_F32 ? run_bin_spread<float>(p, r, q, scratch) : run_bin_spread<double>(p, r, q, scratch);
+        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+    }
+    CU(cudaMemcpyAsync(grid_host, p->grid[0], bytes, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    // scratch columns must be finite for later evaluations
+    CU(cudaMemsetAsync(p->A1[0], 0, 2 * p->esize * n * n * p->Kxp, p->stream));
+    return ENUF_OK;
+}
+
+void enuf_plan_destroy(enuf_plan* p) {
+    if (!p) return;
+    if (p->allocated) cudaStreamSynchronize(p->stream);
+    free_workspace(p);
+    delete p;
+}
+
+int enuf_ncut(double alpha, double L, double delta) {
+    if (!(alpha > 0) || !(L > 0) || !(delta > 0) || !(delta < 1)) return -1;
+    return (int)std::ceil(alpha * L / kPi * std::sqrt(-std::log(delta)));
+}
+
+double enuf_alpha_from_rc(double r_c, double delta) {
+    if (!(r_c > 0) || !(delta > 0) || !(delta < 1)) return NAN;
+    return std::sqrt(-std::log(delta)) / r_c;
+}
+
+double enuf_rc_from_ncut(int n_c, double alpha, double L) {
+    if (n_c < 1 || !(alpha > 0) || !(L > 0)) return NAN;
+    return kPi * n_c / (alpha * alpha * L);
+}
+
+}  // extern "C"

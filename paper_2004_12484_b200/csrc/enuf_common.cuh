@@ -1,0 +1,102 @@
+// Shared declarations of the CUDA ENUF library (sm_100a).  Product code: shares nothing
+// with oracle/.  Notation follows the paper / DESIGN.md: n = sigma*M grid points per
+// dimension, m = window cut-off, W = 2m+1 stencil points, u = n*x grid coordinate,
+// c = floor(u+1/2) nearest grid point, d0 = u - c in [-1/2, 1/2).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/enuf.h"
+
+namespace enuf {
+
+constexpr int kMaxM = 6;            // largest supported window cut-off
+constexpr int kMaxW = 2 * kMaxM + 1;
+constexpr int kLinesPerGroup = 8;   // FFT: consecutive kx handled together (64 B of complex fp32)
+
+template <typename T> struct Cx2;
+template <> struct Cx2<float> { using type = float2; };
+template <> struct Cx2<double> { using type = double2; };
+template <typename T> using Cx = typename Cx2<T>::type;
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { using type = float4; };
+template <> struct Vec4<double> { using type = double4; };
+
+// Window parameters, precomputed on the host in fp64 (step a0).
+struct WindowParams {
+    int kind;          // ENUF_WINDOW_*
+    int m;
+    double b;          // Gaussian: 2 sigma m/((2 sigma-1) pi); Kaiser-Bessel: pi (2 - 1/sigma)
+    double inv_b;      // 1/b (Gaussian)
+    double bm;         // b*m
+    double inv1m;      // 1/(1 - exp(-2 b m))      (Kaiser-Bessel)
+    double A;          // m / sinh(b m)            (Kaiser-Bessel)
+};
+
+// One binned particle: fractional offset d0 per dimension and charge.
+template <typename T> struct alignas(4 * sizeof(T)) PRec { T dx, dy, dz, q; };
+
+// Geometry shared by bin / spread / gather.
+struct TileGeom {
+    int n;        // grid points per dimension
+    int T;        // tile edge in grid cells (8 or 16)
+    int nt;       // tiles per dimension = n / T
+    int ntiles;   // nt^3
+};
+
+__host__ __device__ inline uint32_t pack_cell(int cx, int cy, int cz) {
+    return (uint32_t)cx | ((uint32_t)cy << 10) | ((uint32_t)cz << 20);
+}
+__host__ __device__ inline void unpack_cell(uint32_t p, int& cx, int& cy, int& cz) {
+    cx = p & 1023u; cy = (p >> 10) & 1023u; cz = (p >> 20) & 1023u;
+}
+
+// ---------------------------------------------------------------- math wrappers
+__device__ __forceinline__ float r_exp(float x) { return expf(x); }
+__device__ __forceinline__ double r_exp(double x) { return exp(x); }
+__device__ __forceinline__ float r_expm1(float x) { return expm1f(x); }
+__device__ __forceinline__ double r_expm1(double x) { return expm1(x); }
+__device__ __forceinline__ float r_sqrt(float x) { return sqrtf(x); }
+__device__ __forceinline__ double r_sqrt(double x) { return sqrt(x); }
+
+// Window phi(d) and derivative phi'(d), d in grid units, phi(0) = 1 (R6, R7).
+//   Gaussian:       phi = exp(-d^2/b)
+//   Kaiser-Bessel:  phi = [sinh(b s)/s] * m/sinh(b m), s = sqrt(m^2 - d^2), 0 for |d| > m,
+//                   evaluated overflow-free as (m/s) e^{b(s-m)} (1-e^{-2bs})/(1-e^{-2bm}).
+template <typename T, bool kDeriv>
+__device__ __forceinline__ void window_eval(const WindowParams& wp, T d, T& phi, T& dphi) {
+    if (wp.kind == ENUF_WINDOW_GAUSSIAN) {
+        T ib = (T)wp.inv_b;
+        phi = r_exp(-d * d * ib);
+        if (kDeriv) dphi = -(T)2 * d * ib * phi;
+    } else {
+        T m = (T)wp.m, b = (T)wp.b;
+        T s2 = (m - d) * (m + d);
+        if (s2 > (T)0) {
+            T s = r_sqrt(s2);
+            T e1 = r_exp(b * (s - m));
+            T e2m1 = r_expm1(-(T)2 * b * s);            // e^{-2bs} - 1
+            T G = m * e1 * (T)wp.inv1m;                  // A e^{bs} / 2 ... scaled
+            phi = -G * e2m1 / s;
+            if (kDeriv) {
+                T x = b * s;
+                if (x < (T)1) {
+                    T x2 = x * x;
+                    T ser = (T)(1.0 / 3.0) + x2 * ((T)(1.0 / 30.0) + x2 * ((T)(1.0 / 840.0)
+                            + x2 * ((T)(1.0 / 45360.0) + x2 * (T)(1.0 / 3991680.0))));
+                    dphi = -(T)wp.A * d * b * b * b * ser;
+                } else {
+                    // -d G [b (1+e2) - (1-e2)/s] / s^2
+                    dphi = -d * G * (b * ((T)2 + e2m1) + e2m1 / s) / s2;
+                }
+            }
+        } else {
+            phi = (s2 == (T)0) ? (T)(wp.A * wp.b) : (T)0;
+            if (kDeriv) dphi = (T)0;
+        }
+    }
+}
+
+}  // namespace enuf

@@ -1,0 +1,424 @@
+// Steps a3, a4, a5 -- uniform 3D FFT of the oversampled grid, with
+// the scaling / subdividing steps and the energy sum fused into the z pass.  Hand-written
+// shared-memory FFT, n in {32, 64, 128, 256}; no cuFFT in the product path.
+//
+// One line of length N is transformed by TPL = N/16 threads in two register passes with
+// one shared-memory exchange (four-step FFT, N = RA*RB):
+//   pass A: for each a in [0,RB):  DFT_RA over n1 of x[RB*n1 + a], times W_N^(a*k1)
+//   pass B: for each k1 in [0,RA): DFT_RB over a            ->  X[k1 + RA*k2]
+// forward uses (RA, RB) = (16, N/16), inverse (N/16, 16), so the registers a thread holds
+// after a forward pass B are exactly its inputs of an inverse pass A: the fused z pass goes
+// forward -> scale -> inverse without touching memory in between.
+//
+// Data layout (x fastest everywhere), pruned to the modes the Ewald sphere can reach:
+//   G  [z][y][x]        real      n^3
+//   A1 [z][y][kx]       complex   kx in [0, Kxp), Kxp = roundup(k_cut+1, 8); kx > k_cut are 0
+//   A2 [z][ky'][kx]     complex   ky' in [0, Ky), Ky = 2 k_cut+1; ky' <= k_cut is ky = ky',
+//                                 ky' > k_cut is ky = ky' - Ky (negative frequencies)
+// Passes: X fwd G->A1, Y fwd A1->A2, Z fused A2->A2 (in place), Y inv A2->A1, X inv A1->G.
+#pragma once
+
+#include "enuf_common.cuh"
+
+namespace enuf {
+
+template <typename T> __device__ __forceinline__ Cx<T> cx_make(T a, T b) { Cx<T> r; r.x = a; r.y = b; return r; }
+template <typename C> __device__ __forceinline__ C cx_add(C a, C b) { a.x += b.x; a.y += b.y; return a; }
+template <typename C> __device__ __forceinline__ C cx_sub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
+template <typename C> __device__ __forceinline__ C cx_mul(C a, C b) {
+    C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+
+// d * exp(SIGN * 2 pi i t / 16), t a compile-time constant after unrolling (0 <= t < 8)
+template <typename T, int SIGN>
+__device__ __forceinline__ Cx<T> mul_w16(Cx<T> d, int t) {
+    constexpr double C1 = 0.92387953251128673848, S1 = 0.38268343236508978178, H = 0.70710678118654752440;
+    T c, s;
+    switch (t) {
+        case 0: return d;
+        case 4: return SIGN < 0 ? cx_make<T>(d.y, -d.x) : cx_make<T>(-d.y, d.x);
+        case 1: c = (T)C1; s = (T)S1; break;
+        case 2: c = (T)H; s = (T)H; break;
+        case 3: c = (T)S1; s = (T)C1; break;
+        case 5: c = (T)-S1; s = (T)C1; break;
+        case 6: c = (T)-H; s = (T)H; break;
+        default: c = (T)-C1; s = (T)S1; break;
+    }
+    if (SIGN < 0) s = -s;
+    return cx_make<T>(d.x * c - d.y * s, d.x * s + d.y * c);
+}
+
+__host__ __device__ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
+__host__ __device__ constexpr int bitrev(int i, int bits) {
+    int r = 0;
+    for (int b = 0; b < bits; ++b) r |= ((i >> b) & 1) << (bits - 1 - b);
+    return r;
+}
+
+// In-register DFT of R = 2, 4, 8 or 16 points, natural order in and out.
+template <typename T, int R, int SIGN>
+__device__ __forceinline__ void dft_reg(Cx<T>* v) {
+    constexpr int LOG = ilog2(R);
+#pragma unroll
+    for (int s = 0; s < LOG; ++s) {
+        const int len = R >> s;
+#pragma unroll
+        for (int i = 0; i < R; i += len) {
+#pragma unroll
+            for (int j = 0; j < len / 2; ++j) {
+                Cx<T> a = v[i + j], b = v[i + j + len / 2];
+                v[i + j] = cx_add(a, b);
+                v[i + j + len / 2] = mul_w16<T, SIGN>(cx_sub(a, b), j * (16 / len));
+            }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const int r = bitrev(i, LOG);
+        if (i < r) { Cx<T> t = v[i]; v[i] = v[r]; v[r] = t; }
+    }
+}
+
+template <int N, int SIGN>
+struct FftShape {
+    static constexpr int RA = SIGN < 0 ? 16 : N / 16;
+    static constexpr int RB = N / RA;
+    static constexpr int TPL = N / 16;                 // threads per line
+    static constexpr int ITEMS_A = RB / TPL;           // fwd 1, inv 256/N
+    static constexpr int ITEMS_B = RA / TPL;           // fwd 256/N, inv 1
+    static constexpr int LSP_RAW = RA * (RB + 1);
+    static constexpr int LSP = LSP_RAW | 1;            // odd line pitch in shared memory
+};
+constexpr int kFftThreads = 256;
+template <int N> constexpr int fft_lines_per_cta() { return kFftThreads / (N / 16); }
+template <typename T, int N> constexpr size_t fft_smem_bytes() {
+    // both directions use the same pitch bound: max(16*(N/16+1), (N/16)*17) | 1
+    constexpr int a = FftShape<N, -1>::LSP, b = FftShape<N, +1>::LSP;
+    return sizeof(Cx<T>) * (size_t)fft_lines_per_cta<N>() * (a > b ? a : b);
+}
+template <int N> constexpr int fft_line_pitch() {
+    return FftShape<N, -1>::LSP > FftShape<N, +1>::LSP ? FftShape<N, -1>::LSP : FftShape<N, +1>::LSP;
+}
+
+// Pass A.  v[i*RA + n1] holds x[RB*n1 + a] for item a = t + TPL*i.  Result goes to the
+// line's shared buffer at k1*(RB+1) + a.  tw[j] = exp(-2 pi i j / N).
+template <typename T, int N, int SIGN>
+__device__ __forceinline__ void fft_pass_a(Cx<T>* v, int t, Cx<T>* line, const Cx<T>* __restrict__ tw) {
+    using S = FftShape<N, SIGN>;
+#pragma unroll
+    for (int i = 0; i < S::ITEMS_A; ++i) {
+        const int a = t + S::TPL * i;
+        dft_reg<T, S::RA, SIGN>(v + i * S::RA);
+#pragma unroll
+        for (int k1 = 0; k1 < S::RA; ++k1) {
+            Cx<T> val = v[i * S::RA + k1];
+            if (k1 > 0) {
+                Cx<T> w = __ldg(&tw[a * k1]);
+                if (SIGN > 0) w.y = -w.y;
+                val = cx_mul(val, w);
+            }
+            line[k1 * (S::RB + 1) + a] = val;
+        }
+    }
+}
+
+// Pass B.  After it v[i*RB + k2] holds X[k1 + RA*k2] for k1 = t + TPL*i.
+template <typename T, int N, int SIGN>
+__device__ __forceinline__ void fft_pass_b(Cx<T>* v, int t, const Cx<T>* line) {
+    using S = FftShape<N, SIGN>;
+#pragma unroll
+    for (int i = 0; i < S::ITEMS_B; ++i) {
+        const int k1 = t + S::TPL * i;
+#pragma unroll
+        for (int a = 0; a < S::RB; ++a) v[i * S::RB + a] = line[k1 * (S::RB + 1) + a];
+        dft_reg<T, S::RB, SIGN>(v + i * S::RB);
+    }
+}
+
+struct FftGeom {
+    int n;       // line length = grid points per dimension
+    int kcut;
+    int Kxp;     // padded count of kept kx
+    int Ky;      // 2*kcut + 1
+};
+
+// ---------------------------------------------------------------- X passes (contiguous lines)
+template <typename T, int N>
+__global__ void __launch_bounds__(kFftThreads)
+fft_x_forward_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    using S = FftShape<N, -1>;
+    constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
+    const int t = threadIdx.x % S::TPL, ls = threadIdx.x / S::TPL;
+    const size_t row = (size_t)blockIdx.x * LPC + ls;          // z*n + y; n*n is a multiple of LPC
+    Cx<T> v[16];
+    const T* in = G + row * N;
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) v[n1] = cx_make<T>(in[S::RB * n1 + t], (T)0);
+    Cx<T>* line = sm + ls * PITCH;
+    fft_pass_a<T, N, -1>(v, t, line, tw);
+    __syncthreads();
+    fft_pass_b<T, N, -1>(v, t, line);
+    Cx<T>* out = A1 + row * fg.Kxp;
+#pragma unroll
+    for (int i = 0; i < S::ITEMS_B; ++i)
+#pragma unroll
+        for (int k2 = 0; k2 < S::RB; ++k2) {
+            const int k = t + S::TPL * i + 16 * k2;
+            if (k < fg.Kxp) out[k] = k <= fg.kcut ? v[i * S::RB + k2] : cx_make<T>((T)0, (T)0);
+        }
+}
+
+template <typename T, int N>
+__global__ void __launch_bounds__(kFftThreads)
+fft_x_inverse_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    using S = FftShape<N, +1>;
+    constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
+    const int t = threadIdx.x % S::TPL, ls = threadIdx.x / S::TPL;
+    const size_t row = (size_t)blockIdx.x * LPC + ls;
+    const Cx<T>* in = A1 + row * fg.Kxp;
+    Cx<T> v[16];
+    // Hermitian extension of the half spectrum: X[N-k] = conj X[k]
+#pragma unroll
+    for (int i = 0; i < S::ITEMS_A; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < S::RA; ++n1) {
+            const int e = 16 * n1 + t + S::TPL * i;
+            Cx<T> val = cx_make<T>((T)0, (T)0);
+            if (e <= fg.kcut) val = in[e];
+            else if (N - e <= fg.kcut) { val = in[N - e]; val.y = -val.y; }
+            v[i * S::RA + n1] = val;
+        }
+    Cx<T>* line = sm + ls * PITCH;
+    fft_pass_a<T, N, +1>(v, t, line, tw);
+    __syncthreads();
+    fft_pass_b<T, N, +1>(v, t, line);
+    T* out = G + row * N;
+#pragma unroll
+    for (int k2 = 0; k2 < 16; ++k2) out[t + S::TPL * k2] = v[k2].x;
+}
+
+// ---------------------------------------------------------------- Y passes (strided lines)
+// line id = z*Kxp + kx; consecutive ids are contiguous in memory.
+template <typename T, int N>
+__global__ void __launch_bounds__(kFftThreads)
+fft_y_forward_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    using S = FftShape<N, -1>;
+    constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
+    const int ls = threadIdx.x % LPC, t = threadIdx.x / LPC;
+    const size_t id = (size_t)blockIdx.x * LPC + ls;           // n*Kxp is a multiple of LPC? guarded below
+    const size_t total = (size_t)N * fg.Kxp;
+    const bool live = id < total;
+    const int z = live ? (int)(id / fg.Kxp) : 0, kx = live ? (int)(id % fg.Kxp) : 0;
+    const Cx<T>* in = A1 + (size_t)z * N * fg.Kxp + kx;
+    Cx<T> v[16];
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1)
+        v[n1] = live ? in[(size_t)(S::RB * n1 + t) * fg.Kxp] : cx_make<T>((T)0, (T)0);
+    Cx<T>* line = sm + ls * PITCH;
+    fft_pass_a<T, N, -1>(v, t, line, tw);
+    __syncthreads();
+    fft_pass_b<T, N, -1>(v, t, line);
+    if (!live) return;
+    Cx<T>* out = A2 + (size_t)z * fg.Ky * fg.Kxp + kx;
+#pragma unroll
+    for (int i = 0; i < S::ITEMS_B; ++i)
+#pragma unroll
+        for (int k2 = 0; k2 < S::RB; ++k2) {
+            const int k = t + S::TPL * i + 16 * k2;
+            int kyp = -1;
+            if (k <= fg.kcut) kyp = k;
+            else if (k >= N - fg.kcut) kyp = k - N + fg.Ky;
+            if (kyp >= 0) out[(size_t)kyp * fg.Kxp] = v[i * S::RB + k2];
+        }
+}
+
+template <typename T, int N>
+__global__ void __launch_bounds__(kFftThreads)
+fft_y_inverse_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    using S = FftShape<N, +1>;
+    constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
+    const int ls = threadIdx.x % LPC, t = threadIdx.x / LPC;
+    const size_t id = (size_t)blockIdx.x * LPC + ls;
+    const size_t total = (size_t)N * fg.Kxp;
+    const bool live = id < total;
+    const int z = live ? (int)(id / fg.Kxp) : 0, kx = live ? (int)(id % fg.Kxp) : 0;
+    const Cx<T>* in = A2 + (size_t)z * fg.Ky * fg.Kxp + kx;
+    Cx<T> v[16];
+#pragma unroll
+    for (int i = 0; i < S::ITEMS_A; ++i)
+#pragma unroll
+        for (int n1 = 0; n1 < S::RA; ++n1) {
+            const int e = 16 * n1 + t + S::TPL * i;
+            int kyp = -1;
+            if (e <= fg.kcut) kyp = e;
+            else if (e >= N - fg.kcut) kyp = e - N + fg.Ky;
+            v[i * S::RA + n1] = (live && kyp >= 0) ? in[(size_t)kyp * fg.Kxp] : cx_make<T>((T)0, (T)0);
+        }
+    Cx<T>* line = sm + ls * PITCH;
+    fft_pass_a<T, N, +1>(v, t, line, tw);
+    __syncthreads();
+    fft_pass_b<T, N, +1>(v, t, line);
+    if (!live) return;
+    Cx<T>* out = A1 + (size_t)z * N * fg.Kxp + kx;
+#pragma unroll
+    for (int k2 = 0; k2 < 16; ++k2) out[(size_t)(t + S::TPL * k2) * fg.Kxp] = v[k2];
+}
+
+// ---------------------------------------------------------------- fused Z pass
+// For every kept (kx, ky) line: forward FFT along z, then for each kz with
+// 0 < kx^2+ky^2+kz^2 <= k_cut^2 (R4, R12)
+//     S~ = g^ * iphi[kx] iphi[|ky|] iphi[|kz|]          (scaling, 1/D)
+//     E += mult * wf[|k|^2] |S~|^2                      (Eq. 38; mult = 2 for kx > 0: Hermitian half)
+//     psi^ = wf[|k|^2] * S~ * iphi iphi iphi            (subdividing; zero outside the sphere)
+// and the inverse FFT along z, in place.  wf[s] = f(s)^2 w(s) (Slater factor folded in, R19).
+// NOUT = 1: analytic variant (psi^).  NOUT = 3: ik variant, b^_d = -i n_d psi^ into out0..2.
+struct ScaleTables {
+    const void* iphi;   // [kcut+1]   1/Phi(k)
+    const void* wf;     // [kcut^2+1] f^2 w, entry 0 unused (= 0)
+};
+
+template <typename T, int N, int NOUT>
+__global__ void __launch_bounds__(kFftThreads)
+fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __restrict__ out2, FftGeom fg,
+                   const Cx<T>* __restrict__ tw, ScaleTables st, double* __restrict__ e_partial,
+                   Cx<T>* __restrict__ spectrum) {
+    using SF = FftShape<N, -1>;
+    using SI = FftShape<N, +1>;
+    constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
+    __shared__ double red[kFftThreads / 32];
+    const T* iphi = static_cast<const T*>(st.iphi);
+    const T* wf = static_cast<const T*>(st.wf);
+
+    const int ls = threadIdx.x % LPC, t = threadIdx.x / LPC;
+    const size_t id = (size_t)blockIdx.x * LPC + ls;
+    const size_t total = (size_t)fg.Ky * fg.Kxp;
+    const bool live = id < total;
+    const int kyp = live ? (int)(id / fg.Kxp) : 0, kx = live ? (int)(id % fg.Kxp) : 0;
+    const int ky = kyp <= fg.kcut ? kyp : kyp - fg.Ky;
+    const int kc2 = fg.kcut * fg.kcut;
+    const int kxy2 = kx * kx + ky * ky;
+    const bool inside = live && kx <= fg.kcut && kxy2 <= kc2;
+    const size_t zstride = (size_t)fg.Ky * fg.Kxp;
+    Cx<T>* base = A2 + (size_t)kyp * fg.Kxp + kx;
+    const Cx<T> zero = cx_make<T>((T)0, (T)0);
+
+    // whole CTA outside the cylinder kx^2+ky^2 <= kcut^2: the field spectrum is zero there
+    if (!__syncthreads_or(inside)) {
+        if (live) {
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const size_t o = (size_t)(SF::RB * n1 + t) * zstride;
+                base[o] = zero;
+                if (NOUT == 3) { out1[(base - A2) + o] = zero; out2[(base - A2) + o] = zero; }
+            }
+        }
+        if (threadIdx.x == 0) e_partial[blockIdx.x] = 0.0;
+        return;
+    }
+
+    Cx<T> v[16];
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1)
+        v[n1] = inside ? base[(size_t)(SF::RB * n1 + t) * zstride] : zero;
+    Cx<T>* line = sm + ls * PITCH;
+    fft_pass_a<T, N, -1>(v, t, line, tw);
+    __syncthreads();
+    fft_pass_b<T, N, -1>(v, t, line);
+    __syncthreads();    // shared buffer is reused by the inverse transform
+
+    double e_acc = 0.0;
+    const T ipxy = inside ? iphi[kx] * iphi[ky < 0 ? -ky : ky] : (T)0;
+    const double mult = kx > 0 ? 2.0 : 1.0;
+    int kzs[16];
+#pragma unroll
+    for (int i = 0; i < SF::ITEMS_B; ++i)
+#pragma unroll
+        for (int k2 = 0; k2 < SF::RB; ++k2) {
+            const int r = i * SF::RB + k2;
+            const int k = t + SF::TPL * i + 16 * k2;
+            const int kz = k < N / 2 ? k : k - N;
+            kzs[r] = kz;
+            const int akz = kz < 0 ? -kz : kz;
+            const int s = kxy2 + kz * kz;
+            if (inside && akz <= fg.kcut && s <= kc2 && s > 0) {
+                const T ip3 = ipxy * iphi[akz];
+                const T w = wf[s];
+                Cx<T> S = cx_make<T>(v[r].x * ip3, v[r].y * ip3);
+                e_acc += mult * (double)w * ((double)S.x * (double)S.x + (double)S.y * (double)S.y);
+                if (spectrum) {
+                    const int kzp = kz >= 0 ? kz : kz + fg.Ky;
+                    spectrum[((size_t)kzp * fg.Ky + kyp) * fg.Kxp + kx] = S;
+                }
+                const T sc = w * ip3;
+                v[r] = cx_make<T>(S.x * sc, S.y * sc);
+            } else {
+                v[r] = zero;
+            }
+        }
+
+    Cx<T>* outs[3] = {A2, out1, out2};
+    Cx<T> keep[NOUT == 3 ? 16 : 1];
+    if (NOUT == 3) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) keep[r] = v[r];
+    }
+#pragma unroll
+    for (int d = 0; d < NOUT; ++d) {
+        if (NOUT == 3) {
+            // b^_d = -i n_d psi^ :  -i (x + i y) = y - i x
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const T nd = (T)(d == 0 ? kx : (d == 1 ? ky : kzs[r]));
+                v[r] = cx_make<T>(nd * keep[r].y, -nd * keep[r].x);
+            }
+            if (d > 0) __syncthreads();
+        }
+        fft_pass_a<T, N, +1>(v, t, line, tw);
+        __syncthreads();
+        fft_pass_b<T, N, +1>(v, t, line);
+        if (live) {
+            Cx<T>* ob = outs[d] + (size_t)kyp * fg.Kxp + kx;
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) ob[(size_t)(t + SI::TPL * k2) * zstride] = v[k2];
+        }
+    }
+
+    // deterministic block reduction of the fp64 energy partial
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_xor_sync(0xffffffffu, e_acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = e_acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < kFftThreads / 32; ++w) s += red[w];
+        e_partial[blockIdx.x] = s;
+    }
+}
+
+// Step a7: E = scale * sum of partials, fixed summation order (one CTA).
+static __global__ void __launch_bounds__(256)
+energy_finish_kernel(const double* __restrict__ partial, int count, double scale, double* __restrict__ e_out) {
+    __shared__ double red[256];
+    double s = 0.0;
+    for (int i = threadIdx.x; i < count; i += 256) s += partial[i];
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *e_out = scale * red[0];
+}
+
+}  // namespace enuf

@@ -1,0 +1,10 @@
+// All kernels of the ENUF path instantiated for T = double.
+#include "enuf_launch.cuh"
+
+namespace enuf {
+template int configure_kernels<double>(enuf_plan*);
+template int launch_bin<double>(enuf_plan*, const void*, const void*, void*);
+template int launch_spread<double>(enuf_plan*);
+template int launch_fft<double>(enuf_plan*);
+template int launch_gather<double>(enuf_plan*, void*);
+}  // namespace enuf

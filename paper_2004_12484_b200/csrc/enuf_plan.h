@@ -1,0 +1,63 @@
+// Internal plan structure and per-precision launch entry points (not part of the C ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "enuf_common.cuh"
+
+struct enuf_plan {
+    // problem
+    int64_t N_cap = 0, N = 0;
+    double L = 0, alpha = 0, sigma = 0;
+    int k_cut = 0, M = 0, n = 0, m = 0;
+    // options
+    int precision = ENUF_F32, window = ENUF_WINDOW_KAISER_BESSEL, variant = ENUF_FORCE_ANALYTIC;
+    double lambda = 0.0;
+    bool profile = false, keep_spectrum = false;
+    cudaStream_t stream = nullptr;
+    // derived
+    enuf::TileGeom tg{};
+    enuf::WindowParams wp{};
+    int Kxp = 0, Ky = 0;
+    bool allocated = false, tables_dirty = true, evaluated = false;
+    size_t esize = 4;              // bytes per real
+    size_t workspace_bytes = 0;
+    int launches = 0;
+    // device workspace
+    void* rec = nullptr;           // PRec<T>[N_cap]
+    uint32_t* cell = nullptr;      // [N_cap]
+    uint32_t* idx = nullptr;       // [N_cap]
+    uint32_t* tile_count = nullptr;   // [ntiles]
+    uint32_t* tile_offset = nullptr;  // [ntiles+1]
+    uint32_t* tile_cursor = nullptr;  // [ntiles]
+    void* grid[3] = {nullptr, nullptr, nullptr};   // real n^3 (1 for analytic, 3 for ik)
+    void* A1[3] = {nullptr, nullptr, nullptr};     // complex [n][n][Kxp]
+    void* A2[3] = {nullptr, nullptr, nullptr};     // complex [n][Ky][Kxp]
+    void* spectrum = nullptr;      // complex [Ky][Ky][Kxp] (optional)
+    void* tw = nullptr;            // complex [n]
+    void* iphi = nullptr;          // real [k_cut+1]
+    void* wf = nullptr;            // real [k_cut^2+1]
+    double* e_partial = nullptr;   // [z-pass CTAs]
+    int n_partial = 0;
+    double* e_dev = nullptr;       // [1]
+    double* e_pinned = nullptr;    // [1] host
+    void* r_stage = nullptr;       // host-API staging: r, q, F
+    void* q_stage = nullptr;
+    void* F_stage = nullptr;
+    cudaEvent_t ev[enuf::kMaxW] = {};   // ENUF_NUM_STAGES + 1 used
+    bool events_valid = false;
+};
+
+namespace enuf {
+
+// Implemented once per precision in enuf_kernels_f32.cu / enuf_kernels_f64.cu.
+// Each returns the number of kernel launches it issued, or -1 with the CUDA error left
+// in cudaGetLastError().
+template <typename T> int launch_bin(enuf_plan* p, const void* r, const void* q, void* F);
+template <typename T> int launch_spread(enuf_plan* p);
+template <typename T> int launch_fft(enuf_plan* p);
+template <typename T> int launch_gather(enuf_plan* p, void* F);
+template <typename T> int configure_kernels(enuf_plan* p);   // opt-in shared memory sizes
+
+}  // namespace enuf
