@@ -118,6 +118,12 @@ int enuf_plan_energy(enuf_plan *plan, double *E);
  * Writes min(count, ENUF_NUM_STAGES) floats.  Synchronises the stream. */
 int enuf_plan_stage_ms(enuf_plan *plan, float *ms, int count);
 
+/* Mean per-stage device times over the evaluations made since ENUF_OPT_PROFILE was last
+ * set (at most the last 128; each evaluation records its own CUDA events on the plan's
+ * stream, so no synchronisation happens between evaluations).  *n_evals (may be NULL)
+ * receives how many evaluations were averaged.  Synchronises the stream. */
+int enuf_plan_stage_ms_mean(enuf_plan *plan, float *ms, int count, int *n_evals);
+
 /* Number of kernel launches (this library's kernels, excluding memsets/copies) the last
  * evaluation issued. */
 int enuf_plan_launch_count(const enuf_plan *plan);

@@ -28,7 +28,8 @@ STAGES = ("bin", "spread", "fft", "gather", "energy")
 # every symbol include/enuf.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
     "enuf_plan_create", "enuf_plan_set", "enuf_plan_set_stream", "enuf_energy_forces",
-    "enuf_energy_forces_host", "enuf_plan_energy", "enuf_plan_stage_ms", "enuf_plan_launch_count",
+    "enuf_energy_forces_host", "enuf_plan_energy", "enuf_plan_stage_ms", "enuf_plan_stage_ms_mean",
+    "enuf_plan_launch_count",
     "enuf_plan_copy_field", "enuf_plan_structure_factor", "enuf_spread_only",
     "enuf_plan_workspace_bytes", "enuf_plan_destroy", "enuf_last_error",
     "enuf_ncut", "enuf_alpha_from_rc", "enuf_rc_from_ncut",
@@ -64,6 +65,8 @@ def lib():
         L.enuf_energy_forces_host.argtypes = [vp, vp, vp, vp, C.POINTER(d)]
         L.enuf_plan_energy.restype = i; L.enuf_plan_energy.argtypes = [vp, C.POINTER(d)]
         L.enuf_plan_stage_ms.restype = i; L.enuf_plan_stage_ms.argtypes = [vp, C.POINTER(C.c_float), i]
+        L.enuf_plan_stage_ms_mean.restype = i
+        L.enuf_plan_stage_ms_mean.argtypes = [vp, C.POINTER(C.c_float), i, C.POINTER(i)]
         L.enuf_plan_launch_count.restype = i; L.enuf_plan_launch_count.argtypes = [vp]
         L.enuf_plan_copy_field.restype = i; L.enuf_plan_copy_field.argtypes = [vp, vp]
         L.enuf_plan_structure_factor.restype = i
@@ -188,6 +191,13 @@ class Plan:
         arr = (C.c_float * len(STAGES))()
         _check(lib().enuf_plan_stage_ms(self._h, arr, len(STAGES)))
         return dict(zip(STAGES, (float(x) for x in arr)))
+
+    def stage_ms_mean(self):
+        """(mean per-stage ms, number of evaluations averaged) since profiling was switched on."""
+        arr = (C.c_float * len(STAGES))()
+        ne = C.c_int(0)
+        _check(lib().enuf_plan_stage_ms_mean(self._h, arr, len(STAGES), C.byref(ne)))
+        return dict(zip(STAGES, (float(x) for x in arr))), ne.value
 
     def launch_count(self) -> int:
         return lib().enuf_plan_launch_count(self._h)

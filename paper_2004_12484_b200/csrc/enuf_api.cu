@@ -144,7 +144,13 @@ void free_workspace(enuf_plan* p) {
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev);
     fr(p->r_stage); fr(p->q_stage); fr(p->F_stage);
     if (p->e_pinned) cudaFreeHost(p->e_pinned);
-    if (p->events_valid) for (int i = 0; i <= ENUF_NUM_STAGES; ++i) cudaEventDestroy(p->ev[i]);
+    if (p->ev_ring) {
+        for (int i = 0; i < enuf_plan::kProfRing * enuf_plan::kProfEv; ++i)
+            if (p->ev_ring[i]) cudaEventDestroy(p->ev_ring[i]);
+        delete[] p->ev_ring;
+        p->ev_ring = p->ev = nullptr;
+    }
+    p->prof_evals = 0;
     p->rec = p->spectrum = p->tw = p->iphi = p->wf = p->r_stage = p->q_stage = p->F_stage = nullptr;
     p->cell = p->idx = p->tile_count = p->tile_offset = p->tile_cursor = nullptr;
     p->e_partial = p->e_dev = p->e_pinned = nullptr;
@@ -194,9 +200,13 @@ int ensure_allocated(enuf_plan* p) {
         free_workspace(p);
         return fail(ENUF_ENOMEM, "cudaMallocHost failed");
     }
-    for (int i = 0; i <= ENUF_NUM_STAGES; ++i) {
-        if (cudaEventCreate(&p->ev[i]) != cudaSuccess) { free_workspace(p); return fail(ENUF_ECUDA, "cudaEventCreate failed"); }
+    p->ev_ring = new (std::nothrow) cudaEvent_t[enuf_plan::kProfRing * enuf_plan::kProfEv]();
+    if (!p->ev_ring) { free_workspace(p); return fail(ENUF_ENOMEM, "out of host memory"); }
+    for (int i = 0; i < enuf_plan::kProfRing * enuf_plan::kProfEv; ++i) {
+        if (cudaEventCreate(&p->ev_ring[i]) != cudaSuccess) { free_workspace(p); return fail(ENUF_ECUDA, "cudaEventCreate failed"); }
     }
+    p->ev = p->ev_ring;
+    p->prof_evals = 0;
     p->events_valid = true;
     // pad columns of A1/A2 (kx in (k_cut, Kxp)) must hold finite values
     for (int d = 0; d < nfield; ++d) {
@@ -253,6 +263,10 @@ int run_all(enuf_plan* p, const void* r, const void* q, void* F) {
 
 int evaluate_device(enuf_plan* p, const void* r, const void* q, void* F, double* E) {
     p->launches = 0;
+    if (p->profile) {
+        p->ev = p->ev_ring + (p->prof_evals % enuf_plan::kProfRing) * enuf_plan::kProfEv;
+        ++p->prof_evals;
+    }
     if (p->N == 0) {
         CU(cudaMemsetAsync(p->e_dev, 0, 8, p->stream));
         if (p->profile) for (int i = 0; i <= ENUF_NUM_STAGES; ++i) cudaEventRecord(p->ev[i], p->stream);
@@ -335,6 +349,7 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
             return ENUF_OK;
         case ENUF_OPT_PROFILE:
             p->profile = iv != 0;
+            p->prof_evals = 0;
             return ENUF_OK;
         case ENUF_OPT_KEEP_SPECTRUM:
             if (p->allocated && (iv != 0) != p->keep_spectrum) { cudaStreamSynchronize(p->stream); free_workspace(p); }
@@ -408,6 +423,27 @@ int enuf_plan_stage_ms(enuf_plan* p, float* ms, int count) {
         CU(cudaEventElapsedTime(&t, p->ev[i], p->ev[i + 1]));
         ms[i] = t;
     }
+    return ENUF_OK;
+}
+
+int enuf_plan_stage_ms_mean(enuf_plan* p, float* ms, int count, int* n_evals) {
+    g_err[0] = 0;
+    if (!p || !ms) return fail(ENUF_EINVAL, "plan or ms is NULL");
+    if (!p->profile || p->prof_evals == 0 || !p->ev_ring)
+        return fail(ENUF_ESTATE, "needs ENUF_OPT_PROFILE = 1 and one evaluation");
+    CU(cudaStreamSynchronize(p->stream));
+    const int ne = (int)(p->prof_evals < enuf_plan::kProfRing ? p->prof_evals : enuf_plan::kProfRing);
+    double acc[ENUF_NUM_STAGES] = {0, 0, 0, 0, 0};
+    for (int e = 0; e < ne; ++e) {
+        const cudaEvent_t* ev = p->ev_ring + (size_t)e * enuf_plan::kProfEv;
+        for (int i = 0; i < ENUF_NUM_STAGES; ++i) {
+            float t = 0.f;
+            CU(cudaEventElapsedTime(&t, ev[i], ev[i + 1]));
+            acc[i] += t;
+        }
+    }
+    for (int i = 0; i < count && i < ENUF_NUM_STAGES; ++i) ms[i] = (float)(acc[i] / ne);
+    if (n_evals) *n_evals = ne;
     return ENUF_OK;
 }
 

@@ -45,7 +45,12 @@ struct enuf_plan {
     void* r_stage = nullptr;       // host-API staging: r, q, F
     void* q_stage = nullptr;
     void* F_stage = nullptr;
-    cudaEvent_t ev[enuf::kMaxW] = {};   // ENUF_NUM_STAGES + 1 used
+    // profiling: ring of kProfRing evaluations x (ENUF_NUM_STAGES + 1) events
+    static constexpr int kProfRing = 128;
+    static constexpr int kProfEv = ENUF_NUM_STAGES + 1;
+    cudaEvent_t* ev_ring = nullptr;     // [kProfRing * kProfEv]
+    cudaEvent_t* ev = nullptr;          // slot of the current / last evaluation
+    int64_t prof_evals = 0;             // evaluations recorded since profiling was switched on
     bool events_valid = false;
 };
 

@@ -1,0 +1,92 @@
+"""CPU-only checks of the C-ABI library libenuf_b200.so: it loads, exports every symbol
+include/enuf.h declares, validates arguments, and fails loudly (no CPU fallback) when a
+compute call is made without a CUDA device.  No GPU compute here."""
+import ctypes as C
+import math
+import os
+import re
+
+import pytest
+
+import paper_2004_12484_b200 as enuf
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2004_12484_b200 import build
+    build.build()
+    return enuf.lib()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "enuf.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(enuf_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = _declared_symbols()
+    assert len(names) >= 17
+    for name in names:
+        assert hasattr(lib, name), name
+    assert sorted(enuf.SYMBOLS) == names
+
+
+def test_plan_create_validation(lib):
+    h = C.c_void_p()
+    bad = [
+        dict(N=-1), dict(L=0.0), dict(L=float("nan")), dict(alpha=-1.0), dict(k_cut=0), dict(k_cut=9),
+        dict(M=17), dict(sigma=1.0), dict(m=0), dict(m=7), dict(M=256),
+    ]
+    base = dict(N=10, L=10.0, alpha=0.6, k_cut=8, M=16, sigma=2.0, m=4)
+    for change in bad:
+        a = dict(base, **change)
+        rc = lib.enuf_plan_create(C.byref(h), a["N"], a["L"], a["alpha"], a["k_cut"], a["M"], a["sigma"], a["m"])
+        assert rc == enuf.EINVAL, change
+        assert h.value is None
+        assert lib.enuf_last_error() != b""
+    rc = lib.enuf_plan_create(C.byref(h), *[base[k] for k in ("N", "L", "alpha", "k_cut", "M", "sigma", "m")])
+    assert rc == enuf.OK and h.value
+    assert lib.enuf_plan_set(h, 99, 0.0) == enuf.EINVAL
+    assert lib.enuf_plan_set(h, enuf.OPT_WINDOW, 5.0) == enuf.EINVAL
+    assert lib.enuf_plan_set(h, enuf.OPT_NUM_PARTICLES, 11.0) == enuf.EINVAL
+    assert lib.enuf_plan_set(h, enuf.OPT_NUM_PARTICLES, 7.0) == enuf.OK
+    assert lib.enuf_plan_set(h, enuf.OPT_SLATER_LAMBDA, -0.5) == enuf.EINVAL
+    E = C.c_double()
+    assert lib.enuf_plan_energy(h, C.byref(E)) == enuf.ESTATE       # nothing evaluated yet
+    assert lib.enuf_energy_forces(h, None, None, None, C.byref(E)) == enuf.EINVAL   # NULL pointers, N > 0
+    lib.enuf_plan_destroy(h)
+    lib.enuf_plan_destroy(None)                                     # harmless
+
+
+def test_no_cpu_fallback(lib):
+    """Without a CUDA device every compute call fails with ENUF_ECUDA (loudly)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = C.c_void_p()
+    assert lib.enuf_plan_create(C.byref(h), 4, 10.0, 0.6, 8, 16, 2.0, 4) == enuf.OK
+    buf = (C.c_float * 64)()
+    E = C.c_double()
+    rc = lib.enuf_energy_forces_host(h, buf, buf, buf, C.byref(E))
+    assert rc == enuf.ECUDA
+    assert b"no CPU fallback" in lib.enuf_last_error()
+    lib.enuf_plan_destroy(h)
+    plan = enuf.Plan(4, 10.0, 0.6, 8, 16, m=4)
+    with pytest.raises((enuf.EnufError, TypeError)):
+        plan.energy_forces(torch.zeros(4, 3), torch.zeros(4))
+
+
+def test_parameter_rule_literals(lib):
+    """Eq. 31-32 against the literal plan parameters of the configs."""
+    from enuf_inputs import make_workload
+    for name in ("cfg3", "cfg4"):
+        w = make_workload(name)
+        assert enuf.ncut(w.alpha, w.L, w.meta["delta"]) == w.k_cut
+    a = enuf.alpha_from_rc(10.0, 1e-4)
+    assert abs(a - 0.30348542587702925) < 1e-15
+    assert enuf.ncut(a, 215.0, 1e-4) == 64
+    assert abs(enuf.rc_from_ncut(64, a, 215.0) - math.pi * 64 / (a * a * 215.0)) < 1e-12
+    assert enuf.ncut(-1.0, 1.0, 0.5) < 0 and math.isnan(enuf.alpha_from_rc(0.0, 0.5))

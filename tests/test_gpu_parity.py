@@ -1,0 +1,344 @@
+"""GPU parity: the CUDA path (through the C ABI, paper_2004_12484_b200.Plan) against the
+CPU oracle (oracle/enuf_oracle.c) on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  fp64: relative RMS force error <= 1e-11, relative energy error <= 1e-12
+  fp32 (fp64 energy accumulation): <= 2e-6 and <= 1e-6
+  both vs the direct Ewald sum (Oracle A): within the error the chosen (sigma, m, k_cut,
+  window, variant) predict, per config.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from enuf_inputs import displaced_positions, make_workload, random_neutral_gas
+
+pytestmark = pytest.mark.gpu
+
+F64_F, F64_E = 1e-11, 1e-12
+F32_F, F32_E = 2e-6, 1e-6
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def enuf(torch_cuda):
+    import paper_2004_12484_b200 as e
+    e.lib()   # fails loudly if the library has not been built
+    return e
+
+
+def rel_rms(a, b):
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    return math.sqrt(((a - b) ** 2).sum() / max((b ** 2).sum(), 1e-300))
+
+
+def tols(w):
+    return (F64_F, F64_E) if w.dtype == "f64" else (F32_F, F32_E)
+
+
+def gpu_eval(enuf, torch, w, variant="analytic", r=None, **kw):
+    plan = enuf.Plan.from_workload(w, variant=variant, **kw)
+    rt = torch.from_numpy(w.r if r is None else r).cuda()
+    qt = torch.from_numpy(w.q).cuda()
+    E, F = plan.energy_forces(rt, qt)
+    return plan, E, F.cpu().numpy()
+
+
+# ------------------------------------------------------------------ whole path, configs 1-3
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_small_configs_match_oracle_b(enuf, torch_cuda, oracle, name, variant):
+    w = make_workload(name)
+    ref = oracle.enuf_workload(w, variant=variant)
+    plan, E, F = gpu_eval(enuf, torch_cuda, w, variant)
+    tf, te = tols(w)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"]), (E, ref["E"])
+    assert rel_rms(F, ref["F"]) <= tf
+    if name == "cfg3":    # neutral beads (q = 0) get exactly zero force
+        assert not F[w.q == 0].any()
+    plan.close()
+
+
+@pytest.mark.parametrize("name", ["cfg2_perfect", "cfg2_perfect_k16"])
+def test_perfect_lattice_absolute(enuf, torch_cuda, oracle, name):
+    """R20: for the perfect lattice E_rec is (nearly) zero; compare absolutely against E_self."""
+    w = make_workload(name)
+    ref = oracle.enuf_workload(w)
+    plan, E, F = gpu_eval(enuf, torch_cuda, w)
+    e_self = oracle.self_energy(w.q, w.alpha)
+    assert abs(E - ref["E"]) <= 1e-12 * e_self
+    assert np.abs(F - ref["F"]).max() <= 1e-11 * max(np.abs(ref["F"]).max(), 1e-3 * e_self / w.L)
+    plan.close()
+
+
+# ------------------------------------------------------------------ stage by stage
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
+def test_spread_grid_matches_oracle(enuf, torch_cuda, oracle, name):
+    w = make_workload(name)
+    plan = enuf.Plan.from_workload(w)
+    g = plan.spread_only(torch_cuda.from_numpy(w.r).cuda(), torch_cuda.from_numpy(w.q).cuda()).numpy()
+    ref = oracle.spread(w.r, w.q, w.L, w.n, w.m, w.window, w.sigma)
+    tol = 1e-13 if w.dtype == "f64" else 2e-6
+    assert np.abs(g - ref).max() <= tol * np.abs(ref).max()
+    plan.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
+def test_structure_factor_matches_oracle(enuf, torch_cuda, oracle, name):
+    w = make_workload(name)
+    ref = oracle.enuf_workload(w, forces=False, want_S=True)
+    plan, E, F = gpu_eval(enuf, torch_cuda, w, keep_spectrum=True)
+    ml = oracle.modes(w.k_cut)
+    S = plan.structure_factor(ml)
+    tol = 1e-12 if w.dtype == "f64" else 5e-6
+    assert np.abs(S - ref["S"]).max() <= tol * np.abs(ref["S"]).max()
+    plan.close()
+
+
+def test_field_matches_oracle_inverse_fft(enuf, torch_cuda, oracle):
+    """The real-space field Psi the gather reads = inverse FFT of the scaled spectrum."""
+    w = make_workload("cfg1")
+    ref = oracle.enuf_workload(w, forces=False, want_S=True)
+    plan, E, F = gpu_eval(enuf, torch_cuda, w)
+    psi = plan.field().numpy()
+    n = w.n
+    spec = np.zeros((n, n, n), dtype=np.complex128)
+    for (nx, ny, nz), S in zip(oracle.modes(w.k_cut), ref["S"]):
+        n2 = int(nx) ** 2 + int(ny) ** 2 + int(nz) ** 2
+        D = (oracle.Phi(w.window, w.m, w.sigma, n, nx) * oracle.Phi(w.window, w.m, w.sigma, n, ny)
+             * oracle.Phi(w.window, w.m, w.sigma, n, nz))
+        spec[nz % n, ny % n, nx % n] = oracle.w(n2, w.alpha, w.L) * S / D
+    want = oracle.fft3d(spec, +1).real
+    assert np.abs(psi - want).max() <= 1e-12 * np.abs(want).max()
+    plan.close()
+
+
+# ------------------------------------------------------------------ vs the direct Ewald sum
+
+DIRECT_BOUNDS = {   # (rel E, rel RMS F analytic, rel RMS F ik): DESIGN.md section 5
+    "cfg1": (2e-5, 2e-4, 3e-5),
+    "cfg2": (1e-10, 5e-9, 5e-10),
+    "cfg3": (2e-5, 5e-4, 3e-5),
+}
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
+def test_small_configs_vs_direct_ewald(enuf, torch_cuda, oracle, name):
+    w = make_workload(name)
+    Ea, Fa = oracle.direct(w.r, w.q, w.L, w.alpha, w.k_cut, slater_lambda=w.slater_lambda)
+    be, bfa, bfi = DIRECT_BOUNDS[name]
+    for variant, bf in (("analytic", bfa), ("ik", bfi)):
+        plan, E, F = gpu_eval(enuf, torch_cuda, w, variant)
+        assert abs(E - Ea) <= be * abs(Ea)
+        assert rel_rms(F, Fa) <= bf, (variant, rel_rms(F, Fa))
+        plan.close()
+
+
+def test_ik_variant_conserves_momentum_fp64(enuf, torch_cuda):
+    w = make_workload("cfg1")
+    plan, E, F = gpu_eval(enuf, torch_cuda, w, "ik")
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).max()
+    plan.close()
+
+
+# ------------------------------------------------------------------ large configs (sampled)
+
+def _sampled_check(enuf, torch, oracle, w, r, variant="analytic", nsample=4096, direct_modes=True):
+    rng = np.random.default_rng(w.seed)
+    sample = np.sort(rng.choice(w.N, size=nsample, replace=False))
+    ref = oracle.enuf(r, w.q, w.L, w.alpha, w.k_cut, w.n, w.m, w.window, w.sigma, variant=variant,
+                      slater_lambda=w.slater_lambda, sample=sample, want_S=direct_modes)
+    plan, E, F = gpu_eval(enuf, torch, w, variant, r=r, keep_spectrum=direct_modes)
+    tf, te = tols(w)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"]), (E, ref["E"])
+    err = rel_rms(F[sample], ref["F"])
+    assert err <= tf, err
+    assert np.isfinite(F).all()
+    if direct_modes:
+        # S~ on sampled modes against the oracle's S~ and against the direct sum S (Oracle A)
+        ml = oracle.modes(w.k_cut)
+        pick = np.sort(rng.choice(ml.shape[0], size=256, replace=False))
+        S = plan.structure_factor(ml[pick])
+        scale = np.abs(ref["S"]).max()
+        assert np.abs(S - ref["S"][pick]).max() <= 5e-6 * scale
+        Sd = oracle.direct_S(r, w.q, w.L, ml[pick])
+        assert np.abs(S - Sd).max() <= 5e-6 * scale
+    plan.close()
+    return err
+
+
+@pytest.mark.slow
+def test_cfg4_sampled(enuf, torch_cuda, oracle):
+    w = make_workload("cfg4")
+    _sampled_check(enuf, torch_cuda, oracle, w, w.r)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("step", [0, 1, 99])
+def test_cfg5_sampled_steps(enuf, torch_cuda, oracle, step):
+    """Config 5 in the launch configuration bench.py times; positions after `step` displacements."""
+    w = make_workload("cfg5")
+    r = w.r
+    for s in range(step):
+        r = displaced_positions(r, w.L, w.seed, s, w.meta["step_displacement"])
+    _sampled_check(enuf, torch_cuda, oracle, w, r, direct_modes=(step == 0))
+
+
+@pytest.mark.slow
+def test_cfg5_ik_sampled(enuf, torch_cuda, oracle):
+    w = make_workload("cfg5")
+    _sampled_check(enuf, torch_cuda, oracle, w, w.r, variant="ik", direct_modes=False)
+
+
+def test_cfg5_properties_full_size(enuf, torch_cuda):
+    """Properties that hold at any size: q = 0 inert, repeatability, host API == device API."""
+    torch = torch_cuda
+    w = make_workload("cfg5")
+    plan = enuf.Plan.from_workload(w)
+    r = torch.from_numpy(w.r).cuda(); q = torch.from_numpy(w.q).cuda()
+    E1, F1 = plan.energy_forces(r, q)
+    E2, F2 = plan.energy_forces(r, q)
+    # atomics make the summation order run-dependent (R22): tolerance-level equality only
+    assert abs(E1 - E2) <= 1e-9 * abs(E1)
+    assert rel_rms(F2.cpu().numpy(), F1.cpu().numpy()) <= 5e-7
+    Eh, Fh = plan.energy_forces_host(w.r, w.q)
+    assert abs(Eh - E1) <= 1e-9 * abs(E1)
+    assert rel_rms(Fh.numpy(), F1.cpu().numpy()) <= 5e-7
+    q0 = q.clone(); q0[::3] = 0
+    E3, F3 = plan.energy_forces(r, q0)
+    assert not F3[::3].any().item()
+    assert torch.isfinite(F3).all().item()
+    plan.close()
+
+
+# ------------------------------------------------------------------ shapes: every n, every m
+
+@pytest.mark.parametrize("n,m,window,dtype", [
+    (32, 1, "kaiser_bessel", "f64"), (32, 2, "gaussian", "f64"), (32, 3, "kaiser_bessel", "f32"),
+    (64, 5, "kaiser_bessel", "f64"), (64, 6, "gaussian", "f32"), (128, 4, "kaiser_bessel", "f64"),
+    (128, 6, "gaussian", "f64"), (256, 2, "kaiser_bessel", "f32"), (256, 6, "kaiser_bessel", "f64"),
+])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_all_grid_sizes_and_supports(enuf, torch_cuda, oracle, n, m, window, dtype, variant):
+    torch = torch_cuda
+    N, L = 777, 7.5                    # ragged: not a multiple of any block size
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = random_neutral_gas(N, L, seed=1000 + n + m, dtype=npdt)
+    q = (q * (1.0 + 0.25 * np.arange(N) / N)).astype(npdt)
+    M = n // 2
+    k_cut = min(M // 2, 11)
+    alpha = 0.9 * math.pi * k_cut / (L * 3.0)
+    ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, window, 2.0, variant=variant)
+    plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=2.0, m=m, window=window, variant=variant,
+                     dtype=torch.float64 if dtype == "f64" else torch.float32)
+    E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+    tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+    plan.close()
+
+
+# ------------------------------------------------------------------ edge cases
+
+def test_empty_and_neutral_inputs(enuf, torch_cuda):
+    torch = torch_cuda
+    plan = enuf.Plan(0, 10.0, 0.6, 8, 16, m=4, dtype=torch.float64)
+    E, F = plan.energy_forces(torch.empty((0, 3), dtype=torch.float64, device="cuda"),
+                              torch.empty((0,), dtype=torch.float64, device="cuda"))
+    assert E == 0.0 and F.shape == (0, 3)
+    plan.close()
+    plan = enuf.Plan(50, 10.0, 0.6, 8, 16, m=4, dtype=torch.float64)
+    r = torch.rand((50, 3), dtype=torch.float64, device="cuda") * 10
+    F = torch.full((50, 3), 7.0, dtype=torch.float64, device="cuda")
+    E, F = plan.energy_forces(r, torch.zeros(50, dtype=torch.float64, device="cuda"), F=F)
+    assert E == 0.0 and not F.any().item()          # F overwritten, not accumulated
+    plan.close()
+
+
+def test_single_particle_closed_form(enuf, torch_cuda, oracle):
+    """One charge: S(n) = q e^{-2 pi i n.x}, so E_rec = q^2/(2 pi L) sum_K w(n) (Eq. 38) and F = 0."""
+    torch = torch_cuda
+    L, alpha, kc, M, m = 10.0, 0.7, 8, 16, 6
+    plan = enuf.Plan(1, L, alpha, kc, M, m=m, dtype=torch.float64)
+    r = torch.tensor([[9.99, 0.01, 5.0]], dtype=torch.float64, device="cuda")   # stencil wraps in x and y
+    E, F = plan.energy_forces(r, torch.tensor([1.5], dtype=torch.float64, device="cuda"))
+    want = 1.5 ** 2 / (2 * math.pi * L) * sum(
+        oracle.w(int(a) ** 2 + int(b) ** 2 + int(c) ** 2, alpha, L) for a, b, c in oracle.modes(kc))
+    assert abs(E - want) <= 1e-10 * want            # KB m=6: NFFT error ~1e-12
+    assert np.abs(F.cpu().numpy()).max() <= 1e-6 * want / L     # analytic variant: NFFT-error level (R16)
+    plan.close()
+
+
+def test_positions_outside_box_and_on_boundaries(enuf, torch_cuda, oracle):
+    torch = torch_cuda
+    L, alpha, kc, M, m = 6.0, 1.0, 8, 16, 4
+    r, q = random_neutral_gas(40, L, seed=31)
+    r[0] = [0.0, 0.0, 0.0]; r[1] = [L, L, L]; r[2] = [-1e-17, L - 1e-15, 0.5 * L]
+    r[3] = [L / 64, 3 * L / 64, 5 * L / 64]           # exactly half-way between grid points (tie, R9)
+    shift = np.zeros_like(r); shift[::2] = [3 * L, -2 * L, 5 * L]
+    ref = oracle.enuf(r + shift, q, L, alpha, kc, 32, m, "kaiser_bessel")
+    plan = enuf.Plan(40, L, alpha, kc, M, m=m, dtype=torch.float64)
+    E, F = plan.energy_forces(torch.from_numpy(r + shift).cuda(), torch.from_numpy(q).cuda())
+    assert abs(E - ref["E"]) <= 1e-12 * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= 1e-11
+    plan.close()
+
+
+def test_lower_particle_count_and_reuse(enuf, torch_cuda, oracle):
+    torch = torch_cuda
+    w = make_workload("cfg1")
+    plan = enuf.Plan.from_workload(w)
+    r = torch.from_numpy(w.r).cuda(); q = torch.from_numpy(w.q).cuda()
+    E_full, _ = plan.energy_forces(r, q)
+    plan.set_num_particles(300)
+    E, F = plan.energy_forces(r[:300].contiguous(), q[:300].contiguous())
+    ref = oracle.enuf(w.r[:300], w.q[:300], w.L, w.alpha, w.k_cut, w.n, w.m, w.window)
+    assert abs(E - ref["E"]) <= F64_E * abs(ref["E"]) and rel_rms(F.cpu().numpy(), ref["F"]) <= F64_F
+    plan.set_num_particles(w.N)
+    E_again, _ = plan.energy_forces(r, q)
+    assert abs(E_again - E_full) <= 1e-13 * abs(E_full)
+    assert plan.launch_count() > 0 and plan.workspace_bytes() > 0
+    plan.close()
+
+
+def test_additivity_eq61_on_gpu(enuf, torch_cuda, oracle):
+    """Eq. 61: S~ of the two halves sums to S~ of the whole."""
+    torch = torch_cuda
+    w = make_workload("cfg1")
+    ml = oracle.modes(w.k_cut)
+    r = torch.from_numpy(w.r).cuda(); q = torch.from_numpy(w.q).cuda()
+    plan = enuf.Plan.from_workload(w, keep_spectrum=True)
+    plan.energy_forces(r, q); S = plan.structure_factor(ml)
+    plan.set_num_particles(500)
+    plan.energy_forces(r[:500].contiguous(), q[:500].contiguous()); Sa = plan.structure_factor(ml)
+    plan.energy_forces(r[500:].contiguous(), q[500:].contiguous()); Sb = plan.structure_factor(ml)
+    assert np.abs(S - (Sa + Sb)).max() <= 1e-12 * np.abs(S).max()
+    plan.close()
+
+
+def test_stage_profile_and_streams(enuf, torch_cuda):
+    torch = torch_cuda
+    w = make_workload("cfg3")
+    plan = enuf.Plan.from_workload(w, profile=True)
+    r = torch.from_numpy(w.r).cuda(); q = torch.from_numpy(w.q).cuda()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        E1, F1 = plan.energy_forces(r, q)
+        E2, F2 = plan.energy_forces(r, q, want_energy=False)
+        assert E2 is None and abs(plan.energy() - E1) <= 1e-9 * abs(E1)
+    s.synchronize()
+    ms = plan.stage_ms()
+    assert all(v >= 0 for v in ms.values()) and ms["spread"] > 0 and ms["fft"] > 0 and ms["gather"] > 0
+    mean, ne = plan.stage_ms_mean()
+    assert ne == 2 and mean["fft"] > 0
+    plan.close()
