@@ -75,7 +75,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
             const PRec<T> pr = rec[start + b0 + p];
             T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
             T phi, dphi;
-            window_eval<T, false>(wp, d0 - (T)(k - M_), phi, dphi);
+            window_eval<T, false>(wp, d0, k - M_, phi, dphi);
             if (dim == 0) phi *= pr.q;
             wt[(p * 3 + dim) * 16 + k] = phi;
         }
@@ -175,7 +175,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             int dim = e / W, k = e - dim * W;
             T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
             T phi, dphi = (T)0;
-            window_eval<T, !kIk>(wp, d0 - (T)(k - M_), phi, dphi);
+            window_eval<T, !kIk>(wp, d0, k - M_, phi, dphi);
             wt[dim * 16 + k] = phi;
             if (!kIk) wt[(3 + dim) * 16 + k] = dphi;
         }
