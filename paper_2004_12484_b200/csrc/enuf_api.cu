@@ -81,6 +81,53 @@ void fill_window_params(enuf_plan* p) {
     }
 }
 
+// The window and its analytic continuation beyond |d| = m (Kaiser-Bessel:
+// sinh(b s)/s with s^2 = m^2 - d^2 < 0 becomes sin(b t)/t, t^2 = d^2 - m^2), phi(0) = 1.
+// Only used to fit the polynomial table: the kernels cut the support themselves.
+double window_smooth(const enuf_plan* p, double d) {
+    const double m = p->m, sg = p->sigma;
+    if (p->window == ENUF_WINDOW_GAUSSIAN) {
+        const double b = 2.0 * sg * m / ((2.0 * sg - 1.0) * kPi);
+        return std::exp(-d * d / b);
+    }
+    const double b = kPi * (2.0 - 1.0 / sg), A = m / std::sinh(b * m);
+    const double s2 = (m - d) * (m + d), z = b * b * s2;
+    if (std::fabs(z) < 1e-2)   // sinh(x)/x = 1 + x^2/6 + x^4/120 + x^6/5040 + x^8/362880, x^2 = z
+        return A * b * (1.0 + z * (1.0 / 6.0 + z * (1.0 / 120.0 + z * (1.0 / 5040.0 + z / 362880.0))));
+    if (s2 > 0) { const double s = std::sqrt(s2); return A * std::sinh(b * s) / s; }
+    const double t = std::sqrt(-s2);
+    return A * std::sin(b * t) / t;
+}
+
+// Step a0 (fp32 path): for each stencil offset j the Chebyshev interpolant of degree
+// kPolyDeg of d0 -> phi(d0 - j) on [-1/2, 1/2], converted to monomials in d0, and its
+// exact derivative (enuf_common.cuh, PolyArg).
+void build_poly_table(enuf_plan* p) {
+    constexpr int D = enuf::kPolyDeg, NC = D + 1;
+    for (int j = -p->m; j <= p->m; ++j) {
+        long double a[NC];
+        for (int k = 0; k < NC; ++k) {
+            long double acc = 0;
+            for (int i = 0; i < NC; ++i) {
+                const double th = kPi * (i + 0.5) / NC;
+                acc += (long double)window_smooth(p, 0.5 * std::cos(th) - j) * std::cos(k * th);
+            }
+            a[k] = acc * (k == 0 ? 1.0L : 2.0L) / NC;
+        }
+        // T_0 = 1, T_1 = 2t, T_{k+1} = 4t T_k - T_{k-1} (x = 2t)
+        long double c[NC] = {0}, t0[NC] = {0}, t1[NC] = {0}, t2[NC];
+        t0[0] = 1; t1[1] = 2;
+        for (int e = 0; e < NC; ++e) c[e] = a[0] * t0[e] + a[1] * t1[e];
+        for (int k = 2; k < NC; ++k) {
+            for (int e = 0; e < NC; ++e) t2[e] = (e > 0 ? 4 * t1[e - 1] : 0.0L) - t0[e];
+            for (int e = 0; e < NC; ++e) { c[e] += a[k] * t2[e]; t0[e] = t1[e]; t1[e] = t2[e]; }
+        }
+        const int col = j + p->m;
+        for (int k = 0; k < NC; ++k) p->poly_c[k][col] = (float)c[k];
+        for (int k = 0; k < D; ++k) p->poly_d[k][col] = (float)((k + 1) * c[k + 1]);
+    }
+}
+
 template <typename T>
 int upload(void* dst, const std::vector<double>& src, cudaStream_t s) {
     std::vector<T> tmp(src.size());
@@ -111,6 +158,7 @@ int build_tables(enuf_plan* p) {
         wf[s] = w;
     }
     int rc;
+    build_poly_table(p);
     if (p->precision == ENUF_F32) {
         if ((rc = upload<float>(p->tw, tw, p->stream))) return rc;
         if ((rc = upload<float>(p->iphi, iphi, p->stream))) return rc;
@@ -139,7 +187,8 @@ int dev_alloc(enuf_plan* p, void** ptr, size_t bytes) {
 
 void free_workspace(enuf_plan* p) {
     auto fr = [](void* q) { if (q) cudaFree(q); };
-    fr(p->rec); fr(p->cell); fr(p->idx); fr(p->tile_count); fr(p->tile_offset); fr(p->tile_cursor);
+    fr(p->rec); fr(p->cell); fr(p->idx); fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
+    fr(p->scan_total);
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev);
     fr(p->r_stage); fr(p->q_stage); fr(p->F_stage);
@@ -152,7 +201,7 @@ void free_workspace(enuf_plan* p) {
     }
     p->prof_evals = 0;
     p->rec = p->spectrum = p->tw = p->iphi = p->wf = p->r_stage = p->q_stage = p->F_stage = nullptr;
-    p->cell = p->idx = p->tile_count = p->tile_offset = p->tile_cursor = nullptr;
+    p->cell = p->idx = p->bin_count = p->bin_offset = p->bin_cursor = p->scan_total = nullptr;
     p->e_partial = p->e_dev = p->e_pinned = nullptr;
     p->events_valid = false;
     p->allocated = false;
@@ -178,9 +227,10 @@ int ensure_allocated(enuf_plan* p) {
     ALLOC(p->rec, 4 * es * cap);
     ALLOC(p->cell, 4 * cap);
     ALLOC(p->idx, 4 * cap);
-    ALLOC(p->tile_count, 4 * (size_t)p->tg.ntiles);
-    ALLOC(p->tile_offset, 4 * ((size_t)p->tg.ntiles + 1));
-    ALLOC(p->tile_cursor, 4 * (size_t)p->tg.ntiles);
+    ALLOC(p->bin_count, 4 * (size_t)p->tg.nbins);
+    ALLOC(p->bin_offset, 4 * ((size_t)p->tg.nbins + 1));
+    ALLOC(p->bin_cursor, 4 * (size_t)p->tg.nbins);
+    ALLOC(p->scan_total, 4 * (((size_t)p->tg.nbins + 1023) / 1024));
     for (int d = 0; d < nfield; ++d) {
         ALLOC(p->grid[d], es * n3);
         ALLOC(p->A1[d], 2 * es * n * n * p->Kxp);
@@ -309,9 +359,11 @@ int enuf_plan_create(enuf_plan** out, int64_t N, double L, double alpha, int k_c
     p->N_cap = p->N = N;
     p->L = L; p->alpha = alpha; p->sigma = sigma; p->k_cut = k_cut; p->M = M; p->n = n; p->m = m;
     p->tg.n = n;
-    p->tg.T = n >= 128 ? 16 : 8;
-    p->tg.nt = n / p->tg.T;
-    p->tg.ntiles = p->tg.nt * p->tg.nt * p->tg.nt;
+    p->tg.nt = n / enuf::kTile;
+    p->tg.nbins = p->tg.nt * p->tg.nt * n;
+    // spread: columns x z-chunks; enough CTAs to fill 148 SMs several times over, chunks >= 16 planes
+    p->zchunk = n;
+    while (p->zchunk > 16 && p->tg.nt * p->tg.nt * (n / p->zchunk) < 592) p->zchunk /= 2;
     p->Kxp = ((k_cut + 1 + enuf::kLinesPerGroup - 1) / enuf::kLinesPerGroup) * enuf::kLinesPerGroup;
     p->Ky = 2 * k_cut + 1;
     fill_window_params(p);

@@ -1,5 +1,6 @@
 // Step a1 -- wrap positions (x = r/L; R10) and counting-sort the charged
-// particles by grid tile: histogram -> exclusive scan -> scatter.  The cell index c and
+// particles by bin (16 x 16 column in x, y and grid plane in z; TileGeom in enuf_common.cuh):
+// histogram -> exclusive scan (two launches, any number of bins) -> scatter.  The cell index c and
 // the fractional offset d0 = u - c are formed in fp64 in the order
 //   x = r/L;  x -= floor(x);  u = n*x;  c = floor(u + 1/2)
 // for both precisions (an fp32 u would lose the offset: ulp(256) ~ 1.5e-5 cells), so the
@@ -32,12 +33,11 @@ __device__ __forceinline__ CellOfParticle locate(const T* __restrict__ r, int64_
     return o;
 }
 
-__device__ __forceinline__ int tile_of(const int c[3], const TileGeom& g) {
-    int tx = c[0] / g.T, ty = c[1] / g.T, tz = c[2] / g.T;
-    return (tz * g.nt + ty) * g.nt + tx;
+__device__ __forceinline__ int bin_of(const int c[3], const TileGeom& g) {
+    return ((c[1] / kTile) * g.nt + (c[0] / kTile)) * g.n + c[2];
 }
 
-// Histogram of charged particles per tile; neutral particles get F = 0 here and are dropped.
+// Histogram of charged particles per bin; neutral particles get F = 0 here and are dropped.
 template <typename T>
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict__ F, int64_t N,
@@ -49,63 +49,95 @@ bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict
         return;
     }
     CellOfParticle p = locate(r, j, L, g.n);
-    atomicAdd(&count[tile_of(p.c, g)], 1u);
+    atomicAdd(&count[bin_of(p.c, g)], 1u);
 }
 
-// Exclusive scan of count[0..ntiles) into offset[0..ntiles]; zeroes cursor. One CTA.
-static __global__ void __launch_bounds__(1024)
-bin_scan_kernel(const uint32_t* __restrict__ count, uint32_t* __restrict__ offset,
-                uint32_t* __restrict__ cursor, int ntiles) {
-    __shared__ uint32_t warp_sums[32];
-    __shared__ uint32_t carry_s;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
+// Exclusive scan of count[0..nbins) into offset[0..nbins] (and a copy in cursor[0..nbins),
+// the scatter's running positions).  Two launches of kScanThreads threads per CTA, each
+// CTA owning kScanChunk = 4 * kScanThreads consecutive bins:
+//   bin_scan_totals: total[b] = sum of chunk b
+//   bin_scan_apply : base = sum of total[< b] (few hundred values at most), then a CTA scan.
+constexpr int kScanThreads = 256;
+constexpr int kScanChunk = 4 * kScanThreads;
+
+static __global__ void __launch_bounds__(kScanThreads)
+bin_scan_totals_kernel(const uint32_t* __restrict__ count, int nbins, uint32_t* __restrict__ total) {
+    __shared__ uint32_t ws[kScanThreads / 32];
+    const int i0 = blockIdx.x * kScanChunk + threadIdx.x * 4;
+    uint32_t v = 0;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) if (i0 + e < nbins) v += count[i0 + e];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = v;
     __syncthreads();
-    for (int base = 0; base < ntiles; base += 1024) {
-        int i = base + threadIdx.x;
-        uint32_t v = i < ntiles ? count[i] : 0u;
-        uint32_t inc = v;
+    if (threadIdx.x == 0) {
+        uint32_t s = 0;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) warp_sums[wid] = inc;
-        __syncthreads();
-        if (wid == 0) {
-            uint32_t ws = warp_sums[lane], winc = ws;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
-                if (lane >= o) winc += t;
-            }
-            warp_sums[lane] = winc - ws;   // exclusive prefix of warp totals
-        }
-        __syncthreads();
-        uint32_t carry = carry_s;
-        uint32_t excl = carry + warp_sums[wid] + inc - v;
-        if (i < ntiles) { offset[i] = excl; cursor[i] = 0u; }
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = excl + v;
-        __syncthreads();
+        for (int w = 0; w < kScanThreads / 32; ++w) s += ws[w];
+        total[blockIdx.x] = s;
     }
-    if (threadIdx.x == 0) offset[ntiles] = carry_s;
 }
 
-// Scatter into tile order.  The order inside a tile follows the atomic cursor (any order is
+static __global__ void __launch_bounds__(kScanThreads)
+bin_scan_apply_kernel(const uint32_t* __restrict__ count, int nbins, const uint32_t* __restrict__ total,
+                      uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor) {
+    __shared__ uint32_t ws[kScanThreads / 32];
+    __shared__ uint32_t base_s;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    // base of this chunk
+    uint32_t b = 0;
+    for (int i = threadIdx.x; i < (int)blockIdx.x; i += kScanThreads) b += total[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) b += __shfl_xor_sync(0xffffffffu, b, o);
+    if (lane == 0) ws[wid] = b;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t s = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) s += ws[w];
+        base_s = s;
+    }
+    __syncthreads();
+    const uint32_t base = base_s;
+    __syncthreads();
+    const int i0 = blockIdx.x * kScanChunk + threadIdx.x * 4;
+    uint32_t c[4], sum = 0;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) { c[e] = i0 + e < nbins ? count[i0 + e] : 0u; sum += c[e]; }
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) ws[wid] = inc;
+    __syncthreads();
+    uint32_t wbase = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) if (w < wid) wbase += ws[w];
+    uint32_t run = base + wbase + inc - sum;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        if (i0 + e < nbins) { offset[i0 + e] = run; cursor[i0 + e] = run; }
+        run += c[e];
+    }
+    if (i0 <= nbins - 1 && nbins - 1 < i0 + 4) offset[nbins] = run;   // thread owning the last bin
+}
+
+// Scatter into bin order.  The order inside a bin follows the atomic cursor (any order is
 // a valid sort; sums downstream differ only in rounding order, R22).
 template <typename T>
 __global__ void __launch_bounds__(256)
 bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, double L, TileGeom g,
-                   const uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor,
+                   uint32_t* __restrict__ cursor,
                    PRec<T>* __restrict__ rec, uint32_t* __restrict__ cell, uint32_t* __restrict__ idx) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     T qj = q[j];
     if (qj == (T)0) return;
     CellOfParticle p = locate(r, j, L, g.n);
-    int t = tile_of(p.c, g);
-    uint32_t pos = offset[t] + atomicAdd(&cursor[t], 1u);
+    uint32_t pos = atomicAdd(&cursor[bin_of(p.c, g)], 1u);
     PRec<T> o;
     o.dx = (T)p.d0[0]; o.dy = (T)p.d0[1]; o.dz = (T)p.d0[2]; o.q = qj;
     rec[pos] = o;

@@ -38,12 +38,30 @@ struct WindowParams {
 // One binned particle: fractional offset d0 per dimension and charge.
 template <typename T> struct alignas(4 * sizeof(T)) PRec { T dx, dy, dz, q; };
 
-// Geometry shared by bin / spread / gather.
+// Geometry shared by bin / spread / gather.  Particles are counting-sorted into bins
+//   bin = (Ty * nt + Tx) * n + cz,   Tx = cx / 16, Ty = cy / 16
+// (a column of 16 x 16 cells in x, y; one grid plane in z), so that
+//   - the particles of a z-slab of a column are one contiguous range (spread walks z), and
+//   - the particles of a 16^3 tile are one contiguous range of 16 bins (gather).
+constexpr int kTile = 16;
 struct TileGeom {
     int n;        // grid points per dimension
-    int T;        // tile edge in grid cells (8 or 16)
-    int nt;       // tiles per dimension = n / T
-    int ntiles;   // nt^3
+    int nt;       // columns per dimension = n / 16
+    int nbins;    // nt * nt * n
+};
+
+// Piecewise-polynomial window table for the fp32 path (step a0).  For every stencil offset
+// j in [-m, m] the weight phi(d0 - j), d0 in [-1/2, 1/2], is a polynomial of degree kPolyDeg
+// in d0 (Chebyshev interpolant of the window's analytic continuation, fitted in fp64 on the
+// host; max error <= 3e-11 of phi(0) for m = 1, <= 1e-14 for m = 6).  dphi is the exact
+// derivative of that polynomial.  The table is passed to the kernels BY VALUE as a
+// __grid_constant__ parameter: with fully unrolled loops every coefficient is a constant-bank
+// operand of an FFMA, so a stencil of W weights costs W * kPolyDeg FFMAs and no loads.
+constexpr int kPolyDeg = 12;
+template <int M_>
+struct PolyArg {
+    float c[kPolyDeg + 1][2 * M_ + 1];   // value:      phi_j(d0)  = sum_i c[i][j + m] d0^i
+    float d[kPolyDeg][2 * M_ + 1];       // derivative: phi_j'(d0) = sum_i d[i][j + m] d0^i
 };
 
 __host__ __device__ inline uint32_t pack_cell(int cx, int cy, int cz) {
@@ -107,6 +125,53 @@ __device__ __forceinline__ void window_eval(const WindowParams& wp, T d0, int j,
             phi = (s2 == (T)0) ? (T)(wp.A * wp.b) : (T)0;
             if (kDeriv) dphi = (T)0;
         }
+    }
+}
+
+
+// All W = 2m+1 window weights (and derivatives) of one particle in one dimension:
+//   w[k] = phi(d0 - (k - m)),  dw[k] = phi'(d0 - (k - m)),  k = 0..W-1.
+//   fp32: Horner evaluation of the plan's polynomial table; Kaiser-Bessel support cut
+//         |d| <= m (value) and |d| < m (derivative) exactly as in the closed form.
+//   fp64: the closed form (window_eval).
+template <typename T, int M_, bool kDeriv>
+__device__ __forceinline__ void stencil_weights(const WindowParams& wp, const PolyArg<M_>& pa, T d0,
+                                                T (&w)[2 * M_ + 1], T (&dw)[2 * M_ + 1]) {
+    constexpr int W = 2 * M_ + 1;
+    if (sizeof(T) == 8) {
+#pragma unroll
+        for (int k = 0; k < W; ++k) {
+            dw[k] = (T)0;
+            window_eval<T, kDeriv>(wp, d0, k - M_, w[k], dw[k]);
+        }
+    } else {
+        const float x = (float)d0;
+        float v[W], dv[W];
+#pragma unroll
+        for (int j = 0; j < W; ++j) v[j] = pa.c[kPolyDeg][j];
+#pragma unroll
+        for (int i = kPolyDeg - 1; i >= 0; --i)
+#pragma unroll
+            for (int j = 0; j < W; ++j) v[j] = fmaf(v[j], x, pa.c[i][j]);
+        if (kDeriv) {
+#pragma unroll
+            for (int j = 0; j < W; ++j) dv[j] = pa.d[kPolyDeg - 1][j];
+#pragma unroll
+            for (int i = kPolyDeg - 2; i >= 0; --i)
+#pragma unroll
+                for (int j = 0; j < W; ++j) dv[j] = fmaf(dv[j], x, pa.d[i][j]);
+        } else {
+#pragma unroll
+            for (int j = 0; j < W; ++j) dv[j] = 0.f;
+        }
+        if (wp.kind == ENUF_WINDOW_KAISER_BESSEL) {
+            // |d0 - j| > m only for j = +m (d0 < 0) and j = -m (d0 > 0); phi' = 0 at |d| = m
+            if (x < 0.f) { v[W - 1] = 0.f; dv[W - 1] = 0.f; }
+            if (x > 0.f) { v[0] = 0.f; dv[0] = 0.f; }
+            if (x == 0.f) { dv[0] = 0.f; dv[W - 1] = 0.f; }
+        }
+#pragma unroll
+        for (int j = 0; j < W; ++j) { w[j] = (T)v[j]; dw[j] = (T)dv[j]; }
     }
 }
 

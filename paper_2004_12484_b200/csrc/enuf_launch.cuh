@@ -5,6 +5,7 @@
 
 #include "enuf_bin.cuh"
 #include "enuf_fft.cuh"
+#include "enuf_gather.cuh"
 #include "enuf_plan.h"
 #include "enuf_spread.cuh"
 
@@ -12,15 +13,18 @@ namespace enuf {
 
 template <int V> using IntC = std::integral_constant<int, V>;
 
-// f(IntC<m>, IntC<tile>) -> int
+// f(IntC<m>) -> int
 template <typename F>
-static inline int dispatch_mt(const enuf_plan* p, F&& f) {
-#define ENUF_CASE_M(mv) case mv: return p->tg.T == 16 ? f(IntC<mv>{}, IntC<16>{}) : f(IntC<mv>{}, IntC<8>{});
+static inline int dispatch_m(const enuf_plan* p, F&& f) {
     switch (p->m) {
-        ENUF_CASE_M(1) ENUF_CASE_M(2) ENUF_CASE_M(3) ENUF_CASE_M(4) ENUF_CASE_M(5) ENUF_CASE_M(6)
+        case 1: return f(IntC<1>{});
+        case 2: return f(IntC<2>{});
+        case 3: return f(IntC<3>{});
+        case 4: return f(IntC<4>{});
+        case 5: return f(IntC<5>{});
+        case 6: return f(IntC<6>{});
         default: return -1;
     }
-#undef ENUF_CASE_M
 }
 
 // f(IntC<n>) -> int
@@ -35,6 +39,16 @@ static inline int dispatch_n(int n, F&& f) {
     }
 }
 
+template <int M_>
+static inline PolyArg<M_> make_poly_arg(const enuf_plan* p) {
+    PolyArg<M_> a;
+    for (int j = 0; j < 2 * M_ + 1; ++j) {
+        for (int k = 0; k <= kPolyDeg; ++k) a.c[k][j] = p->poly_c[k][j];
+        for (int k = 0; k < kPolyDeg; ++k) a.d[k][j] = p->poly_d[k][j];
+    }
+    return a;
+}
+
 template <typename K>
 static inline bool set_smem(K kernel, size_t bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
@@ -42,11 +56,11 @@ static inline bool set_smem(K kernel, size_t bytes) {
 
 template <typename T>
 int configure_kernels(enuf_plan* p) {
-    int rc = dispatch_mt(p, [&](auto mc, auto tc) -> int {
-        constexpr int M_ = decltype(mc)::value, TL = decltype(tc)::value;
-        bool ok = set_smem(spread_kernel<T, M_, TL>, spread_smem_bytes<T, M_, TL>());
-        ok = ok && set_smem(gather_kernel<T, M_, TL, false>, gather_smem_bytes<T, M_, TL>());
-        ok = ok && set_smem(gather_kernel<T, M_, TL, true>, gather_smem_bytes<T, M_, TL>());
+    int rc = dispatch_m(p, [&](auto mc) -> int {
+        constexpr int M_ = decltype(mc)::value;
+        bool ok = set_smem(spread_kernel<T, M_>, spread_smem_bytes<T, M_>());
+        ok = ok && set_smem(gather_kernel<T, M_, false>, gather_smem_bytes<T, M_>());
+        ok = ok && set_smem(gather_kernel<T, M_, true>, gather_smem_bytes<T, M_>());
         return ok ? 0 : -1;
     });
     if (rc) return rc;
@@ -64,28 +78,31 @@ template <typename T>
 int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     cudaStream_t s = p->stream;
     const int64_t N = p->N;
-    if (cudaMemsetAsync(p->tile_count, 0, sizeof(uint32_t) * p->tg.ntiles, s) != cudaSuccess) return -1;
+    const int nbins = p->tg.nbins;
+    if (cudaMemsetAsync(p->bin_count, 0, sizeof(uint32_t) * nbins, s) != cudaSuccess) return -1;
     const unsigned blocks = (unsigned)((N + 255) / 256);
+    const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
     bin_count_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q),
-                                               static_cast<T*>(F), N, p->L, p->tg, p->tile_count);
-    bin_scan_kernel<<<1, 1024, 0, s>>>(p->tile_count, p->tile_offset, p->tile_cursor, p->tg.ntiles);
+                                               static_cast<T*>(F), N, p->L, p->tg, p->bin_count);
+    bin_scan_totals_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total);
+    bin_scan_apply_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total, p->bin_offset,
+                                                          p->bin_cursor);
     bin_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
-                                                 p->tg, p->tile_offset, p->tile_cursor,
-                                                 static_cast<PRec<T>*>(p->rec), p->cell, p->idx);
-    return cudaGetLastError() == cudaSuccess ? 3 : -1;
+                                                 p->tg, p->bin_cursor, static_cast<PRec<T>*>(p->rec), p->cell,
+                                                 p->idx);
+    return cudaGetLastError() == cudaSuccess ? 4 : -1;
 }
 
 template <typename T>
 int launch_spread(enuf_plan* p) {
     cudaStream_t s = p->stream;
-    const size_t n3 = (size_t)p->n * p->n * p->n;
-    if (cudaMemsetAsync(p->grid[0], 0, sizeof(T) * n3, s) != cudaSuccess) return -1;
-    int rc = dispatch_mt(p, [&](auto mc, auto tc) -> int {
-        constexpr int M_ = decltype(mc)::value, TL = decltype(tc)::value;
-        using C = TileCfg<M_, TL>;
-        spread_kernel<T, M_, TL><<<p->tg.ntiles, C::SPREAD_THREADS, spread_smem_bytes<T, M_, TL>(), s>>>(
-            static_cast<const PRec<T>*>(p->rec), p->cell, p->tile_offset, p->tg, p->wp,
-            static_cast<T*>(p->grid[0]));
+    int rc = dispatch_m(p, [&](auto mc) -> int {
+        constexpr int M_ = decltype(mc)::value;
+        using C = SpreadCfg<M_>;
+        const dim3 grid((unsigned)(p->tg.nt * p->tg.nt), (unsigned)((p->n + p->zchunk - 1) / p->zchunk));
+        spread_kernel<T, M_><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
+            static_cast<const PRec<T>*>(p->rec), p->cell, p->bin_offset, p->tg, p->wp, make_poly_arg<M_>(p),
+            p->zchunk, static_cast<T*>(p->grid[0]));
         return 0;
     });
     if (rc) return -1;
@@ -142,23 +159,25 @@ template <typename T>
 int launch_gather(enuf_plan* p, void* F) {
     cudaStream_t s = p->stream;
     const double PI = 3.14159265358979323846;
-    int launches = dispatch_mt(p, [&](auto mc, auto tc) -> int {
-        constexpr int M_ = decltype(mc)::value, TL = decltype(tc)::value;
+    int launches = dispatch_m(p, [&](auto mc) -> int {
+        constexpr int M_ = decltype(mc)::value;
         int launches = 0;
-        using C = TileCfg<M_, TL>;
-        const size_t sb = gather_smem_bytes<T, M_, TL>();
+        using C = GatherCfg<M_>;
+        const size_t sb = gather_smem_bytes<T, M_>();
+        const unsigned ntiles = (unsigned)(p->tg.nt * p->tg.nt * (p->n / kTile));
+        const PolyArg<M_> pa = make_poly_arg<M_>(p);
         if (p->variant == ENUF_FORCE_ANALYTIC) {
             const T pre = (T)(-(double)p->n / (PI * p->L * p->L));
-            gather_kernel<T, M_, TL, false><<<p->tg.ntiles, C::GATHER_WARPS * 32, sb, s>>>(
+            gather_kernel<T, M_, false><<<ntiles, C::NT, sb, s>>>(
                 static_cast<const T*>(p->grid[0]), static_cast<const PRec<T>*>(p->rec), p->cell, p->idx,
-                p->tile_offset, p->tg, p->wp, pre, 0, static_cast<T*>(F));
+                p->bin_offset, p->tg, p->wp, pa, pre, 0, static_cast<T*>(F));
             launches = 1;
         } else {
             const T pre = (T)(2.0 / (p->L * p->L));
             for (int d = 0; d < 3; ++d)
-                gather_kernel<T, M_, TL, true><<<p->tg.ntiles, C::GATHER_WARPS * 32, sb, s>>>(
+                gather_kernel<T, M_, true><<<ntiles, C::NT, sb, s>>>(
                     static_cast<const T*>(p->grid[d]), static_cast<const PRec<T>*>(p->rec), p->cell, p->idx,
-                    p->tile_offset, p->tg, p->wp, pre, d, static_cast<T*>(F));
+                    p->bin_offset, p->tg, p->wp, pa, pre, d, static_cast<T*>(F));
             launches = 3;
         }
         return launches;

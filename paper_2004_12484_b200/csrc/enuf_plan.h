@@ -28,9 +28,13 @@ struct enuf_plan {
     void* rec = nullptr;           // PRec<T>[N_cap]
     uint32_t* cell = nullptr;      // [N_cap]
     uint32_t* idx = nullptr;       // [N_cap]
-    uint32_t* tile_count = nullptr;   // [ntiles]
-    uint32_t* tile_offset = nullptr;  // [ntiles+1]
-    uint32_t* tile_cursor = nullptr;  // [ntiles]
+    uint32_t* bin_count = nullptr;    // [nbins]
+    uint32_t* bin_offset = nullptr;   // [nbins+1]
+    uint32_t* bin_cursor = nullptr;   // [nbins]
+    uint32_t* scan_total = nullptr;   // [ceil(nbins / kScanChunk)]
+    float poly_c[enuf::kPolyDeg + 1][enuf::kMaxW] = {};   // host copy of the polynomial window table
+    float poly_d[enuf::kPolyDeg][enuf::kMaxW] = {};       // (fp32 path; packed into PolyArg<m> per launch)
+    int zchunk = 0;                   // grid planes per spread CTA
     void* grid[3] = {nullptr, nullptr, nullptr};   // real n^3 (1 for analytic, 3 for ik)
     void* A1[3] = {nullptr, nullptr, nullptr};     // complex [n][n][Kxp]
     void* A2[3] = {nullptr, nullptr, nullptr};     // complex [n][Ky][Kxp]

@@ -1,227 +1,202 @@
 // Step a2 -- spreading (adjoint NFFT, part 1):
 //   g[l] = sum_j q_j phi(u_jx - l_x) phi(u_jy - l_y) phi(u_jz - l_z), l periodic.
-// Step a6 -- interpolating (forward NFFT, last part; Eq. 42 :340).
 //
-// Both run one CTA per grid tile of TILE^3 cells on the tile's particles (binned by a1),
-// with the tile plus a halo of m cells per side ((TILE+2m)^3 values) held in shared memory
-// and the 3*(2m+1) window values of a particle computed once per particle and kept on
-// chip (the paper's "window values computed in local memory").
-//
-// Spread -- no shared-memory atomics (fp32 atomicAdd on shared memory is a CAS loop on
-// sm_100a).  Instead every shared cell has exactly one owner thread: thread (ty, tz) owns
-// all cells with ly = ty (mod W), lz = tz (mod W).  A (2m+1)^2 block of (y, z) rows hits
-// every residue pair exactly once, so all W*W threads work on every particle, each doing
-// the W cells of one x-row, and the read-modify-write of a cell is always done by the
-// same thread in program order: race-free without atomics or barriers, and the summation
-// order inside a tile is the sorted particle order.  Only the flush of the padded tile to
-// the global grid uses (global) atomic adds, because halos of neighbouring tiles overlap.
+// Output-stationary, sliding z-window.  A CTA owns a 16 x 16 column of grid cells in
+// (x, y) and a chunk [z0, z1) of grid planes.  Every lane owns two x-adjacent cells of the
+// column and keeps, in registers, the partial sums of those two cells on the W = 2m+1
+// consecutive planes z = s-m .. s+m that the particles of slab s (nearest plane c_z = s)
+// can reach.  The CTA walks s upwards: after slab s, plane s-m is complete, is written to
+// the grid with one plain coalesced store, and the window slides by one plane.  So
+//   - every grid value is written exactly once: no atomics, no clearing of the grid,
+//     and the sum for a cell is formed in registers (no shared-memory read-modify-write);
+//   - per (warp, particle) visit the work is W packed FMAs acc[k] += (a0, a1) * wz[k],
+//     with a0, a1 = wx[cell] * wy[cell] read from zero-padded per-particle rows.
+// The particles of slab s that reach the column come from the 3 x 3 neighbouring columns'
+// bins (TileGeom); they are culled against the column's halo of m cells, their 3 W window
+// values are computed once per CTA (the paper's "window values computed in local memory",
+// PAPER.md:519) and staged in shared memory; each of the four warps (8 x 8 cells) then
+// visits only the particles whose stencil overlaps its cells.
 #pragma once
 
 #include "enuf_common.cuh"
 
 namespace enuf {
 
-template <int M_, int TILE>
-struct TileCfg {
+template <typename T> struct Pair2;
+template <> struct Pair2<float> { using type = float2; };
+template <> struct Pair2<double> { using type = double2; };
+
+// acc += a * w (both halves), one FFMA2 for fp32 on sm_100a
+__device__ __forceinline__ void fma_pair(float2& acc, const float2 a, const float w) {
+    unsigned long long A, C, Wv;
+    const float2 w2 = make_float2(w, w);
+    A = *reinterpret_cast<const unsigned long long*>(&a);
+    C = *reinterpret_cast<unsigned long long*>(&acc);
+    Wv = *reinterpret_cast<const unsigned long long*>(&w2);
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(C) : "l"(A), "l"(Wv));
+    acc = *reinterpret_cast<float2*>(&C);
+}
+__device__ __forceinline__ void fma_pair(double2& acc, const double2 a, const double w) {
+    acc.x = fma(a.x, w, acc.x);
+    acc.y = fma(a.y, w, acc.y);
+}
+
+template <int M_>
+struct SpreadCfg {
     static constexpr int W = 2 * M_ + 1;
-    static constexpr int TP = TILE + 2 * M_;                    // padded tile edge
-    static constexpr int SX = (TP % 2 == 0) ? TP + 1 : TP;      // odd row stride (bank spread)
-    static constexpr int SPL = TP * SX + ((TP * SX) % 2 == 0 ? 1 : 0) + 2;  // plane stride
-    static constexpr int CELLS = ((TP * SPL + 3) / 4) * 4;      // shared tile size in elements (16 B multiple)
-    static constexpr int PB = 16;                               // particles per weight batch
-    static constexpr int SPREAD_THREADS = ((W * W + 31) / 32) * 32;
-    static constexpr int GATHER_WARPS = 8;
+    static constexpr int NT = 128;          // 4 warps: 2 x 2 patches of 8 x 8 cells
+    static constexpr int CAP = NT;          // staged particles per chunk (one candidate per thread)
+    static constexpr int ROW = 16;          // row length of the staged x / y / z weight rows
 };
 
-template <typename T, int M_, int TILE>
+template <typename T, int M_>
 constexpr size_t spread_smem_bytes() {
-    using C = TileCfg<M_, TILE>;
-    return sizeof(T) * ((size_t)C::CELLS + 2 * C::PB * 3 * 16) + sizeof(int) * 2 * C::PB * 4;
+    using C = SpreadCfg<M_>;
+    return sizeof(T) * (size_t)C::CAP * (3 * C::ROW + 4) + sizeof(int) * (size_t)C::CAP;
 }
 
-template <typename T, int M_, int TILE>
-__global__ void __launch_bounds__(TileCfg<M_, TILE>::SPREAD_THREADS)
+template <typename T, int M_>
+__global__ void __launch_bounds__(SpreadCfg<M_>::NT)
 spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell,
-              const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp, T* __restrict__ grid) {
-    using C = TileCfg<M_, TILE>;
-    constexpr int W = C::W, TP = C::TP, SX = C::SX, SPL = C::SPL, PB = C::PB;
-    constexpr int NT = C::SPREAD_THREADS;
-
-    const int tile = blockIdx.x;
-    const uint32_t start = offset[tile];
-    const int cnt = (int)(offset[tile + 1] - start);
-    if (cnt == 0) return;
+              const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
+              const __grid_constant__ PolyArg<M_> pa, int zchunk, T* __restrict__ grid) {
+    using C = SpreadCfg<M_>;
+    using P2 = typename Pair2<T>::type;
+    constexpr int W = C::W, NT = C::NT, CAP = C::CAP, ROW = C::ROW;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* tile_s = reinterpret_cast<T*>(smem_raw);
-    T* wtab = tile_s + C::CELLS;                         // [2][PB][3][16]
-    int* base_s = reinterpret_cast<int*>(wtab + 2 * PB * 3 * 16);   // [2][PB][4]
-
-    const int tid = threadIdx.x;
-    for (int e = tid; e < C::CELLS; e += NT) tile_s[e] = (T)0;
-
-    const int tx0 = (tile % g.nt) * TILE, ty0 = ((tile / g.nt) % g.nt) * TILE, tz0 = (tile / (g.nt * g.nt)) * TILE;
-    const int ty = tid % W, tz = tid / W;               // owned residues (tid < W*W)
-    constexpr int KW = ((TILE + W - 1) / W) * W;        // multiple of W >= TILE
-
-    int buf = 0;
-    for (int b0 = 0; b0 < cnt; b0 += PB, buf ^= 1) {
-        const int nb = min(PB, cnt - b0);
-        T* wt = wtab + buf * (PB * 3 * 16);
-        int* bs = base_s + buf * (PB * 4);
-        // window values of the batch, once per particle (q folded into the x weights)
-        for (int e = tid; e < nb * 3 * W; e += NT) {
-            int p = e / (3 * W), rem = e - p * 3 * W, dim = rem / W, k = rem - dim * W;
-            const PRec<T> pr = rec[start + b0 + p];
-            T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
-            T phi, dphi;
-            window_eval<T, false>(wp, d0, k - M_, phi, dphi);
-            if (dim == 0) phi *= pr.q;
-            wt[(p * 3 + dim) * 16 + k] = phi;
-        }
-        for (int p = tid; p < nb; p += NT) {
-            int cx, cy, cz;
-            unpack_cell(cell[start + b0 + p], cx, cy, cz);
-            bs[p * 4 + 0] = cx - tx0; bs[p * 4 + 1] = cy - ty0; bs[p * 4 + 2] = cz - tz0;
-        }
-        __syncthreads();   // with double buffering this is the only barrier per batch
-        if (tid < W * W) {
-            for (int p = 0; p < nb; ++p) {
-                const int bx = bs[p * 4], by = bs[p * 4 + 1], bz = bs[p * 4 + 2];
-                const int oy = (ty - by + KW) % W, oz = (tz - bz + KW) % W;
-                const T* wp_ = wt + p * 3 * 16;
-                const T a = wp_[16 + oy] * wp_[32 + oz];
-                T* row = tile_s + (bz + oz) * SPL + (by + oy) * SX + bx;
-                T wx[16];
-                if (sizeof(T) == 4) {
-#pragma unroll
-                    for (int v = 0; v < 4; ++v)
-                        *reinterpret_cast<float4*>(&wx[4 * v]) = *reinterpret_cast<const float4*>(&wp_[4 * v]);
-                } else {
-#pragma unroll
-                    for (int v = 0; v < 8; ++v)
-                        *reinterpret_cast<double2*>(&wx[2 * v]) = *reinterpret_cast<const double2*>(&wp_[2 * v]);
-                }
-#pragma unroll
-                for (int k = 0; k < W; ++k) row[k] += a * wx[k];
-            }
-        }
-    }
-    __syncthreads();
-    // flush padded tile (origin = tile origin - m) to the periodic global grid
-    for (int e = tid; e < TP * TP * TP; e += NT) {
-        int lx = e % TP, t2 = e / TP, ly = t2 % TP, lz = t2 / TP;
-        T v = tile_s[lz * SPL + ly * SX + lx];
-        if (v != (T)0) {
-            int gx = tx0 - M_ + lx, gy = ty0 - M_ + ly, gz = tz0 - M_ + lz;
-            gx += gx < 0 ? g.n : 0; gx -= gx >= g.n ? g.n : 0;
-            gy += gy < 0 ? g.n : 0; gy -= gy >= g.n ? g.n : 0;
-            gz += gz < 0 ? g.n : 0; gz -= gz >= g.n ? g.n : 0;
-            atomicAdd(&grid[((size_t)gz * g.n + gy) * g.n + gx], v);
-        }
-    }
-}
-
-// ------------------------------------------------------------------------ gather
-template <typename T, int M_, int TILE>
-constexpr size_t gather_smem_bytes() {
-    using C = TileCfg<M_, TILE>;
-    return sizeof(T) * ((size_t)C::CELLS + C::GATHER_WARPS * 6 * 16);
-}
-
-// kIk = false: analytic-derivative variant, F = pre*q * sum Psi[l] grad(phi phi phi)
-//              with pre = -n/(pi L^2)  (exact gradient of the ENUF energy).
-// kIk = true : one component d of the paper's ik variant, F[.,d] = pre*q * sum B_d[l] phi phi phi
-//              with pre = 2/L^2 (Eq. 42).
-template <typename T, int M_, int TILE, bool kIk>
-__global__ void __launch_bounds__(TileCfg<M_, TILE>::GATHER_WARPS * 32)
-gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
-              const uint32_t* __restrict__ cell, const uint32_t* __restrict__ idx,
-              const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp, T pre,
-              int component, T* __restrict__ F) {
-    using C = TileCfg<M_, TILE>;
-    constexpr int W = C::W, TP = C::TP, SX = C::SX, SPL = C::SPL;
-    constexpr int NT = C::GATHER_WARPS * 32;
-
-    const int tile = blockIdx.x;
-    const uint32_t start = offset[tile];
-    const int cnt = (int)(offset[tile + 1] - start);
-    if (cnt == 0) return;
-
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* tile_s = reinterpret_cast<T*>(smem_raw);
-    T* wtab = tile_s + C::CELLS;    // [warps][6][16]: phi x,y,z then phi' x,y,z
+    T* wxr = reinterpret_cast<T*>(smem_raw);          // [CAP][ROW] x weights on the column's 16 cells
+    T* wyr = wxr + CAP * ROW;                          // [CAP][ROW]
+    T* wzr = wyr + CAP * ROW;                          // [CAP][ROW] q * z weights, k = 0..W-1
+    T* sd = wzr + CAP * ROW;                           // [CAP][4]   d0x, d0y, d0z, q
+    int* sb = reinterpret_cast<int*>(sd + CAP * 4);    // [CAP]      (bx + m) | (by + m) << 8
+    __shared__ int rng_start[2][9], rng_cnt[2][9];
+    __shared__ int nslot_s;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tx0 = (tile % g.nt) * TILE, ty0 = ((tile / g.nt) % g.nt) * TILE, tz0 = (tile / (g.nt * g.nt)) * TILE;
+    const int Tx = blockIdx.x % g.nt, Ty = blockIdx.x / g.nt;
+    const int z0 = blockIdx.y * zchunk, z1 = min(g.n, z0 + zchunk);
+    const int px = (warp & 1) * 8, py = (warp >> 1) * 8;           // warp patch origin in the column
+    const int lx = px + (lane & 3) * 2, ly = py + (lane >> 2);     // this lane's two cells: (lx, ly), (lx+1, ly)
 
-    for (int e = tid; e < TP * TP * TP; e += NT) {
-        int lx = e % TP, t2 = e / TP, ly = t2 % TP, lz = t2 / TP;
-        int gx = tx0 - M_ + lx, gy = ty0 - M_ + ly, gz = tz0 - M_ + lz;
-        gx += gx < 0 ? g.n : 0; gx -= gx >= g.n ? g.n : 0;
-        gy += gy < 0 ? g.n : 0; gy -= gy >= g.n ? g.n : 0;
-        gz += gz < 0 ? g.n : 0; gz -= gz >= g.n ? g.n : 0;
-        tile_s[lz * SPL + ly * SX + lx] = field[((size_t)gz * g.n + gy) * g.n + gx];
+    // the 9 neighbouring columns (tid < 9): bin of plane 0
+    int nb_bin0 = 0;
+    if (tid < 9) {
+        int ty = Ty + tid / 3 - 1, tx = Tx + tid % 3 - 1;
+        ty += ty < 0 ? g.nt : 0; ty -= ty >= g.nt ? g.nt : 0;
+        tx += tx < 0 ? g.nt : 0; tx -= tx >= g.nt ? g.nt : 0;
+        nb_bin0 = (ty * g.nt + tx) * g.n;
     }
-    __syncthreads();
+    auto load_ranges = [&](int s, int buf) {
+        if (tid < 9) {
+            const int cz = s < 0 ? s + g.n : (s >= g.n ? s - g.n : s);
+            const uint32_t st = offset[nb_bin0 + cz];
+            rng_start[buf][tid] = (int)st;
+            rng_cnt[buf][tid] = (int)(offset[nb_bin0 + cz + 1] - st);
+        }
+    };
+    if (tid == 0) nslot_s = 0;
+    load_ranges(z0 - M_, 0);
 
-    T* wt = wtab + warp * 6 * 16;
-    for (int p = warp; p < cnt; p += C::GATHER_WARPS) {
-        const PRec<T> pr = rec[start + p];
-        int cx, cy, cz;
-        unpack_cell(cell[start + p], cx, cy, cz);
-        const int bx = cx - tx0, by = cy - ty0, bz = cz - tz0;
-        for (int e = lane; e < 3 * W; e += 32) {
-            int dim = e / W, k = e - dim * W;
-            T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
-            T phi, dphi = (T)0;
-            window_eval<T, !kIk>(wp, d0, k - M_, phi, dphi);
-            wt[dim * 16 + k] = phi;
-            if (!kIk) wt[(3 + dim) * 16 + k] = dphi;
-        }
-        __syncwarp();
-        T wx[W], dwx[W];
+    P2 acc[W];
 #pragma unroll
-        for (int k = 0; k < W; ++k) { wx[k] = wt[k]; if (!kIk) dwx[k] = wt[48 + k]; }
-        T fx = (T)0, fy = (T)0, fz = (T)0;
-        for (int rr = lane; rr < W * W; rr += 32) {
-            const int rz = rr / W, ry = rr - rz * W;
-            const T* row = tile_s + (bz + rz) * SPL + (by + ry) * SX + bx;
-            T s0 = (T)0, s1 = (T)0;
+    for (int k = 0; k < W; ++k) { acc[k].x = (T)0; acc[k].y = (T)0; }
+
+    T* gout = grid + ((size_t)(Ty * kTile + ly)) * g.n + Tx * kTile + lx;
+
+    int buf = 0;
+    for (int s = z0 - M_; s < z1 + M_; ++s, buf ^= 1) {
+        __syncthreads();      // ranges of slab s visible; all warps are done with the previous slab
+        if (s + 1 < z1 + M_) load_ranges(s + 1, buf ^ 1);
+        int pref[10];
+        pref[0] = 0;
 #pragma unroll
-            for (int k = 0; k < W; ++k) {
-                T v = row[k];
-                s0 += v * wx[k];
-                if (!kIk) s1 += v * dwx[k];
-            }
-            const T wy = wt[16 + ry], wz = wt[32 + rz];
-            if (kIk) {
-                fx += s0 * (wy * wz);
-            } else {
-                const T dwy = wt[64 + ry], dwz = wt[80 + rz];
-                fx += s1 * (wy * wz);
-                fy += s0 * (dwy * wz);
-                fz += s0 * (wy * dwz);
-            }
-        }
+        for (int i = 0; i < 9; ++i) pref[i + 1] = pref[i] + rng_cnt[buf][i];
+        const int total = pref[9];
+
+        for (int c0 = 0; c0 < total; c0 += NT) {
+            // ---- cull: one candidate per thread
+            const int c = c0 + tid;
+            bool take = false;
+            int bxm = 0, bym = 0;
+            uint32_t pidx = 0;
+            if (c < total) {
+                int i = 0;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            fx += __shfl_xor_sync(0xffffffffu, fx, o);
-            if (!kIk) {
-                fy += __shfl_xor_sync(0xffffffffu, fy, o);
-                fz += __shfl_xor_sync(0xffffffffu, fz, o);
+                for (int e = 1; e < 9; ++e) i += (c >= pref[e]) ? 1 : 0;
+                int pb = 0;
+#pragma unroll
+                for (int e = 1; e < 9; ++e) pb = (i == e) ? pref[e] : pb;
+                pidx = (uint32_t)(rng_start[buf][i] + (c - pb));
+                int cx, cy, czp;
+                unpack_cell(cell[pidx], cx, cy, czp);
+                bxm = (cx & (kTile - 1)) + (i % 3 - 1) * kTile + M_;      // bx + m, bx relative to the column
+                bym = (cy & (kTile - 1)) + (i / 3 - 1) * kTile + M_;
+                take = (unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_);
             }
-        }
-        if (lane == 0) {
-            const size_t j = idx[start + p];
-            const T s = pre * pr.q;
-            if (kIk) {
-                F[3 * j + component] = s * fx;
-            } else {
-                F[3 * j] = s * fx; F[3 * j + 1] = s * fy; F[3 * j + 2] = s * fz;
+            const unsigned tmask = __ballot_sync(0xffffffffu, take);
+            if (tmask) {
+                int base = 0;
+                if (lane == 0) base = atomicAdd(&nslot_s, __popc(tmask));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (take) {
+                    const int slot = base + __popc(tmask & ((1u << lane) - 1u));
+                    const PRec<T> pr = rec[pidx];
+                    sd[slot * 4 + 0] = pr.dx; sd[slot * 4 + 1] = pr.dy; sd[slot * 4 + 2] = pr.dz; sd[slot * 4 + 3] = pr.q;
+                    sb[slot] = bxm | (bym << 8);
+                }
             }
+            __syncthreads();
+            const int ns = nslot_s;
+            // ---- window values: one task per (dimension, slot); dimension-major so warps stay uniform
+            for (int t = tid; t < 3 * ns; t += NT) {
+                const int dim = t / ns, slot = t - dim * ns;
+                T w[W], dw[W];
+                stencil_weights<T, M_, false>(wp, pa, sd[slot * 4 + dim], w, dw);
+                if (dim == 2) {
+                    const T q = sd[slot * 4 + 3];
+#pragma unroll
+                    for (int k = 0; k < W; ++k) wzr[slot * ROW + k] = w[k] * q;
+                } else {
+                    T* row = (dim == 0 ? wxr : wyr) + slot * ROW;
+#pragma unroll
+                    for (int e = 0; e < ROW; ++e) row[e] = (T)0;
+                    const int X0 = (dim == 0 ? (sb[slot] & 255) : (sb[slot] >> 8)) - 2 * M_;   // cell of k = 0
+#pragma unroll
+                    for (int k = 0; k < W; ++k)
+                        if ((unsigned)(X0 + k) < (unsigned)kTile) row[X0 + k] = w[k];
+                }
+            }
+            __syncthreads();
+            if (tid == 0) nslot_s = 0;      // every thread has read ns; the next cull starts after a barrier
+            // ---- accumulate: each warp visits the staged particles that overlap its 8 x 8 cells
+            for (int e0 = 0; e0 < ns; e0 += 32) {
+                bool ov = false;
+                if (e0 + lane < ns) {
+                    const int v = sb[e0 + lane];
+                    const int bx2 = v & 255, by2 = v >> 8;            // stencil covers [b - 2m, b] in column cells
+                    ov = bx2 >= px && bx2 - 2 * M_ <= px + 7 && by2 >= py && by2 - 2 * M_ <= py + 7;
+                }
+                unsigned om = __ballot_sync(0xffffffffu, ov);
+                while (om) {
+                    const int e = e0 + __ffs(om) - 1;
+                    om &= om - 1;
+                    const P2 wx2 = *reinterpret_cast<const P2*>(&wxr[e * ROW + lx]);
+                    const T wy = wyr[e * ROW + ly];
+                    P2 a; a.x = wx2.x * wy; a.y = wx2.y * wy;
+                    const T* wz = &wzr[e * ROW];
+#pragma unroll
+                    for (int k = 0; k < W; ++k) fma_pair(acc[k], a, wz[k]);
+                }
+            }
+            if (c0 + NT < total) __syncthreads();     // staging buffers are reused by the next chunk
         }
-        __syncwarp();
+        // ---- plane z = s - m is complete: store it and slide the window
+        const int zo = s - M_;
+        if (zo >= z0) *reinterpret_cast<P2*>(gout + (size_t)zo * g.n * g.n) = acc[0];
+#pragma unroll
+        for (int k = 0; k + 1 < W; ++k) acc[k] = acc[k + 1];
+        acc[W - 1].x = (T)0; acc[W - 1].y = (T)0;
     }
 }
 

@@ -341,7 +341,7 @@ def test_stage_profile_and_streams(enuf, torch_cuda):
     with torch.cuda.stream(s):
         E1, F1 = plan.energy_forces(r, q)
         E2, F2 = plan.energy_forces(r, q, want_energy=False)
-        assert E2 is None and abs(plan.energy() - E1) <= 1e-9 * abs(E1)
+        assert E2 is None and abs(plan.energy() - E1) <= 5e-8 * abs(E1)   # R22: order of fp32 sums is run-dependent
     s.synchronize()
     ms = plan.stage_ms()
     assert all(v >= 0 for v in ms.values()) and ms["spread"] > 0 and ms["fft"] > 0 and ms["gather"] > 0
