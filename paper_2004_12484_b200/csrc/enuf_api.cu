@@ -99,13 +99,14 @@ double window_smooth(const enuf_plan* p, double d) {
     return A * std::sin(b * t) / t;
 }
 
-// Step a0 (fp32 path): for each stencil offset j the Chebyshev interpolant of degree
-// kPolyDeg of d0 -> phi(d0 - j) on [-1/2, 1/2], converted to monomials in d0, and its
-// exact derivative (enuf_common.cuh, PolyArg).
+// Step a0 (fp32 path): for each stencil offset j = 0..m the Chebyshev interpolant of degree
+// D = poly_degree(m) of d0 -> phi(d0 - j) on [-1/2, 1/2], converted to monomials in d0, and
+// its exact derivative (enuf_common.cuh, PolyArg).
 void build_poly_table(enuf_plan* p) {
-    constexpr int D = enuf::kPolyDeg, NC = D + 1;
-    for (int j = -p->m; j <= p->m; ++j) {
-        long double a[NC];
+    constexpr int NCMAX = enuf::kPolyMaxDeg + 1;
+    const int D = enuf::poly_degree(p->m), NC = D + 1;
+    for (int j = 0; j <= p->m; ++j) {
+        long double a[NCMAX];
         for (int k = 0; k < NC; ++k) {
             long double acc = 0;
             for (int i = 0; i < NC; ++i) {
@@ -115,16 +116,15 @@ void build_poly_table(enuf_plan* p) {
             a[k] = acc * (k == 0 ? 1.0L : 2.0L) / NC;
         }
         // T_0 = 1, T_1 = 2t, T_{k+1} = 4t T_k - T_{k-1} (x = 2t)
-        long double c[NC] = {0}, t0[NC] = {0}, t1[NC] = {0}, t2[NC];
+        long double c[NCMAX] = {0}, t0[NCMAX] = {0}, t1[NCMAX] = {0}, t2[NCMAX];
         t0[0] = 1; t1[1] = 2;
         for (int e = 0; e < NC; ++e) c[e] = a[0] * t0[e] + a[1] * t1[e];
         for (int k = 2; k < NC; ++k) {
             for (int e = 0; e < NC; ++e) t2[e] = (e > 0 ? 4 * t1[e - 1] : 0.0L) - t0[e];
             for (int e = 0; e < NC; ++e) { c[e] += a[k] * t2[e]; t0[e] = t1[e]; t1[e] = t2[e]; }
         }
-        const int col = j + p->m;
-        for (int k = 0; k < NC; ++k) p->poly_c[k][col] = (float)c[k];
-        for (int k = 0; k < D; ++k) p->poly_d[k][col] = (float)((k + 1) * c[k + 1]);
+        for (int k = 0; k < NC; ++k) p->poly_c[k][j] = (float)c[k];
+        for (int k = 0; k < D; ++k) p->poly_d[k][j] = (float)((k + 1) * c[k + 1]);
     }
 }
 

@@ -51,17 +51,21 @@ struct TileGeom {
 };
 
 // Piecewise-polynomial window table for the fp32 path (step a0).  For every stencil offset
-// j in [-m, m] the weight phi(d0 - j), d0 in [-1/2, 1/2], is a polynomial of degree kPolyDeg
-// in d0 (Chebyshev interpolant of the window's analytic continuation, fitted in fp64 on the
-// host; max error <= 3e-11 of phi(0) for m = 1, <= 1e-14 for m = 6).  dphi is the exact
-// derivative of that polynomial.  The table is passed to the kernels BY VALUE as a
-// __grid_constant__ parameter: with fully unrolled loops every coefficient is a constant-bank
-// operand of an FFMA, so a stencil of W weights costs W * kPolyDeg FFMAs and no loads.
-constexpr int kPolyDeg = 12;
+// j in [0, m] the weight phi(d0 - j), d0 in [-1/2, 1/2], is a polynomial p_j of degree
+// poly_degree(m) in d0 (Chebyshev interpolant of the window's analytic continuation, fitted
+// in fp64 on the host; max error <= 5e-11 of phi(0), <= 2e-9 of max|phi'| for the
+// derivative); since phi is even, p_{-j}(d0) = p_j(-d0),
+// so with p_j = E_j(d0^2) + d0 O_j(d0^2) both come out of one evaluation of E_j and O_j.
+// dphi is the exact derivative of that polynomial.  The table is passed to the kernels BY
+// VALUE as a __grid_constant__ parameter: with fully unrolled loops every coefficient is a
+// constant-bank operand of an FFMA, so the W weights of a stencil cost ~6 W FFMAs, no loads.
+__host__ __device__ constexpr int poly_degree(int m) { return m >= 4 ? 10 : 12; }
+constexpr int kPolyMaxDeg = 12;
 template <int M_>
 struct PolyArg {
-    float c[kPolyDeg + 1][2 * M_ + 1];   // value:      phi_j(d0)  = sum_i c[i][j + m] d0^i
-    float d[kPolyDeg][2 * M_ + 1];       // derivative: phi_j'(d0) = sum_i d[i][j + m] d0^i
+    static constexpr int D = poly_degree(M_);
+    float c[D + 1][M_ + 1];   // value:      p_j(d0)  = sum_i c[i][j] d0^i,  j = 0..m
+    float d[D][M_ + 1];       // derivative: p_j'(d0) = sum_i d[i][j] d0^i
 };
 
 __host__ __device__ inline uint32_t pack_cell(int cx, int cy, int cz) {
@@ -131,7 +135,7 @@ __device__ __forceinline__ void window_eval(const WindowParams& wp, T d0, int j,
 
 // All W = 2m+1 window weights (and derivatives) of one particle in one dimension:
 //   w[k] = phi(d0 - (k - m)),  dw[k] = phi'(d0 - (k - m)),  k = 0..W-1.
-//   fp32: Horner evaluation of the plan's polynomial table; Kaiser-Bessel support cut
+//   fp32: the plan's polynomial table (even/odd Horner in d0^2); Kaiser-Bessel support cut
 //         |d| <= m (value) and |d| < m (derivative) exactly as in the closed form.
 //   fp64: the closed form (window_eval).
 template <typename T, int M_, bool kDeriv>
@@ -145,21 +149,43 @@ __device__ __forceinline__ void stencil_weights(const WindowParams& wp, const Po
             window_eval<T, kDeriv>(wp, d0, k - M_, w[k], dw[k]);
         }
     } else {
-        const float x = (float)d0;
+        constexpr int D = PolyArg<M_>::D;
+        constexpr int DE = D - (D & 1), DO = D - 1 + (D & 1);      // highest even / odd power of p
+        const float x = (float)d0, y = x * x;
         float v[W], dv[W];
+        {
+            float E[M_ + 1], O[M_ + 1];
 #pragma unroll
-        for (int j = 0; j < W; ++j) v[j] = pa.c[kPolyDeg][j];
+            for (int j = 0; j <= M_; ++j) { E[j] = pa.c[DE][j]; O[j] = pa.c[DO][j]; }
 #pragma unroll
-        for (int i = kPolyDeg - 1; i >= 0; --i)
+            for (int i = DE - 2; i >= 0; i -= 2)
 #pragma unroll
-            for (int j = 0; j < W; ++j) v[j] = fmaf(v[j], x, pa.c[i][j]);
+                for (int j = 0; j <= M_; ++j) E[j] = fmaf(E[j], y, pa.c[i][j]);
+#pragma unroll
+            for (int i = DO - 2; i >= 1; i -= 2)
+#pragma unroll
+                for (int j = 1; j <= M_; ++j) O[j] = fmaf(O[j], y, pa.c[i][j]);
+            v[M_] = E[0];
+#pragma unroll
+            for (int j = 1; j <= M_; ++j) { v[M_ + j] = fmaf(x, O[j], E[j]); v[M_ - j] = fmaf(-x, O[j], E[j]); }
+        }
         if (kDeriv) {
+            constexpr int D1 = D - 1;
+            constexpr int DE1 = D1 - (D1 & 1), DO1 = D1 - 1 + (D1 & 1);
+            float E[M_ + 1], O[M_ + 1];
 #pragma unroll
-            for (int j = 0; j < W; ++j) dv[j] = pa.d[kPolyDeg - 1][j];
+            for (int j = 0; j <= M_; ++j) { E[j] = pa.d[DE1][j]; O[j] = pa.d[DO1][j]; }
 #pragma unroll
-            for (int i = kPolyDeg - 2; i >= 0; --i)
+            for (int i = DE1 - 2; i >= 0; i -= 2)
 #pragma unroll
-                for (int j = 0; j < W; ++j) dv[j] = fmaf(dv[j], x, pa.d[i][j]);
+                for (int j = 1; j <= M_; ++j) E[j] = fmaf(E[j], y, pa.d[i][j]);
+#pragma unroll
+            for (int i = DO1 - 2; i >= 1; i -= 2)
+#pragma unroll
+                for (int j = 0; j <= M_; ++j) O[j] = fmaf(O[j], y, pa.d[i][j]);
+            dv[M_] = x * O[0];                                       // p_0 is even: p_0' is odd
+#pragma unroll
+            for (int j = 1; j <= M_; ++j) { dv[M_ + j] = fmaf(x, O[j], E[j]); dv[M_ - j] = fmaf(x, O[j], -E[j]); }
         } else {
 #pragma unroll
             for (int j = 0; j < W; ++j) dv[j] = 0.f;

@@ -2,11 +2,12 @@
 //
 // One CTA per 16^3 grid tile, working on the tile's particles (a contiguous range of 16
 // bins, TileGeom), with the tile plus a halo of m cells per side ((16+2m)^3 values) held in
-// shared memory.  Particles are taken in batches: first the 3 W window values and
-// derivatives of every particle of the batch are computed once (one thread per particle and
-// dimension) and kept on chip, then one warp per particle contracts the
-// (2m+1)^3 stencil: every lane owns x-rows of the stencil (row strides chosen so that the 32
-// rows a warp reads at once fall in 32 different banks), forms s = sum_x Psi (phi, phi') with
+// shared memory (staged with cp.async).  Every warp takes the tile's particles five at a
+// time: first the 3 W window values and derivatives of those particles are computed once
+// (one lane per particle and dimension) and kept on chip, then the warp
+// contracts the (2m+1)^3 stencil of one particle after the other: every lane owns x-rows of
+// the stencil (row strides chosen so that the 32 rows a warp reads at once fall in 32
+// different banks), forms s = sum_x Psi (phi, phi') with
 // packed FMAs, and the three force components come out of one pass over the field
 // ("forces in 3D packed into a single calculation entity").
 #pragma once
@@ -33,20 +34,27 @@ struct GatherCfg {
     static constexpr int CELLS = ((TP * SPL + 3) / 4) * 4;      // shared tile size in elements (16 B multiple)
     static constexpr int WARPS = 8;
     static constexpr int NT = WARPS * 32;
-    static constexpr int PB = 32;                               // particles per batch
+    static constexpr int PBW = 5;                               // particles per warp batch
     static constexpr int ITER = (W * W + 31) / 32;              // stencil rows per lane
 };
 
 template <typename T, int M_>
 constexpr size_t gather_smem_bytes() {
     using C = GatherCfg<M_>;
-    // tile + per batch: (phi, phi') pairs [PB][3][16] + (q, idx, base offset) per particle
-    return sizeof(T) * ((size_t)C::CELLS + (size_t)C::PB * 3 * 16 * 2 + C::PB) + sizeof(int) * 2 * C::PB;
+    // tile + per warp and batch particle: (phi, phi') pairs [3][16], pre*q, tile offset, caller index
+    return sizeof(T) * ((size_t)C::CELLS + (size_t)C::WARPS * C::PBW * (3 * 16 * 2 + 1))
+           + sizeof(int) * 2 * C::WARPS * C::PBW;
 }
 
-// acc += w2 * v  (both halves, scalar v)
-__device__ __forceinline__ void fma_pair_s(float2& acc, const float2 w2, const float v) { fma_pair(acc, w2, v); }
-__device__ __forceinline__ void fma_pair_s(double2& acc, const double2 w2, const double v) { fma_pair(acc, w2, v); }
+__device__ __forceinline__ void cp_async_4(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_8(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // kIk = false: analytic-derivative variant, F = pre*q * sum Psi[l] grad(phi phi phi)
 //              with pre = -n/(pi L^2)  (exact gradient of the ENUF energy).
@@ -60,7 +68,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
               const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F) {
     using C = GatherCfg<M_>;
     using P2 = typename Pair2<T>::type;
-    constexpr int W = C::W, TP = C::TP, SX = C::SX, SPL = C::SPL, NT = C::NT, PB = C::PB, ITER = C::ITER;
+    constexpr int W = C::W, TP = C::TP, SX = C::SX, SPL = C::SPL, PBW = C::PBW, ITER = C::ITER;
 
     // tile (Tx, Ty, Tz): bins (Ty*nt + Tx)*n + 16 Tz .. + 16
     const int ntz = g.n / kTile;
@@ -73,24 +81,33 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* tile_s = reinterpret_cast<T*>(smem_raw);
-    P2* wtab = reinterpret_cast<P2*>(tile_s + C::CELLS);        // [PB][3][16] (phi, phi')
-    T* q_s = reinterpret_cast<T*>(wtab + PB * 3 * 16);          // [PB] pre * q
-    int* base_s = reinterpret_cast<int*>(q_s + PB);             // [PB] tile offset of the stencil origin
-    int* idx_s = base_s + PB;                                   // [PB] caller index
+    P2* wtab_all = reinterpret_cast<P2*>(tile_s + C::CELLS);            // [WARPS][PBW][3][16] (phi, phi')
+    T* q_all = reinterpret_cast<T*>(wtab_all + C::WARPS * PBW * 3 * 16); // [WARPS][PBW] pre * q
+    int* base_all = reinterpret_cast<int*>(q_all + C::WARPS * PBW);     // [WARPS][PBW] tile offset of the stencil origin
+    int* idx_all = base_all + C::WARPS * PBW;                           // [WARPS][PBW] caller index
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tx0 = Tx * kTile, ty0 = Ty * kTile, tz0 = Tz * kTile;
 
-    // ---- stage the padded tile: one row of TP values per warp pass
-    for (int rw = warp; rw < TP * TP; rw += C::WARPS) {
-        const int lz = rw / TP, ly = rw - lz * TP;
-        int gy = ty0 - M_ + ly, gz = tz0 - M_ + lz;
-        gy += gy < 0 ? g.n : 0; gy -= gy >= g.n ? g.n : 0;
-        gz += gz < 0 ? g.n : 0; gz -= gz >= g.n ? g.n : 0;
-        if (lane < TP) {
-            int gx = tx0 - M_ + lane;
-            gx += gx < 0 ? g.n : 0; gx -= gx >= g.n ? g.n : 0;
-            tile_s[lz * SPL + ly * SX + lane] = field[((size_t)gz * g.n + gy) * g.n + gx];
+    // ---- stage the padded tile asynchronously: one row of TP values per warp and step
+    {
+        int gx = tx0 - M_ + lane;
+        gx += gx < 0 ? g.n : 0; gx -= gx >= g.n ? g.n : 0;
+        for (int lz = 0; lz < TP; ++lz) {
+            int gz = tz0 - M_ + lz;
+            gz += gz < 0 ? g.n : 0; gz -= gz >= g.n ? g.n : 0;
+            const T* plane = field + (size_t)gz * g.n * g.n + gx;
+            T* dst = tile_s + lz * SPL + lane;
+#pragma unroll
+            for (int r = 0; r < (TP + C::WARPS - 1) / C::WARPS; ++r) {
+                const int ly = warp + r * C::WARPS;
+                int gy = ty0 - M_ + ly;
+                gy += gy < 0 ? g.n : 0; gy -= gy >= g.n ? g.n : 0;
+                if (ly < TP && lane < TP) {
+                    if (sizeof(T) == 4) cp_async_4(dst + ly * SX, plane + (size_t)gy * g.n);
+                    else cp_async_8(dst + ly * SX, plane + (size_t)gy * g.n);
+                }
+            }
         }
     }
 
@@ -105,13 +122,15 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
         rzo[it] = 32 + rz;
     }
 
-    for (int b0 = 0; b0 < cnt; b0 += PB) {
-        const int nb = min(PB, cnt - b0);
-        __syncthreads();        // tile staged / previous batch consumed
-        // ---- window values of the batch: one task per (dimension, particle)
-        for (int t = tid; t < 3 * nb; t += NT) {
-            const int dim = t / nb, slot = t - dim * nb;
-            const PRec<T> pr = rec[start + b0 + slot];
+    P2* wtab = wtab_all + warp * PBW * 3 * 16;
+    T* q_s = q_all + warp * PBW;
+    int* base_s = base_all + warp * PBW;
+    int* idx_s = idx_all + warp * PBW;
+    // window values of one warp batch: one lane per (dimension, particle)
+    auto batch_weights = [&](int p0, int nb) {
+        if (lane < 3 * nb) {
+            const int dim = lane / nb, slot = lane - dim * nb;
+            const PRec<T> pr = rec[start + p0 + slot];
             const T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
             T w[W], dw[W];
             stencil_weights<T, M_, !kIk>(wp, pa, d0, w, dw);
@@ -120,15 +139,27 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             for (int k = 0; k < W; ++k) { P2 v; v.x = w[k]; v.y = dw[k]; row[k] = v; }
             if (dim == 0) {
                 int cx, cy, cz;
-                unpack_cell(cell[start + b0 + slot], cx, cy, cz);
+                unpack_cell(cell[start + p0 + slot], cx, cy, cz);
                 base_s[slot] = (cz - tz0) * SPL + (cy - ty0) * SX + (cx - tx0);
                 q_s[slot] = pre * pr.q;
-                idx_s[slot] = (int)idx[start + b0 + slot];
+                idx_s[slot] = (int)idx[start + p0 + slot];
             }
         }
-        __syncthreads();
-        // ---- one warp per particle
-        for (int slot = warp; slot < nb; slot += C::WARPS) {
+    };
+
+    // the first batch's weights overlap the tile copy
+    if (warp * PBW < cnt) batch_weights(warp * PBW, min(PBW, cnt - warp * PBW));
+    cp_async_wait_all();
+    __syncthreads();
+
+    for (int p0 = warp * PBW; p0 < cnt; p0 += C::WARPS * PBW) {
+        const int nb = min(PBW, cnt - p0);
+        if (p0 != warp * PBW) {
+            batch_weights(p0, nb);
+            __syncwarp();
+        }
+        // ---- one particle after the other
+        for (int slot = 0; slot < nb; ++slot) {
             const P2* wt = wtab + slot * 3 * 16;
             P2 wx[W];
 #pragma unroll
@@ -137,18 +168,22 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             T fx = (T)0, fy = (T)0, fz = (T)0;
 #pragma unroll
             for (int it = 0; it < ITER; ++it) {
-                if (lane + 32 * it < W * W) {
+                if (it + 1 < ITER || lane + 32 * it < W * W) {
                     const T* row = origin + rowoff[it];
-                    P2 s; s.x = (T)0; s.y = (T)0;
+                    P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
 #pragma unroll
-                    for (int k = 0; k < W; ++k) fma_pair_s(s, wx[k], row[k]);
+                    for (int k = 0; k < W; ++k) {
+                        if (k & 1) fma_pair(sb2, wx[k], row[k]);
+                        else fma_pair(sa, wx[k], row[k]);
+                    }
+                    const T s0 = sa.x + sb2.x, s1 = sa.y + sb2.y;
                     const P2 wy = wt[ryo[it]], wz = wt[rzo[it]];
                     if (kIk) {
-                        fx += s.x * (wy.x * wz.x);
+                        fx += s0 * (wy.x * wz.x);
                     } else {
-                        fx += s.y * (wy.x * wz.x);
-                        fy += s.x * (wy.y * wz.x);
-                        fz += s.x * (wy.x * wz.y);
+                        fx += s1 * (wy.x * wz.x);
+                        fy += s0 * (wy.y * wz.x);
+                        fz += s0 * (wy.x * wz.y);
                     }
                 }
             }
@@ -170,6 +205,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
                 }
             }
         }
+        __syncwarp();
     }
 }
 

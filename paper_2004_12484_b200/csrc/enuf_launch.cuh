@@ -42,9 +42,10 @@ static inline int dispatch_n(int n, F&& f) {
 template <int M_>
 static inline PolyArg<M_> make_poly_arg(const enuf_plan* p) {
     PolyArg<M_> a;
-    for (int j = 0; j < 2 * M_ + 1; ++j) {
-        for (int k = 0; k <= kPolyDeg; ++k) a.c[k][j] = p->poly_c[k][j];
-        for (int k = 0; k < kPolyDeg; ++k) a.d[k][j] = p->poly_d[k][j];
+    constexpr int D = PolyArg<M_>::D;
+    for (int j = 0; j <= M_; ++j) {
+        for (int k = 0; k <= D; ++k) a.c[k][j] = p->poly_c[k][j];
+        for (int k = 0; k < D; ++k) a.d[k][j] = p->poly_d[k][j];
     }
     return a;
 }

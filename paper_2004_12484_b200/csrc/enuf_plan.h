@@ -32,8 +32,8 @@ struct enuf_plan {
     uint32_t* bin_offset = nullptr;   // [nbins+1]
     uint32_t* bin_cursor = nullptr;   // [nbins]
     uint32_t* scan_total = nullptr;   // [ceil(nbins / kScanChunk)]
-    float poly_c[enuf::kPolyDeg + 1][enuf::kMaxW] = {};   // host copy of the polynomial window table
-    float poly_d[enuf::kPolyDeg][enuf::kMaxW] = {};       // (fp32 path; packed into PolyArg<m> per launch)
+    float poly_c[enuf::kPolyMaxDeg + 1][enuf::kMaxM + 1] = {};   // host copy of the polynomial window table
+    float poly_d[enuf::kPolyMaxDeg][enuf::kMaxM + 1] = {};       // (fp32 path; packed into PolyArg<m> per launch)
     int zchunk = 0;                   // grid planes per spread CTA
     void* grid[3] = {nullptr, nullptr, nullptr};   // real n^3 (1 for analytic, 3 for ik)
     void* A1[3] = {nullptr, nullptr, nullptr};     // complex [n][n][Kxp]

@@ -46,30 +46,29 @@ struct SpreadCfg {
     static constexpr int W = 2 * M_ + 1;
     static constexpr int NT = 128;          // 4 warps: 2 x 2 patches of 8 x 8 cells
     static constexpr int CAP = NT;          // staged particles per chunk (one candidate per thread)
-    static constexpr int ROW = 16;          // row length of the staged x / y / z weight rows
+    // staged record of one particle: x row [16], y row [16], q * z row [16], (d0x, d0y, d0z, q).
+    // Pitch 52 = 20 mod 32: the 16-byte stores of 8 consecutive slots cover all 32 banks.
+    static constexpr int RP = 52, OX = 0, OY = 16, OZ = 32, OD = 48;
 };
 
 template <typename T, int M_>
 constexpr size_t spread_smem_bytes() {
     using C = SpreadCfg<M_>;
-    return sizeof(T) * (size_t)C::CAP * (3 * C::ROW + 4) + sizeof(int) * (size_t)C::CAP;
+    return sizeof(T) * (size_t)C::CAP * C::RP + sizeof(int) * (size_t)C::CAP;
 }
 
 template <typename T, int M_>
-__global__ void __launch_bounds__(SpreadCfg<M_>::NT)
+__global__ void __launch_bounds__(SpreadCfg<M_>::NT, sizeof(T) == 4 ? 8 : 2)
 spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
               const __grid_constant__ PolyArg<M_> pa, int zchunk, T* __restrict__ grid) {
     using C = SpreadCfg<M_>;
     using P2 = typename Pair2<T>::type;
-    constexpr int W = C::W, NT = C::NT, CAP = C::CAP, ROW = C::ROW;
+    constexpr int W = C::W, NT = C::NT, CAP = C::CAP, RP = C::RP, OX = C::OX, OY = C::OY, OZ = C::OZ, OD = C::OD;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* wxr = reinterpret_cast<T*>(smem_raw);          // [CAP][ROW] x weights on the column's 16 cells
-    T* wyr = wxr + CAP * ROW;                          // [CAP][ROW]
-    T* wzr = wyr + CAP * ROW;                          // [CAP][ROW] q * z weights, k = 0..W-1
-    T* sd = wzr + CAP * ROW;                           // [CAP][4]   d0x, d0y, d0z, q
-    int* sb = reinterpret_cast<int*>(sd + CAP * 4);    // [CAP]      (bx + m) | (by + m) << 8
+    T* st = reinterpret_cast<T*>(smem_raw);            // [CAP][RP] staged particle records
+    int* sb = reinterpret_cast<int*>(st + CAP * RP);   // [CAP]     (bx + m) | (by + m) << 8
     __shared__ int rng_start[2][9], rng_cnt[2][9];
     __shared__ int nslot_s;
 
@@ -142,7 +141,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                 if (take) {
                     const int slot = base + __popc(tmask & ((1u << lane) - 1u));
                     const PRec<T> pr = rec[pidx];
-                    sd[slot * 4 + 0] = pr.dx; sd[slot * 4 + 1] = pr.dy; sd[slot * 4 + 2] = pr.dz; sd[slot * 4 + 3] = pr.q;
+                    *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = pr;
                     sb[slot] = bxm | (bym << 8);
                 }
             }
@@ -152,15 +151,24 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
             for (int t = tid; t < 3 * ns; t += NT) {
                 const int dim = t / ns, slot = t - dim * ns;
                 T w[W], dw[W];
-                stencil_weights<T, M_, false>(wp, pa, sd[slot * 4 + dim], w, dw);
+                stencil_weights<T, M_, false>(wp, pa, st[slot * RP + OD + dim], w, dw);
+                using V4 = typename Vec4<T>::type;
                 if (dim == 2) {
-                    const T q = sd[slot * 4 + 3];
+                    const T q = st[slot * RP + OD + 3];
+                    T r16[16];
 #pragma unroll
-                    for (int k = 0; k < W; ++k) wzr[slot * ROW + k] = w[k] * q;
+                    for (int k = 0; k < 16; ++k) r16[k] = k < W ? w[k < W ? k : 0] * q : (T)0;
+                    V4* row4 = reinterpret_cast<V4*>(st + slot * RP + OZ);
+#pragma unroll
+                    for (int v = 0; v < 4; ++v) {
+                        V4 o; o.x = r16[4 * v]; o.y = r16[4 * v + 1]; o.z = r16[4 * v + 2]; o.w = r16[4 * v + 3];
+                        row4[v] = o;
+                    }
                 } else {
-                    T* row = (dim == 0 ? wxr : wyr) + slot * ROW;
+                    T* row = st + slot * RP + (dim == 0 ? OX : OY);
+                    V4 z; z.x = (T)0; z.y = (T)0; z.z = (T)0; z.w = (T)0;
 #pragma unroll
-                    for (int e = 0; e < ROW; ++e) row[e] = (T)0;
+                    for (int v = 0; v < 4; ++v) reinterpret_cast<V4*>(row)[v] = z;
                     const int X0 = (dim == 0 ? (sb[slot] & 255) : (sb[slot] >> 8)) - 2 * M_;   // cell of k = 0
 #pragma unroll
                     for (int k = 0; k < W; ++k)
@@ -178,15 +186,27 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                     ov = bx2 >= px && bx2 - 2 * M_ <= px + 7 && by2 >= py && by2 - 2 * M_ <= py + 7;
                 }
                 unsigned om = __ballot_sync(0xffffffffu, ov);
+                // two particles per trip: the loads of the second overlap the FMAs of the first
                 while (om) {
-                    const int e = e0 + __ffs(om) - 1;
+                    const int e1 = e0 + __ffs(om) - 1;
                     om &= om - 1;
-                    const P2 wx2 = *reinterpret_cast<const P2*>(&wxr[e * ROW + lx]);
-                    const T wy = wyr[e * ROW + ly];
-                    P2 a; a.x = wx2.x * wy; a.y = wx2.y * wy;
-                    const T* wz = &wzr[e * ROW];
+                    const bool two = om != 0;
+                    const int e2 = two ? e0 + __ffs(om) - 1 : e1;
+                    om &= om - 1;
+                    const P2 wx1 = *reinterpret_cast<const P2*>(&st[e1 * RP + OX + lx]);
+                    const T wy1 = st[e1 * RP + OY + ly];
+                    const P2 wx2 = *reinterpret_cast<const P2*>(&st[e2 * RP + OX + lx]);
+                    const T wy2 = two ? st[e2 * RP + OY + ly] : (T)0;
+                    P2 a1; a1.x = wx1.x * wy1; a1.y = wx1.y * wy1;
+                    P2 a2; a2.x = wx2.x * wy2; a2.y = wx2.y * wy2;
+                    const T* wz1 = &st[e1 * RP + OZ];
+                    const T* wz2 = &st[e2 * RP + OZ];
 #pragma unroll
-                    for (int k = 0; k < W; ++k) fma_pair(acc[k], a, wz[k]);
+                    for (int k = 0; k < W; ++k) fma_pair(acc[k], a1, wz1[k]);
+                    if (two) {
+#pragma unroll
+                        for (int k = 0; k < W; ++k) fma_pair(acc[k], a2, wz2[k]);
+                    }
                 }
             }
             if (c0 + NT < total) __syncthreads();     // staging buffers are reused by the next chunk
