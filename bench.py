@@ -307,10 +307,27 @@ def run_ours(args):
         gbs = abytes[st] / (stage_ms[st] * 1e-3) / 1e9 if stage_ms[st] > 0 else 0.0
         stages[st] = {"ms": stage_ms[st], "algorithmic_bytes": abytes[st], "GBps": gbs, "hbm_frac": gbs / peak}
     dom = max(stages, key=lambda k: stages[k]["ms"])
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": stages[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                "frac": stages[dom]["hbm_frac"], "traffic": recorded_traffic(dom), "peak_source": peak_src,
-                "events_averaged": n_prof,
-                "note": "spread and gather are bound by the shared-memory pipe, not HBM (DESIGN.md section 7)"}
+    if dom in ("spread", "gather"):
+        # these two stages are bound by FP32 FMA issue, not by HBM.  Algorithmic
+        # work = (2m+1)^3 FMAs per charged particle (spread), twice that for the analytic gather
+        # (field x window and field x window derivative), three times for the ik gather.
+        W3 = (2 * w.m + 1) ** 3
+        per = {"spread": 1, "gather": 3 if args.variant == "ik" else 2}[dom]
+        flops = 2.0 * per * W3 * n_charged
+        sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+        peak_tf = 148 * 128 * 2 * sm_max * 1e6 / 1e12
+        ach = flops / (stages[dom]["ms"] * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
+                    "frac": ach / peak_tf, "traffic": recorded_traffic(dom),
+                    "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x clocks.max.sm (B200_PROFILING.md nominal table; "
+                                   "DESIGN.md section 7)",
+                    "algorithmic_flops": flops, "events_averaged": n_prof,
+                    "hbm": {"achieved": stages[dom]["GBps"], "peak": peak, "unit": "GB/s",
+                            "frac": stages[dom]["hbm_frac"], "peak_source": peak_src}}
+    else:
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": stages[dom]["GBps"], "peak": peak, "unit": "GB/s",
+                    "frac": stages[dom]["hbm_frac"], "traffic": recorded_traffic(dom), "peak_source": peak_src,
+                    "events_averaged": n_prof}
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
