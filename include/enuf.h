@@ -53,7 +53,9 @@ enum enuf_option {
     ENUF_OPT_SLATER_LAMBDA = 4,  /* decay length of the Slater density Eq. 51 (:407); 0 = point (R19) */
     ENUF_OPT_NUM_PARTICLES = 5,  /* lower N for the next calls, 0 <= N <= planned capacity          */
     ENUF_OPT_PROFILE = 6,        /* 1: record per-stage CUDA-event times (enuf_plan_stage_ms)        */
-    ENUF_OPT_KEEP_SPECTRUM = 7   /* 1: also store S~(n) so enuf_plan_structure_factor() can read it  */
+    ENUF_OPT_KEEP_SPECTRUM = 7,  /* 1: also store S~(n) so enuf_plan_structure_factor() can read it  */
+    ENUF_OPT_SPREAD_ZCHUNK = 8   /* tuning: grid planes per spreading CTA (power of two, 8..n);
+                                    default fills the SMs several times over                         */
 };
 
 enum { ENUF_F32 = 0, ENUF_F64 = 1 };

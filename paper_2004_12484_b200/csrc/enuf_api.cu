@@ -407,6 +407,10 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
             if (p->allocated && (iv != 0) != p->keep_spectrum) { cudaStreamSynchronize(p->stream); free_workspace(p); }
             p->keep_spectrum = iv != 0;
             return ENUF_OK;
+        case ENUF_OPT_SPREAD_ZCHUNK:
+            if (iv < 8 || iv > p->n || (iv & (iv - 1))) return fail(ENUF_EINVAL, "zchunk must be a power of two in [8, n]");
+            p->zchunk = iv;
+            return ENUF_OK;
         default:
             return fail(ENUF_EINVAL, "unknown option key %d", key);
     }

@@ -32,17 +32,18 @@ struct GatherCfg {
     static constexpr int SX = GatherStride<M_>::SX;
     static constexpr int SPL = GatherStride<M_>::SPL;
     static constexpr int CELLS = ((TP * SPL + 3) / 4) * 4;      // shared tile size in elements (16 B multiple)
-    static constexpr int WARPS = 8;
+    static constexpr int WARPS = 12;
     static constexpr int NT = WARPS * 32;
-    static constexpr int PBW = 5;                               // particles per warp batch
+    static constexpr int PBW = 4;                               // particles per warp batch
     static constexpr int ITER = (W * W + 31) / 32;              // stencil rows per lane
+    static constexpr int WP = 18;                               // pitch of a (phi, phi') weight row: 16-byte aligned, rows spread over banks
 };
 
 template <typename T, int M_>
 constexpr size_t gather_smem_bytes() {
     using C = GatherCfg<M_>;
-    // tile + per warp and batch particle: (phi, phi') pairs [3][16], pre*q, tile offset, caller index
-    return sizeof(T) * ((size_t)C::CELLS + (size_t)C::WARPS * C::PBW * (3 * 16 * 2 + 1))
+    // tile + per warp and batch particle: (phi, phi') pairs [3][WP], pre*q, tile offset, caller index
+    return sizeof(T) * ((size_t)C::CELLS + (size_t)C::WARPS * C::PBW * (3 * C::WP * 2 + 1))
            + sizeof(int) * 2 * C::WARPS * C::PBW;
 }
 
@@ -68,7 +69,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
               const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F) {
     using C = GatherCfg<M_>;
     using P2 = typename Pair2<T>::type;
-    constexpr int W = C::W, TP = C::TP, SX = C::SX, SPL = C::SPL, PBW = C::PBW, ITER = C::ITER;
+    constexpr int W = C::W, TP = C::TP, SX = C::SX, SPL = C::SPL, PBW = C::PBW, ITER = C::ITER, WP = C::WP;
 
     // tile (Tx, Ty, Tz): bins (Ty*nt + Tx)*n + 16 Tz .. + 16
     const int ntz = g.n / kTile;
@@ -81,8 +82,8 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* tile_s = reinterpret_cast<T*>(smem_raw);
-    P2* wtab_all = reinterpret_cast<P2*>(tile_s + C::CELLS);            // [WARPS][PBW][3][16] (phi, phi')
-    T* q_all = reinterpret_cast<T*>(wtab_all + C::WARPS * PBW * 3 * 16); // [WARPS][PBW] pre * q
+    P2* wtab_all = reinterpret_cast<P2*>(tile_s + C::CELLS);            // [WARPS][PBW][3][WP] (phi, phi')
+    T* q_all = reinterpret_cast<T*>(wtab_all + C::WARPS * PBW * 3 * WP); // [WARPS][PBW] pre * q
     int* base_all = reinterpret_cast<int*>(q_all + C::WARPS * PBW);     // [WARPS][PBW] tile offset of the stencil origin
     int* idx_all = base_all + C::WARPS * PBW;                           // [WARPS][PBW] caller index
 
@@ -118,11 +119,11 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
         const int rr = lane + 32 * it;
         const int rz = rr / W, ry = rr - rz * W;
         rowoff[it] = rz * SPL + ry * SX;
-        ryo[it] = 16 + ry;          // index into the particle's [3][16] weight rows
-        rzo[it] = 32 + rz;
+        ryo[it] = WP + ry;          // index into the particle's [3][WP] weight rows
+        rzo[it] = 2 * WP + rz;
     }
 
-    P2* wtab = wtab_all + warp * PBW * 3 * 16;
+    P2* wtab = wtab_all + warp * PBW * 3 * WP;
     T* q_s = q_all + warp * PBW;
     int* base_s = base_all + warp * PBW;
     int* idx_s = idx_all + warp * PBW;
@@ -134,7 +135,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             const T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
             T w[W], dw[W];
             stencil_weights<T, M_, !kIk>(wp, pa, d0, w, dw);
-            P2* row = wtab + (slot * 3 + dim) * 16;
+            P2* row = wtab + (slot * 3 + dim) * WP;
 #pragma unroll
             for (int k = 0; k < W; ++k) { P2 v; v.x = w[k]; v.y = dw[k]; row[k] = v; }
             if (dim == 0) {
@@ -160,10 +161,17 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
         }
         // ---- one particle after the other
         for (int slot = 0; slot < nb; ++slot) {
-            const P2* wt = wtab + slot * 3 * 16;
-            P2 wx[W];
+            const P2* wt = wtab + slot * 3 * WP;
+            P2 wx[W + 1];
+            {
+                using V4 = typename Vec4<T>::type;
+                const V4* w4 = reinterpret_cast<const V4*>(wt);
 #pragma unroll
-            for (int k = 0; k < W; ++k) wx[k] = wt[k];
+                for (int v = 0; v < (W + 1) / 2; ++v) {
+                    const V4 t4 = w4[v];
+                    wx[2 * v].x = t4.x; wx[2 * v].y = t4.y; wx[2 * v + 1].x = t4.z; wx[2 * v + 1].y = t4.w;
+                }
+            }
             const T* origin = tile_s + base_s[slot];
             T fx = (T)0, fy = (T)0, fz = (T)0;
 #pragma unroll
