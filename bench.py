@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--variant", default="analytic", choices=["analytic", "ik"])
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-comparisons", action="store_true",
+                    help="skip the context timings (cuFFT round trip, ik force variant)")
     return ap.parse_args()
 
 
@@ -203,6 +205,26 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ---------------------------------------------------------------------- rank plumbing (replicas only)
+
+def reduce_over_ranks(x: float, op: str, device: str = "cuda") -> float:
+    """max / sum of a scalar over all ranks (identity when torch.distributed is not initialised).
+    The only collectives of the N > 1 run: the path itself has no data-path exchange (DESIGN.md
+    section 9).  Covered on CPU by tests/test_multirank_gloo.py (gloo, world_size 2)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def whole_job_value(n_particles: int, world: int, ms_step_max: float) -> float:
+    """Whole-job throughput of `world` independent replicas: all ranks' particles / slowest rank's time."""
+    return n_particles * world / (ms_step_max * 1e-3)
+
+
 # ---------------------------------------------------------------------- this repo's arm
 
 def run_ours(args):
@@ -225,18 +247,10 @@ def run_ours(args):
             dist.barrier()
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_over_ranks(x, "max", "cuda")
 
     def sum_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return reduce_over_ranks(x, "sum", "cuda")
 
     w = make_workload(args.workload)
     K, W = args.steps, args.warmup
@@ -271,7 +285,7 @@ def run_ours(args):
     E_last = plan.energy()
     stage_ms, n_prof = plan.stage_ms_mean()
     ms_step = ms_total / K
-    value = w.N * world / (ms_step * 1e-3)
+    value = whole_job_value(w.N, world, ms_step)
     total_launches = int(sum_over_ranks(float(launches)))
 
     # ---- end to end: host buffers in, host forces + energy out, through the C ABI
@@ -329,6 +343,39 @@ def run_ours(args):
                     "frac": stages[dom]["hbm_frac"], "traffic": recorded_traffic(dom), "peak_source": peak_src,
                     "events_averaged": n_prof}
 
+    # ---- context timings asked for by north_star (not on the product path, not the headline)
+    comparisons = None
+    if world == 1 and not args.no_comparisons:
+        comparisons = {}
+        # (1) cuFFT (torch.fft) real-to-complex + complex-to-real round trip of the full n^3 grid,
+        #     against this library's pruned 5-pass FFT + scale + energy ("fft" stage above)
+        g = torch.randn((w.n, w.n, w.n), dtype=tdtype, device="cuda")
+        for _ in range(3):
+            torch.fft.irfftn(torch.fft.rfftn(g), s=g.shape)
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); c0.record()
+        for _ in range(10):
+            torch.fft.irfftn(torch.fft.rfftn(g), s=g.shape)
+        c1.record(); torch.cuda.synchronize()
+        comparisons["cufft_rfftn_irfftn_ms"] = c0.elapsed_time(c1) / 10
+        comparisons["own_fft_scale_energy_ms"] = stage_ms["fft"]
+        del g
+        # (2) the paper's ik force variant (three inverse FFTs and three gathers, Eq. 41-42)
+        other = "ik" if args.variant == "analytic" else "analytic"
+        plan2 = enuf.Plan.from_workload(w, variant=other, profile=False)
+        for s_ in range(3):
+            plan2.energy_forces(pos_dev[s_], q_dev, F=F_dev, want_energy=False)
+        plan2.set(enuf.OPT_PROFILE, 1)
+        torch.cuda.synchronize(); c0.record()
+        Kc = min(10, K)
+        for s_ in range(Kc):
+            plan2.energy_forces(pos_dev[W + s_], q_dev, F=F_dev, want_energy=False)
+        c1.record(); torch.cuda.synchronize()
+        st2, _ = plan2.stage_ms_mean()
+        comparisons[other + "_variant"] = {"ms_per_step": c0.elapsed_time(c1) / Kc,
+                                           "stages_ms": {k: st2[k] for k in ("bin", "spread", "fft", "gather")}}
+        plan2.close()
+
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
         from oracle import enuf_oracle as O
@@ -350,7 +397,7 @@ def run_ours(args):
         "evals_per_sec": world / (ms_step * 1e-3),
         "energy_last_step": E_last,
         "clocks": clocks, "e2e": e2e, "gpu_launches": total_launches,
-        "roofline": roofline, "stages": stages, "cpu_baseline": cpu_baseline,
+        "roofline": roofline, "stages": stages, "cpu_baseline": cpu_baseline, "comparisons": comparisons,
     }
     print(json.dumps(line), flush=True)
     plan.close()
