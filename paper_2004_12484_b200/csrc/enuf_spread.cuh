@@ -58,7 +58,7 @@ constexpr size_t spread_smem_bytes() {
 }
 
 template <typename T, int M_>
-__global__ void __launch_bounds__(SpreadCfg<M_>::NT, sizeof(T) == 4 ? 8 : 2)
+__global__ void __launch_bounds__(SpreadCfg<M_>::NT, sizeof(T) == 4 ? 7 : 2)
 spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
               const __grid_constant__ PolyArg<M_> pa, int zchunk, T* __restrict__ grid) {
