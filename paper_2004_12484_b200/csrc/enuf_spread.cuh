@@ -113,40 +113,47 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
         for (int i = 0; i < 9; ++i) pref[i + 1] = pref[i] + rng_cnt[buf][i];
         const int total = pref[9];
 
-        for (int c0 = 0; c0 < total; c0 += NT) {
-            // ---- cull: one candidate per thread
-            const int c = c0 + tid;
-            bool take = false;
-            int bxm = 0, bym = 0;
-            uint32_t pidx = 0;
-            if (c < total) {
+        // cull candidates [c0, c0 + span) against the column's halo: accepted ones are staged
+        // (record + packed position) while slots last; returns nothing, the count is nslot_s
+        auto cull = [&](int c0, int span) {
+            for (int c = c0 + tid; c < min(total, c0 + span); c += NT) {
                 int i = 0;
 #pragma unroll
                 for (int e = 1; e < 9; ++e) i += (c >= pref[e]) ? 1 : 0;
                 int pb = 0;
 #pragma unroll
                 for (int e = 1; e < 9; ++e) pb = (i == e) ? pref[e] : pb;
-                pidx = (uint32_t)(rng_start[buf][i] + (c - pb));
+                const uint32_t pidx = (uint32_t)(rng_start[buf][i] + (c - pb));
                 int cx, cy, czp;
                 unpack_cell(cell[pidx], cx, cy, czp);
-                bxm = (cx & (kTile - 1)) + (i % 3 - 1) * kTile + M_;      // bx + m, bx relative to the column
-                bym = (cy & (kTile - 1)) + (i / 3 - 1) * kTile + M_;
-                take = (unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_);
-            }
-            const unsigned tmask = __ballot_sync(0xffffffffu, take);
-            if (tmask) {
-                int base = 0;
-                if (lane == 0) base = atomicAdd(&nslot_s, __popc(tmask));
-                base = __shfl_sync(0xffffffffu, base, 0);
-                if (take) {
-                    const int slot = base + __popc(tmask & ((1u << lane) - 1u));
-                    const PRec<T> pr = rec[pidx];
-                    *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = pr;
-                    sb[slot] = bxm | (bym << 8);
+                const int bxm = (cx & (kTile - 1)) + (i % 3 - 1) * kTile + M_;   // bx + m, bx relative to the column
+                const int bym = (cy & (kTile - 1)) + (i / 3 - 1) * kTile + M_;
+                if ((unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_)) {
+                    const int slot = atomicAdd(&nslot_s, 1);
+                    if (slot < CAP) {
+                        *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = rec[pidx];
+                        sb[slot] = bxm | (bym << 8);
+                    }
                 }
             }
+        };
+
+        for (int c0 = 0; c0 < total;) {
+            // ---- cull: two candidates per thread; if more than CAP were accepted (dense clusters),
+            //      redo the chunk with one candidate per thread (at most NT = CAP accepted)
+            int span = 2 * NT;
+            cull(c0, span);
             __syncthreads();
-            const int ns = nslot_s;
+            int ns = nslot_s;
+            if (ns > CAP) {
+                __syncthreads();                 // every thread has read ns
+                if (tid == 0) nslot_s = 0;
+                __syncthreads();
+                span = NT;
+                cull(c0, span);
+                __syncthreads();
+                ns = nslot_s;
+            }
             // ---- window values: one task per (dimension, slot); dimension-major so warps stay uniform
             for (int t = tid; t < 3 * ns; t += NT) {
                 const int dim = t / ns, slot = t - dim * ns;
@@ -209,7 +216,8 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                     }
                 }
             }
-            if (c0 + NT < total) __syncthreads();     // staging buffers are reused by the next chunk
+            c0 += span;
+            if (c0 < total) __syncthreads();           // staging buffers are reused by the next chunk
         }
         // ---- plane z = s - m is complete: store it and slide the window
         const int zo = s - M_;

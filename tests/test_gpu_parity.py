@@ -354,3 +354,26 @@ def test_stage_profile_and_streams(enuf, torch_cuda):
     mean, ne = plan.stage_ms_mean()
     assert ne == 2 and mean["fft"] > 0
     plan.close()
+
+
+def test_dense_cluster_many_particles_per_bin(enuf, torch_cuda, oracle):
+    """3000 charges inside a ball of two grid cells: hundreds of particles per bin and z-slab, so the
+    spread's staging area overflows and takes its one-candidate-per-thread path; plus a dilute rest."""
+    torch = torch_cuda
+    N, L, n, m = 3600, 9.0, 64, 4
+    rng = np.random.default_rng(77)
+    r = rng.uniform(0, L, size=(N, 3))
+    r[:3000] = np.array([4.1, 0.05, 8.9]) + rng.normal(0, 2 * L / n / 3, size=(3000, 3))   # wraps across faces
+    q = np.where(np.arange(N) % 2 == 0, 1.0, -1.0) * (1 + 0.1 * rng.uniform(size=N))
+    M, k_cut = n // 2, n // 4
+    alpha = 0.9 * math.pi * k_cut / (L * 3.0)
+    for dtype, npdt in (("f64", np.float64), ("f32", np.float32)):
+        rr, qq = r.astype(npdt), q.astype(npdt)
+        ref = oracle.enuf(rr, qq, L, alpha, k_cut, n, m, "kaiser_bessel", 2.0, variant="ik")
+        plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=2.0, m=m, window="kaiser_bessel", variant="ik",
+                         dtype=torch.float64 if dtype == "f64" else torch.float32)
+        E, F = plan.energy_forces(torch.from_numpy(rr).cuda(), torch.from_numpy(qq).cuda())
+        tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+        assert abs(E - ref["E"]) <= te * abs(ref["E"])
+        assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+        plan.close()
