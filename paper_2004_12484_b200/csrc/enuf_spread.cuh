@@ -28,13 +28,7 @@ template <> struct Pair2<double> { using type = double2; };
 
 // acc += a * w (both halves), one FFMA2 for fp32 on sm_100a
 __device__ __forceinline__ void fma_pair(float2& acc, const float2 a, const float w) {
-    unsigned long long A, C, Wv;
-    const float2 w2 = make_float2(w, w);
-    A = *reinterpret_cast<const unsigned long long*>(&a);
-    C = *reinterpret_cast<unsigned long long*>(&acc);
-    Wv = *reinterpret_cast<const unsigned long long*>(&w2);
-    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(C) : "l"(A), "l"(Wv));
-    acc = *reinterpret_cast<float2*>(&C);
+    acc = __ffma2_rn(a, make_float2(w, w), acc);
 }
 __device__ __forceinline__ void fma_pair(double2& acc, const double2 a, const double w) {
     acc.x = fma(a.x, w, acc.x);
@@ -102,6 +96,9 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
     for (int k = 0; k < W; ++k) { acc[k].x = (T)0; acc[k].y = (T)0; }
 
     T* gout = grid + ((size_t)(Ty * kTile + ly)) * g.n + Tx * kTile + lx;
+    const char* lane_xb = reinterpret_cast<const char*>(st + OX + lx);   // this lane's entries of slot 0's rows
+    const char* lane_yb = reinterpret_cast<const char*>(st + OY + ly);
+    const char* st_zb = reinterpret_cast<const char*>(st + OZ);
 
     int buf = 0;
     for (int s = z0 - M_; s < z1 + M_; ++s, buf ^= 1) {
@@ -200,14 +197,15 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                     const bool two = om != 0;
                     const int e2 = two ? e0 + __ffs(om) - 1 : e1;
                     om &= om - 1;
-                    const P2 wx1 = *reinterpret_cast<const P2*>(&st[e1 * RP + OX + lx]);
-                    const T wy1 = st[e1 * RP + OY + ly];
-                    const P2 wx2 = *reinterpret_cast<const P2*>(&st[e2 * RP + OX + lx]);
-                    const T wy2 = two ? st[e2 * RP + OY + ly] : (T)0;
+                    const unsigned o1 = (unsigned)e1 * (RP * sizeof(T)), o2 = (unsigned)e2 * (RP * sizeof(T));   // warp-uniform
+                    const P2 wx1 = *reinterpret_cast<const P2*>(lane_xb + o1);
+                    const T wy1 = *reinterpret_cast<const T*>(lane_yb + o1);
+                    const P2 wx2 = *reinterpret_cast<const P2*>(lane_xb + o2);
+                    const T wy2 = two ? *reinterpret_cast<const T*>(lane_yb + o2) : (T)0;
                     P2 a1; a1.x = wx1.x * wy1; a1.y = wx1.y * wy1;
                     P2 a2; a2.x = wx2.x * wy2; a2.y = wx2.y * wy2;
-                    const T* wz1 = &st[e1 * RP + OZ];
-                    const T* wz2 = &st[e2 * RP + OZ];
+                    const T* wz1 = reinterpret_cast<const T*>(st_zb + o1);
+                    const T* wz2 = reinterpret_cast<const T*>(st_zb + o2);
 #pragma unroll
                     for (int k = 0; k < W; ++k) fma_pair(acc[k], a1, wz1[k]);
                     if (two) {
