@@ -141,10 +141,18 @@ int upload(void* dst, const std::vector<double>& src, cudaStream_t s) {
 int build_tables(enuf_plan* p) {
     fill_window_params(p);
     const int n = p->n, kc = p->k_cut;
-    std::vector<double> tw(2 * (size_t)n), iphi((size_t)kc + 1), wf((size_t)kc * kc + 1);
-    for (int j = 0; j < n; ++j) {
-        tw[2 * j] = std::cos(2.0 * kPi * j / n);
-        tw[2 * j + 1] = -std::sin(2.0 * kPi * j / n);
+    // twiddles of the four-step FFT, one table per direction, laid out [k1][a] (enuf_fft.cuh):
+    // forward (RA, RB) = (16, n/16), inverse (n/16, 16); entry = exp(-2 pi i a k1 / n)
+    std::vector<double> tw(4 * (size_t)n), iphi((size_t)kc + 1), wf((size_t)kc * kc + 1);
+    for (int dir = 0; dir < 2; ++dir) {
+        const int RA = dir == 0 ? 16 : n / 16, RB = n / RA;
+        for (int k1 = 0; k1 < RA; ++k1)
+            for (int a = 0; a < RB; ++a) {
+                const size_t e = (size_t)dir * n + (size_t)k1 * RB + a;
+                const int j = (a * k1) % n;
+                tw[2 * e] = std::cos(2.0 * kPi * j / n);
+                tw[2 * e + 1] = -std::sin(2.0 * kPi * j / n);
+            }
     }
     for (int k = 0; k <= kc; ++k) iphi[k] = 1.0 / window_transform(p, k);
     wf[0] = 0.0;
@@ -237,7 +245,7 @@ int ensure_allocated(enuf_plan* p) {
         ALLOC(p->A2[d], 2 * es * n * p->Ky * p->Kxp);
     }
     if (p->keep_spectrum) ALLOC(p->spectrum, 2 * es * (size_t)p->Ky * p->Ky * p->Kxp);
-    ALLOC(p->tw, 2 * es * n);
+    ALLOC(p->tw, 4 * es * n);
     ALLOC(p->iphi, es * ((size_t)p->k_cut + 1));
     ALLOC(p->wf, es * ((size_t)p->k_cut * p->k_cut + 1));
     const int lpc = 256 / (p->n / 16);

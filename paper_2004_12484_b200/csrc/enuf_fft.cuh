@@ -101,7 +101,7 @@ template <int N> constexpr int fft_line_pitch() {
 }
 
 // Pass A.  v[i*RA + n1] holds x[RB*n1 + a] for item a = t + TPL*i.  Result goes to the
-// line's shared buffer at k1*(RB+1) + a.  tw[j] = exp(-2 pi i j / N).
+// line's shared buffer at k1*(RB+1) + a.  tw[(SIGN<0 ? 0 : N) + k1*RB + a] = exp(-2 pi i a k1 / N).
 template <typename T, int N, int SIGN>
 __device__ __forceinline__ void fft_pass_a(Cx<T>* v, int t, Cx<T>* line, const Cx<T>* __restrict__ tw) {
     using S = FftShape<N, SIGN>;
@@ -113,7 +113,9 @@ __device__ __forceinline__ void fft_pass_a(Cx<T>* v, int t, Cx<T>* line, const C
         for (int k1 = 0; k1 < S::RA; ++k1) {
             Cx<T> val = v[i * S::RA + k1];
             if (k1 > 0) {
-                Cx<T> w = __ldg(&tw[a * k1]);
+                // table laid out [direction][k1][a]: the lanes of a line (consecutive a) read consecutive
+                // entries -- 4 sectors per request instead of ~13 for the a*k1-indexed table
+                Cx<T> w = __ldg(&tw[(SIGN < 0 ? 0 : N) + k1 * S::RB + a]);
                 if (SIGN > 0) w.y = -w.y;
                 val = cx_mul(val, w);
             }
