@@ -172,6 +172,8 @@ fft_x_forward_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg
         }
 }
 
+// Complex-to-real, two rows per transform: with Z = X1 + i X2 (X1, X2 the Hermitian spectra of two
+// real rows) one complex inverse FFT returns row 1 in the real and row 2 in the imaginary part.
 template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_x_inverse_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeom fg, const Cx<T>* __restrict__ tw) {
@@ -180,27 +182,34 @@ fft_x_inverse_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeom fg
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
     const int t = threadIdx.x % S::TPL, ls = threadIdx.x / S::TPL;
-    const size_t row = (size_t)blockIdx.x * LPC + ls;
-    const Cx<T>* in = A1 + row * fg.Kxp;
+    const size_t row = 2 * ((size_t)blockIdx.x * LPC + ls);    // rows (row, row+1); n*n is a multiple of 2*LPC
+    const Cx<T>* in0 = A1 + row * fg.Kxp;
+    const Cx<T>* in1 = in0 + fg.Kxp;
     Cx<T> v[16];
-    // Hermitian extension of the half spectrum: X[N-k] = conj X[k]
+    // Hermitian extension of the half spectra: X[N-k] = conj X[k];  Z = X1 + i X2
 #pragma unroll
     for (int i = 0; i < S::ITEMS_A; ++i)
 #pragma unroll
         for (int n1 = 0; n1 < S::RA; ++n1) {
             const int e = 16 * n1 + t + S::TPL * i;
             Cx<T> val = cx_make<T>((T)0, (T)0);
-            if (e <= fg.kcut) val = in[e];
-            else if (N - e <= fg.kcut) { val = in[N - e]; val.y = -val.y; }
+            if (e <= fg.kcut) {
+                const Cx<T> a = in0[e], b = in1[e];
+                val = cx_make<T>(a.x - b.y, a.y + b.x);
+            } else if (N - e <= fg.kcut) {
+                const Cx<T> a = in0[N - e], b = in1[N - e];       // conj(a) + i conj(b)
+                val = cx_make<T>(a.x + b.y, b.x - a.y);
+            }
             v[i * S::RA + n1] = val;
         }
     Cx<T>* line = sm + ls * PITCH;
     fft_pass_a<T, N, +1>(v, t, line, tw);
     __syncthreads();
     fft_pass_b<T, N, +1>(v, t, line);
-    T* out = G + row * N;
+    T* out0 = G + row * N;
+    T* out1 = out0 + N;
 #pragma unroll
-    for (int k2 = 0; k2 < 16; ++k2) out[t + S::TPL * k2] = v[k2].x;
+    for (int k2 = 0; k2 < 16; ++k2) { out0[t + S::TPL * k2] = v[k2].x; out1[t + S::TPL * k2] = v[k2].y; }
 }
 
 // ---------------------------------------------------------------- Y passes (strided lines)

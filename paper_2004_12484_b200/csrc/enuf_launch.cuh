@@ -143,7 +143,7 @@ int launch_fft(enuf_plan* p) {
         for (int d = 0; d < nout; ++d) {
             fft_y_inverse_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A2[d]),
                                                                    static_cast<Cx<T>*>(p->A1[d]), fg, tw);
-            fft_x_inverse_kernel<T, N_><<<bx, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[d]),
+            fft_x_inverse_kernel<T, N_><<<bx / 2, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[d]),
                                                                    static_cast<T*>(p->grid[d]), fg, tw);
             launches += 2;
         }
