@@ -145,30 +145,53 @@ struct FftGeom {
 };
 
 // ---------------------------------------------------------------- X passes (contiguous lines)
+// Real-to-complex, two rows per transform: z = x1 + i x2, then X1[k] = (Z[k] + conj Z[N-k])/2 and
+// X2[k] = (Z[k] - conj Z[N-k])/(2i).  Z[N-k] lives in another thread of the line, so the spectrum
+// goes through the line's shared buffer once more (a line's threads are lanes of one warp).
 template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_x_forward_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg, const Cx<T>* __restrict__ tw) {
     using S = FftShape<N, -1>;
+    static_assert(S::TPL <= 32, "a line must fit in one warp");
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
+    static_assert(PITCH >= N, "line buffer holds a full spectrum");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
     const int t = threadIdx.x % S::TPL, ls = threadIdx.x / S::TPL;
-    const size_t row = (size_t)blockIdx.x * LPC + ls;          // z*n + y; n*n is a multiple of LPC
+    const size_t row = 2 * ((size_t)blockIdx.x * LPC + ls);    // rows (row, row+1); n*n is a multiple of 2*LPC
     Cx<T> v[16];
-    const T* in = G + row * N;
+    const T* in0 = G + row * N;
+    const T* in1 = in0 + N;
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) v[n1] = cx_make<T>(in[S::RB * n1 + t], (T)0);
+    for (int n1 = 0; n1 < 16; ++n1) v[n1] = cx_make<T>(in0[S::RB * n1 + t], in1[S::RB * n1 + t]);
     Cx<T>* line = sm + ls * PITCH;
     fft_pass_a<T, N, -1>(v, t, line, tw);
     __syncthreads();
     fft_pass_b<T, N, -1>(v, t, line);
-    Cx<T>* out = A1 + row * fg.Kxp;
+    __syncwarp();                                              // every lane of the line has read pass A's data
+#pragma unroll
+    for (int i = 0; i < S::ITEMS_B; ++i)
+#pragma unroll
+        for (int k2 = 0; k2 < S::RB; ++k2) line[t + S::TPL * i + 16 * k2] = v[i * S::RB + k2];
+    __syncwarp();
+    Cx<T>* out0 = A1 + row * fg.Kxp;
+    Cx<T>* out1 = out0 + fg.Kxp;
+    const T half = (T)0.5;
 #pragma unroll
     for (int i = 0; i < S::ITEMS_B; ++i)
 #pragma unroll
         for (int k2 = 0; k2 < S::RB; ++k2) {
             const int k = t + S::TPL * i + 16 * k2;
-            if (k < fg.Kxp) out[k] = k <= fg.kcut ? v[i * S::RB + k2] : cx_make<T>((T)0, (T)0);
+            if (k < fg.Kxp) {
+                Cx<T> x1 = cx_make<T>((T)0, (T)0), x2 = x1;
+                if (k <= fg.kcut) {
+                    const Cx<T> zk = v[i * S::RB + k2], zn = line[(N - k) & (N - 1)];
+                    x1 = cx_make<T>(half * (zk.x + zn.x), half * (zk.y - zn.y));
+                    x2 = cx_make<T>(half * (zk.y + zn.y), half * (zn.x - zk.x));
+                }
+                out0[k] = x1;
+                out1[k] = x2;
+            }
         }
 }
 

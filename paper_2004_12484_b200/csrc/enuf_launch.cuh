@@ -126,7 +126,7 @@ int launch_fft(enuf_plan* p) {
         const unsigned by = (unsigned)(((size_t)N_ * p->Kxp + LPC - 1) / LPC);
         const unsigned bz = (unsigned)(((size_t)p->Ky * p->Kxp + LPC - 1) / LPC);
         if ((int)bz > p->n_partial) return -1;
-        fft_x_forward_kernel<T, N_><<<bx, kFftThreads, sb, s>>>(static_cast<const T*>(p->grid[0]),
+        fft_x_forward_kernel<T, N_><<<bx / 2, kFftThreads, sb, s>>>(static_cast<const T*>(p->grid[0]),
                                                                static_cast<Cx<T>*>(p->A1[0]), fg, tw);
         fft_y_forward_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[0]),
                                                                static_cast<Cx<T>*>(p->A2[0]), fg, tw);
