@@ -17,31 +17,39 @@
 
 namespace enuf {
 
-template <int M_> struct GatherStride;   // (row stride, plane stride) of the shared tile: conflict-free
-template <> struct GatherStride<1> { static constexpr int SX = 18, SPL = 325; };
-template <> struct GatherStride<2> { static constexpr int SX = 21, SPL = 425; };
-template <> struct GatherStride<3> { static constexpr int SX = 23, SPL = 513; };
-template <> struct GatherStride<4> { static constexpr int SX = 25, SPL = 609; };
-template <> struct GatherStride<5> { static constexpr int SX = 27, SPL = 713; };
-template <> struct GatherStride<6> { static constexpr int SX = 29, SPL = 825; };
+// (row stride, plane stride) of the shared tile, found by search: the 32 stencil rows (rz, ry) =
+// divmod(lane + 32 it, WE) a warp reads at once fall in 32 different banks.  kTrim: WE = 2m.
+template <int M_, bool kTrim> struct GatherStride;
+template <> struct GatherStride<1, false> { static constexpr int SX = 18, SPL = 325; };
+template <> struct GatherStride<2, false> { static constexpr int SX = 21, SPL = 425; };
+template <> struct GatherStride<3, false> { static constexpr int SX = 23, SPL = 513; };
+template <> struct GatherStride<4, false> { static constexpr int SX = 25, SPL = 609; };
+template <> struct GatherStride<5, false> { static constexpr int SX = 27, SPL = 713; };
+template <> struct GatherStride<6, false> { static constexpr int SX = 29, SPL = 825; };
+template <> struct GatherStride<5, true> { static constexpr int SX = 27, SPL = 718; };
+template <> struct GatherStride<6, true> { static constexpr int SX = 29, SPL = 828; };
 
-template <int M_>
+// kTrim (fp32 Kaiser-Bessel, m >= 5; enuf_common.cuh): the window vanishes beyond |d| = m, so of the
+// 2m+1 stencil points per dimension the outermost one on the far side of the particle carries an exact
+// zero.  The kernels then work on the WE = 2m points [c - m + ks, c + m - 1 + ks], ks = (d0 > 0).
+template <int M_, bool kTrim = false>
 struct GatherCfg {
     static constexpr int W = 2 * M_ + 1;
+    static constexpr int WE = W - (kTrim ? 1 : 0);              // stencil points per dimension actually visited
     static constexpr int TP = kTile + 2 * M_;                   // padded tile edge
-    static constexpr int SX = GatherStride<M_>::SX;
-    static constexpr int SPL = GatherStride<M_>::SPL;
+    static constexpr int SX = GatherStride<M_, kTrim>::SX;
+    static constexpr int SPL = GatherStride<M_, kTrim>::SPL;
     static constexpr int CELLS = ((TP * SPL + 3) / 4) * 4;      // shared tile size in elements (16 B multiple)
     static constexpr int WARPS = 12;
     static constexpr int NT = WARPS * 32;
     static constexpr int PBW = 4;                               // particles per warp batch
-    static constexpr int ITER = (W * W + 31) / 32;              // stencil rows per lane
+    static constexpr int ITER = (WE * WE + 31) / 32;            // stencil rows per lane
     static constexpr int WP = 18;                               // pitch of a (phi, phi') weight row: 16-byte aligned, rows spread over banks
 };
 
-template <typename T, int M_>
+template <typename T, int M_, bool kTrim = false>
 constexpr size_t gather_smem_bytes() {
-    using C = GatherCfg<M_>;
+    using C = GatherCfg<M_, kTrim>;
     // tile + per warp and batch particle: (phi, phi') pairs [3][WP], pre*q, tile offset, caller index
     return sizeof(T) * ((size_t)C::CELLS + (size_t)C::WARPS * C::PBW * (3 * C::WP * 2 + 1))
            + sizeof(int) * 2 * C::WARPS * C::PBW;
@@ -61,15 +69,15 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 //              with pre = -n/(pi L^2)  (exact gradient of the ENUF energy).
 // kIk = true : one component d of the paper's ik variant, F[.,d] = pre*q * sum B_d[l] phi phi phi
 //              with pre = 2/L^2 (Eq. 42).
-template <typename T, int M_, bool kIk>
-__global__ void __launch_bounds__(GatherCfg<M_>::NT)
+template <typename T, int M_, bool kIk, bool kTrim = false>
+__global__ void __launch_bounds__(GatherCfg<M_, kTrim>::NT)
 gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
               const uint32_t* __restrict__ cell, const uint32_t* __restrict__ idx,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
               const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F) {
-    using C = GatherCfg<M_>;
+    using C = GatherCfg<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
-    constexpr int W = C::W, TP = C::TP, SX = C::SX, SPL = C::SPL, PBW = C::PBW, ITER = C::ITER, WP = C::WP;
+    constexpr int W = C::W, WE = C::WE, TP = C::TP, SX = C::SX, SPL = C::SPL, PBW = C::PBW, ITER = C::ITER, WP = C::WP;
 
     // tile (Tx, Ty, Tz): bins (Ty*nt + Tx)*n + 16 Tz .. + 16
     const int ntz = g.n / kTile;
@@ -117,7 +125,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
 #pragma unroll
     for (int it = 0; it < ITER; ++it) {
         const int rr = lane + 32 * it;
-        const int rz = rr / W, ry = rr - rz * W;
+        const int rz = rr / WE, ry = rr - rz * WE;
         rowoff[it] = rz * SPL + ry * SX;
         ryo[it] = WP + ry;          // index into the particle's [3][WP] weight rows
         rzo[it] = 2 * WP + rz;
@@ -136,11 +144,20 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             T w[W], dw[W];
             stencil_weights<T, M_, !kIk>(wp, pa, d0, w, dw);
             P2* row = wtab + (slot * 3 + dim) * WP;
+            const bool sh = kTrim && d0 > (T)0;                 // ks = 1: the k = 0 point is the zero one
 #pragma unroll
-            for (int k = 0; k < W; ++k) { P2 v; v.x = w[k]; v.y = dw[k]; row[k] = v; }
+            for (int k = 0; k < WE; ++k) {
+                P2 v;
+                v.x = (kTrim && sh) ? w[k + (kTrim ? 1 : 0)] : w[k];
+                v.y = (kTrim && sh) ? dw[k + (kTrim ? 1 : 0)] : dw[k];
+                row[k] = v;
+            }
             if (dim == 0) {
                 int cx, cy, cz;
                 unpack_cell(cell[start + p0 + slot], cx, cy, cz);
+                if (kTrim) {
+                    cx += pr.dx > (T)0 ? 1 : 0; cy += pr.dy > (T)0 ? 1 : 0; cz += pr.dz > (T)0 ? 1 : 0;
+                }
                 base_s[slot] = (cz - tz0) * SPL + (cy - ty0) * SX + (cx - tx0);
                 q_s[slot] = pre * pr.q;
                 idx_s[slot] = (int)idx[start + p0 + slot];
@@ -162,12 +179,12 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
         // ---- one particle after the other
         for (int slot = 0; slot < nb; ++slot) {
             const P2* wt = wtab + slot * 3 * WP;
-            P2 wx[W + 1];
+            P2 wx[WE + 1];
             {
                 using V4 = typename Vec4<T>::type;
                 const V4* w4 = reinterpret_cast<const V4*>(wt);
 #pragma unroll
-                for (int v = 0; v < (W + 1) / 2; ++v) {
+                for (int v = 0; v < (WE + 1) / 2; ++v) {
                     const V4 t4 = w4[v];
                     wx[2 * v].x = t4.x; wx[2 * v].y = t4.y; wx[2 * v + 1].x = t4.z; wx[2 * v + 1].y = t4.w;
                 }
@@ -176,11 +193,11 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             T fx = (T)0, fy = (T)0, fz = (T)0;
 #pragma unroll
             for (int it = 0; it < ITER; ++it) {
-                if (it + 1 < ITER || lane + 32 * it < W * W) {
+                if (it + 1 < ITER || lane + 32 * it < WE * WE) {
                     const T* row = origin + rowoff[it];
                     P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
 #pragma unroll
-                    for (int k = 0; k < W; ++k) {
+                    for (int k = 0; k < WE; ++k) {
                         if (k & 1) fma_pair(sb2, wx[k], row[k]);
                         else fma_pair(sa, wx[k], row[k]);
                     }

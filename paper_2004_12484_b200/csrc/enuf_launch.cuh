@@ -62,6 +62,10 @@ int configure_kernels(enuf_plan* p) {
         bool ok = set_smem(spread_kernel<T, M_>, spread_smem_bytes<T, M_>());
         ok = ok && set_smem(gather_kernel<T, M_, false>, gather_smem_bytes<T, M_>());
         ok = ok && set_smem(gather_kernel<T, M_, true>, gather_smem_bytes<T, M_>());
+        if constexpr (M_ >= 5 && sizeof(T) == 4) {
+            ok = ok && set_smem(gather_kernel<T, M_, false, true>, gather_smem_bytes<T, M_, true>());
+            ok = ok && set_smem(gather_kernel<T, M_, true, true>, gather_smem_bytes<T, M_, true>());
+        }
         return ok ? 0 : -1;
     });
     if (rc) return rc;
@@ -162,26 +166,30 @@ int launch_gather(enuf_plan* p, void* F) {
     const double PI = 3.14159265358979323846;
     int launches = dispatch_m(p, [&](auto mc) -> int {
         constexpr int M_ = decltype(mc)::value;
-        int launches = 0;
-        using C = GatherCfg<M_>;
-        const size_t sb = gather_smem_bytes<T, M_>();
         const unsigned ntiles = (unsigned)(p->tg.nt * p->tg.nt * (p->n / kTile));
         const PolyArg<M_> pa = make_poly_arg<M_>(p);
-        if (p->variant == ENUF_FORCE_ANALYTIC) {
-            const T pre = (T)(-(double)p->n / (PI * p->L * p->L));
-            gather_kernel<T, M_, false><<<ntiles, C::NT, sb, s>>>(
-                static_cast<const T*>(p->grid[0]), static_cast<const PRec<T>*>(p->rec), p->cell, p->idx,
-                p->bin_offset, p->tg, p->wp, pa, pre, 0, static_cast<T*>(F));
-            launches = 1;
-        } else {
+        auto run = [&](auto trim_c) -> int {
+            constexpr bool kTrim = decltype(trim_c)::value != 0;
+            using C = GatherCfg<M_, kTrim>;
+            const size_t sb = gather_smem_bytes<T, M_, kTrim>();
+            if (p->variant == ENUF_FORCE_ANALYTIC) {
+                const T pre = (T)(-(double)p->n / (PI * p->L * p->L));
+                gather_kernel<T, M_, false, kTrim><<<ntiles, C::NT, sb, s>>>(
+                    static_cast<const T*>(p->grid[0]), static_cast<const PRec<T>*>(p->rec), p->cell, p->idx,
+                    p->bin_offset, p->tg, p->wp, pa, pre, 0, static_cast<T*>(F));
+                return 1;
+            }
             const T pre = (T)(2.0 / (p->L * p->L));
             for (int d = 0; d < 3; ++d)
-                gather_kernel<T, M_, true><<<ntiles, C::NT, sb, s>>>(
+                gather_kernel<T, M_, true, kTrim><<<ntiles, C::NT, sb, s>>>(
                     static_cast<const T*>(p->grid[d]), static_cast<const PRec<T>*>(p->rec), p->cell, p->idx,
                     p->bin_offset, p->tg, p->wp, pa, pre, d, static_cast<T*>(F));
-            launches = 3;
+            return 3;
+        };
+        if constexpr (M_ >= 5 && sizeof(T) == 4) {
+            if (p->trim) return run(IntC<1>{});
         }
-        return launches;
+        return run(IntC<0>{});
     });
     if (launches < 0) return -1;
     return cudaGetLastError() == cudaSuccess ? launches : -1;

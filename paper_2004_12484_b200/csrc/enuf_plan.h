@@ -15,6 +15,7 @@ struct enuf_plan {
     int precision = ENUF_F32, window = ENUF_WINDOW_KAISER_BESSEL, variant = ENUF_FORCE_ANALYTIC;
     double lambda = 0.0;
     bool profile = false, keep_spectrum = false;
+    bool trim = false;             // fp32 Kaiser-Bessel m >= 5: kernels visit 2m stencil points per dimension
     cudaStream_t stream = nullptr;
     // derived
     enuf::TileGeom tg{};

@@ -229,6 +229,7 @@ def test_cfg5_properties_full_size(enuf, torch_cuda):
     (32, 1, "kaiser_bessel", "f64"), (32, 2, "gaussian", "f64"), (32, 3, "kaiser_bessel", "f32"),
     (64, 5, "kaiser_bessel", "f64"), (64, 6, "gaussian", "f32"), (128, 4, "kaiser_bessel", "f64"),
     (128, 6, "gaussian", "f64"), (256, 2, "kaiser_bessel", "f32"), (256, 6, "kaiser_bessel", "f64"),
+    (64, 5, "kaiser_bessel", "f32"), (128, 6, "kaiser_bessel", "f32"),     # trimmed 2m-point stencils (fp32, m >= 5)
 ])
 @pytest.mark.parametrize("variant", ["analytic", "ik"])
 def test_all_grid_sizes_and_supports(enuf, torch_cuda, oracle, n, m, window, dtype, variant):
@@ -376,4 +377,28 @@ def test_dense_cluster_many_particles_per_bin(enuf, torch_cuda, oracle):
         tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
         assert abs(E - ref["E"]) <= te * abs(ref["E"])
         assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+        plan.close()
+
+
+def test_fp32_particles_exactly_on_grid_points(enuf, torch_cuda, oracle):
+    """fp32 Kaiser-Bessel m = 6 visits 2m stencil points per dimension (the far outermost one is an
+    exact zero) -- except for a particle exactly on a grid point, where both ends carry
+    b m / sinh(b m) = 2.9e-11 of the peak and one of them is dropped: far below the fp32 bar."""
+    torch = torch_cuda
+    n, m, L = 64, 6, 8.0
+    rng = np.random.default_rng(5)
+    N = 600
+    cells = rng.integers(0, n, size=(N, 3))
+    r = (cells * (L / n)).astype(np.float32)                 # multiples of 1/8: exact in fp32, d0 = 0
+    r[N // 2:] += rng.uniform(0, L / n, size=(N - N // 2, 3)).astype(np.float32)
+    q = np.where(np.arange(N) % 2 == 0, 1.0, -1.0).astype(np.float32)
+    M, k_cut = n // 2, n // 4
+    alpha = 0.9 * math.pi * k_cut / (L * 3.0)
+    for variant in ("analytic", "ik"):
+        ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, "kaiser_bessel", 2.0, variant=variant)
+        plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=2.0, m=m, window="kaiser_bessel", variant=variant,
+                         dtype=torch.float32)
+        E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+        assert abs(E - ref["E"]) <= F32_E * abs(ref["E"])
+        assert rel_rms(F.cpu().numpy(), ref["F"]) <= F32_F
         plan.close()
