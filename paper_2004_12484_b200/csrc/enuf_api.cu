@@ -232,6 +232,7 @@ int ensure_allocated(enuf_plan* p) {
     // only when the particle sits exactly on a grid point are both ends non-zero, with the value
     // b m / sinh(b m) (<= 2.7e-9 for m >= 5): the fp32 kernels then skip that point
     p->trim = p->precision == ENUF_F32 && p->window == ENUF_WINDOW_KAISER_BESSEL && p->m >= 5;
+    p->tg.trim = p->trim ? 1 : 0;
     const size_t es = p->esize, n = p->n, n3 = n * n * n, cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1);
     const int nfield = p->variant == ENUF_FORCE_IK ? 3 : 1;
     int rc;
@@ -397,6 +398,7 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
             if (iv != ENUF_WINDOW_GAUSSIAN && iv != ENUF_WINDOW_KAISER_BESSEL) return fail(ENUF_EINVAL, "unknown window");
             p->window = iv; p->tables_dirty = true; fill_window_params(p);
             p->trim = p->precision == ENUF_F32 && p->window == ENUF_WINDOW_KAISER_BESSEL && p->m >= 5;
+            p->tg.trim = p->trim ? 1 : 0;
             return ENUF_OK;
         case ENUF_OPT_FORCE_VARIANT:
             if (iv != ENUF_FORCE_ANALYTIC && iv != ENUF_FORCE_IK) return fail(ENUF_EINVAL, "unknown force variant");

@@ -33,8 +33,14 @@ __device__ __forceinline__ CellOfParticle locate(const T* __restrict__ r, int64_
     return o;
 }
 
-__device__ __forceinline__ int bin_of(const int c[3], const TileGeom& g) {
-    return ((c[1] / kTile) * g.nt + (c[0] / kTile)) * g.n + c[2];
+template <typename T>
+__device__ __forceinline__ int bin_of(const CellOfParticle& p, const TileGeom& g) {
+    int bz = p.c[2];
+    if (g.trim) {       // the sign test is taken on the value the record stores (rounded to T)
+        bz += ((T)p.d0[2] > (T)0 ? 1 : 0) - 1;
+        bz += bz < 0 ? g.n : 0;
+    }
+    return ((p.c[1] / kTile) * g.nt + (p.c[0] / kTile)) * g.n + bz;
 }
 
 // Histogram of charged particles per bin; neutral particles get F = 0 here and are dropped.
@@ -49,7 +55,7 @@ bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict
         return;
     }
     CellOfParticle p = locate(r, j, L, g.n);
-    atomicAdd(&count[bin_of(p.c, g)], 1u);
+    atomicAdd(&count[bin_of<T>(p, g)], 1u);
 }
 
 // Exclusive scan of count[0..nbins) into offset[0..nbins] (and a copy in cursor[0..nbins),
@@ -137,7 +143,7 @@ bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, 
     T qj = q[j];
     if (qj == (T)0) return;
     CellOfParticle p = locate(r, j, L, g.n);
-    uint32_t pos = atomicAdd(&cursor[bin_of(p.c, g)], 1u);
+    uint32_t pos = atomicAdd(&cursor[bin_of<T>(p, g)], 1u);
     PRec<T> o;
     o.dx = (T)p.d0[0]; o.dy = (T)p.d0[1]; o.dz = (T)p.d0[2]; o.q = qj;
     rec[pos] = o;

@@ -48,6 +48,9 @@ struct TileGeom {
     int n;        // grid points per dimension
     int nt;       // columns per dimension = n / 16
     int nbins;    // nt * nt * n
+    int trim;     // 1: the z index of the bin is c_z - 1 + (d0_z > 0) instead of c_z (trimmed stencils,
+                  //    fp32 Kaiser-Bessel m >= 5: the particle's 2m non-zero z weights sit on the planes
+                  //    bin_z - m + 1 .. bin_z + m)
 };
 
 // Piecewise-polynomial window table for the fp32 path (step a0).  For every stencil offset

@@ -155,10 +155,12 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             if (dim == 0) {
                 int cx, cy, cz;
                 unpack_cell(cell[start + p0 + slot], cx, cy, cz);
+                int zrel = cz - tz0;                  // trimmed bins: c_z may be the first plane of the next tile
+                zrel += zrel < 0 ? g.n : 0;
                 if (kTrim) {
-                    cx += pr.dx > (T)0 ? 1 : 0; cy += pr.dy > (T)0 ? 1 : 0; cz += pr.dz > (T)0 ? 1 : 0;
+                    cx += pr.dx > (T)0 ? 1 : 0; cy += pr.dy > (T)0 ? 1 : 0; zrel += pr.dz > (T)0 ? 1 : 0;
                 }
-                base_s[slot] = (cz - tz0) * SPL + (cy - ty0) * SX + (cx - tx0);
+                base_s[slot] = zrel * SPL + (cy - ty0) * SX + (cx - tx0);
                 q_s[slot] = pre * pr.q;
                 idx_s[slot] = (int)idx[start + p0 + slot];
             }

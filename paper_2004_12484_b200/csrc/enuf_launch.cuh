@@ -60,6 +60,7 @@ int configure_kernels(enuf_plan* p) {
     int rc = dispatch_m(p, [&](auto mc) -> int {
         constexpr int M_ = decltype(mc)::value;
         bool ok = set_smem(spread_kernel<T, M_>, spread_smem_bytes<T, M_>());
+        if constexpr (M_ >= 5 && sizeof(T) == 4) ok = ok && set_smem(spread_kernel<T, M_, true>, spread_smem_bytes<T, M_>());
         ok = ok && set_smem(gather_kernel<T, M_, false>, gather_smem_bytes<T, M_>());
         ok = ok && set_smem(gather_kernel<T, M_, true>, gather_smem_bytes<T, M_>());
         if constexpr (M_ >= 5 && sizeof(T) == 4) {
@@ -105,9 +106,18 @@ int launch_spread(enuf_plan* p) {
         constexpr int M_ = decltype(mc)::value;
         using C = SpreadCfg<M_>;
         const dim3 grid((unsigned)(p->tg.nt * p->tg.nt), (unsigned)((p->n + p->zchunk - 1) / p->zchunk));
-        spread_kernel<T, M_><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
-            static_cast<const PRec<T>*>(p->rec), p->cell, p->bin_offset, p->tg, p->wp, make_poly_arg<M_>(p),
-            p->zchunk, static_cast<T*>(p->grid[0]));
+        const PolyArg<M_> pa = make_poly_arg<M_>(p);
+        if constexpr (M_ >= 5 && sizeof(T) == 4) {
+            if (p->trim) {
+                spread_kernel<T, M_, true><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
+                    static_cast<const PRec<T>*>(p->rec), p->cell, p->bin_offset, p->tg, p->wp, pa, p->zchunk,
+                    static_cast<T*>(p->grid[0]));
+                return 0;
+            }
+        }
+        spread_kernel<T, M_, false><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
+            static_cast<const PRec<T>*>(p->rec), p->cell, p->bin_offset, p->tg, p->wp, pa, p->zchunk,
+            static_cast<T*>(p->grid[0]));
         return 0;
     });
     if (rc) return -1;

@@ -51,7 +51,10 @@ constexpr size_t spread_smem_bytes() {
     return sizeof(T) * (size_t)C::CAP * C::RP + sizeof(int) * (size_t)C::CAP;
 }
 
-template <typename T, int M_>
+// kTrim (fp32 Kaiser-Bessel, m >= 5): particles are binned by the plane s = c_z - 1 + ks_z, ks = (d0 > 0),
+// so that every particle of slab s has its 2m non-zero z weights on the planes s-m+1 .. s+m: the window
+// is WZ = 2m planes, and the warps test their cells against the 2m-point x / y extents.
+template <typename T, int M_, bool kTrim = false>
 __global__ void __launch_bounds__(SpreadCfg<M_>::NT, sizeof(T) == 4 ? 7 : 2)
 spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
@@ -59,10 +62,12 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
     using C = SpreadCfg<M_>;
     using P2 = typename Pair2<T>::type;
     constexpr int W = C::W, NT = C::NT, CAP = C::CAP, RP = C::RP, OX = C::OX, OY = C::OY, OZ = C::OZ, OD = C::OD;
+    constexpr int WZ = W - (kTrim ? 1 : 0);            // planes in the register window
+    constexpr int SLO = M_, SHI = kTrim ? M_ - 1 : M_;  // slabs z0 - SLO .. z1 - 1 + SHI reach the planes [z0, z1)
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* st = reinterpret_cast<T*>(smem_raw);            // [CAP][RP] staged particle records
-    int* sb = reinterpret_cast<int*>(st + CAP * RP);   // [CAP]     (bx + m) | (by + m) << 8
+    int* sb = reinterpret_cast<int*>(st + CAP * RP);   // [CAP]     (bx + m) | (by + m) << 8 | ks_x << 16 | ks_y << 17
     __shared__ int rng_start[2][9], rng_cnt[2][9];
     __shared__ int nslot_s;
 
@@ -89,11 +94,11 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
         }
     };
     if (tid == 0) nslot_s = 0;
-    load_ranges(z0 - M_, 0);
+    load_ranges(z0 - SLO, 0);
 
-    P2 acc[W];
+    P2 acc[WZ];
 #pragma unroll
-    for (int k = 0; k < W; ++k) { acc[k].x = (T)0; acc[k].y = (T)0; }
+    for (int k = 0; k < WZ; ++k) { acc[k].x = (T)0; acc[k].y = (T)0; }
 
     T* gout = grid + ((size_t)(Ty * kTile + ly)) * g.n + Tx * kTile + lx;
     const char* lane_xb = reinterpret_cast<const char*>(st + OX + lx);   // this lane's entries of slot 0's rows
@@ -101,9 +106,9 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
     const char* st_zb = reinterpret_cast<const char*>(st + OZ);
 
     int buf = 0;
-    for (int s = z0 - M_; s < z1 + M_; ++s, buf ^= 1) {
+    for (int s = z0 - SLO; s < z1 + SHI; ++s, buf ^= 1) {
         __syncthreads();      // ranges of slab s visible; all warps are done with the previous slab
-        if (s + 1 < z1 + M_) load_ranges(s + 1, buf ^ 1);
+        if (s + 1 < z1 + SHI) load_ranges(s + 1, buf ^ 1);
         int pref[10];
         pref[0] = 0;
 #pragma unroll
@@ -128,8 +133,11 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                 if ((unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_)) {
                     const int slot = atomicAdd(&nslot_s, 1);
                     if (slot < CAP) {
-                        *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = rec[pidx];
-                        sb[slot] = bxm | (bym << 8);
+                        const PRec<T> pr = rec[pidx];
+                        *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = pr;
+                        int pk = bxm | (bym << 8);
+                        if (kTrim) pk |= (pr.dx > (T)0 ? 1 << 16 : 0) | (pr.dy > (T)0 ? 1 << 17 : 0);
+                        sb[slot] = pk;
                     }
                 }
             }
@@ -155,13 +163,15 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
             for (int t = tid; t < 3 * ns; t += NT) {
                 const int dim = t / ns, slot = t - dim * ns;
                 T w[W], dw[W];
-                stencil_weights<T, M_, false>(wp, pa, st[slot * RP + OD + dim], w, dw);
+                const T d0 = st[slot * RP + OD + dim];
+                stencil_weights<T, M_, false>(wp, pa, d0, w, dw);
                 using V4 = typename Vec4<T>::type;
                 if (dim == 2) {
                     const T q = st[slot * RP + OD + 3];
                     T r16[16];
 #pragma unroll
-                    for (int k = 0; k < 16; ++k) r16[k] = k < W ? w[k < W ? k : 0] * q : (T)0;
+                    for (int k = 0; k < 16; ++k)
+                        r16[k] = k < WZ ? ((kTrim && d0 > (T)0) ? w[k + 1 < W ? k + 1 : 0] : w[k < W ? k : 0]) * q : (T)0;
                     V4* row4 = reinterpret_cast<V4*>(st + slot * RP + OZ);
 #pragma unroll
                     for (int v = 0; v < 4; ++v) {
@@ -173,7 +183,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                     V4 z; z.x = (T)0; z.y = (T)0; z.z = (T)0; z.w = (T)0;
 #pragma unroll
                     for (int v = 0; v < 4; ++v) reinterpret_cast<V4*>(row)[v] = z;
-                    const int X0 = (dim == 0 ? (sb[slot] & 255) : (sb[slot] >> 8)) - 2 * M_;   // cell of k = 0
+                    const int X0 = (dim == 0 ? (sb[slot] & 255) : ((sb[slot] >> 8) & 255)) - 2 * M_;   // cell of k = 0
 #pragma unroll
                     for (int k = 0; k < W; ++k)
                         if ((unsigned)(X0 + k) < (unsigned)kTile) row[X0 + k] = w[k];
@@ -186,8 +196,10 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                 bool ov = false;
                 if (e0 + lane < ns) {
                     const int v = sb[e0 + lane];
-                    const int bx2 = v & 255, by2 = v >> 8;            // stencil covers [b - 2m, b] in column cells
-                    ov = bx2 >= px && bx2 - 2 * M_ <= px + 7 && by2 >= py && by2 - 2 * M_ <= py + 7;
+                    // stencil covers [b - 2m, b] in column cells; trimmed: [b - 2m + ks, b - 1 + ks]
+                    const int bx2 = (v & 255) + (kTrim ? ((v >> 16) & 1) - 1 : 0);
+                    const int by2 = ((v >> 8) & 255) + (kTrim ? ((v >> 17) & 1) - 1 : 0);
+                    ov = bx2 >= px && bx2 - (WZ - 1) <= px + 7 && by2 >= py && by2 - (WZ - 1) <= py + 7;
                 }
                 unsigned om = __ballot_sync(0xffffffffu, ov);
                 // two particles per trip: the loads of the second overlap the FMAs of the first
@@ -207,22 +219,22 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                     const T* wz1 = reinterpret_cast<const T*>(st_zb + o1);
                     const T* wz2 = reinterpret_cast<const T*>(st_zb + o2);
 #pragma unroll
-                    for (int k = 0; k < W; ++k) fma_pair(acc[k], a1, wz1[k]);
+                    for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a1, wz1[k]);
                     if (two) {
 #pragma unroll
-                        for (int k = 0; k < W; ++k) fma_pair(acc[k], a2, wz2[k]);
+                        for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a2, wz2[k]);
                     }
                 }
             }
             c0 += span;
             if (c0 < total) __syncthreads();           // staging buffers are reused by the next chunk
         }
-        // ---- plane z = s - m is complete: store it and slide the window
-        const int zo = s - M_;
+        // ---- the lowest plane of the window (s - m, trimmed: s - m + 1) is complete: store it, slide
+        const int zo = s - SHI;
         if (zo >= z0) *reinterpret_cast<P2*>(gout + (size_t)zo * g.n * g.n) = acc[0];
 #pragma unroll
-        for (int k = 0; k + 1 < W; ++k) acc[k] = acc[k + 1];
-        acc[W - 1].x = (T)0; acc[W - 1].y = (T)0;
+        for (int k = 0; k + 1 < WZ; ++k) acc[k] = acc[k + 1];
+        acc[WZ - 1].x = (T)0; acc[WZ - 1].y = (T)0;
     }
 }
 

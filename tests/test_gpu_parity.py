@@ -212,10 +212,13 @@ def test_cfg5_properties_full_size(enuf, torch_cuda):
     # per mode and E (a sum over ~1e6 modes with random signs) by ~1e-7/sqrt(1e3..1e6): allow 5e-8,
     # 20x below the fp32 parity bar.
     assert abs(E1 - E2) <= 5e-8 * abs(E1)
-    assert rel_rms(F2.cpu().numpy(), F1.cpu().numpy()) <= 5e-7
+    # Forces: the order inside a bin and inside a slab's staging list is arrival order, so each run carries
+    # its own fp32 summation noise (~3.6e-7 relative RMS measured); two runs differ by sqrt(2) of it.
+    # Bound: half the fp32 parity bar.
+    assert rel_rms(F2.cpu().numpy(), F1.cpu().numpy()) <= 1e-6
     Eh, Fh = plan.energy_forces_host(w.r, w.q)
     assert abs(Eh - E1) <= 5e-8 * abs(E1)
-    assert rel_rms(Fh.numpy(), F1.cpu().numpy()) <= 5e-7
+    assert rel_rms(Fh.numpy(), F1.cpu().numpy()) <= 1e-6
     q0 = q.clone(); q0[::3] = 0
     E3, F3 = plan.energy_forces(r, q0)
     assert not F3[::3].any().item()
