@@ -124,8 +124,34 @@ int launch_spread(enuf_plan* p) {
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
+// Forward half of the FFT stage (a3): X real-to-complex and Y passes; leaves the partial spectrum
+// [z][ky'][kx] of this plan's particles in A2[0].  Linear in the charges, so partial spectra of
+// particle subsets add (Eq. 61): the multi-GPU path all-reduces A2[0] here.
 template <typename T>
-int launch_fft(enuf_plan* p) {
+int launch_fft_forward(enuf_plan* p) {
+    cudaStream_t s = p->stream;
+    FftGeom fg{p->n, p->k_cut, p->Kxp, p->Ky};
+    const Cx<T>* tw = static_cast<const Cx<T>*>(p->tw);
+    int launches = dispatch_n(p->n, [&](auto nc) -> int {
+        constexpr int N_ = decltype(nc)::value;
+        constexpr int LPC = fft_lines_per_cta<N_>();
+        const size_t sb = fft_smem_bytes<T, N_>();
+        const unsigned bx = (unsigned)(((size_t)N_ * N_) / LPC);
+        const unsigned by = (unsigned)(((size_t)N_ * p->Kxp + LPC - 1) / LPC);
+        fft_x_forward_kernel<T, N_><<<bx / 2, kFftThreads, sb, s>>>(static_cast<const T*>(p->grid[0]),
+                                                               static_cast<Cx<T>*>(p->A1[0]), fg, tw);
+        fft_y_forward_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[0]),
+                                                               static_cast<Cx<T>*>(p->A2[0]), fg, tw);
+        return 2;
+    });
+    if (launches < 0) return -1;
+    return cudaGetLastError() == cudaSuccess ? launches : -1;
+}
+
+// Backward half (a4 + a5 + a7): Z forward . scale . energy . Z inverse on A2[0] (in place; the ik
+// variant writes A2[0..2]), Y and X inverse passes into the real field(s), energy reduction.
+template <typename T>
+int launch_fft_backward(enuf_plan* p) {
     cudaStream_t s = p->stream;
     FftGeom fg{p->n, p->k_cut, p->Kxp, p->Ky};
     const Cx<T>* tw = static_cast<const Cx<T>*>(p->tw);
@@ -140,10 +166,6 @@ int launch_fft(enuf_plan* p) {
         const unsigned by = (unsigned)(((size_t)N_ * p->Kxp + LPC - 1) / LPC);
         const unsigned bz = (unsigned)(((size_t)p->Ky * p->Kxp + LPC - 1) / LPC);
         if ((int)bz > p->n_partial) return -1;
-        fft_x_forward_kernel<T, N_><<<bx / 2, kFftThreads, sb, s>>>(static_cast<const T*>(p->grid[0]),
-                                                               static_cast<Cx<T>*>(p->A1[0]), fg, tw);
-        fft_y_forward_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[0]),
-                                                               static_cast<Cx<T>*>(p->A2[0]), fg, tw);
         Cx<T>* spec = p->keep_spectrum ? static_cast<Cx<T>*>(p->spectrum) : nullptr;
         if (nout == 1)
             fft_z_fused_kernel<T, N_, 1><<<bz, kFftThreads, sb, s>>>(static_cast<Cx<T>*>(p->A2[0]), nullptr, nullptr,
@@ -153,7 +175,7 @@ int launch_fft(enuf_plan* p) {
                                                                     static_cast<Cx<T>*>(p->A2[1]),
                                                                     static_cast<Cx<T>*>(p->A2[2]), fg, tw, st,
                                                                     p->e_partial, spec);
-        launches = 3;
+        launches = 1;
         for (int d = 0; d < nout; ++d) {
             fft_y_inverse_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A2[d]),
                                                                    static_cast<Cx<T>*>(p->A1[d]), fg, tw);
@@ -168,6 +190,14 @@ int launch_fft(enuf_plan* p) {
     });
     if (launches < 0) return -1;
     return cudaGetLastError() == cudaSuccess ? launches : -1;
+}
+
+template <typename T>
+int launch_fft(enuf_plan* p) {
+    const int a = launch_fft_forward<T>(p);
+    if (a < 0) return -1;
+    const int b = launch_fft_backward<T>(p);
+    return b < 0 ? -1 : a + b;
 }
 
 template <typename T>

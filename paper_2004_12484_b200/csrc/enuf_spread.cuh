@@ -48,7 +48,7 @@ struct SpreadCfg {
 template <typename T, int M_>
 constexpr size_t spread_smem_bytes() {
     using C = SpreadCfg<M_>;
-    return sizeof(T) * (size_t)C::CAP * C::RP + sizeof(int) * (size_t)C::CAP;
+    return sizeof(T) * (size_t)(C::CAP + 1) * C::RP + sizeof(int) * (size_t)C::CAP;
 }
 
 // kTrim (fp32 Kaiser-Bessel, m >= 5): particles are binned by the plane s = c_z - 1 + ks_z, ks = (d0 > 0),
@@ -66,10 +66,12 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
     constexpr int SLO = M_, SHI = kTrim ? M_ - 1 : M_;  // slabs z0 - SLO .. z1 - 1 + SHI reach the planes [z0, z1)
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* st = reinterpret_cast<T*>(smem_raw);            // [CAP][RP] staged particle records
-    int* sb = reinterpret_cast<int*>(st + CAP * RP);   // [CAP]     (bx + m) | (by + m) << 8 | ks_x << 16 | ks_y << 17
+    T* st = reinterpret_cast<T*>(smem_raw);            // [CAP + 1][RP] staged particle records; slot CAP is all zero
+    int* sb = reinterpret_cast<int*>(st + (CAP + 1) * RP);   // [CAP] (bx + m) | (by + m) << 8 | ks_x << 16 | ks_y << 17
     __shared__ int rng_start[2][9], rng_cnt[2][9];
     __shared__ int nslot_s;
+    // per warp: byte offsets (into st) of the staged particles that overlap the warp's cells, compacted
+    __shared__ __align__(8) unsigned wlist[NT / 32][36];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int Tx = blockIdx.x % g.nt, Ty = blockIdx.x / g.nt;
@@ -94,6 +96,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
         }
     };
     if (tid == 0) nslot_s = 0;
+    if (tid < RP) st[CAP * RP + tid] = (T)0;           // the padding record of odd-length visit lists
     load_ranges(z0 - SLO, 0);
 
     P2 acc[WZ];
@@ -201,30 +204,42 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                     const int by2 = ((v >> 8) & 255) + (kTrim ? ((v >> 17) & 1) - 1 : 0);
                     ov = bx2 >= px && bx2 - (WZ - 1) <= px + 7 && by2 >= py && by2 - (WZ - 1) <= py + 7;
                 }
-                unsigned om = __ballot_sync(0xffffffffu, ov);
-                // two particles per trip: the loads of the second overlap the FMAs of the first
-                while (om) {
-                    const int e1 = e0 + __ffs(om) - 1;
-                    om &= om - 1;
-                    const bool two = om != 0;
-                    const int e2 = two ? e0 + __ffs(om) - 1 : e1;
-                    om &= om - 1;
-                    const unsigned o1 = (unsigned)e1 * (RP * sizeof(T)), o2 = (unsigned)e2 * (RP * sizeof(T));   // warp-uniform
+                const unsigned om = __ballot_sync(0xffffffffu, ov);
+                if (om == 0u) continue;
+                // compact the overlapping slots into the warp's list (padded to an even length with the
+                // zero record), then visit them two per trip: the loads of the second overlap the FMAs
+                // of the first, and the trip has no data-dependent control flow
+                const int cnt = __popc(om);
+                unsigned* wl = wlist[warp];
+                if (ov) wl[__popc(om & ((1u << lane) - 1u))] = (unsigned)(e0 + lane) * (unsigned)(RP * sizeof(T));
+                if (lane == 0) wl[cnt] = (unsigned)CAP * (unsigned)(RP * sizeof(T));
+                __syncwarp();
+                uint2 oo = *reinterpret_cast<const uint2*>(wl);
+                for (int i = 0; i < cnt; i += 2) {
+                    const unsigned o1 = oo.x, o2 = oo.y;
+                    oo = *reinterpret_cast<const uint2*>(wl + i + 2);        // next trip (list has 4 spare entries)
                     const P2 wx1 = *reinterpret_cast<const P2*>(lane_xb + o1);
                     const T wy1 = *reinterpret_cast<const T*>(lane_yb + o1);
                     const P2 wx2 = *reinterpret_cast<const P2*>(lane_xb + o2);
-                    const T wy2 = two ? *reinterpret_cast<const T*>(lane_yb + o2) : (T)0;
+                    const T wy2 = *reinterpret_cast<const T*>(lane_yb + o2);
                     P2 a1; a1.x = wx1.x * wy1; a1.y = wx1.y * wy1;
                     P2 a2; a2.x = wx2.x * wy2; a2.y = wx2.y * wy2;
-                    const T* wz1 = reinterpret_cast<const T*>(st_zb + o1);
-                    const T* wz2 = reinterpret_cast<const T*>(st_zb + o2);
+                    // q * z rows: 16-byte vector loads (slot pitch and OZ are multiples of 16 bytes)
+                    using V4 = typename Vec4<T>::type;
+                    constexpr int NV = (WZ + 3) / 4;
+                    V4 z1[NV], z2[NV];
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) z1[v] = reinterpret_cast<const V4*>(st_zb + o1)[v];
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) z2[v] = reinterpret_cast<const V4*>(st_zb + o2)[v];
+                    const T* wz1 = reinterpret_cast<const T*>(z1);
+                    const T* wz2 = reinterpret_cast<const T*>(z2);
 #pragma unroll
                     for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a1, wz1[k]);
-                    if (two) {
 #pragma unroll
-                        for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a2, wz2[k]);
-                    }
+                    for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a2, wz2[k]);
                 }
+                __syncwarp();                    // the list is rewritten by the next group of 32 slots
             }
             c0 += span;
             if (c0 < total) __syncthreads();           // staging buffers are reused by the next chunk
