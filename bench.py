@@ -40,6 +40,10 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--variant", default="analytic", choices=["analytic", "ik"])
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "sharded"],
+                    help="N > 1: independent replicas (weak scaling, no data-path collective; default) or ONE "
+                         "system sharded by particle with an all-reduce of the partial spectra (strong scaling; "
+                         "DESIGN.md section 9)")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-comparisons", action="store_true",
@@ -63,11 +67,11 @@ def step_positions(w, steps: int, rank: int):
 
 # ---------------------------------------------------------------------- algorithmic bytes
 
-def algorithmic_bytes(w, variant: str, n_charged: int) -> dict:
+def algorithmic_bytes(w, variant: str, n_charged: int, n_local: int = None) -> dict:
     """Bytes each stage must move per evaluation: every input read
     once, every output written once, at the pruned sizes."""
     B = 8 if w.dtype == "f64" else 4
-    n, kc, N = w.n, w.k_cut, w.N
+    n, kc, N = w.n, w.k_cut, (w.N if n_local is None else n_local)
     kx, ky = kc + 1, 2 * kc + 1
     n3 = n ** 3
     a1 = n * n * kx * 2 * B          # [z][y][kx] complex
@@ -255,17 +259,33 @@ def run_ours(args):
     w = make_workload(args.workload)
     K, W = args.steps, args.warmup
     tdtype = torch.float64 if w.dtype == "f64" else torch.float32
-    pos_host = step_positions(w, W + K, rank)                       # (W+K, N, 3)
+    sharded = args.parallel == "sharded"
+    N_sys = w.N
+    if sharded:
+        # ONE system, the same on every rank; this rank owns the particles [lo, hi)
+        lo, hi = enuf.shard_bounds(w.N, rank, world)
+        pos_host = np.ascontiguousarray(step_positions(w, W + K, 0)[:, lo:hi])
+        q_host = np.ascontiguousarray(w.q[lo:hi])
+    else:
+        lo, hi = 0, w.N
+        pos_host = step_positions(w, W + K, rank)                   # (W+K, N, 3)
+        q_host = w.q
+    N_loc = hi - lo
     pos_pinned = torch.from_numpy(pos_host).pin_memory()
-    q_pinned = torch.from_numpy(w.q).pin_memory()
+    q_pinned = torch.from_numpy(q_host).pin_memory()
     pos_dev = pos_pinned.cuda()
     q_dev = q_pinned.cuda()
-    F_dev = torch.empty((w.N, 3), dtype=tdtype, device="cuda")
-    n_charged = int(np.count_nonzero(w.q))
+    F_dev = torch.empty((N_loc, 3), dtype=tdtype, device="cuda")
+    n_charged = int(np.count_nonzero(q_host))
 
     plan = enuf.Plan.from_workload(w, variant=args.variant, profile=False)
+    if sharded:
+        plan.close()
+        plan = enuf.Plan(N_loc, w.L, w.alpha, w.k_cut, w.M, sigma=w.sigma, m=w.m, dtype=tdtype, window=w.window,
+                         variant=args.variant, slater_lambda=w.slater_lambda)
+    evaluate = plan.energy_forces_sharded if sharded else plan.energy_forces
     for s in range(W):
-        plan.energy_forces(pos_dev[s], q_dev, F=F_dev, want_energy=False)
+        evaluate(pos_dev[s], q_dev, F=F_dev, want_energy=False)
     plan.set(enuf.OPT_PROFILE, 1)                                  # per-stage events from here on
     torch.cuda.synchronize()
     barrier()
@@ -275,7 +295,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     ev0.record()
     for s in range(K):
-        plan.energy_forces(pos_dev[W + s], q_dev, F=F_dev, want_energy=False)
+        evaluate(pos_dev[W + s], q_dev, F=F_dev, want_energy=False)
         launches += plan.launch_count()
     ev1.record()
     torch.cuda.synchronize()
@@ -285,27 +305,40 @@ def run_ours(args):
     E_last = plan.energy()
     stage_ms, n_prof = plan.stage_ms_mean()
     ms_step = ms_total / K
-    value = whole_job_value(w.N, world, ms_step)
+    value = N_sys / (ms_step * 1e-3) if sharded else whole_job_value(w.N, world, ms_step)
     total_launches = int(sum_over_ranks(float(launches)))
 
     # ---- end to end: host buffers in, host forces + energy out, through the C ABI
     plan.set(enuf.OPT_PROFILE, 0)
     Ke = max(1, min(args.e2e_steps, K))
-    F_host = torch.empty((w.N, 3), dtype=tdtype).pin_memory()
+    F_host = torch.empty((N_loc, 3), dtype=tdtype).pin_memory()
+    if sharded:
+        r_st, q_st = torch.empty_like(pos_dev[0]), torch.empty_like(q_dev)
+
+        def host_step(s_):       # pinned host shard -> device, sharded evaluation, forces + energy back
+            r_st.copy_(pos_pinned[s_], non_blocking=True); q_st.copy_(q_pinned, non_blocking=True)
+            plan.energy_forces_sharded(r_st, q_st, F=F_dev, want_energy=False)
+            F_host.copy_(F_dev, non_blocking=True)
+            return plan.energy()
+        api = "Plan.energy_forces_sharded (pinned host shard -> device, all-reduce, host F, E)"
+    else:
+        def host_step(s_):
+            return plan.energy_forces_host(pos_pinned[s_], q_pinned, F=F_host)[0]
+        api = "enuf_energy_forces_host (pinned host r, q -> host F, E)"
     for s in range(2):
-        plan.energy_forces_host(pos_pinned[s], q_pinned, F=F_host)
+        host_step(s)
     torch.cuda.synchronize()
     barrier()
     t0 = time.perf_counter()
     for s in range(Ke):
-        E_h, _ = plan.energy_forces_host(pos_pinned[W + s], q_pinned, F=F_host)
+        E_h = host_step(W + s)
     torch.cuda.synchronize()
     t_e2e = max_over_ranks((time.perf_counter() - t0) / Ke)
     barrier()
     esz = 8 if w.dtype == "f64" else 4
-    e2e = {"value": w.N * world / t_e2e, "unit": UNIT, "ms_per_step": 1e3 * t_e2e, "steps": Ke,
-           "h2d_bytes_per_step": int(w.N * 4 * esz), "d2h_bytes_per_step": int(w.N * 3 * esz + 8),
-           "api": "enuf_energy_forces_host (pinned host r, q -> host F, E)"}
+    e2e = {"value": (N_sys if sharded else w.N * world) / t_e2e, "unit": UNIT, "ms_per_step": 1e3 * t_e2e, "steps": Ke,
+           "h2d_bytes_per_step": int(N_loc * 4 * esz), "d2h_bytes_per_step": int(N_loc * 3 * esz + 8),
+           "api": api}
 
     if rank != 0:
         plan.close()
@@ -315,7 +348,7 @@ def run_ours(args):
 
     # ---- roofline of the dominant stage (CUDA events recorded on the plan's stream, per evaluation)
     peak, peak_src = measured_hbm_peak()
-    abytes = algorithmic_bytes(w, args.variant, n_charged)
+    abytes = algorithmic_bytes(w, args.variant, n_charged, N_loc)
     stages = {}
     for st in ("bin", "spread", "fft", "gather"):
         gbs = abytes[st] / (stage_ms[st] * 1e-3) / 1e9 if stage_ms[st] > 0 else 0.0
@@ -387,14 +420,15 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
         "config": {"workload": args.workload, "N": int(w.N), "L": w.L, "alpha": w.alpha, "k_cut": w.k_cut,
                    "M": w.M, "sigma": w.sigma, "n": w.n, "m": w.m, "window": w.window, "variant": args.variant,
-                   "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                   "parallelism": (f"sharded by particle x{world}, all-reduce of the partial spectrum" if sharded else
+                                   f"replicas x{world}") if world > 1 else "single GPU",
                    "l2": "no explicit flush: positions differ every step and the per-step working set "
                          "(grid + spectra + particles, ~165 MB) exceeds the 126 MB L2"},
-        "evals_per_sec": world / (ms_step * 1e-3),
+        "evals_per_sec": (1 if sharded else world) / (ms_step * 1e-3),
         "energy_last_step": E_last,
         "clocks": clocks, "e2e": e2e, "gpu_launches": total_launches,
         "roofline": roofline, "stages": stages, "cpu_baseline": cpu_baseline, "comparisons": comparisons,

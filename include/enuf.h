@@ -113,6 +113,37 @@ int enuf_energy_forces(enuf_plan *plan, const void *r, const void *q, void *F, d
 int enuf_energy_forces_host(enuf_plan *plan, const void *r_host, const void *q_host,
                             void *F_host, double *E);
 
+/*
+ * Sharded evaluation over several GPUs (the paper's HP-ENUF, section III.B).
+ * The structure factor is additive over arbitrary particle subsets (Eq. 61, :533-540): every
+ * rank holds a plan with the SAME (L, alpha, k_cut, M, sigma, m, options) and its OWN particles,
+ * and one evaluation is
+ *
+ *   enuf_spectrum_partial(plan, r, q, F)       a1, a2 and the X, Y forward FFT passes on the
+ *                                              rank's particles (F of its q == 0 particles is
+ *                                              zeroed here, so F is the same buffer as below)
+ *   all-reduce (sum) over ranks of the buffer  enuf_plan_spectrum_buffer() returns: `count`
+ *                                              reals of the plan's precision, the half spectrum
+ *                                              [z][ky'][kx] (complex, kx < Kxp, ky' < 2 k_cut + 1)
+ *                                              after the X and Y passes -- linear in the charges.
+ *                                              The caller does it (ncclAllReduce / torch.distributed
+ *                                              on the plan's stream): "sums S_i(n) ... broadcasts",
+ *                                              PAPER.md:542.  With one rank it is skipped.
+ *   enuf_forces_from_spectrum(plan, F, E)      a4 .. a7 on the summed buffer: Z pass with scaling
+ *                                              and energy, inverse passes (replicated on every
+ *                                              rank), gather onto the rank's own particles.
+ *
+ * E is the energy of the WHOLE system (identical on all ranks up to nothing: same input bytes,
+ * same fixed-order reduction); F holds the forces on the rank's own particles from all
+ * particles of all ranks.  No force exchange is needed.  The device pointer returned by
+ * enuf_plan_spectrum_buffer stays valid (and the same) until an option that reallocates the
+ * workspace changes or the plan is destroyed.  enuf_forces_from_spectrum returns ENUF_ESTATE
+ * unless enuf_spectrum_partial ran directly before it on this plan.
+ */
+int enuf_spectrum_partial(enuf_plan *plan, const void *r, const void *q, void *F);
+int enuf_plan_spectrum_buffer(enuf_plan *plan, void **dev_ptr, size_t *count);
+int enuf_forces_from_spectrum(enuf_plan *plan, void *F, double *E);
+
 /* Synchronise the plan's stream and return the energy of the last evaluation. */
 int enuf_plan_energy(enuf_plan *plan, double *E);
 

@@ -30,6 +30,7 @@ SYMBOLS = (
     "enuf_plan_create", "enuf_plan_set", "enuf_plan_set_stream", "enuf_energy_forces",
     "enuf_energy_forces_host", "enuf_plan_energy", "enuf_plan_stage_ms", "enuf_plan_stage_ms_mean",
     "enuf_plan_launch_count",
+    "enuf_spectrum_partial", "enuf_plan_spectrum_buffer", "enuf_forces_from_spectrum",
     "enuf_plan_copy_field", "enuf_plan_structure_factor", "enuf_spread_only",
     "enuf_plan_workspace_bytes", "enuf_plan_destroy", "enuf_last_error",
     "enuf_ncut", "enuf_alpha_from_rc", "enuf_rc_from_ncut",
@@ -64,6 +65,10 @@ def lib():
         L.enuf_energy_forces_host.restype = i
         L.enuf_energy_forces_host.argtypes = [vp, vp, vp, vp, C.POINTER(d)]
         L.enuf_plan_energy.restype = i; L.enuf_plan_energy.argtypes = [vp, C.POINTER(d)]
+        L.enuf_spectrum_partial.restype = i; L.enuf_spectrum_partial.argtypes = [vp, vp, vp, vp]
+        L.enuf_plan_spectrum_buffer.restype = i
+        L.enuf_plan_spectrum_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_size_t)]
+        L.enuf_forces_from_spectrum.restype = i; L.enuf_forces_from_spectrum.argtypes = [vp, vp, C.POINTER(d)]
         L.enuf_plan_stage_ms.restype = i; L.enuf_plan_stage_ms.argtypes = [vp, C.POINTER(C.c_float), i]
         L.enuf_plan_stage_ms_mean.restype = i
         L.enuf_plan_stage_ms_mean.argtypes = [vp, C.POINTER(C.c_float), i, C.POINTER(i)]
@@ -100,6 +105,33 @@ def alpha_from_rc(r_c: float, delta: float) -> float:
 def rc_from_ncut(n_c: int, alpha: float, L: float) -> float:
     """Eq. 32: r_c = pi n_c / (alpha^2 L)."""
     return lib().enuf_rc_from_ncut(n_c, alpha, L)
+
+
+def shard_bounds(N: int, rank: int, world: int):
+    """[lo, hi) of the particles rank `rank` of `world` owns when N particles are split by index
+    into contiguous, near-equal shards (HP-ENUF partitions by particle)."""
+    if not (0 <= rank < world):
+        raise ValueError("rank must be in [0, world)")
+    base, rem = divmod(int(N), int(world))
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def all_reduce_sum_(t, group=None):
+    """In-place sum of a tensor over the ranks of `group` (identity without an initialised
+    process group or with one rank): the one exchange step of the sharded path."""
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return t
+
+
+class _DeviceBuffer:
+    """A plan-owned device buffer exposed through __cuda_array_interface__ (no copy)."""
+
+    def __init__(self, ptr: int, count: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (count,), "typestr": typestr, "data": (ptr, False),
+                                         "version": 2, "strides": None}
 
 
 class Plan:
@@ -181,6 +213,47 @@ class Plan:
         _check(lib().enuf_energy_forces_host(self._h, C.c_void_p(r_t.data_ptr()), C.c_void_p(q_t.data_ptr()),
                                              C.c_void_p(F.data_ptr()), C.byref(E)))
         return E.value, F
+
+    # ---- sharded evaluation (include/enuf.h, "Sharded evaluation")
+    def spectrum_partial(self, r, q, F):
+        """a1, a2 and the X, Y forward passes on this rank's particles."""
+        N = self.N
+        self._use_current_stream()
+        _check(lib().enuf_spectrum_partial(self._h, self._dev(r, (N, 3), "r"), self._dev(q, (N,), "q"),
+                                           self._dev(F, (N, 3), "F")))
+
+    def spectrum_tensor(self):
+        """The plan-owned partial-spectrum buffer as a flat CUDA tensor (a view, no copy): the
+        tensor to all-reduce (sum) over ranks between the two halves."""
+        torch = self._torch
+        ptr, cnt = C.c_void_p(), C.c_size_t(0)
+        _check(lib().enuf_plan_spectrum_buffer(self._h, C.byref(ptr), C.byref(cnt)))
+        key = (ptr.value, cnt.value)
+        if getattr(self, "_spec_key", None) != key:
+            buf = _DeviceBuffer(ptr.value, cnt.value, "<f4" if self.dtype == torch.float32 else "<f8")
+            self._spec_view = torch.as_tensor(buf, device="cuda")
+            self._spec_key = key
+        return self._spec_view
+
+    def forces_from_spectrum(self, F, want_energy=True):
+        """a4 .. a7 on the (summed) spectrum buffer; forces on this rank's particles."""
+        self._use_current_stream()
+        E = C.c_double(0.0)
+        _check(lib().enuf_forces_from_spectrum(self._h, self._dev(F, (self.N, 3), "F"),
+                                               C.byref(E) if want_energy else None))
+        return (E.value if want_energy else None), F
+
+    def energy_forces_sharded(self, r, q, F=None, group=None, want_energy=True):
+        """One evaluation of a system whose particles are spread over the ranks of `group`
+        (each rank passes its own r, q).  Returns (E of the whole system, F of the own particles)."""
+        torch = self._torch
+        if not torch.cuda.is_available():
+            raise EnufError(ECUDA, "no CUDA device available; this library has no CPU fallback")
+        if F is None:
+            F = torch.empty((self.N, 3), dtype=self.dtype, device=r.device)
+        self.spectrum_partial(r, q, F)
+        all_reduce_sum_(self.spectrum_tensor(), group)
+        return self.forces_from_spectrum(F, want_energy=want_energy)
 
     def energy(self) -> float:
         E = C.c_double(0.0)

@@ -212,6 +212,7 @@ void free_workspace(enuf_plan* p) {
     p->cell = p->idx = p->bin_count = p->bin_offset = p->bin_cursor = p->scan_total = nullptr;
     p->e_partial = p->e_dev = p->e_pinned = nullptr;
     p->events_valid = false;
+    p->partial_ready = false;
     p->allocated = false;
     p->workspace_bytes = 0;
     (void)cudaGetLastError();
@@ -314,6 +315,31 @@ int run_all(enuf_plan* p, const void* r, const void* q, void* F) {
     if (p->profile) cudaEventRecord(p->ev[0], p->stream);
     if (run_bin_spread<T>(p, r, q, F)) return -1;
     int l = enuf::launch_fft<T>(p);
+    if (l < 0) return -1;
+    p->launches += l;
+    if (p->profile) cudaEventRecord(p->ev[3], p->stream);
+    l = enuf::launch_gather<T>(p, F);
+    if (l < 0) return -1;
+    p->launches += l;
+    if (p->profile) { cudaEventRecord(p->ev[4], p->stream); cudaEventRecord(p->ev[5], p->stream); }
+    return 0;
+}
+
+// Multi-GPU halves (enuf.h, "Sharded evaluation"): a1 + a2 + the X, Y forward passes ...
+template <typename T>
+int run_partial(enuf_plan* p, const void* r, const void* q, void* F) {
+    if (p->profile) cudaEventRecord(p->ev[0], p->stream);
+    if (run_bin_spread<T>(p, r, q, F)) return -1;
+    const int l = enuf::launch_fft_forward<T>(p);
+    if (l < 0) return -1;
+    p->launches += l;
+    return 0;
+}
+
+// ... and Z forward . scale . energy . Z inverse, Y and X inverse passes, gather (a4 .. a7)
+template <typename T>
+int run_finish(enuf_plan* p, void* F) {
+    int l = enuf::launch_fft_backward<T>(p);
     if (l < 0) return -1;
     p->launches += l;
     if (p->profile) cudaEventRecord(p->ev[3], p->stream);
@@ -470,6 +496,68 @@ int enuf_energy_forces_host(enuf_plan* p, const void* r_host, const void* q_host
     CU(cudaMemcpyAsync(p->e_pinned, p->e_dev, 8, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));
     if (E) *E = *p->e_pinned;
+    return ENUF_OK;
+}
+
+int enuf_spectrum_partial(enuf_plan* p, const void* r, const void* q, void* F) {
+    g_err[0] = 0;
+    if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    if (p->N > 0 && (!r || !q || !F)) return fail(ENUF_EINVAL, "r, q and F must be non-NULL when N > 0");
+    int rc = prepare(p);
+    if (rc) return rc;
+    p->launches = 0;
+    p->partial_ready = false;
+    if (p->profile) {
+        p->ev = p->ev_ring + (p->prof_evals % enuf_plan::kProfRing) * enuf_plan::kProfEv;
+        ++p->prof_evals;
+    }
+    if (p->N == 0) {
+        // no particles on this rank: its partial spectrum is zero
+        CU(cudaMemsetAsync(p->A2[0], 0, 2 * p->esize * (size_t)p->n * p->Ky * p->Kxp, p->stream));
+        if (p->profile) for (int i = 0; i <= 2; ++i) cudaEventRecord(p->ev[i], p->stream);
+    } else {
+        rc = p->precision == ENUF_F32 ? run_partial<float>(p, r, q, F) : run_partial<double>(p, r, q, F);
+        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+    }
+    p->partial_ready = true;
+    return ENUF_OK;
+}
+
+int enuf_plan_spectrum_buffer(enuf_plan* p, void** dev_ptr, size_t* count) {
+    g_err[0] = 0;
+    if (!p || !dev_ptr || !count) return fail(ENUF_EINVAL, "plan, dev_ptr or count is NULL");
+    int rc = prepare(p);
+    if (rc) return rc;
+    *dev_ptr = p->A2[0];
+    *count = 2 * (size_t)p->n * p->Ky * p->Kxp;
+    return ENUF_OK;
+}
+
+int enuf_forces_from_spectrum(enuf_plan* p, void* F, double* E) {
+    g_err[0] = 0;
+    if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    if (!p->allocated || !p->partial_ready)
+        return fail(ENUF_ESTATE, "enuf_forces_from_spectrum needs a preceding enuf_spectrum_partial");
+    if (p->N > 0 && !F) return fail(ENUF_EINVAL, "F must be non-NULL when N > 0");
+    p->partial_ready = false;
+    const int before = p->launches;
+    int rc;
+    if (p->N == 0) {
+        // no particles to interpolate onto, but the energy of the summed spectrum is still produced
+        rc = p->precision == ENUF_F32 ? enuf::launch_fft_backward<float>(p) : enuf::launch_fft_backward<double>(p);
+        if (rc < 0) return fail_cuda(cudaGetLastError(), "kernel launch");
+        p->launches = before + rc;
+        if (p->profile) for (int i = 3; i <= ENUF_NUM_STAGES; ++i) cudaEventRecord(p->ev[i], p->stream);
+    } else {
+        rc = p->precision == ENUF_F32 ? run_finish<float>(p, F) : run_finish<double>(p, F);
+        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+    }
+    p->evaluated = true;
+    if (E) {
+        CU(cudaMemcpyAsync(p->e_pinned, p->e_dev, 8, cudaMemcpyDeviceToHost, p->stream));
+        CU(cudaStreamSynchronize(p->stream));
+        *E = *p->e_pinned;
+    }
     return ENUF_OK;
 }
 

@@ -6,5 +6,7 @@ template int configure_kernels<float>(enuf_plan*);
 template int launch_bin<float>(enuf_plan*, const void*, const void*, void*);
 template int launch_spread<float>(enuf_plan*);
 template int launch_fft<float>(enuf_plan*);
+template int launch_fft_forward<float>(enuf_plan*);
+template int launch_fft_backward<float>(enuf_plan*);
 template int launch_gather<float>(enuf_plan*, void*);
 }  // namespace enuf

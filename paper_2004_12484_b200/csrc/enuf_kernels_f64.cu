@@ -6,5 +6,7 @@ template int configure_kernels<double>(enuf_plan*);
 template int launch_bin<double>(enuf_plan*, const void*, const void*, void*);
 template int launch_spread<double>(enuf_plan*);
 template int launch_fft<double>(enuf_plan*);
+template int launch_fft_forward<double>(enuf_plan*);
+template int launch_fft_backward<double>(enuf_plan*);
 template int launch_gather<double>(enuf_plan*, void*);
 }  // namespace enuf

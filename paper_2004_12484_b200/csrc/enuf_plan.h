@@ -22,6 +22,7 @@ struct enuf_plan {
     enuf::WindowParams wp{};
     int Kxp = 0, Ky = 0;
     bool allocated = false, tables_dirty = true, evaluated = false;
+    bool partial_ready = false;    // enuf_spectrum_partial has run and enuf_forces_from_spectrum has not yet
     size_t esize = 4;              // bytes per real
     size_t workspace_bytes = 0;
     int launches = 0;
@@ -66,7 +67,9 @@ namespace enuf {
 // in cudaGetLastError().
 template <typename T> int launch_bin(enuf_plan* p, const void* r, const void* q, void* F);
 template <typename T> int launch_spread(enuf_plan* p);
-template <typename T> int launch_fft(enuf_plan* p);
+template <typename T> int launch_fft(enuf_plan* p);            // = forward + backward
+template <typename T> int launch_fft_forward(enuf_plan* p);    // X, Y forward passes -> A2[0] (partial spectrum)
+template <typename T> int launch_fft_backward(enuf_plan* p);   // Z fused + inverse passes + energy
 template <typename T> int launch_gather(enuf_plan* p, void* F);
 template <typename T> int configure_kernels(enuf_plan* p);   // opt-in shared memory sizes
 
