@@ -140,6 +140,13 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                         *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = pr;
                         int pk = bxm | (bym << 8);
                         if (kTrim) pk |= (pr.dx > (T)0 ? 1 << 16 : 0) | (pr.dy > (T)0 ? 1 << 17 : 0);
+                        // which of the four 8 x 8 warp patches the stencil touches (bits 20..23, warp order):
+                        // it covers the column cells [b - (WZ-1), b], b = bxm (trimmed: bxm - 1 + ks)
+                        const int bx2 = bxm + (kTrim ? (pr.dx > (T)0 ? 0 : -1) : 0);
+                        const int by2 = bym + (kTrim ? (pr.dy > (T)0 ? 0 : -1) : 0);
+                        const int ox = (bx2 >= 0 && bx2 - (WZ - 1) <= 7 ? 1 : 0) | (bx2 >= 8 && bx2 - (WZ - 1) <= 15 ? 2 : 0);
+                        const int oy = (by2 >= 0 && by2 - (WZ - 1) <= 7 ? 1 : 0) | (by2 >= 8 && by2 - (WZ - 1) <= 15 ? 2 : 0);
+                        pk |= ((oy & 1 ? ox : 0) | (oy & 2 ? ox << 2 : 0)) << 20;
                         sb[slot] = pk;
                     }
                 }
@@ -196,14 +203,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
             if (tid == 0) nslot_s = 0;      // every thread has read ns; the next cull starts after a barrier
             // ---- accumulate: each warp visits the staged particles that overlap its 8 x 8 cells
             for (int e0 = 0; e0 < ns; e0 += 32) {
-                bool ov = false;
-                if (e0 + lane < ns) {
-                    const int v = sb[e0 + lane];
-                    // stencil covers [b - 2m, b] in column cells; trimmed: [b - 2m + ks, b - 1 + ks]
-                    const int bx2 = (v & 255) + (kTrim ? ((v >> 16) & 1) - 1 : 0);
-                    const int by2 = ((v >> 8) & 255) + (kTrim ? ((v >> 17) & 1) - 1 : 0);
-                    ov = bx2 >= px && bx2 - (WZ - 1) <= px + 7 && by2 >= py && by2 - (WZ - 1) <= py + 7;
-                }
+                const bool ov = e0 + lane < ns && ((sb[e0 + lane] >> (20 + warp)) & 1);   // patch mask from the cull
                 const unsigned om = __ballot_sync(0xffffffffu, ov);
                 if (om == 0u) continue;
                 // compact the overlapping slots into the warp's list (padded to an even length with the
