@@ -26,8 +26,10 @@ template <> struct GatherStride<3, false> { static constexpr int SX = 23, SPL = 
 template <> struct GatherStride<4, false> { static constexpr int SX = 25, SPL = 609; };
 template <> struct GatherStride<5, false> { static constexpr int SX = 27, SPL = 713; };
 template <> struct GatherStride<6, false> { static constexpr int SX = 29, SPL = 825; };
-template <> struct GatherStride<5, true> { static constexpr int SX = 27, SPL = 718; };
-template <> struct GatherStride<6, true> { static constexpr int SX = 29, SPL = 828; };
+// Trimmed fp32 plans read the stencil rows with 8-byte loads (kPair below): even row stride, and a plane
+// stride = 8 (m = 6) / 12 (m = 5) mod 32 so that the 16 rows x 2 words of each half-warp hit 32 different banks.
+template <> struct GatherStride<5, true> { static constexpr int SX = 30, SPL = 26 * 30; };
+template <> struct GatherStride<6, true> { static constexpr int SX = 30, SPL = 28 * 30; };
 
 // kTrim (fp32 Kaiser-Bessel, m >= 5; enuf_common.cuh): the window vanishes beyond |d| = m, so of the
 // 2m+1 stencil points per dimension the outermost one on the far side of the particle carries an exact
@@ -37,6 +39,11 @@ struct GatherCfg {
     static constexpr int W = 2 * M_ + 1;
     static constexpr int WE = W - (kTrim ? 1 : 0);              // stencil points per dimension actually visited
     static constexpr int TP = kTile + 2 * M_;                   // padded tile edge
+    // kPair: the x rows of the shared tile start on an even grid column (halo XS = m rounded up to even) so
+    // that staging copies and stencil-row loads move aligned pairs (Psi[x], Psi[x+1])
+    static constexpr bool kPair = kTrim;
+    static constexpr int XS = kPair ? ((M_ + 1) & ~1) : M_;     // x halo on the low side
+    static constexpr int TPX = kTile + 2 * XS;                  // staged row length
     static constexpr int SX = GatherStride<M_, kTrim>::SX;
     static constexpr int SPL = GatherStride<M_, kTrim>::SPL;
     static constexpr int CELLS = ((TP * SPL + 3) / 4) * 4;      // shared tile size in elements (16 B multiple)
@@ -98,8 +105,32 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tx0 = Tx * kTile, ty0 = Ty * kTile, tz0 = Tz * kTile;
 
-    // ---- stage the padded tile asynchronously: one row of TP values per warp and step
-    {
+    // ---- stage the padded tile asynchronously
+    if constexpr (C::kPair && sizeof(T) == 4) {
+        // 8-byte copies: a warp takes whole planes (lz = warp, warp + WARPS, ..), each half-warp moving one
+        // row of TPX / 2 pairs per step
+        constexpr int PAIRS = C::TPX / 2;
+        const int half = lane >> 4, pxi = lane & 15;
+        int gx = tx0 - C::XS + 2 * pxi;
+        gx += gx < 0 ? g.n : 0; gx -= gx >= g.n ? g.n : 0;
+        int gy0 = ty0 - M_ + half;
+        gy0 += gy0 < 0 ? g.n : 0;
+        const size_t nn = (size_t)g.n;
+        if (pxi < PAIRS) {
+            for (int lz = warp; lz < TP; lz += C::WARPS) {
+                int gz = tz0 - M_ + lz;
+                gz += gz < 0 ? g.n : 0; gz -= gz >= g.n ? g.n : 0;
+                const T* src = field + (size_t)gz * nn * nn + gx;
+                T* dst = tile_s + lz * SPL + half * SX + 2 * pxi;
+                int gy = gy0;
+#pragma unroll
+                for (int j = 0; j < (TP + 1) / 2; ++j) {
+                    if (2 * j + 1 < TP || half == 0) cp_async_8(dst + 2 * j * SX, src + (size_t)gy * nn);
+                    gy += 2; gy -= gy >= g.n ? g.n : 0;
+                }
+            }
+        }
+    } else {
         int gx = tx0 - M_ + lane;
         gx += gx < 0 ? g.n : 0; gx -= gx >= g.n ? g.n : 0;
         for (int lz = 0; lz < TP; ++lz) {
@@ -160,7 +191,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
                 if (kTrim) {
                     cx += pr.dx > (T)0 ? 1 : 0; cy += pr.dy > (T)0 ? 1 : 0; zrel += pr.dz > (T)0 ? 1 : 0;
                 }
-                base_s[slot] = zrel * SPL + (cy - ty0) * SX + (cx - tx0);
+                base_s[slot] = zrel * SPL + (cy - ty0) * SX + (cx - tx0) + (C::XS - M_);
                 q_s[slot] = pre * pr.q;
                 idx_s[slot] = (int)idx[start + p0 + slot];
             }
@@ -191,26 +222,64 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
                     wx[2 * v].x = t4.x; wx[2 * v].y = t4.y; wx[2 * v + 1].x = t4.z; wx[2 * v + 1].y = t4.w;
                 }
             }
-            const T* origin = tile_s + base_s[slot];
+            const int base = base_s[slot];
+            const T* origin = tile_s + base;
             T fx = (T)0, fy = (T)0, fz = (T)0;
+            // one stencil row: s = sum_k (phi, phi')[k] * v[k], then the y, z weights of the row
+            auto finish_row = [&](int it, const T (&v)[WE]) {
+                P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
 #pragma unroll
-            for (int it = 0; it < ITER; ++it) {
-                if (it + 1 < ITER || lane + 32 * it < WE * WE) {
-                    const T* row = origin + rowoff[it];
-                    P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
+                for (int k = 0; k < WE; ++k) {
+                    if (k & 1) fma_pair(sb2, wx[k], v[k]);
+                    else fma_pair(sa, wx[k], v[k]);
+                }
+                const T s0 = sa.x + sb2.x, s1 = sa.y + sb2.y;
+                const P2 wy = wt[ryo[it]], wz = wt[rzo[it]];
+                if (kIk) {
+                    fx += s0 * (wy.x * wz.x);
+                } else {
+                    fx += s1 * (wy.x * wz.x);
+                    fy += s0 * (wy.y * wz.x);
+                    fz += s0 * (wy.x * wz.y);
+                }
+            };
+            if constexpr (C::kPair && sizeof(T) == 4) {
+                // 8-byte loads of aligned pairs; the row starts on an even or an odd column (warp-uniform)
+                if ((base & 1) == 0) {
 #pragma unroll
-                    for (int k = 0; k < WE; ++k) {
-                        if (k & 1) fma_pair(sb2, wx[k], row[k]);
-                        else fma_pair(sa, wx[k], row[k]);
+                    for (int it = 0; it < ITER; ++it) {
+                        if (it + 1 < ITER || lane + 32 * it < WE * WE) {
+                            const P2* row = reinterpret_cast<const P2*>(origin + rowoff[it]);
+                            T v[WE];
+#pragma unroll
+                            for (int j = 0; j < WE / 2; ++j) { const P2 t2 = row[j]; v[2 * j] = t2.x; v[2 * j + 1] = t2.y; }
+                            finish_row(it, v);
+                        }
                     }
-                    const T s0 = sa.x + sb2.x, s1 = sa.y + sb2.y;
-                    const P2 wy = wt[ryo[it]], wz = wt[rzo[it]];
-                    if (kIk) {
-                        fx += s0 * (wy.x * wz.x);
-                    } else {
-                        fx += s1 * (wy.x * wz.x);
-                        fy += s0 * (wy.y * wz.x);
-                        fz += s0 * (wy.x * wz.y);
+                } else {
+#pragma unroll
+                    for (int it = 0; it < ITER; ++it) {
+                        if (it + 1 < ITER || lane + 32 * it < WE * WE) {
+                            const T* rowf = origin + rowoff[it];
+                            const P2* row = reinterpret_cast<const P2*>(rowf + 1);
+                            T v[WE];
+                            v[0] = rowf[0];
+#pragma unroll
+                            for (int j = 0; j < WE / 2 - 1; ++j) { const P2 t2 = row[j]; v[2 * j + 1] = t2.x; v[2 * j + 2] = t2.y; }
+                            v[WE - 1] = rowf[WE - 1];
+                            finish_row(it, v);
+                        }
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int it = 0; it < ITER; ++it) {
+                    if (it + 1 < ITER || lane + 32 * it < WE * WE) {
+                        const T* row = origin + rowoff[it];
+                        T v[WE];
+#pragma unroll
+                        for (int k = 0; k < WE; ++k) v[k] = row[k];
+                        finish_row(it, v);
                     }
                 }
             }
