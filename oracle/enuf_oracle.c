@@ -15,7 +15,11 @@
  *             (PAPER.md:491-499 spreading / FFT / scaling, subdividing / inverse FFT /
  *             interpolating), both force variants.
  *   Helpers   real-space + self energy (Eq. 17, 24, 25) used
- *             only by the Madelung / Wigner pins; the parameter rule Eq. 31-32 (:256-259).
+ *             by the Madelung / Wigner pins; the parameter rule Eq. 31-32 (:256-259).
+ *   Oracle R  (orc_real_forces)  the real-space part of the Ewald sum, energy per particle
+ *             and forces (Eq. 16-17, 29) with the Slater factors
+ *             B_U, B_F of Eq. 57-58 (:434-436); pinned by finite differences of the
+ *             Madelung-pinned orc_real_energy, Newton's third law, Eq. 59-60 limits.
  *
  * Pins (tests/test_oracle_pins.py): rock-salt Madelung constant, cubic Wigner constant,
  * alpha-independence of the total energy, forces = -dE/dr by central differences,
@@ -309,6 +313,64 @@ double orc_self_energy(int64_t N, const double *q, double alpha)
     double s = 0.0;
     for (int64_t i = 0; i < N; ++i) s += q[i] * q[i];
     return alpha / sqrt(ORC_PI) * s;
+}
+
+/* Slater correction factors of the real-space pair energy and force, Eq. 57-58
+ * with beta r* = d/lambda; lambda = 0: point charges, both 1.      */
+double orc_slater_BU(double d, double lambda)
+{
+    if (lambda <= 0.0) return 1.0;
+    double x = d / lambda;
+    return 1.0 - (1.0 + x) * exp(-2.0 * x);
+}
+
+double orc_slater_BF(double d, double lambda)
+{
+    if (lambda <= 0.0) return 1.0;
+    double x = d / lambda;
+    return 1.0 - (1.0 + 2.0 * x * (1.0 + x)) * exp(-2.0 * x);
+}
+
+/* Real-space (short-range) Ewald part on a sample of particles (all if ns == 0):
+ *   e_i = 1/2 q_i sum'_{j,n} q_j B_U(d) erfc(alpha d)/d                 (Eq. 16-17)
+ *   F_i = q_i sum'_{j,n} q_j B_F(d) [erfc(alpha d)/d^2 + (2 alpha/sqrt(pi)) exp(-alpha^2 d^2)/d] dvec/d
+ * with dvec = r_i - r_j - nL, d = |dvec| <= r_cut, images |n_t| <= shells, the prime dropping
+ * i = j in the home cell.  Eq. 29 prints the bracket without q_i, the unit
+ * vector and the 1/d of the Gaussian term (reading R24: the bracket above is -d/dd of
+ * erfc(alpha d)/d; pinned by finite differences of orc_real_energy).  B_U, B_F scale the
+ * real-space energy and force terms as the paper states ("B_U and B_F are only applied on
+ * real space summations"); lambda = 0 switches them off.
+ * Sum_i e_i over all particles is the real-space energy.  F is ns x 3 (or N x 3).      */
+void orc_real_forces(int64_t N, const double *r, const double *q, double L, double alpha,
+                     double r_cut, int shells, double lambda, int64_t ns, const int64_t *sample,
+                     double *F, double *e)
+{
+    const int64_t cnt = ns ? ns : N;
+    const double two_a_sqrtpi = 2.0 * alpha / sqrt(ORC_PI);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t t = 0; t < cnt; ++t) {
+        const int64_t i = ns ? sample[t] : t;
+        double fx = 0.0, fy = 0.0, fz = 0.0, ei = 0.0;
+        for (int64_t j = 0; j < N; ++j)
+            for (int a = -shells; a <= shells; ++a)
+                for (int b = -shells; b <= shells; ++b)
+                    for (int c = -shells; c <= shells; ++c) {
+                        if (i == j && a == 0 && b == 0 && c == 0) continue;
+                        double dx = r[3 * i] - r[3 * j] - a * L;
+                        double dy = r[3 * i + 1] - r[3 * j + 1] - b * L;
+                        double dz = r[3 * i + 2] - r[3 * j + 2] - c * L;
+                        double d2 = dx * dx + dy * dy + dz * dz;
+                        if (d2 > r_cut * r_cut) continue;
+                        double d = sqrt(d2);
+                        double ec = erfc(alpha * d);
+                        ei += q[j] * orc_slater_BU(d, lambda) * ec / d;
+                        double g = orc_slater_BF(d, lambda)
+                                   * (ec / d2 + two_a_sqrtpi * exp(-alpha * alpha * d2) / d) / d;
+                        fx += q[j] * g * dx; fy += q[j] * g * dy; fz += q[j] * g * dz;
+                    }
+        if (F) { F[3 * t] = q[i] * fx; F[3 * t + 1] = q[i] * fy; F[3 * t + 2] = q[i] * fz; }
+        if (e) e[t] = 0.5 * q[i] * ei;
+    }
 }
 
 /* ------------------------------------------------------------------ Oracle B */

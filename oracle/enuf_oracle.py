@@ -57,6 +57,10 @@ def lib():
         L.orc_slater_f2.restype = d; L.orc_slater_f2.argtypes = [i, d, d]
         L.orc_ncut.restype = i; L.orc_ncut.argtypes = [d, d, d]
         L.orc_alpha_from_rc.restype = d; L.orc_alpha_from_rc.argtypes = [d, d]
+        L.orc_slater_BU.restype = d; L.orc_slater_BU.argtypes = [d, d]
+        L.orc_slater_BF.restype = d; L.orc_slater_BF.argtypes = [d, d]
+        L.orc_real_forces.restype = None
+        L.orc_real_forces.argtypes = [i64, p, p, d, d, d, i, d, i64, pi64, p, p]
         L.orc_direct_S.restype = None
         L.orc_direct_S.argtypes = [i64, p, p, d, i64, pi32, p, p]
         L.orc_modes.restype = i64; L.orc_modes.argtypes = [i, pi32]
@@ -152,6 +156,29 @@ def direct(r, q, L, alpha, k_cut, slater_lambda=0.0, forces=True, sample=None):
 def real_energy(r, q, L, alpha, r_cut, shells=1):
     r, q = _f64(r), _f64(q)
     return lib().orc_real_energy(q.shape[0], _dp(r), _dp(q), L, alpha, r_cut, shells)
+
+
+def slater_BU(d, lam):
+    return lib().orc_slater_BU(float(d), float(lam))
+
+
+def slater_BF(d, lam):
+    return lib().orc_slater_BF(float(d), float(lam))
+
+
+def real_forces(r, q, L, alpha, r_cut, shells=1, slater_lambda=0.0, sample=None):
+    """Oracle R: real-space Ewald part. Returns (e_i, F) for all particles or for `sample`;
+    e_i = 1/2 q_i sum_j q_j B_U erfc(alpha d)/d, so e_i summed over ALL particles is E_real."""
+    r, q = _f64(r), _f64(q)
+    N = q.shape[0]
+    ns, sp = 0, None
+    if sample is not None:
+        sample = np.ascontiguousarray(np.asarray(sample, dtype=np.int64))
+        ns, sp = sample.shape[0], sample.ctypes.data_as(C.POINTER(C.c_int64))
+    cnt = ns if ns else N
+    F = np.zeros((cnt, 3)); e = np.zeros(cnt)
+    lib().orc_real_forces(N, _dp(r), _dp(q), L, alpha, r_cut, shells, slater_lambda, ns, sp, _dp(F), _dp(e))
+    return e, F
 
 
 def self_energy(q, alpha):

@@ -360,3 +360,68 @@ def test_predicted_error_cfg2(oracle):
         out = oracle.enuf_workload(w, variant=variant)
         assert abs(out["E"] - Ea) < 1e-10 * abs(Ea)
         assert _rel_rms(out["F"], Fa) < tol
+
+
+# ------------------------------------------------------------------ Oracle R (real-space part)
+
+def test_real_forces_are_minus_gradient_of_pinned_energy(oracle):
+    """Eq. 29 (garbled; reading R24): F_i^R = -dU^R/dr_i, with U^R the real-space
+    energy that the Madelung / Wigner pins fix.  Central differences, images included."""
+    L, alpha, rc = 3.0, 1.3, 4.0
+    r, q = random_neutral_gas(20, L, seed=5)
+    e_i, F = oracle.real_forces(r, q, L, alpha, rc, shells=2)
+    assert abs(e_i.sum() - oracle.real_energy(r, q, L, alpha, rc, 2)) <= 1e-13 * abs(e_i.sum())
+    # cutoff-crossing pairs make U^R discontinuous at the 1e-7 level only if a pair sits within h of r_cut
+    h = 1e-5
+    for i in (0, 7, 19):
+        for t in range(3):
+            rp, rm = r.copy(), r.copy()
+            rp[i, t] += h; rm[i, t] -= h
+            fd = -(oracle.real_energy(rp, q, L, alpha, rc, 2) - oracle.real_energy(rm, q, L, alpha, rc, 2)) / (2 * h)
+            assert abs(fd - F[i, t]) <= 2e-7 * np.abs(F).max() + 5e-6 * math.erfc(alpha * rc)
+
+
+def test_real_forces_newton_third_law_and_two_particles(oracle):
+    L, alpha = 10.0, 0.4
+    r, q = random_neutral_gas(50, L, seed=9)
+    _, F = oracle.real_forces(r, q, L, alpha, L / 2)
+    assert np.abs(F.sum(axis=0)).max() <= 1e-13 * np.abs(F).max()
+    # two opposite charges at distance d along x: F_0 = -q^2 [erfc(a d)/d^2 + 2a/sqrt(pi) exp(-a^2 d^2)/d] (attractive)
+    d = 1.7
+    r2 = np.array([[1.0, 2.0, 3.0], [1.0 + d, 2.0, 3.0]]); q2 = np.array([1.0, -1.0])
+    e2, F2 = oracle.real_forces(r2, q2, L, alpha, 4.0)
+    mag = math.erfc(alpha * d) / d ** 2 + 2 * alpha / math.sqrt(math.pi) * math.exp(-(alpha * d) ** 2) / d
+    assert F2[0, 0] == pytest.approx(mag, rel=1e-14) and F2[1, 0] == pytest.approx(-mag, rel=1e-14)
+    assert np.abs(F2[:, 1:]).max() == 0.0
+    assert e2.sum() == pytest.approx(-math.erfc(alpha * d) / d, rel=1e-14)
+
+
+def test_real_forces_sample_matches_full(oracle):
+    L, alpha = 6.0, 0.8
+    r, q = random_neutral_gas(64, L, seed=3)
+    e, F = oracle.real_forces(r, q, L, alpha, 3.0)
+    es, Fs = oracle.real_forces(r, q, L, alpha, 3.0, sample=[5, 0, 63])
+    assert np.array_equal(Fs, F[[5, 0, 63]]) and np.array_equal(es, e[[5, 0, 63]])
+
+
+def test_slater_real_space_factors(oracle):
+    """Eq. 57-60 (PAPER.md:434-442): B_U/r -> 1/lambda and B_F -> 0 as r -> 0; B_U, B_F -> 1 at large r;
+    Eq. 53 -> 54: -d/dr [B_U(r)/r] = B_F(r)/r^2 (central differences); lambda = 0 is the point charge."""
+    lam = 0.25
+    for d in (1e-6, 1e-5):
+        assert oracle.slater_BU(d, lam) / d == pytest.approx(1.0 / lam, rel=1e-4)
+        assert abs(oracle.slater_BF(d, lam)) < 1e-8
+    assert oracle.slater_BU(40 * lam, lam) == pytest.approx(1.0, abs=1e-30 + 1e-15)
+    assert oracle.slater_BF(40 * lam, lam) == pytest.approx(1.0, abs=1e-15)
+    assert oracle.slater_BU(0.7, 0.0) == 1.0 and oracle.slater_BF(0.7, 0.0) == 1.0
+    h = 1e-6
+    for d in (0.05, 0.2, 0.6, 1.5):
+        dU = (oracle.slater_BU(d + h, lam) / (d + h) - oracle.slater_BU(d - h, lam) / (d - h)) / (2 * h)
+        assert -dU == pytest.approx(oracle.slater_BF(d, lam) / d ** 2, rel=2e-8)
+    # beta = R_c/lambda = 1.125 (PAPER.md:446): B_U, B_F "converge to unity when r >= 3.0 R_c" (:463): 0.5 % and 3.6 % off
+    assert abs(oracle.slater_BU(3.0, 1 / 1.125) - 1) < 1e-2 and abs(oracle.slater_BF(3.0, 1 / 1.125) - 1) < 5e-2
+    # in the pair sum the factors multiply the energy and force terms (two particles, alpha -> 0: erfc -> 1)
+    r2 = np.array([[0.0, 0.0, 0.0], [0.3, 0.0, 0.0]]); q2 = np.array([1.0, 1.0])
+    e2, F2 = oracle.real_forces(r2, q2, 50.0, 1e-9, 1.0, slater_lambda=lam)
+    assert e2.sum() == pytest.approx(oracle.slater_BU(0.3, lam) / 0.3, rel=1e-8)
+    assert F2[1, 0] == pytest.approx(oracle.slater_BF(0.3, lam) / 0.09, rel=1e-8)
