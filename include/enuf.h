@@ -144,6 +144,28 @@ int enuf_spectrum_partial(enuf_plan *plan, const void *r, const void *q, void *F
 int enuf_plan_spectrum_buffer(enuf_plan *plan, void **dev_ptr, size_t *count);
 int enuf_forces_from_spectrum(enuf_plan *plan, void *F, double *E);
 
+/*
+ * Real-space (short-range) part of the Ewald sum and the self term -- the other two terms of
+ * Eq. 25, so that E_total = E_real + E_rec - E_self on the device:
+ *   E_real = 1/2 sum'_{i,j} q_i q_j B_U(d) erfc(alpha d)/d    over minimum-image pairs with d <= r_cut
+ *            (Eq. 16-17, :176-181)
+ *   F_i    = q_i sum'_j q_j B_F(d) [erfc(alpha d)/d^2 + (2 alpha/sqrt(pi)) exp(-alpha^2 d^2)/d] (r_i-r_j)/d
+ *            (Eq. 29, :243 -- printed without q_i, the unit vector and the 1/d of the Gaussian term;
+ *            the bracket here is -d/dd [erfc(alpha d)/d], reading R24)
+ *   E_self = (alpha/sqrt(pi)) sum_i q_i^2                      (Eq. 24, :216; SUBTRACTED in Eq. 25, R13)
+ * B_U, B_F are the Slater factors of Eq. 57-58 (:434-436) with r/lambda, lambda = ENUF_OPT_SLATER_LAMBDA;
+ * lambda = 0 (default): point charges, B_U = B_F = 1.  Particles are sorted into a linked-cell list
+ * with cells smaller than the cutoff (the paper's "Near Distance" scheme, :511-515).
+ *   r, q       device pointers as in enuf_energy_forces (plan's N, L, alpha, precision, stream)
+ *   r_cut      real-space cutoff, 0 < r_cut <= L/2 (minimum image)
+ *   accumulate 0: F is OVERWRITTEN with the real-space forces (F = 0 for q == 0 particles);
+ *              1: they are ADDED to F (e.g. after enuf_energy_forces wrote the reciprocal part)
+ *   F          device pointer N x 3, caller's particle order
+ *   E_real, E_self  host pointers or NULL; if either is non-NULL the stream is synchronised.
+ */
+int enuf_real_space(enuf_plan *plan, const void *r, const void *q, double r_cut, int accumulate,
+                    void *F, double *E_real, double *E_self);
+
 /* Synchronise the plan's stream and return the energy of the last evaluation. */
 int enuf_plan_energy(enuf_plan *plan, double *E);
 

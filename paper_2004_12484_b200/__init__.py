@@ -31,6 +31,7 @@ SYMBOLS = (
     "enuf_energy_forces_host", "enuf_plan_energy", "enuf_plan_stage_ms", "enuf_plan_stage_ms_mean",
     "enuf_plan_launch_count",
     "enuf_spectrum_partial", "enuf_plan_spectrum_buffer", "enuf_forces_from_spectrum",
+    "enuf_real_space",
     "enuf_plan_copy_field", "enuf_plan_structure_factor", "enuf_spread_only",
     "enuf_plan_workspace_bytes", "enuf_plan_destroy", "enuf_last_error",
     "enuf_ncut", "enuf_alpha_from_rc", "enuf_rc_from_ncut",
@@ -65,6 +66,8 @@ def lib():
         L.enuf_energy_forces_host.restype = i
         L.enuf_energy_forces_host.argtypes = [vp, vp, vp, vp, C.POINTER(d)]
         L.enuf_plan_energy.restype = i; L.enuf_plan_energy.argtypes = [vp, C.POINTER(d)]
+        L.enuf_real_space.restype = i
+        L.enuf_real_space.argtypes = [vp, vp, vp, d, i, vp, C.POINTER(d), C.POINTER(d)]
         L.enuf_spectrum_partial.restype = i; L.enuf_spectrum_partial.argtypes = [vp, vp, vp, vp]
         L.enuf_plan_spectrum_buffer.restype = i
         L.enuf_plan_spectrum_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_size_t)]
@@ -254,6 +257,24 @@ class Plan:
         self.spectrum_partial(r, q, F)
         all_reduce_sum_(self.spectrum_tensor(), group)
         return self.forces_from_spectrum(F, want_energy=want_energy)
+
+    def real_space(self, r, q, r_cut, F=None, accumulate=False, want_energy=True):
+        """Real-space Ewald part and self term (enuf_real_space). Returns (E_real, E_self, F);
+        with accumulate=True the forces are added to F."""
+        torch = self._torch
+        if not torch.cuda.is_available():
+            raise EnufError(ECUDA, "no CUDA device available; this library has no CPU fallback")
+        N = self.N
+        if F is None:
+            if accumulate:
+                raise ValueError("accumulate=True needs F")
+            F = torch.empty((N, 3), dtype=self.dtype, device=r.device)
+        self._use_current_stream()
+        Er, Es = C.c_double(0.0), C.c_double(0.0)
+        _check(lib().enuf_real_space(self._h, self._dev(r, (N, 3), "r"), self._dev(q, (N,), "q"), float(r_cut),
+                                     int(bool(accumulate)), self._dev(F, (N, 3), "F"),
+                                     C.byref(Er) if want_energy else None, C.byref(Es) if want_energy else None))
+        return (Er.value if want_energy else None), (Es.value if want_energy else None), F
 
     def energy(self) -> float:
         E = C.c_double(0.0)

@@ -200,6 +200,12 @@ void free_workspace(enuf_plan* p) {
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev);
     fr(p->r_stage); fr(p->q_stage); fr(p->F_stage);
+    fr(p->real_pos); fr(p->real_idx); fr(p->real_count); fr(p->real_offset); fr(p->real_cursor);
+    fr(p->real_scan_total); fr(p->real_partial); fr(p->real_e_dev);
+    if (p->real_e_pinned) cudaFreeHost(p->real_e_pinned);
+    p->real_pos = nullptr; p->real_idx = p->real_count = p->real_offset = p->real_cursor = p->real_scan_total = nullptr;
+    p->real_partial = p->real_e_dev = p->real_e_pinned = nullptr;
+    p->real_ncells_cap = 0;
     if (p->e_pinned) cudaFreeHost(p->e_pinned);
     if (p->ev_ring) {
         for (int i = 0; i < enuf_plan::kProfRing * enuf_plan::kProfEv; ++i)
@@ -557,6 +563,63 @@ int enuf_forces_from_spectrum(enuf_plan* p, void* F, double* E) {
         CU(cudaMemcpyAsync(p->e_pinned, p->e_dev, 8, cudaMemcpyDeviceToHost, p->stream));
         CU(cudaStreamSynchronize(p->stream));
         *E = *p->e_pinned;
+    }
+    return ENUF_OK;
+}
+
+int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, int accumulate, void* F,
+                    double* E_real, double* E_self) {
+    g_err[0] = 0;
+    if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    if (p->N > 0 && (!r || !q || !F)) return fail(ENUF_EINVAL, "r, q and F must be non-NULL when N > 0");
+    if (!(r_cut > 0) || !(r_cut <= 0.5 * p->L))
+        return fail(ENUF_EINVAL, "r_cut = %g must satisfy 0 < r_cut <= L/2 = %g (minimum image)", r_cut, 0.5 * p->L);
+    int rc = prepare(p);
+    if (rc) return rc;
+    // cells of side L/ncd >= r_cut/2, neighbour range s = 2 cells, needs 2 s + 1 <= ncd; smaller boxes
+    // (r_cut > 0.4 L) use one cell, i.e. all minimum-image pairs.  The table is capped at 256^3 cells
+    // (cells then are larger than needed, which is still correct).
+    int s = 2, ncd = (int)std::floor(2.0 * p->L / r_cut);
+    if (ncd < 5) { s = 0; ncd = 1; }
+    if (ncd > 256) ncd = 256;
+    const int ncells = ncd * ncd * ncd;
+    const size_t cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1), es = p->esize;
+    if (!p->real_pos) {
+        if ((rc = dev_alloc(p, &p->real_pos, 4 * es * cap))) return rc;
+        if ((rc = dev_alloc(p, (void**)&p->real_idx, 4 * cap))) return rc;
+        if ((rc = dev_alloc(p, (void**)&p->real_partial, 16 * ((cap + 127) / 128)))) return rc;
+        if ((rc = dev_alloc(p, (void**)&p->real_e_dev, 16))) return rc;
+        if (cudaMallocHost((void**)&p->real_e_pinned, 16) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return fail(ENUF_ENOMEM, "cudaMallocHost failed");
+        }
+    }
+    if (ncells > p->real_ncells_cap) {
+        CU(cudaStreamSynchronize(p->stream));
+        if (p->real_count) { cudaFree(p->real_count); cudaFree(p->real_offset); cudaFree(p->real_cursor); cudaFree(p->real_scan_total); }
+        p->real_count = p->real_offset = p->real_cursor = p->real_scan_total = nullptr;
+        p->real_ncells_cap = 0;
+        if ((rc = dev_alloc(p, (void**)&p->real_count, 4 * (size_t)ncells))) return rc;
+        if ((rc = dev_alloc(p, (void**)&p->real_offset, 4 * ((size_t)ncells + 1)))) return rc;
+        if ((rc = dev_alloc(p, (void**)&p->real_cursor, 4 * (size_t)ncells))) return rc;
+        if ((rc = dev_alloc(p, (void**)&p->real_scan_total, 4 * (((size_t)ncells + 1023) / 1024)))) return rc;
+        p->real_ncells_cap = ncells;
+    }
+    p->real_ncd = ncd; p->real_s = s;
+    p->launches = 0;
+    if (p->N == 0) {
+        CU(cudaMemsetAsync(p->real_e_dev, 0, 16, p->stream));
+    } else {
+        const int l = p->precision == ENUF_F32 ? enuf::launch_real<float>(p, r, q, r_cut, accumulate, F)
+                                               : enuf::launch_real<double>(p, r, q, r_cut, accumulate, F);
+        if (l < 0) return fail_cuda(cudaGetLastError(), "kernel launch");
+        p->launches = l;
+    }
+    if (E_real || E_self) {
+        CU(cudaMemcpyAsync(p->real_e_pinned, p->real_e_dev, 16, cudaMemcpyDeviceToHost, p->stream));
+        CU(cudaStreamSynchronize(p->stream));
+        if (E_real) *E_real = p->real_e_pinned[0];
+        if (E_self) *E_self = p->real_e_pinned[1];
     }
     return ENUF_OK;
 }

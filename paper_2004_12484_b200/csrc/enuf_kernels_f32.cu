@@ -9,4 +9,5 @@ template int launch_fft<float>(enuf_plan*);
 template int launch_fft_forward<float>(enuf_plan*);
 template int launch_fft_backward<float>(enuf_plan*);
 template int launch_gather<float>(enuf_plan*, void*);
+template int launch_real<float>(enuf_plan*, const void*, const void*, double, int, void*);
 }  // namespace enuf

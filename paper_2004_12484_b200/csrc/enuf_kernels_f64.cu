@@ -9,4 +9,5 @@ template int launch_fft<double>(enuf_plan*);
 template int launch_fft_forward<double>(enuf_plan*);
 template int launch_fft_backward<double>(enuf_plan*);
 template int launch_gather<double>(enuf_plan*, void*);
+template int launch_real<double>(enuf_plan*, const void*, const void*, double, int, void*);
 }  // namespace enuf

@@ -7,6 +7,7 @@
 #include "enuf_fft.cuh"
 #include "enuf_gather.cuh"
 #include "enuf_plan.h"
+#include "enuf_real.cuh"
 #include "enuf_spread.cuh"
 
 namespace enuf {
@@ -233,6 +234,38 @@ int launch_gather(enuf_plan* p, void* F) {
     });
     if (launches < 0) return -1;
     return cudaGetLastError() == cudaSuccess ? launches : -1;
+}
+
+template <typename T>
+int launch_real(enuf_plan* p, const void* r, const void* q, double r_cut, int accumulate, void* F) {
+    cudaStream_t s = p->stream;
+    const int64_t N = p->N;
+    const RealGeom g{p->real_ncd, p->real_s, p->L};
+    const int ncells = g.ncd * g.ncd * g.ncd;
+    using V4 = typename Vec4<T>::type;
+    if (cudaMemsetAsync(p->real_count, 0, sizeof(uint32_t) * ncells, s) != cudaSuccess) return -1;
+    const unsigned blocks = (unsigned)((N + 255) / 256);
+    const unsigned sblocks = (unsigned)((ncells + kScanChunk - 1) / kScanChunk);
+    real_count_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), static_cast<T*>(F),
+                                                accumulate ? 0 : 1, N, g, p->real_count);
+    bin_scan_totals_kernel<<<sblocks, kScanThreads, 0, s>>>(p->real_count, ncells, p->real_scan_total);
+    bin_scan_apply_kernel<<<sblocks, kScanThreads, 0, s>>>(p->real_count, ncells, p->real_scan_total, p->real_offset,
+                                                          p->real_cursor);
+    real_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, g,
+                                                  p->real_cursor, static_cast<V4*>(p->real_pos), p->real_idx);
+    const unsigned fblocks = (unsigned)((N + kRealThreads - 1) / kRealThreads);
+    const T alpha = (T)p->alpha, rc2 = (T)(r_cut * r_cut);
+    if (p->lambda > 0.0)
+        real_force_kernel<T, true><<<fblocks, kRealThreads, 0, s>>>(
+            static_cast<const V4*>(p->real_pos), p->real_idx, p->real_offset, ncells, g, alpha, rc2,
+            (T)(1.0 / p->lambda), accumulate, static_cast<T*>(F), p->real_partial);
+    else
+        real_force_kernel<T, false><<<fblocks, kRealThreads, 0, s>>>(
+            static_cast<const V4*>(p->real_pos), p->real_idx, p->real_offset, ncells, g, alpha, rc2, (T)0,
+            accumulate, static_cast<T*>(F), p->real_partial);
+    real_energy_finish_kernel<<<1, 256, 0, s>>>(p->real_partial, (int)fblocks, 0.5,
+                                               p->alpha * 0.56418958354775628694807945156077, p->real_e_dev);
+    return cudaGetLastError() == cudaSuccess ? 6 : -1;
 }
 
 }  // namespace enuf

@@ -48,6 +48,18 @@ struct enuf_plan {
     int n_partial = 0;
     double* e_dev = nullptr;       // [1]
     double* e_pinned = nullptr;    // [1] host
+    // real-space part (enuf_real_space; allocated at its first call)
+    void* real_pos = nullptr;         // Vec4<T>[N_cap]: wrapped position + charge, cell order
+    uint32_t* real_idx = nullptr;     // [N_cap] caller index
+    uint32_t* real_count = nullptr;   // [real_ncells]
+    uint32_t* real_offset = nullptr;  // [real_ncells + 1]
+    uint32_t* real_cursor = nullptr;  // [real_ncells]
+    uint32_t* real_scan_total = nullptr;
+    double* real_partial = nullptr;   // [2 * ceil(N_cap / 128)]
+    double* real_e_dev = nullptr;     // [2] E_real, E_self
+    double* real_e_pinned = nullptr;  // [2] host
+    int real_ncells_cap = 0;          // cells the count/offset/cursor buffers hold
+    int real_ncd = 0, real_s = 0;     // geometry of the last call
     void* r_stage = nullptr;       // host-API staging: r, q, F
     void* q_stage = nullptr;
     void* F_stage = nullptr;
@@ -72,5 +84,7 @@ template <typename T> int launch_fft_forward(enuf_plan* p);    // X, Y forward p
 template <typename T> int launch_fft_backward(enuf_plan* p);   // Z fused + inverse passes + energy
 template <typename T> int launch_gather(enuf_plan* p, void* F);
 template <typename T> int configure_kernels(enuf_plan* p);   // opt-in shared memory sizes
+// real-space part: cell sort + pair kernel + energy reduction (enuf_real.cuh)
+template <typename T> int launch_real(enuf_plan* p, const void* r, const void* q, double r_cut, int accumulate, void* F);
 
 }  // namespace enuf
