@@ -408,6 +408,19 @@ def run_ours(args):
         comparisons[other + "_variant"] = {"ms_per_step": c0.elapsed_time(c1) / Kc,
                                            "stages_ms": {k: st2[k] for k in ("bin", "spread", "fft", "gather")}}
         plan2.close()
+        # (3) the other two terms of Eq. 25 on the device (not part of the metric): real-space
+        #     sum at the cutoff the config tunes alpha for, self term; forces accumulated onto the reciprocal ones
+        r_cut = w.meta.get("r_c")
+        if r_cut and r_cut <= 0.5 * w.L and not sharded:
+            for s_ in range(2):
+                plan.real_space(pos_dev[s_], q_dev, r_cut, F=F_dev, accumulate=True, want_energy=False)
+            torch.cuda.synchronize(); c0.record()
+            for s_ in range(5):
+                plan.real_space(pos_dev[W + s_], q_dev, r_cut, F=F_dev, accumulate=True, want_energy=False)
+            c1.record(); torch.cuda.synchronize()
+            E_real, E_self, _ = plan.real_space(pos_dev[W + K - 1], q_dev, r_cut, F=F_dev, accumulate=True)
+            comparisons["real_space"] = {"ms_per_step": c0.elapsed_time(c1) / 5, "r_cut": r_cut, "E_real": E_real,
+                                         "E_self": E_self, "E_total_last_step": E_real + E_last - E_self}
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
