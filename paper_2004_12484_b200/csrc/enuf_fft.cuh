@@ -23,10 +23,29 @@
 namespace enuf {
 
 template <typename T> __device__ __forceinline__ Cx<T> cx_make(T a, T b) { Cx<T> r; r.x = a; r.y = b; return r; }
-template <typename C> __device__ __forceinline__ C cx_add(C a, C b) { a.x += b.x; a.y += b.y; return a; }
-template <typename C> __device__ __forceinline__ C cx_sub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
-template <typename C> __device__ __forceinline__ C cx_mul(C a, C b) {
-    C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+// Complex arithmetic.  fp32 uses the packed two-lane instructions of sm_100a (FADD2 / FMUL2 / FFMA2 on
+// (re, im) register pairs): a complex add or subtract is one instruction, a complex multiply two.
+__device__ __forceinline__ double2 cx_add(double2 a, double2 b) { a.x += b.x; a.y += b.y; return a; }
+__device__ __forceinline__ double2 cx_sub(double2 a, double2 b) { a.x -= b.x; a.y -= b.y; return a; }
+__device__ __forceinline__ double2 cx_mul(double2 a, double2 b) {
+    double2 r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+__device__ __forceinline__ float2 cx_add(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 cx_sub(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
+// a * b = a.x (b.x, b.y) + a.y (-b.y, b.x)
+__device__ __forceinline__ float2 cx_mul(float2 a, float2 b) {
+    const float2 r = __fmul2_rn(b, make_float2(a.x, a.x));
+    return __ffma2_rn(make_float2(-b.y, b.x), make_float2(a.y, a.y), r);
+}
+__device__ __forceinline__ float2 cx_scale(float2 a, float f) { return __fmul2_rn(a, make_float2(f, f)); }
+__device__ __forceinline__ double2 cx_scale(double2 a, double f) { a.x *= f; a.y *= f; return a; }
+// d * (c + i s), c and s compile-time constants after unrolling
+__device__ __forceinline__ float2 cx_mul_const(float2 d, float c, float s) {
+    const float2 r = __fmul2_rn(make_float2(c, s), make_float2(d.x, d.x));
+    return __ffma2_rn(make_float2(-s, c), make_float2(d.y, d.y), r);
+}
+__device__ __forceinline__ double2 cx_mul_const(double2 d, double c, double s) {
+    double2 r; r.x = d.x * c - d.y * s; r.y = d.x * s + d.y * c; return r;
 }
 
 // d * exp(SIGN * 2 pi i t / 16), t a compile-time constant after unrolling (0 <= t < 8)
@@ -45,7 +64,7 @@ __device__ __forceinline__ Cx<T> mul_w16(Cx<T> d, int t) {
         default: c = (T)-C1; s = (T)S1; break;
     }
     if (SIGN < 0) s = -s;
-    return cx_make<T>(d.x * c - d.y * s, d.x * s + d.y * c);
+    return cx_mul_const(d, c, s);
 }
 
 __host__ __device__ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
@@ -185,9 +204,12 @@ fft_x_forward_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg
             if (k < fg.Kxp) {
                 Cx<T> x1 = cx_make<T>((T)0, (T)0), x2 = x1;
                 if (k <= fg.kcut) {
+                    // X1 = (Z[k] + conj Z[N-k])/2,  X2 = -i (Z[k] - conj Z[N-k])/2
                     const Cx<T> zk = v[i * S::RB + k2], zn = line[(N - k) & (N - 1)];
-                    x1 = cx_make<T>(half * (zk.x + zn.x), half * (zk.y - zn.y));
-                    x2 = cx_make<T>(half * (zk.y + zn.y), half * (zn.x - zk.x));
+                    const Cx<T> zc = cx_make<T>(zn.x, -zn.y);
+                    const Cx<T> sum = cx_add(zk, zc), dif = cx_sub(zk, zc);
+                    x1 = cx_scale(sum, half);
+                    x2 = cx_scale(cx_make<T>(dif.y, -dif.x), half);
                 }
                 out0[k] = x1;
                 out1[k] = x2;
