@@ -235,6 +235,13 @@ int ensure_allocated(enuf_plan* p) {
                     e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
     }
     p->esize = p->precision == ENUF_F32 ? 4 : 8;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            p->num_sms = sms;
+        (void)cudaGetLastError();
+    }
     // the outermost stencil point on the far side of a particle is an exact zero for Kaiser-Bessel;
     // only when the particle sits exactly on a grid point are both ends non-zero, with the value
     // b m / sinh(b m) (<= 2.7e-9 for m >= 5): the fp32 kernels then skip that point

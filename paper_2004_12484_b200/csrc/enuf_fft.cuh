@@ -257,6 +257,115 @@ fft_x_inverse_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeom fg
     for (int k2 = 0; k2 < 16; ++k2) { out0[t + S::TPL * k2] = v[k2].x; out1[t + S::TPL * k2] = v[k2].y; }
 }
 
+// ---------------------------------------------------------------- X passes, rows staged through TMA
+// Persistent variants of the two X passes: a CTA walks tiles (LPC lines = 2 LPC rows, contiguous in memory)
+// blockIdx.x, blockIdx.x + gridDim.x, ...  The rows of a tile are brought into shared memory by the TMA
+// unit (cp.async.bulk, one 1-D bulk copy per line = two rows, completion on an mbarrier; the line pitch in
+// shared memory is padded by 64 bytes so that the two lines a warp reads fall in different banks).  There
+// is ONE staging buffer: as soon as every thread has taken its tile out of it into registers, the copy of
+// the CTA's next tile is issued, so it runs under the whole transform + store of the current tile.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared bulk copy (TMA, 1-D): bytes is a multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <typename T, int N> constexpr int fft_xf_stage_pitch() { return 2 * N + 64 / (int)sizeof(T); }      // in T
+template <typename T, int N> constexpr size_t fft_xf_tma_smem_bytes() {
+    return fft_smem_bytes<T, N>() + sizeof(T) * (size_t)fft_lines_per_cta<N>() * fft_xf_stage_pitch<T, N>() + 16;
+}
+
+template <typename T, int N>
+__global__ void __launch_bounds__(kFftThreads)
+fft_x_forward_tma_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg, const Cx<T>* __restrict__ tw,
+                         int ntiles) {
+    using S = FftShape<N, -1>;
+    static_assert(S::TPL <= 32, "a line must fit in one warp");
+    constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>(), SP = fft_xf_stage_pitch<T, N>();
+    constexpr uint32_t LINE_BYTES = 2 * N * sizeof(T);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
+    T* stage = reinterpret_cast<T*>(smem_raw + fft_smem_bytes<T, N>());
+    uint64_t* bar = reinterpret_cast<uint64_t*>(stage + (size_t)LPC * SP);
+    const int t = threadIdx.x % S::TPL, ls = threadIdx.x / S::TPL;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    // producer side: thread 0 arms the barrier with the tile's bytes, the first thread of every line copies it
+    auto issue = [&](int tile) {
+        if (threadIdx.x == 0) mbar_expect_tx(bar, LINE_BYTES * LPC);
+        __syncthreads();                                    // the expectation is armed before any copy can complete
+        if (t == 0) tma_load_1d(stage + (size_t)ls * SP, G + (2 * ((size_t)tile * LPC + ls)) * N, LINE_BYTES, bar);
+    };
+    int tile = blockIdx.x;
+    if (tile < ntiles) issue(tile);
+    uint32_t parity = 0;
+    const T half = (T)0.5;
+    for (; tile < ntiles; tile += gridDim.x) {
+        mbar_wait(bar, parity);
+        parity ^= 1u;
+        const size_t row = 2 * ((size_t)tile * LPC + ls);
+        Cx<T> v[16];
+        const T* in0 = stage + (size_t)ls * SP;
+        const T* in1 = in0 + N;
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) v[n1] = cx_make<T>(in0[S::RB * n1 + t], in1[S::RB * n1 + t]);
+        __syncthreads();                                    // every thread holds its tile: the buffer is free
+        if (tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x);
+        Cx<T>* line = sm + ls * PITCH;
+        fft_pass_a<T, N, -1>(v, t, line, tw);
+        __syncthreads();
+        fft_pass_b<T, N, -1>(v, t, line);
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < S::ITEMS_B; ++i)
+#pragma unroll
+            for (int k2 = 0; k2 < S::RB; ++k2) line[t + S::TPL * i + 16 * k2] = v[i * S::RB + k2];
+        __syncwarp();
+        Cx<T>* out0 = A1 + row * fg.Kxp;
+        Cx<T>* out1 = out0 + fg.Kxp;
+#pragma unroll
+        for (int i = 0; i < S::ITEMS_B; ++i)
+#pragma unroll
+            for (int k2 = 0; k2 < S::RB; ++k2) {
+                const int k = t + S::TPL * i + 16 * k2;
+                if (k < fg.Kxp) {
+                    Cx<T> x1 = cx_make<T>((T)0, (T)0), x2 = x1;
+                    if (k <= fg.kcut) {
+                        const Cx<T> zk = v[i * S::RB + k2], zn = line[(N - k) & (N - 1)];
+                        const Cx<T> zc = cx_make<T>(zn.x, -zn.y);
+                        const Cx<T> sum = cx_add(zk, zc), dif = cx_sub(zk, zc);
+                        x1 = cx_scale(sum, half);
+                        x2 = cx_scale(cx_make<T>(dif.y, -dif.x), half);
+                    }
+                    out0[k] = x1;
+                    out1[k] = x2;
+                }
+            }
+        __syncthreads();                                    // the line buffers are rewritten by the next tile
+    }
+}
+
 // ---------------------------------------------------------------- Y passes (strided lines)
 // line id = z*Kxp + kx; consecutive ids are contiguous in memory.
 template <typename T, int N>

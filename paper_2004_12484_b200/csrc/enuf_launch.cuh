@@ -75,6 +75,7 @@ int configure_kernels(enuf_plan* p) {
         constexpr int N_ = decltype(nc)::value;
         const size_t sb = fft_smem_bytes<T, N_>();
         bool ok = set_smem(fft_x_forward_kernel<T, N_>, sb) && set_smem(fft_x_inverse_kernel<T, N_>, sb)
+                  && set_smem(fft_x_forward_tma_kernel<T, N_>, fft_xf_tma_smem_bytes<T, N_>())
                   && set_smem(fft_y_forward_kernel<T, N_>, sb) && set_smem(fft_y_inverse_kernel<T, N_>, sb)
                   && set_smem(fft_z_fused_kernel<T, N_, 1>, sb) && set_smem(fft_z_fused_kernel<T, N_, 3>, sb);
         return ok ? 0 : -1;
@@ -139,8 +140,15 @@ int launch_fft_forward(enuf_plan* p) {
         const size_t sb = fft_smem_bytes<T, N_>();
         const unsigned bx = (unsigned)(((size_t)N_ * N_) / LPC);
         const unsigned by = (unsigned)(((size_t)N_ * p->Kxp + LPC - 1) / LPC);
-        fft_x_forward_kernel<T, N_><<<bx / 2, kFftThreads, sb, s>>>(static_cast<const T*>(p->grid[0]),
-                                                               static_cast<Cx<T>*>(p->A1[0]), fg, tw);
+        {
+            // persistent, rows staged through TMA; CTAs per SM by shared memory (<= 3 for fp32, 1-2 for fp64)
+            const size_t sbt = fft_xf_tma_smem_bytes<T, N_>();
+            const int per_sm = (int)((size_t)(227 * 1024) / (sbt + 1024));
+            const int ntiles = (int)(bx / 2);
+            const int gridx = ntiles < p->num_sms * per_sm ? ntiles : p->num_sms * per_sm;
+            fft_x_forward_tma_kernel<T, N_><<<gridx, kFftThreads, sbt, s>>>(static_cast<const T*>(p->grid[0]),
+                                                                           static_cast<Cx<T>*>(p->A1[0]), fg, tw, ntiles);
+        }
         fft_y_forward_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[0]),
                                                                static_cast<Cx<T>*>(p->A2[0]), fg, tw);
         return 2;

@@ -26,6 +26,7 @@ struct enuf_plan {
     size_t esize = 4;              // bytes per real
     size_t workspace_bytes = 0;
     int launches = 0;
+    int num_sms = 148;             // multiProcessorCount of the current device (persistent FFT grids)
     // device workspace
     void* rec = nullptr;           // PRec<T>[N_cap]
     uint32_t* cell = nullptr;      // [N_cap]
