@@ -366,6 +366,76 @@ fft_x_forward_tma_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeo
     }
 }
 
+// X inverse (complex-to-real) with the half-spectrum rows staged through TMA; same structure as above.
+// A line = the two consecutive rows (row, row + 1) of A1 = 2 Kxp complex values, contiguous.
+template <typename T> constexpr int fft_xi_stage_pad() { return 16 / (int)sizeof(Cx<T>) * 2; }    // complex values
+template <typename T, int N> size_t fft_xi_tma_smem_bytes(int Kxp) {
+    return fft_smem_bytes<T, N>() + sizeof(Cx<T>) * (size_t)fft_lines_per_cta<N>() * (2 * Kxp + fft_xi_stage_pad<T>()) + 16;
+}
+
+template <typename T, int N>
+__global__ void __launch_bounds__(kFftThreads)
+fft_x_inverse_tma_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeom fg, const Cx<T>* __restrict__ tw,
+                         int ntiles) {
+    using S = FftShape<N, +1>;
+    constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);
+    Cx<T>* stage = reinterpret_cast<Cx<T>*>(smem_raw + fft_smem_bytes<T, N>());
+    const int SP = 2 * fg.Kxp + fft_xi_stage_pad<T>();                       // line pitch in complex values
+    const uint32_t LINE_BYTES = 2u * (uint32_t)fg.Kxp * (uint32_t)sizeof(Cx<T>);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(stage + (size_t)LPC * SP);
+    const int t = threadIdx.x % S::TPL, ls = threadIdx.x / S::TPL;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    auto issue = [&](int tile) {
+        if (threadIdx.x == 0) mbar_expect_tx(bar, LINE_BYTES * LPC);
+        __syncthreads();
+        if (t == 0) tma_load_1d(stage + (size_t)ls * SP, A1 + (2 * ((size_t)tile * LPC + ls)) * fg.Kxp, LINE_BYTES, bar);
+    };
+    int tile = blockIdx.x;
+    if (tile < ntiles) issue(tile);
+    uint32_t parity = 0;
+    for (; tile < ntiles; tile += gridDim.x) {
+        mbar_wait(bar, parity);
+        parity ^= 1u;
+        const size_t row = 2 * ((size_t)tile * LPC + ls);
+        const Cx<T>* in0 = stage + (size_t)ls * SP;
+        const Cx<T>* in1 = in0 + fg.Kxp;
+        Cx<T> v[16];
+        // Hermitian extension of the half spectra: X[N-k] = conj X[k];  Z = X1 + i X2
+#pragma unroll
+        for (int i = 0; i < S::ITEMS_A; ++i)
+#pragma unroll
+            for (int n1 = 0; n1 < S::RA; ++n1) {
+                const int e = 16 * n1 + t + S::TPL * i;
+                Cx<T> val = cx_make<T>((T)0, (T)0);
+                if (e <= fg.kcut) {
+                    const Cx<T> a = in0[e], b = in1[e];
+                    val = cx_make<T>(a.x - b.y, a.y + b.x);
+                } else if (N - e <= fg.kcut) {
+                    const Cx<T> a = in0[N - e], b = in1[N - e];       // conj(a) + i conj(b)
+                    val = cx_make<T>(a.x + b.y, b.x - a.y);
+                }
+                v[i * S::RA + n1] = val;
+            }
+        __syncthreads();                                    // every thread holds its tile: the buffer is free
+        if (tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x);
+        Cx<T>* line = sm + ls * PITCH;
+        fft_pass_a<T, N, +1>(v, t, line, tw);
+        __syncthreads();
+        fft_pass_b<T, N, +1>(v, t, line);
+        T* out0 = G + row * N;
+        T* out1 = out0 + N;
+#pragma unroll
+        for (int k2 = 0; k2 < 16; ++k2) { out0[t + S::TPL * k2] = v[k2].x; out1[t + S::TPL * k2] = v[k2].y; }
+        __syncthreads();                                    // the line buffers are rewritten by the next tile
+    }
+}
+
 // ---------------------------------------------------------------- Y passes (strided lines)
 // line id = z*Kxp + kx; consecutive ids are contiguous in memory.
 template <typename T, int N>

@@ -76,6 +76,7 @@ int configure_kernels(enuf_plan* p) {
         const size_t sb = fft_smem_bytes<T, N_>();
         bool ok = set_smem(fft_x_forward_kernel<T, N_>, sb) && set_smem(fft_x_inverse_kernel<T, N_>, sb)
                   && set_smem(fft_x_forward_tma_kernel<T, N_>, fft_xf_tma_smem_bytes<T, N_>())
+                  && set_smem(fft_x_inverse_tma_kernel<T, N_>, fft_xi_tma_smem_bytes<T, N_>(p->Kxp))
                   && set_smem(fft_y_forward_kernel<T, N_>, sb) && set_smem(fft_y_inverse_kernel<T, N_>, sb)
                   && set_smem(fft_z_fused_kernel<T, N_, 1>, sb) && set_smem(fft_z_fused_kernel<T, N_, 3>, sb);
         return ok ? 0 : -1;
@@ -188,8 +189,14 @@ int launch_fft_backward(enuf_plan* p) {
         for (int d = 0; d < nout; ++d) {
             fft_y_inverse_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A2[d]),
                                                                    static_cast<Cx<T>*>(p->A1[d]), fg, tw);
-            fft_x_inverse_kernel<T, N_><<<bx / 2, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[d]),
-                                                                   static_cast<T*>(p->grid[d]), fg, tw);
+            {
+                const size_t sbt = fft_xi_tma_smem_bytes<T, N_>(p->Kxp);
+                const int per_sm = (int)((size_t)(227 * 1024) / (sbt + 1024));
+                const int ntiles = (int)(bx / 2);
+                const int cap = p->num_sms * (per_sm < 4 ? per_sm : 4);
+                fft_x_inverse_tma_kernel<T, N_><<<ntiles < cap ? ntiles : cap, kFftThreads, sbt, s>>>(
+                    static_cast<const Cx<T>*>(p->A1[d]), static_cast<T*>(p->grid[d]), fg, tw, ntiles);
+            }
             launches += 2;
         }
         energy_finish_kernel<<<1, 256, 0, s>>>(p->e_partial, (int)bz, 1.0 / (2.0 * 3.14159265358979323846 * p->L),
