@@ -198,7 +198,7 @@ void free_workspace(enuf_plan* p) {
     fr(p->rec); fr(p->cell); fr(p->idx); fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
     fr(p->scan_total);
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
-    fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev);
+    fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev); fr(p->fft_done);
     fr(p->r_stage); fr(p->q_stage); fr(p->F_stage);
     fr(p->real_pos); fr(p->real_idx); fr(p->real_count); fr(p->real_offset); fr(p->real_cursor);
     fr(p->real_scan_total); fr(p->real_partial); fr(p->real_e_dev);
@@ -217,6 +217,7 @@ void free_workspace(enuf_plan* p) {
     p->rec = p->spectrum = p->tw = p->iphi = p->wf = p->r_stage = p->q_stage = p->F_stage = nullptr;
     p->cell = p->idx = p->bin_count = p->bin_offset = p->bin_cursor = p->scan_total = nullptr;
     p->e_partial = p->e_dev = p->e_pinned = nullptr;
+    p->fft_done = nullptr;
     p->events_valid = false;
     p->partial_ready = false;
     p->allocated = false;
@@ -271,6 +272,7 @@ int ensure_allocated(enuf_plan* p) {
     p->n_partial = (int)(((size_t)p->Ky * p->Kxp + lpc - 1) / lpc);
     ALLOC(p->e_partial, 8 * (size_t)p->n_partial);
     ALLOC(p->e_dev, 8);
+    ALLOC(p->fft_done, 4);
 #undef ALLOC
     if (cudaMallocHost((void**)&p->e_pinned, 8) != cudaSuccess) {
         (void)cudaGetLastError();
@@ -292,6 +294,7 @@ int ensure_allocated(enuf_plan* p) {
     }
     if (p->spectrum) cudaMemsetAsync(p->spectrum, 0, 2 * es * (size_t)p->Ky * p->Ky * p->Kxp, p->stream);
     cudaMemsetAsync(p->e_dev, 0, 8, p->stream);
+    cudaMemsetAsync(p->fft_done, 0, 4, p->stream);
     rc = p->precision == ENUF_F32 ? enuf::configure_kernels<float>(p) : enuf::configure_kernels<double>(p);
     if (rc) {
         cudaError_t le = cudaGetLastError();

@@ -520,11 +520,40 @@ struct ScaleTables {
     const void* wf;     // [kcut^2+1] f^2 w, entry 0 unused (= 0)
 };
 
+// Step a7 inside the Z pass: every CTA publishes its fp64 energy partial (thread 0's `mine`); the CTA that
+// finishes last sums all partials in a fixed order (strided per thread, then a tree: the same order whichever
+// CTA it is, so E is reproducible) and writes E = scale * sum.  The counter resets itself for the next call.
+// Must be called by all threads of the CTA.
+__device__ __forceinline__ void z_pass_energy_finish(double mine, double* __restrict__ e_partial,
+                                                     unsigned* __restrict__ done_count, double e_scale,
+                                                     double* __restrict__ e_out) {
+    __shared__ bool is_last;
+    __shared__ double fin[kFftThreads];
+    if (threadIdx.x == 0) {
+        e_partial[blockIdx.x] = mine;
+        __threadfence();
+        is_last = atomicAdd(done_count, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    double s = 0.0;
+    for (unsigned i = threadIdx.x; i < gridDim.x; i += kFftThreads) s += __ldcg(&e_partial[i]);
+    fin[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = kFftThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) fin[threadIdx.x] += fin[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { *e_out = e_scale * fin[0]; *done_count = 0u; }
+}
+
 template <typename T, int N, int NOUT>
 __global__ void __launch_bounds__(kFftThreads)
 fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __restrict__ out2, FftGeom fg,
                    const Cx<T>* __restrict__ tw, ScaleTables st, double* __restrict__ e_partial,
-                   Cx<T>* __restrict__ spectrum) {
+                   Cx<T>* __restrict__ spectrum, unsigned* __restrict__ done_count, double e_scale,
+                   double* __restrict__ e_out) {
     using SF = FftShape<N, -1>;
     using SI = FftShape<N, +1>;
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
@@ -557,7 +586,7 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
                 if (NOUT == 3) { out1[(base - A2) + o] = zero; out2[(base - A2) + o] = zero; }
             }
         }
-        if (threadIdx.x == 0) e_partial[blockIdx.x] = 0.0;
+        z_pass_energy_finish(0.0, e_partial, done_count, e_scale, e_out);
         return;
     }
 
@@ -633,27 +662,13 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
     for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_xor_sync(0xffffffffu, e_acc, o);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = e_acc;
     __syncthreads();
+    double s = 0.0;
     if (threadIdx.x == 0) {
-        double s = 0.0;
 #pragma unroll
         for (int w = 0; w < kFftThreads / 32; ++w) s += red[w];
-        e_partial[blockIdx.x] = s;
     }
+    z_pass_energy_finish(s, e_partial, done_count, e_scale, e_out);
 }
 
-// Step a7: E = scale * sum of partials, fixed summation order (one CTA).
-static __global__ void __launch_bounds__(256)
-energy_finish_kernel(const double* __restrict__ partial, int count, double scale, double* __restrict__ e_out) {
-    __shared__ double red[256];
-    double s = 0.0;
-    for (int i = threadIdx.x; i < count; i += 256) s += partial[i];
-    red[threadIdx.x] = s;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) *e_out = scale * red[0];
-}
 
 }  // namespace enuf

@@ -177,14 +177,16 @@ int launch_fft_backward(enuf_plan* p) {
         const unsigned bz = (unsigned)(((size_t)p->Ky * p->Kxp + LPC - 1) / LPC);
         if ((int)bz > p->n_partial) return -1;
         Cx<T>* spec = p->keep_spectrum ? static_cast<Cx<T>*>(p->spectrum) : nullptr;
+        const double e_scale = 1.0 / (2.0 * 3.14159265358979323846 * p->L);   // Eq. 38: C/(2 pi L), C = 1
         if (nout == 1)
             fft_z_fused_kernel<T, N_, 1><<<bz, kFftThreads, sb, s>>>(static_cast<Cx<T>*>(p->A2[0]), nullptr, nullptr,
-                                                                    fg, tw, st, p->e_partial, spec);
+                                                                    fg, tw, st, p->e_partial, spec, p->fft_done,
+                                                                    e_scale, p->e_dev);
         else
             fft_z_fused_kernel<T, N_, 3><<<bz, kFftThreads, sb, s>>>(static_cast<Cx<T>*>(p->A2[0]),
                                                                     static_cast<Cx<T>*>(p->A2[1]),
                                                                     static_cast<Cx<T>*>(p->A2[2]), fg, tw, st,
-                                                                    p->e_partial, spec);
+                                                                    p->e_partial, spec, p->fft_done, e_scale, p->e_dev);
         launches = 1;
         for (int d = 0; d < nout; ++d) {
             fft_y_inverse_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A2[d]),
@@ -199,9 +201,6 @@ int launch_fft_backward(enuf_plan* p) {
             }
             launches += 2;
         }
-        energy_finish_kernel<<<1, 256, 0, s>>>(p->e_partial, (int)bz, 1.0 / (2.0 * 3.14159265358979323846 * p->L),
-                                              p->e_dev);
-        launches += 1;
         return launches;
     });
     if (launches < 0) return -1;

@@ -48,6 +48,7 @@ struct enuf_plan {
     double* e_partial = nullptr;   // [z-pass CTAs]
     int n_partial = 0;
     double* e_dev = nullptr;       // [1]
+    unsigned* fft_done = nullptr;  // [1] CTAs of the Z pass that have published their energy partial
     double* e_pinned = nullptr;    // [1] host
     // real-space part (enuf_real_space; allocated at its first call)
     void* real_pos = nullptr;         // Vec4<T>[N_cap]: wrapped position + charge, cell order
