@@ -454,7 +454,7 @@ fft_y_forward_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, FftGe
     Cx<T> v[16];
 #pragma unroll
     for (int n1 = 0; n1 < 16; ++n1)
-        v[n1] = live ? in[(size_t)(S::RB * n1 + t) * fg.Kxp] : cx_make<T>((T)0, (T)0);
+        v[n1] = live ? in[(unsigned)(S::RB * n1 + t) * (unsigned)fg.Kxp] : cx_make<T>((T)0, (T)0);
     Cx<T>* line = sm + ls * PITCH;
     fft_pass_a<T, N, -1>(v, t, line, tw);
     __syncthreads();
@@ -469,7 +469,7 @@ fft_y_forward_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, FftGe
             int kyp = -1;
             if (k <= fg.kcut) kyp = k;
             else if (k >= N - fg.kcut) kyp = k - N + fg.Ky;
-            if (kyp >= 0) out[(size_t)kyp * fg.Kxp] = v[i * S::RB + k2];
+            if (kyp >= 0) out[(unsigned)kyp * (unsigned)fg.Kxp] = v[i * S::RB + k2];
         }
 }
 
@@ -495,7 +495,7 @@ fft_y_inverse_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, FftGe
             int kyp = -1;
             if (e <= fg.kcut) kyp = e;
             else if (e >= N - fg.kcut) kyp = e - N + fg.Ky;
-            v[i * S::RA + n1] = (live && kyp >= 0) ? in[(size_t)kyp * fg.Kxp] : cx_make<T>((T)0, (T)0);
+            v[i * S::RA + n1] = (live && kyp >= 0) ? in[(unsigned)kyp * (unsigned)fg.Kxp] : cx_make<T>((T)0, (T)0);
         }
     Cx<T>* line = sm + ls * PITCH;
     fft_pass_a<T, N, +1>(v, t, line, tw);
@@ -504,7 +504,7 @@ fft_y_inverse_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, FftGe
     if (!live) return;
     Cx<T>* out = A1 + (size_t)z * N * fg.Kxp + kx;
 #pragma unroll
-    for (int k2 = 0; k2 < 16; ++k2) out[(size_t)(t + S::TPL * k2) * fg.Kxp] = v[k2];
+    for (int k2 = 0; k2 < 16; ++k2) out[(unsigned)(t + S::TPL * k2) * (unsigned)fg.Kxp] = v[k2];
 }
 
 // ---------------------------------------------------------------- fused Z pass
@@ -572,7 +572,7 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
     const int kc2 = fg.kcut * fg.kcut;
     const int kxy2 = kx * kx + ky * ky;
     const bool inside = live && kx <= fg.kcut && kxy2 <= kc2;
-    const size_t zstride = (size_t)fg.Ky * fg.Kxp;
+    const unsigned zstride = (unsigned)fg.Ky * (unsigned)fg.Kxp;   // all offsets fit 32 bits (<= 2^23 elements)
     Cx<T>* base = A2 + (size_t)kyp * fg.Kxp + kx;
     const Cx<T> zero = cx_make<T>((T)0, (T)0);
 
@@ -581,7 +581,7 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
         if (live) {
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
-                const size_t o = (size_t)(SF::RB * n1 + t) * zstride;
+                const unsigned o = (unsigned)(SF::RB * n1 + t) * zstride;
                 base[o] = zero;
                 if (NOUT == 3) { out1[(base - A2) + o] = zero; out2[(base - A2) + o] = zero; }
             }
@@ -593,7 +593,7 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
     Cx<T> v[16];
 #pragma unroll
     for (int n1 = 0; n1 < 16; ++n1)
-        v[n1] = inside ? base[(size_t)(SF::RB * n1 + t) * zstride] : zero;
+        v[n1] = inside ? base[(unsigned)(SF::RB * n1 + t) * zstride] : zero;
     Cx<T>* line = sm + ls * PITCH;
     fft_pass_a<T, N, -1>(v, t, line, tw);
     __syncthreads();
@@ -653,7 +653,7 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
         if (live) {
             Cx<T>* ob = outs[d] + (size_t)kyp * fg.Kxp + kx;
 #pragma unroll
-            for (int k2 = 0; k2 < 16; ++k2) ob[(size_t)(t + SI::TPL * k2) * zstride] = v[k2];
+            for (int k2 = 0; k2 < 16; ++k2) ob[(unsigned)(t + SI::TPL * k2) * zstride] = v[k2];
         }
     }
 
