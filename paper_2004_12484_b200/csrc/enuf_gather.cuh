@@ -199,13 +199,17 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
     };
 
     // the first batch's weights overlap the tile copy
-    if (warp * PBW < cnt) batch_weights(warp * PBW, min(PBW, cnt - warp * PBW));
+    // every warp takes one contiguous share of the tile's particles (sizes differ by at most one), in
+    // batches of PBW: the CTA ends within one particle of perfect balance
+    const int share = cnt / C::WARPS, extra = cnt - share * C::WARPS;
+    const int wbeg = warp * share + min(warp, extra), wend = wbeg + share + (warp < extra ? 1 : 0);
+    if (wbeg < wend) batch_weights(wbeg, min(PBW, wend - wbeg));
     cp_async_wait_all();
     __syncthreads();
 
-    for (int p0 = warp * PBW; p0 < cnt; p0 += C::WARPS * PBW) {
-        const int nb = min(PBW, cnt - p0);
-        if (p0 != warp * PBW) {
+    for (int p0 = wbeg; p0 < wend; p0 += PBW) {
+        const int nb = min(PBW, wend - p0);
+        if (p0 != wbeg) {
             batch_weights(p0, nb);
             __syncwarp();
         }
