@@ -49,9 +49,9 @@ struct GatherCfg {
     static constexpr int CELLS = ((TP * SPL + 3) / 4) * 4;      // shared tile size in elements (16 B multiple)
     static constexpr int WARPS = 12;
     static constexpr int NT = WARPS * 32;
-    static constexpr int PBW = 4;                               // particles per warp batch
+    static constexpr int PBW = 5;                               // particles per warp batch (15 lanes compute weights)
     static constexpr int ITER = (WE * WE + 31) / 32;            // stencil rows per lane
-    static constexpr int WP = 18;                               // pitch of a (phi, phi') weight row: 16-byte aligned, rows spread over banks
+    static constexpr int WP = 14;                               // pitch of a (phi, phi') weight row: >= W + 1, 16-byte aligned
 };
 
 template <typename T, int M_, bool kTrim = false>
