@@ -134,20 +134,23 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                 const int bxm = (cx & (kTile - 1)) + (i % 3 - 1) * kTile + M_;   // bx + m, bx relative to the column
                 const int bym = (cy & (kTile - 1)) + (i / 3 - 1) * kTile + M_;
                 if ((unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_)) {
-                    const int slot = atomicAdd(&nslot_s, 1);
-                    if (slot < CAP) {
-                        const PRec<T> pr = rec[pidx];
-                        *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = pr;
-                        int pk = bxm | (bym << 8);
-                        if (kTrim) pk |= (pr.dx > (T)0 ? 1 << 16 : 0) | (pr.dy > (T)0 ? 1 << 17 : 0);
-                        // which of the four 8 x 8 warp patches the stencil touches (bits 20..23, warp order):
-                        // it covers the column cells [b - (WZ-1), b], b = bxm (trimmed: bxm - 1 + ks)
-                        const int bx2 = bxm + (kTrim ? (pr.dx > (T)0 ? 0 : -1) : 0);
-                        const int by2 = bym + (kTrim ? (pr.dy > (T)0 ? 0 : -1) : 0);
-                        const int ox = (bx2 >= 0 && bx2 - (WZ - 1) <= 7 ? 1 : 0) | (bx2 >= 8 && bx2 - (WZ - 1) <= 15 ? 2 : 0);
-                        const int oy = (by2 >= 0 && by2 - (WZ - 1) <= 7 ? 1 : 0) | (by2 >= 8 && by2 - (WZ - 1) <= 15 ? 2 : 0);
-                        pk |= ((oy & 1 ? ox : 0) | (oy & 2 ? ox << 2 : 0)) << 20;
-                        sb[slot] = pk;
+                    const PRec<T> pr = rec[pidx];
+                    int pk = bxm | (bym << 8);
+                    if (kTrim) pk |= (pr.dx > (T)0 ? 1 << 16 : 0) | (pr.dy > (T)0 ? 1 << 17 : 0);
+                    // which of the four 8 x 8 warp patches the stencil touches (bits 20..23, warp order):
+                    // it covers the column cells [b - (WZ-1), b], b = bxm (trimmed: bxm - 1 + ks)
+                    const int bx2 = bxm + (kTrim ? (pr.dx > (T)0 ? 0 : -1) : 0);
+                    const int by2 = bym + (kTrim ? (pr.dy > (T)0 ? 0 : -1) : 0);
+                    const int ox = (bx2 >= 0 && bx2 - (WZ - 1) <= 7 ? 1 : 0) | (bx2 >= 8 && bx2 - (WZ - 1) <= 15 ? 2 : 0);
+                    const int oy = (by2 >= 0 && by2 - (WZ - 1) <= 7 ? 1 : 0) | (by2 >= 8 && by2 - (WZ - 1) <= 15 ? 2 : 0);
+                    const int mask = (oy & 1 ? ox : 0) | (oy & 2 ? ox << 2 : 0);
+                    // a trimmed stencil at the far edge of the halo misses the column altogether: not staged
+                    if (mask != 0) {
+                        const int slot = atomicAdd(&nslot_s, 1);
+                        if (slot < CAP) {
+                            *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = pr;
+                            sb[slot] = pk | (mask << 20);
+                        }
                     }
                 }
             }
