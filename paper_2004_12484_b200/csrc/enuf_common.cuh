@@ -66,9 +66,17 @@ __host__ __device__ constexpr int poly_degree(int m) { return m >= 4 ? 10 : 12; 
 constexpr int kPolyMaxDeg = 12;
 template <int M_>
 struct PolyArg {
-    static constexpr int D = poly_degree(M_);
+    static constexpr int D = poly_degree(M_);          // even
     float c[D + 1][M_ + 1];   // value:      p_j(d0)  = sum_i c[i][j] d0^i,  j = 0..m
     float d[D][M_ + 1];       // derivative: p_j'(d0) = sum_i d[i][j] d0^i
+    // The same coefficients paired for the packed evaluation (stencil_weights<.., kPacked = true>):
+    // p_j(d0) = E_j(y) + d0 O_j(y), y = d0^2; the two Horner chains advance together in one FFMA2 per step,
+    // vp[k][j] = (c_(D-2-2k), c_(D-1-2k)), top[j] = c_D starts E_j one step early (it has one coefficient more);
+    // p_j' (degree D-1, odd) has D/2 coefficients in both chains: dp[k][j] = (d_(D-2-2k), d_(D-1-2k)).
+    static constexpr int NP = D / 2;
+    alignas(8) float top[M_ + 1 + ((M_ + 1) & 1)];
+    float2 vp[NP][M_ + 1];
+    float2 dp[NP][M_ + 1];
 };
 
 __host__ __device__ inline uint32_t pack_cell(int cx, int cy, int cz) {
@@ -141,7 +149,7 @@ __device__ __forceinline__ void window_eval(const WindowParams& wp, T d0, int j,
 //   fp32: the plan's polynomial table (even/odd Horner in d0^2); Kaiser-Bessel support cut
 //         |d| <= m (value) and |d| < m (derivative) exactly as in the closed form.
 //   fp64: the closed form (window_eval).
-template <typename T, int M_, bool kDeriv>
+template <typename T, int M_, bool kDeriv, bool kPacked = false>
 __device__ __forceinline__ void stencil_weights(const WindowParams& wp, const PolyArg<M_>& pa, T d0,
                                                 T (&w)[2 * M_ + 1], T (&dw)[2 * M_ + 1]) {
     constexpr int W = 2 * M_ + 1;
@@ -152,46 +160,81 @@ __device__ __forceinline__ void stencil_weights(const WindowParams& wp, const Po
             window_eval<T, kDeriv>(wp, d0, k - M_, w[k], dw[k]);
         }
     } else {
-        constexpr int D = PolyArg<M_>::D;
-        constexpr int DE = D - (D & 1), DO = D - 1 + (D & 1);      // highest even / odd power of p
         const float x = (float)d0, y = x * x;
         float v[W], dv[W];
-        {
-            float E[M_ + 1], O[M_ + 1];
+        if constexpr (kPacked) {
+            const float2 yy = make_float2(y, y);
+            constexpr int NP = PolyArg<M_>::NP;
+            {
+                float2 EO[M_ + 1];                                     // (E_j, O_j)
 #pragma unroll
-            for (int j = 0; j <= M_; ++j) { E[j] = pa.c[DE][j]; O[j] = pa.c[DO][j]; }
+                for (int j = 0; j <= M_; ++j) {
+                    EO[j] = pa.vp[0][j];
+                    EO[j].x = fmaf(pa.top[j], y, EO[j].x);
+                }
 #pragma unroll
-            for (int i = DE - 2; i >= 0; i -= 2)
+                for (int k = 1; k < NP; ++k)
 #pragma unroll
-                for (int j = 0; j <= M_; ++j) E[j] = fmaf(E[j], y, pa.c[i][j]);
+                    for (int j = 0; j <= M_; ++j) EO[j] = __ffma2_rn(EO[j], yy, pa.vp[k][j]);
+                v[M_] = EO[0].x;                                       // p_0 is even
 #pragma unroll
-            for (int i = DO - 2; i >= 1; i -= 2)
+                for (int j = 1; j <= M_; ++j) { v[M_ + j] = fmaf(x, EO[j].y, EO[j].x); v[M_ - j] = fmaf(-x, EO[j].y, EO[j].x); }
+            }
+            if (kDeriv) {
+                float2 EO[M_ + 1];                                     // (E'_j, O'_j) of p_j'
 #pragma unroll
-                for (int j = 1; j <= M_; ++j) O[j] = fmaf(O[j], y, pa.c[i][j]);
-            v[M_] = E[0];
+                for (int j = 0; j <= M_; ++j) EO[j] = pa.dp[0][j];
 #pragma unroll
-            for (int j = 1; j <= M_; ++j) { v[M_ + j] = fmaf(x, O[j], E[j]); v[M_ - j] = fmaf(-x, O[j], E[j]); }
-        }
-        if (kDeriv) {
-            constexpr int D1 = D - 1;
-            constexpr int DE1 = D1 - (D1 & 1), DO1 = D1 - 1 + (D1 & 1);
-            float E[M_ + 1], O[M_ + 1];
+                for (int k = 1; k < NP; ++k)
 #pragma unroll
-            for (int j = 0; j <= M_; ++j) { E[j] = pa.d[DE1][j]; O[j] = pa.d[DO1][j]; }
+                    for (int j = 0; j <= M_; ++j) EO[j] = __ffma2_rn(EO[j], yy, pa.dp[k][j]);
+                dv[M_] = x * EO[0].y;                                  // p_0 is even: p_0' is odd
 #pragma unroll
-            for (int i = DE1 - 2; i >= 0; i -= 2)
+                for (int j = 1; j <= M_; ++j) { dv[M_ + j] = fmaf(x, EO[j].y, EO[j].x); dv[M_ - j] = fmaf(x, EO[j].y, -EO[j].x); }
+            } else {
 #pragma unroll
-                for (int j = 1; j <= M_; ++j) E[j] = fmaf(E[j], y, pa.d[i][j]);
-#pragma unroll
-            for (int i = DO1 - 2; i >= 1; i -= 2)
-#pragma unroll
-                for (int j = 0; j <= M_; ++j) O[j] = fmaf(O[j], y, pa.d[i][j]);
-            dv[M_] = x * O[0];                                       // p_0 is even: p_0' is odd
-#pragma unroll
-            for (int j = 1; j <= M_; ++j) { dv[M_ + j] = fmaf(x, O[j], E[j]); dv[M_ - j] = fmaf(x, O[j], -E[j]); }
+                for (int j = 0; j < W; ++j) dv[j] = 0.f;
+            }
         } else {
+            constexpr int D = PolyArg<M_>::D;
+            constexpr int DE = D - (D & 1), DO = D - 1 + (D & 1);      // highest even / odd power of p
+            {
+                float E[M_ + 1], O[M_ + 1];
 #pragma unroll
-            for (int j = 0; j < W; ++j) dv[j] = 0.f;
+                for (int j = 0; j <= M_; ++j) { E[j] = pa.c[DE][j]; O[j] = pa.c[DO][j]; }
+#pragma unroll
+                for (int i = DE - 2; i >= 0; i -= 2)
+#pragma unroll
+                    for (int j = 0; j <= M_; ++j) E[j] = fmaf(E[j], y, pa.c[i][j]);
+#pragma unroll
+                for (int i = DO - 2; i >= 1; i -= 2)
+#pragma unroll
+                    for (int j = 1; j <= M_; ++j) O[j] = fmaf(O[j], y, pa.c[i][j]);
+                v[M_] = E[0];
+#pragma unroll
+                for (int j = 1; j <= M_; ++j) { v[M_ + j] = fmaf(x, O[j], E[j]); v[M_ - j] = fmaf(-x, O[j], E[j]); }
+            }
+            if (kDeriv) {
+                constexpr int D1 = D - 1;
+                constexpr int DE1 = D1 - (D1 & 1), DO1 = D1 - 1 + (D1 & 1);
+                float E[M_ + 1], O[M_ + 1];
+#pragma unroll
+                for (int j = 0; j <= M_; ++j) { E[j] = pa.d[DE1][j]; O[j] = pa.d[DO1][j]; }
+#pragma unroll
+                for (int i = DE1 - 2; i >= 0; i -= 2)
+#pragma unroll
+                    for (int j = 1; j <= M_; ++j) E[j] = fmaf(E[j], y, pa.d[i][j]);
+#pragma unroll
+                for (int i = DO1 - 2; i >= 1; i -= 2)
+#pragma unroll
+                    for (int j = 0; j <= M_; ++j) O[j] = fmaf(O[j], y, pa.d[i][j]);
+                dv[M_] = x * O[0];                                       // p_0 is even: p_0' is odd
+#pragma unroll
+                for (int j = 1; j <= M_; ++j) { dv[M_ + j] = fmaf(x, O[j], E[j]); dv[M_ - j] = fmaf(x, O[j], -E[j]); }
+            } else {
+#pragma unroll
+                for (int j = 0; j < W; ++j) dv[j] = 0.f;
+            }
         }
         if (wp.kind == ENUF_WINDOW_KAISER_BESSEL) {
             // |d0 - j| > m only for j = +m (d0 < 0) and j = -m (d0 > 0); phi' = 0 at |d| = m

@@ -173,7 +173,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             const PRec<T> pr = rec[start + p0 + slot];
             const T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
             T w[W], dw[W];
-            stencil_weights<T, M_, !kIk>(wp, pa, d0, w, dw);
+            stencil_weights<T, M_, !kIk, true>(wp, pa, d0, w, dw);   // packed Horner chains
             P2* row = wtab + (slot * 3 + dim) * WP;
             const bool sh = kTrim && d0 > (T)0;                 // ks = 1: the k = 0 point is the zero one
 #pragma unroll

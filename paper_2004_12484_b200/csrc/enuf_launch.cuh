@@ -42,11 +42,17 @@ static inline int dispatch_n(int n, F&& f) {
 
 template <int M_>
 static inline PolyArg<M_> make_poly_arg(const enuf_plan* p) {
-    PolyArg<M_> a;
-    constexpr int D = PolyArg<M_>::D;
+    PolyArg<M_> a{};
+    constexpr int D = PolyArg<M_>::D, NP = PolyArg<M_>::NP;
+    static_assert(D % 2 == 0, "packed Horner chains assume an even degree");
     for (int j = 0; j <= M_; ++j) {
         for (int k = 0; k <= D; ++k) a.c[k][j] = p->poly_c[k][j];
         for (int k = 0; k < D; ++k) a.d[k][j] = p->poly_d[k][j];
+        a.top[j] = p->poly_c[D][j];
+        for (int k = 0; k < NP; ++k) {
+            a.vp[k][j] = make_float2(p->poly_c[D - 2 - 2 * k][j], p->poly_c[D - 1 - 2 * k][j]);
+            a.dp[k][j] = make_float2(p->poly_d[D - 2 - 2 * k][j], p->poly_d[D - 1 - 2 * k][j]);
+        }
     }
     return a;
 }
