@@ -237,14 +237,15 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
                     if (k & 1) fma_pair(sb2, wx[k], v[k]);
                     else fma_pair(sa, wx[k], v[k]);
                 }
-                const T s0 = sa.x + sb2.x, s1 = sa.y + sb2.y;
+                const P2 s2 = pair_add(sa, sb2);                       // (sum Psi phi_x, sum Psi phi_x')
                 const P2 wy = wt[ryo[it]], wz = wt[rzo[it]];
                 if (kIk) {
-                    fx += s0 * (wy.x * wz.x);
+                    fx += s2.x * (wy.x * wz.x);
                 } else {
-                    fx += s1 * (wy.x * wz.x);
-                    fy += s0 * (wy.y * wz.x);
-                    fz += s0 * (wy.x * wz.y);
+                    const P2 yz = pair_scale(wy, wz.x);                // (phi_y phi_z, phi_y' phi_z)
+                    fx += s2.y * yz.x;
+                    fy += s2.x * yz.y;
+                    fz += s2.x * (wy.x * wz.y);
                 }
             };
             if constexpr (C::kPair && sizeof(T) == 4) {

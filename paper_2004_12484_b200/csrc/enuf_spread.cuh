@@ -35,6 +35,12 @@ __device__ __forceinline__ void fma_pair(double2& acc, const double2 a, const do
     acc.y = fma(a.y, w, acc.y);
 }
 
+// elementwise a + b and a * f on a pair (one packed instruction for fp32)
+__device__ __forceinline__ float2 pair_add(const float2 a, const float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ double2 pair_add(double2 a, const double2 b) { a.x += b.x; a.y += b.y; return a; }
+__device__ __forceinline__ float2 pair_scale(const float2 a, const float f) { return __fmul2_rn(a, make_float2(f, f)); }
+__device__ __forceinline__ double2 pair_scale(double2 a, const double f) { a.x *= f; a.y *= f; return a; }
+
 template <int M_>
 struct SpreadCfg {
     static constexpr int W = 2 * M_ + 1;
