@@ -180,7 +180,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
             }
             // ---- window values: one task per (dimension, slot); dimension-major so warps stay uniform
             for (int t = tid; t < 3 * ns; t += NT) {
-                const int dim = t / ns, slot = t - dim * ns;
+                const int dim = (t >= ns ? 1 : 0) + (t >= 2 * ns ? 1 : 0), slot = t - dim * ns;   // t < 3 ns
                 T w[W], dw[W];
                 const T d0 = st[slot * RP + OD + dim];
                 stencil_weights<T, M_, false>(wp, pa, d0, w, dw);
@@ -231,8 +231,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                     const T wy1 = *reinterpret_cast<const T*>(lane_yb + o1);
                     const P2 wx2 = *reinterpret_cast<const P2*>(lane_xb + o2);
                     const T wy2 = *reinterpret_cast<const T*>(lane_yb + o2);
-                    P2 a1; a1.x = wx1.x * wy1; a1.y = wx1.y * wy1;
-                    P2 a2; a2.x = wx2.x * wy2; a2.y = wx2.y * wy2;
+                    const P2 a1 = pair_scale(wx1, wy1), a2 = pair_scale(wx2, wy2);
                     // q * z rows: 16-byte vector loads (slot pitch and OZ are multiples of 16 bytes)
                     using V4 = typename Vec4<T>::type;
                     constexpr int NV = (WZ + 3) / 4;
