@@ -77,7 +77,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
     __shared__ int rng_start[2][9], rng_cnt[2][9];
     __shared__ int nslot_s;
     // per warp: byte offsets (into st) of the staged particles that overlap the warp's cells, compacted
-    __shared__ __align__(8) unsigned wlist[NT / 32][36];
+    __shared__ __align__(8) unsigned wlist[NT / 32][68];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int Tx = blockIdx.x % g.nt, Ty = blockIdx.x / g.nt;
@@ -211,16 +211,20 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
             __syncthreads();
             if (tid == 0) nslot_s = 0;      // every thread has read ns; the next cull starts after a barrier
             // ---- accumulate: each warp visits the staged particles that overlap its 8 x 8 cells
-            for (int e0 = 0; e0 < ns; e0 += 32) {
-                const bool ov = e0 + lane < ns && ((sb[e0 + lane] >> (20 + warp)) & 1);   // patch mask from the cull
-                const unsigned om = __ballot_sync(0xffffffffu, ov);
-                if (om == 0u) continue;
+            for (int e0 = 0; e0 < ns; e0 += 64) {                      // 64 staged slots per pass
+                // patch mask from the cull: does slot e0 + lane / e0 + 32 + lane touch this warp's cells?
+                const bool ov0 = e0 + lane < ns && ((sb[e0 + lane] >> (20 + warp)) & 1);
+                const bool ov1 = e0 + 32 + lane < ns && ((sb[e0 + 32 + lane] >> (20 + warp)) & 1);
+                const unsigned om0 = __ballot_sync(0xffffffffu, ov0), om1 = __ballot_sync(0xffffffffu, ov1);
+                const int cnt0 = __popc(om0), cnt = cnt0 + __popc(om1);
+                if (cnt == 0) continue;
                 // compact the overlapping slots into the warp's list (padded to an even length with the
                 // zero record), then visit them two per trip: the loads of the second overlap the FMAs
                 // of the first, and the trip has no data-dependent control flow
-                const int cnt = __popc(om);
                 unsigned* wl = wlist[warp];
-                if (ov) wl[__popc(om & ((1u << lane) - 1u))] = (unsigned)(e0 + lane) * (unsigned)(RP * sizeof(T));
+                const unsigned below = (1u << lane) - 1u;
+                if (ov0) wl[__popc(om0 & below)] = (unsigned)(e0 + lane) * (unsigned)(RP * sizeof(T));
+                if (ov1) wl[cnt0 + __popc(om1 & below)] = (unsigned)(e0 + 32 + lane) * (unsigned)(RP * sizeof(T));
                 if (lane == 0) wl[cnt] = (unsigned)CAP * (unsigned)(RP * sizeof(T));
                 __syncwarp();
                 uint2 oo = *reinterpret_cast<const uint2*>(wl);
@@ -247,7 +251,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
 #pragma unroll
                     for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a2, wz2[k]);
                 }
-                __syncwarp();                    // the list is rewritten by the next group of 32 slots
+                __syncwarp();                    // the list is rewritten by the next group of 64 slots
             }
             c0 += span;
             if (c0 < total) __syncthreads();           // staging buffers are reused by the next chunk
