@@ -74,7 +74,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* st = reinterpret_cast<T*>(smem_raw);            // [CAP + 1][RP] staged particle records; slot CAP is all zero
     int* sb = reinterpret_cast<int*>(st + (CAP + 1) * RP);   // [CAP] (bx + m) | (by + m) << 8 | ks_x << 16 | ks_y << 17
-    __shared__ int rng_start[2][9], rng_cnt[2][9];
+    __shared__ int rng_start[2][9], rng_cnt[2][9], rng_max[2];
     __shared__ int nslot_s;
     // per warp: byte offsets (into st) of the staged particles that overlap the warp's cells, compacted
     __shared__ __align__(8) unsigned wlist[NT / 32][68];
@@ -97,10 +97,19 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
         if (tid < 9) {
             const int cz = s < 0 ? s + g.n : (s >= g.n ? s - g.n : s);
             const uint32_t st = offset[nb_bin0 + cz];
+            const int cnt = (int)(offset[nb_bin0 + cz + 1] - st);
             rng_start[buf][tid] = (int)st;
-            rng_cnt[buf][tid] = (int)(offset[nb_bin0 + cz + 1] - st);
+            rng_cnt[buf][tid] = cnt;
+            const int mx = __reduce_max_sync(0x1ffu, cnt);       // lanes 0..8 of warp 0
+            if (tid == 0) rng_max[buf] = mx;
         }
     };
+    // cull mapping: kCullT threads per neighbouring column (9 x 14 = 126 of the 128 threads), thread
+    // (cull_i, cull_k) tests the candidates cull_k, cull_k + 14, .. of column cull_i's bin -- no search for
+    // the range a candidate belongs to
+    constexpr int kCullT = NT / 9;
+    const int cull_i = tid / kCullT < 9 ? tid / kCullT : -1, cull_k = tid % kCullT;
+    const int cull_dx = (cull_i % 3 - 1) * kTile + M_, cull_dy = (cull_i / 3 - 1) * kTile + M_;
     if (tid == 0) nslot_s = 0;
     if (tid < RP) st[CAP * RP + tid] = (T)0;           // the padding record of odd-length visit lists
     load_ranges(z0 - SLO, 0);
@@ -118,27 +127,19 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
     for (int s = z0 - SLO; s < z1 + SHI; ++s, buf ^= 1) {
         __syncthreads();      // ranges of slab s visible; all warps are done with the previous slab
         if (s + 1 < z1 + SHI) load_ranges(s + 1, buf ^ 1);
-        int pref[10];
-        pref[0] = 0;
-#pragma unroll
-        for (int i = 0; i < 9; ++i) pref[i + 1] = pref[i] + rng_cnt[buf][i];
-        const int total = pref[9];
+        const int total = rng_max[buf];                        // candidates of the fullest of the 9 bins
+        const int my_start = cull_i >= 0 ? rng_start[buf][cull_i] : 0;
+        const int my_cnt = cull_i >= 0 ? rng_cnt[buf][cull_i] : 0;
 
-        // cull candidates [c0, c0 + span) against the column's halo: accepted ones are staged
-        // (record + packed position) while slots last; returns nothing, the count is nslot_s
+        // cull the candidates [c0, c0 + span) of every bin against the column's halo: accepted ones are
+        // staged (record + packed position) while slots last; returns nothing, the count is nslot_s
         auto cull = [&](int c0, int span) {
-            for (int c = c0 + tid; c < min(total, c0 + span); c += NT) {
-                int i = 0;
-#pragma unroll
-                for (int e = 1; e < 9; ++e) i += (c >= pref[e]) ? 1 : 0;
-                int pb = 0;
-#pragma unroll
-                for (int e = 1; e < 9; ++e) pb = (i == e) ? pref[e] : pb;
-                const uint32_t pidx = (uint32_t)(rng_start[buf][i] + (c - pb));
+            for (int c = c0 + cull_k; c < min(my_cnt, c0 + span); c += kCullT) {
+                const uint32_t pidx = (uint32_t)(my_start + c);
                 int cx, cy, czp;
                 unpack_cell(cell[pidx], cx, cy, czp);
-                const int bxm = (cx & (kTile - 1)) + (i % 3 - 1) * kTile + M_;   // bx + m, bx relative to the column
-                const int bym = (cy & (kTile - 1)) + (i / 3 - 1) * kTile + M_;
+                const int bxm = (cx & (kTile - 1)) + cull_dx;   // bx + m, bx relative to the column
+                const int bym = (cy & (kTile - 1)) + cull_dy;
                 if ((unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_)) {
                     const PRec<T> pr = rec[pidx];
                     int pk = bxm | (bym << 8);
@@ -164,8 +165,8 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
 
         for (int c0 = 0; c0 < total;) {
             // ---- cull: two candidates per thread; if more than CAP were accepted (dense clusters),
-            //      redo the chunk with one candidate per thread (at most NT = CAP accepted)
-            int span = 2 * NT;
+            //      redo the chunk with one candidate per thread (at most 9 * kCullT <= CAP accepted)
+            int span = 2 * kCullT;
             cull(c0, span);
             __syncthreads();
             int ns = nslot_s;
@@ -173,7 +174,7 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
                 __syncthreads();                 // every thread has read ns
                 if (tid == 0) nslot_s = 0;
                 __syncthreads();
-                span = NT;
+                span = kCullT;
                 cull(c0, span);
                 __syncthreads();
                 ns = nslot_s;
