@@ -195,7 +195,7 @@ int dev_alloc(enuf_plan* p, void** ptr, size_t bytes) {
 
 void free_workspace(enuf_plan* p) {
     auto fr = [](void* q) { if (q) cudaFree(q); };
-    fr(p->rec); fr(p->cell); fr(p->idx); fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
+    fr(p->rec); fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
     fr(p->scan_total);
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev); fr(p->fft_done);
@@ -215,7 +215,7 @@ void free_workspace(enuf_plan* p) {
     }
     p->prof_evals = 0;
     p->rec = p->spectrum = p->tw = p->iphi = p->wf = p->r_stage = p->q_stage = p->F_stage = nullptr;
-    p->cell = p->idx = p->bin_count = p->bin_offset = p->bin_cursor = p->scan_total = nullptr;
+    p->bin_count = p->bin_offset = p->bin_cursor = p->scan_total = nullptr;
     p->e_partial = p->e_dev = p->e_pinned = nullptr;
     p->fft_done = nullptr;
     p->events_valid = false;
@@ -252,9 +252,7 @@ int ensure_allocated(enuf_plan* p) {
     const int nfield = p->variant == ENUF_FORCE_IK ? 3 : 1;
     int rc;
 #define ALLOC(ptr, bytes) if ((rc = dev_alloc(p, (void**)&(ptr), (bytes)))) { free_workspace(p); return rc; }
-    ALLOC(p->rec, 4 * es * cap);
-    ALLOC(p->cell, 4 * cap);
-    ALLOC(p->idx, 4 * cap);
+    ALLOC(p->rec, (es == 4 ? sizeof(enuf::PSlot<float>) : sizeof(enuf::PSlot<double>)) * cap);
     ALLOC(p->bin_count, 4 * (size_t)p->tg.nbins);
     ALLOC(p->bin_offset, 4 * ((size_t)p->tg.nbins + 1));
     ALLOC(p->bin_cursor, 4 * (size_t)p->tg.nbins);

@@ -136,19 +136,18 @@ bin_scan_apply_kernel(const uint32_t* __restrict__ count, int nbins, const uint3
 template <typename T>
 __global__ void __launch_bounds__(256)
 bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, double L, TileGeom g,
-                   uint32_t* __restrict__ cursor,
-                   PRec<T>* __restrict__ rec, uint32_t* __restrict__ cell, uint32_t* __restrict__ idx) {
+                   uint32_t* __restrict__ cursor, PSlot<T>* __restrict__ slots) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     T qj = q[j];
     if (qj == (T)0) return;
     CellOfParticle p = locate(r, j, L, g.n);
     uint32_t pos = atomicAdd(&cursor[bin_of<T>(p, g)], 1u);
-    PRec<T> o;
-    o.dx = (T)p.d0[0]; o.dy = (T)p.d0[1]; o.dz = (T)p.d0[2]; o.q = qj;
-    rec[pos] = o;
-    cell[pos] = pack_cell(p.c[0], p.c[1], p.c[2]);
-    idx[pos] = (uint32_t)j;
+    PSlot<T> o;
+    o.rec.dx = (T)p.d0[0]; o.rec.dy = (T)p.d0[1]; o.rec.dz = (T)p.d0[2]; o.rec.q = qj;
+    o.cell = pack_cell(p.c[0], p.c[1], p.c[2]);
+    o.idx = (uint32_t)j;
+    slots[pos] = o;
 }
 
 }  // namespace enuf

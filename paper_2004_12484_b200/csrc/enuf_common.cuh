@@ -37,6 +37,10 @@ struct WindowParams {
 
 // One binned particle: fractional offset d0 per dimension and charge.
 template <typename T> struct alignas(4 * sizeof(T)) PRec { T dx, dy, dz, q; };
+// The sorted particle array: record, packed nearest cell and caller index side by side, so that the
+// scatter writes one 32-byte sector per particle (fp32) and the spreading cull, which first reads the
+// cell and then -- for the particles it keeps -- the record, finds the record in the line it just fetched.
+template <typename T> struct alignas(sizeof(T) == 4 ? 32 : 16) PSlot { PRec<T> rec; uint32_t cell, idx; };
 
 // Geometry shared by bin / spread / gather.  Particles are counting-sorted into bins
 //   bin = (Ty * nt + Tx) * n + cz,   Tx = cx / 16, Ty = cy / 16

@@ -78,8 +78,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 //              with pre = 2/L^2 (Eq. 42).
 template <typename T, int M_, bool kIk, bool kTrim = false>
 __global__ void __launch_bounds__(GatherCfg<M_, kTrim>::NT)
-gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
-              const uint32_t* __restrict__ cell, const uint32_t* __restrict__ idx,
+gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
               const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F) {
     using C = GatherCfg<M_, kTrim>;
@@ -170,7 +169,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
     auto batch_weights = [&](int p0, int nb) {
         if (lane < 3 * nb) {
             const int dim = lane / nb, slot = lane - dim * nb;
-            const PRec<T> pr = rec[start + p0 + slot];
+            const PRec<T> pr = slots[start + p0 + slot].rec;
             const T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
             T w[W], dw[W];
             stencil_weights<T, M_, !kIk, true>(wp, pa, d0, w, dw);   // packed Horner chains
@@ -185,7 +184,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
             }
             if (dim == 0) {
                 int cx, cy, cz;
-                unpack_cell(cell[start + p0 + slot], cx, cy, cz);
+                unpack_cell(slots[start + p0 + slot].cell, cx, cy, cz);
                 int zrel = cz - tz0;                  // trimmed bins: c_z may be the first plane of the next tile
                 zrel += zrel < 0 ? g.n : 0;
                 if (kTrim) {
@@ -193,7 +192,7 @@ gather_kernel(const T* __restrict__ field, const PRec<T>* __restrict__ rec,
                 }
                 base_s[slot] = zrel * SPL + (cy - ty0) * SX + (cx - tx0) + (C::XS - M_);
                 q_s[slot] = pre * pr.q;
-                idx_s[slot] = (int)idx[start + p0 + slot];
+                idx_s[slot] = (int)slots[start + p0 + slot].idx;
             }
         }
     };

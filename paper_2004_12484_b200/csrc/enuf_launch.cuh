@@ -103,8 +103,7 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     bin_scan_apply_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total, p->bin_offset,
                                                           p->bin_cursor);
     bin_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
-                                                 p->tg, p->bin_cursor, static_cast<PRec<T>*>(p->rec), p->cell,
-                                                 p->idx);
+                                                 p->tg, p->bin_cursor, static_cast<PSlot<T>*>(p->rec));
     return cudaGetLastError() == cudaSuccess ? 4 : -1;
 }
 
@@ -119,13 +118,13 @@ int launch_spread(enuf_plan* p) {
         if constexpr (M_ >= 5 && sizeof(T) == 4) {
             if (p->trim) {
                 spread_kernel<T, M_, true><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
-                    static_cast<const PRec<T>*>(p->rec), p->cell, p->bin_offset, p->tg, p->wp, pa, p->zchunk,
+                    static_cast<const PSlot<T>*>(p->rec), p->bin_offset, p->tg, p->wp, pa, p->zchunk,
                     static_cast<T*>(p->grid[0]));
                 return 0;
             }
         }
         spread_kernel<T, M_, false><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
-            static_cast<const PRec<T>*>(p->rec), p->cell, p->bin_offset, p->tg, p->wp, pa, p->zchunk,
+            static_cast<const PSlot<T>*>(p->rec), p->bin_offset, p->tg, p->wp, pa, p->zchunk,
             static_cast<T*>(p->grid[0]));
         return 0;
     });
@@ -236,14 +235,14 @@ int launch_gather(enuf_plan* p, void* F) {
             if (p->variant == ENUF_FORCE_ANALYTIC) {
                 const T pre = (T)(-(double)p->n / (PI * p->L * p->L));
                 gather_kernel<T, M_, false, kTrim><<<ntiles, C::NT, sb, s>>>(
-                    static_cast<const T*>(p->grid[0]), static_cast<const PRec<T>*>(p->rec), p->cell, p->idx,
+                    static_cast<const T*>(p->grid[0]), static_cast<const PSlot<T>*>(p->rec),
                     p->bin_offset, p->tg, p->wp, pa, pre, 0, static_cast<T*>(F));
                 return 1;
             }
             const T pre = (T)(2.0 / (p->L * p->L));
             for (int d = 0; d < 3; ++d)
                 gather_kernel<T, M_, true, kTrim><<<ntiles, C::NT, sb, s>>>(
-                    static_cast<const T*>(p->grid[d]), static_cast<const PRec<T>*>(p->rec), p->cell, p->idx,
+                    static_cast<const T*>(p->grid[d]), static_cast<const PSlot<T>*>(p->rec),
                     p->bin_offset, p->tg, p->wp, pa, pre, d, static_cast<T*>(F));
             return 3;
         };

@@ -28,9 +28,7 @@ struct enuf_plan {
     int launches = 0;
     int num_sms = 148;             // multiProcessorCount of the current device (persistent FFT grids)
     // device workspace
-    void* rec = nullptr;           // PRec<T>[N_cap]
-    uint32_t* cell = nullptr;      // [N_cap]
-    uint32_t* idx = nullptr;       // [N_cap]
+    void* rec = nullptr;           // PSlot<T>[N_cap]: record, packed cell, caller index (bin order)
     uint32_t* bin_count = nullptr;    // [nbins]
     uint32_t* bin_offset = nullptr;   // [nbins+1]
     uint32_t* bin_cursor = nullptr;   // [nbins]

@@ -62,7 +62,7 @@ constexpr size_t spread_smem_bytes() {
 // is WZ = 2m planes, and the warps test their cells against the 2m-point x / y extents.
 template <typename T, int M_, bool kTrim = false>
 __global__ void __launch_bounds__(SpreadCfg<M_>::NT, sizeof(T) == 4 ? 7 : 2)
-spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell,
+spread_kernel(const PSlot<T>* __restrict__ slots,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
               const __grid_constant__ PolyArg<M_> pa, int zchunk, T* __restrict__ grid) {
     using C = SpreadCfg<M_>;
@@ -137,11 +137,11 @@ spread_kernel(const PRec<T>* __restrict__ rec, const uint32_t* __restrict__ cell
             for (int c = c0 + cull_k; c < min(my_cnt, c0 + span); c += kCullT) {
                 const uint32_t pidx = (uint32_t)(my_start + c);
                 int cx, cy, czp;
-                unpack_cell(cell[pidx], cx, cy, czp);
+                unpack_cell(slots[pidx].cell, cx, cy, czp);
                 const int bxm = (cx & (kTile - 1)) + cull_dx;   // bx + m, bx relative to the column
                 const int bym = (cy & (kTile - 1)) + cull_dy;
                 if ((unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_)) {
-                    const PRec<T> pr = rec[pidx];
+                    const PRec<T> pr = slots[pidx].rec;
                     int pk = bxm | (bym << 8);
                     if (kTrim) pk |= (pr.dx > (T)0 ? 1 << 16 : 0) | (pr.dy > (T)0 ? 1 << 17 : 0);
                     // which of the four 8 x 8 warp patches the stencil touches (bits 20..23, warp order):
