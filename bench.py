@@ -353,16 +353,22 @@ def run_ours(args):
     for st in ("bin", "spread", "fft", "gather"):
         gbs = abytes[st] / (stage_ms[st] * 1e-3) / 1e9 if stage_ms[st] > 0 else 0.0
         stages[st] = {"ms": stage_ms[st], "algorithmic_bytes": abytes[st], "GBps": gbs, "hbm_frac": gbs / peak}
+    # spread and gather are bound by FP32 FMA issue, not by HBM: their ALU fractions too
+    W3 = (2 * w.m + 1) ** 3
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak_tf = 148 * 128 * 2 * sm_max * 1e6 / 1e12
+    for st, per in (("spread", 1), ("gather", 3 if args.variant == "ik" else 2)):
+        if stages[st]["ms"] > 0:
+            tf = 2.0 * per * W3 * n_charged / (stages[st]["ms"] * 1e-3) / 1e12
+            stages[st]["alu_TFLOPs"] = tf
+            stages[st]["alu_frac"] = tf / peak_tf
     dom = max(stages, key=lambda k: stages[k]["ms"])
     if dom in ("spread", "gather"):
         # these two stages are bound by FP32 FMA issue, not by HBM.  Algorithmic
         # work = (2m+1)^3 FMAs per charged particle (spread), twice that for the analytic gather
         # (field x window and field x window derivative), three times for the ik gather.
-        W3 = (2 * w.m + 1) ** 3
         per = {"spread": 1, "gather": 3 if args.variant == "ik" else 2}[dom]
         flops = 2.0 * per * W3 * n_charged
-        sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
-        peak_tf = 148 * 128 * 2 * sm_max * 1e6 / 1e12
         ach = flops / (stages[dom]["ms"] * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
                     "frac": ach / peak_tf, "traffic": recorded_traffic(dom),
