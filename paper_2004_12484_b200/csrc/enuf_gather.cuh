@@ -2,8 +2,8 @@
 //
 // One CTA per 16^3 grid tile, working on the tile's particles (a contiguous range of 16
 // bins, TileGeom), with the tile plus a halo of m cells per side ((16+2m)^3 values) held in
-// shared memory (staged with cp.async).  Every warp takes the tile's particles five at a
-// time: first the 3 W window values and derivatives of those particles are computed once
+// shared memory (staged with cp.async).  Every warp takes a contiguous share of the tile's
+// particles (shares differ by at most one), five at a time: first the 3 W window values and derivatives of those particles are computed once
 // (one lane per particle and dimension) and kept on chip, then the warp
 // contracts the (2m+1)^3 stencil of one particle after the other: every lane owns x-rows of
 // the stencil (row strides chosen so that the 32 rows a warp reads at once fall in 32
