@@ -575,6 +575,36 @@ int enuf_forces_from_spectrum(enuf_plan* p, void* F, double* E) {
     return ENUF_OK;
 }
 
+namespace {
+// Chebyshev interpolant of degree kErfcDeg of g(t) = exp(x^2) erfc(x) / t, x = 2 (1/t - 1), on t in
+// [1/(1 + xmax/2), 1], converted to monomials in u = ua t + ub in [-1, 1] (enuf_real.cuh, ErfcFit).
+void build_erfc_fit(enuf_plan* p, double xmax) {
+    constexpr int D = enuf::kErfcDeg, NC = D + 1;
+    const double tmin = 1.0 / (1.0 + 0.5 * xmax), ua = 2.0 / (1.0 - tmin), ub = -(1.0 + tmin) / (1.0 - tmin);
+    long double a[NC];
+    for (int k = 0; k < NC; ++k) {
+        long double acc = 0;
+        for (int i = 0; i < NC; ++i) {
+            const double th = kPi * (i + 0.5) / NC, u = std::cos(th);
+            const double t = (u - ub) / ua, x = 2.0 * (1.0 / t - 1.0);
+            acc += (long double)(std::exp(x * x) * std::erfc(x) / t) * std::cos(k * th);
+        }
+        a[k] = acc * (k == 0 ? 1.0L : 2.0L) / NC;
+    }
+    // T_0 = 1, T_1 = u, T_{k+1} = 2 u T_k - T_{k-1}
+    long double c[NC] = {0}, t0[NC] = {0}, t1[NC] = {0}, t2[NC];
+    t0[0] = 1; t1[1] = 1;
+    for (int e = 0; e < NC; ++e) c[e] = a[0] * t0[e] + a[1] * t1[e];
+    for (int k = 2; k < NC; ++k) {
+        for (int e = 0; e < NC; ++e) t2[e] = (e > 0 ? 2 * t1[e - 1] : 0.0L) - t0[e];
+        for (int e = 0; e < NC; ++e) { c[e] += a[k] * t2[e]; t0[e] = t1[e]; t1[e] = t2[e]; }
+    }
+    for (int k = 0; k < NC; ++k) p->erfc_c[k] = (float)c[k];
+    p->erfc_ua = (float)ua; p->erfc_ub = (float)ub;
+    p->erfc_xmax = xmax;
+}
+}  // namespace
+
 int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, int accumulate, void* F,
                     double* E_real, double* E_self) {
     g_err[0] = 0;
@@ -614,6 +644,10 @@ int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, in
         p->real_ncells_cap = ncells;
     }
     p->real_ncd = ncd; p->real_s = s;
+    {
+        const double xmax = p->alpha * r_cut * 1.0001;       // x = alpha d <= alpha r_cut
+        if (xmax > p->erfc_xmax || xmax < 0.5 * p->erfc_xmax) build_erfc_fit(p, xmax);
+    }
     p->launches = 0;
     if (p->N == 0) {
         CU(cudaMemsetAsync(p->real_e_dev, 0, 16, p->stream));

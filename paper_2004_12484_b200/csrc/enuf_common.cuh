@@ -13,6 +13,7 @@ namespace enuf {
 
 constexpr int kMaxM = 6;            // largest supported window cut-off
 constexpr int kMaxW = 2 * kMaxM + 1;
+constexpr int kErfcDeg = 10;        // degree of the fp32 erfc fit of the real-space pair term (enuf_real.cuh)
 constexpr int kLinesPerGroup = 8;   // FFT: consecutive kx handled together (64 B of complex fp32)
 
 template <typename T> struct Cx2;

@@ -274,14 +274,17 @@ int launch_real(enuf_plan* p, const void* r, const void* q, double r_cut, int ac
                                                   p->real_cursor, static_cast<V4*>(p->real_pos), p->real_idx);
     const unsigned fblocks = (unsigned)((N + kRealThreads - 1) / kRealThreads);
     const T alpha = (T)p->alpha, rc2 = (T)(r_cut * r_cut);
+    ErfcFit ef;
+    for (int k = 0; k <= kErfcDeg; ++k) ef.c[k] = p->erfc_c[k];
+    ef.ua = p->erfc_ua; ef.ub = p->erfc_ub;
     if (p->lambda > 0.0)
         real_force_kernel<T, true><<<fblocks, kRealThreads, 0, s>>>(
             static_cast<const V4*>(p->real_pos), p->real_idx, p->real_offset, ncells, g, alpha, rc2,
-            (T)(1.0 / p->lambda), accumulate, static_cast<T*>(F), p->real_partial);
+            (T)(1.0 / p->lambda), ef, accumulate, static_cast<T*>(F), p->real_partial);
     else
         real_force_kernel<T, false><<<fblocks, kRealThreads, 0, s>>>(
             static_cast<const V4*>(p->real_pos), p->real_idx, p->real_offset, ncells, g, alpha, rc2, (T)0,
-            accumulate, static_cast<T*>(F), p->real_partial);
+            ef, accumulate, static_cast<T*>(F), p->real_partial);
     real_energy_finish_kernel<<<1, 256, 0, s>>>(p->real_partial, (int)fblocks, 0.5,
                                                p->alpha * 0.56418958354775628694807945156077, p->real_e_dev);
     return cudaGetLastError() == cudaSuccess ? 6 : -1;

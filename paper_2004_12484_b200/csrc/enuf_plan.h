@@ -60,6 +60,9 @@ struct enuf_plan {
     double* real_e_pinned = nullptr;  // [2] host
     int real_ncells_cap = 0;          // cells the count/offset/cursor buffers hold
     int real_ncd = 0, real_s = 0;     // geometry of the last call
+    float erfc_c[16] = {};            // fp32 erfc fit of the pair term (enuf_real.cuh, ErfcFit), for x <= erfc_xmax
+    float erfc_ua = 0.f, erfc_ub = 0.f;
+    double erfc_xmax = -1.0;
     void* r_stage = nullptr;       // host-API staging: r, q, F
     void* q_stage = nullptr;
     void* F_stage = nullptr;

@@ -18,6 +18,16 @@
 
 namespace enuf {
 
+// erfc for the fp32 pair term: erfc(x) = exp(-x^2) t P(u), t = 1/(1 + x/2), u = ua t + ub in [-1, 1], with P
+// the degree-10 Chebyshev interpolant (as monomials in u) of exp(x^2) erfc(x)/t on 0 <= x <= alpha r_cut,
+// fitted in fp64 when the real-space part is first used (relative error <= 4e-9 for alpha r_cut <= 8, far
+// below fp32 rounding).  The exponential is the one the Gaussian term of the force needs anyway, so the
+// pair term costs one expf instead of erfcf + expf.
+struct ErfcFit {
+    float c[kErfcDeg + 1];
+    float ua, ub;
+};
+
 struct RealGeom {
     int ncd;        // cells per dimension
     int s;          // neighbour range in cells (0: single cell, all pairs)
@@ -94,7 +104,8 @@ template <typename T, bool kSlater>
 __global__ void __launch_bounds__(kRealThreads)
 real_force_kernel(const typename Vec4<T>::type* __restrict__ pos, const uint32_t* __restrict__ idx,
                   const uint32_t* __restrict__ offset, int ncells, RealGeom g, T alpha, T r_cut2,
-                  T inv_lambda, int accumulate, T* __restrict__ F, double* __restrict__ partial) {
+                  T inv_lambda, const __grid_constant__ ErfcFit ef, int accumulate, T* __restrict__ F,
+                  double* __restrict__ partial) {
     using V4 = typename Vec4<T>::type;
     const uint32_t i = blockIdx.x * kRealThreads + threadIdx.x;
     const uint32_t n_sorted = offset[ncells];          // number of charged particles
@@ -117,9 +128,19 @@ real_force_kernel(const typename Vec4<T>::type* __restrict__ pos, const uint32_t
             if (d2 <= r_cut2 && other) {
                 const T d = r_sqrt(d2), inv_d = (T)1 / d;
                 const T ad = alpha * d;
-                const T ec = r_erfc(ad);
+                const T ex = r_exp(-ad * ad);
+                T ec;
+                if (sizeof(T) == 4) {
+                    const float t = __frcp_rn(fmaf(0.5f, (float)ad, 1.0f)), u = fmaf(t, ef.ua, ef.ub);
+                    float P = ef.c[kErfcDeg];
+#pragma unroll
+                    for (int k = kErfcDeg - 1; k >= 0; --k) P = fmaf(P, u, ef.c[k]);
+                    ec = (T)(t * P) * ex;
+                } else {
+                    ec = r_erfc(ad);
+                }
                 T eterm = ec * inv_d;
-                T g_ = (eterm * inv_d + two_a_sqrtpi * r_exp(-ad * ad) * inv_d) * inv_d;
+                T g_ = (eterm * inv_d + two_a_sqrtpi * ex * inv_d) * inv_d;
                 if (kSlater) {
                     const T x = d * inv_lambda, ex = r_exp(-(T)2 * x);
                     eterm *= (T)1 - ((T)1 + x) * ex;                           // B_U, Eq. 57
