@@ -74,8 +74,9 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* st = reinterpret_cast<T*>(smem_raw);            // [CAP + 1][RP] staged particle records; slot CAP is all zero
     int* sb = reinterpret_cast<int*>(st + (CAP + 1) * RP);   // [CAP] (bx + m) | (by + m) << 8 | ks_x << 16 | ks_y << 17
-    __shared__ int rng_start[2][9], rng_cnt[2][9], rng_max[2];
-    __shared__ int nslot_s;
+    __shared__ int rng_start[3][9], rng_cnt[3][9], rng_max[3];   // bin ranges of the slabs s - 1 / s / s + 1 / s + 2 (ring)
+    __shared__ int nslot_s[2];                                   // staged count of the current / next round
+    __shared__ unsigned char smask[CAP];                         // patch mask of a staged slot (copy of sb >> 20)
     // per warp: byte offsets (into st) of the staged particles that overlap the warp's cells, compacted
     __shared__ __align__(8) unsigned wlist[NT / 32][68];
 
@@ -110,9 +111,12 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
     constexpr int kCullT = NT / 9;
     const int cull_i = tid / kCullT < 9 ? tid / kCullT : -1, cull_k = tid % kCullT;
     const int cull_dx = (cull_i % 3 - 1) * kTile + M_, cull_dy = (cull_i / 3 - 1) * kTile + M_;
-    if (tid == 0) nslot_s = 0;
+    const int s_begin = z0 - SLO, s_end = z1 + SHI;
+    if (tid == 0) { nslot_s[0] = 0; nslot_s[1] = 0; }
     if (tid < RP) st[CAP * RP + tid] = (T)0;           // the padding record of odd-length visit lists
-    load_ranges(z0 - SLO, 0);
+    load_ranges(s_begin, 0);
+    if (s_begin + 1 < s_end) load_ranges(s_begin + 1, 1);
+    __syncthreads();
 
     P2 acc[WZ];
 #pragma unroll
@@ -123,17 +127,20 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
     const char* lane_yb = reinterpret_cast<const char*>(st + OY + ly);
     const char* st_zb = reinterpret_cast<const char*>(st + OZ);
 
-    int buf = 0;
-    for (int s = z0 - SLO; s < z1 + SHI; ++s, buf ^= 1) {
-        __syncthreads();      // ranges of slab s visible; all warps are done with the previous slab
-        if (s + 1 < z1 + SHI) load_ranges(s + 1, buf ^ 1);
-        const int total = rng_max[buf];                        // candidates of the fullest of the 9 bins
-        const int my_start = cull_i >= 0 ? rng_start[buf][cull_i] : 0;
-        const int my_cnt = cull_i >= 0 ? rng_cnt[buf][cull_i] : 0;
-
+    // The kernel proceeds in rounds: one round = one chunk of candidates of one slab (a slab is a single round
+    // unless a bin holds more than 2 kCullT particles or more than CAP were accepted):
+    //   cull -> barrier -> window values -> barrier -> accumulate -> [slab done: store a plane, slide] -> cull of the
+    //   NEXT round.  The cull only writes the packed positions sb[] and the raw records (words OD..OD+3 of a slot),
+    //   which the accumulate phase does not read (it uses the rows and smask[]), so a warp that finishes its visits
+    //   early culls the next round while the others are still accumulating: two barriers per round, and the
+    //   cull's global-load latency overlaps the tail of the accumulate phase.
+    int s = s_begin, rb = 0, c0 = 0, kk = 0, span = 2 * kCullT;
+    {
         // cull the candidates [c0, c0 + span) of every bin against the column's halo: accepted ones are
         // staged (record + packed position) while slots last; returns nothing, the count is nslot_s
-        auto cull = [&](int c0, int span) {
+        auto cull = [&](int rbuf, int c0, int span, int kk) {
+            const int my_start = cull_i >= 0 ? rng_start[rbuf][cull_i] : 0;
+            const int my_cnt = cull_i >= 0 ? rng_cnt[rbuf][cull_i] : 0;
             for (int c = c0 + cull_k; c < min(my_cnt, c0 + span); c += kCullT) {
                 const uint32_t pidx = (uint32_t)(my_start + c);
                 int cx, cy, czp;
@@ -153,7 +160,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
                     const int mask = (oy & 1 ? ox : 0) | (oy & 2 ? ox << 2 : 0);
                     // a trimmed stencil at the far edge of the halo misses the column altogether: not staged
                     if (mask != 0) {
-                        const int slot = atomicAdd(&nslot_s, 1);
+                        const int slot = atomicAdd(&nslot_s[kk], 1);
                         if (slot < CAP) {
                             *reinterpret_cast<PRec<T>*>(st + slot * RP + OD) = pr;
                             sb[slot] = pk | (mask << 20);
@@ -163,22 +170,23 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
             }
         };
 
-        for (int c0 = 0; c0 < total;) {
-            // ---- cull: two candidates per thread; if more than CAP were accepted (dense clusters),
-            //      redo the chunk with one candidate per thread (at most 9 * kCullT <= CAP accepted)
-            int span = 2 * kCullT;
-            cull(c0, span);
-            __syncthreads();
-            int ns = nslot_s;
+        cull(rb, c0, span, kk);                                // round 0
+        for (;;) {
+            __syncthreads();                                   // this round's cull is complete; rows and smask are free
+            int ns = nslot_s[kk];
             if (ns > CAP) {
+                // more than CAP accepted (dense clusters): redo the chunk with one candidate per thread
+                // (at most 9 * kCullT <= CAP accepted)
                 __syncthreads();                 // every thread has read ns
-                if (tid == 0) nslot_s = 0;
+                if (tid == 0) nslot_s[kk] = 0;
                 __syncthreads();
                 span = kCullT;
-                cull(c0, span);
+                cull(rb, c0, span, kk);
                 __syncthreads();
-                ns = nslot_s;
+                ns = nslot_s[kk];
             }
+            if (tid == 0) nslot_s[kk ^ 1] = 0;                 // counter of the next round (nobody touches it now)
+            if (c0 == 0 && s + 2 < s_end) load_ranges(s + 2, rb == 0 ? 2 : rb - 1);   // ring slot of slab s - 1
             // ---- window values: one task per (dimension, slot); dimension-major so warps stay uniform
             for (int t = tid; t < 3 * ns; t += NT) {
                 const int dim = (t >= ns ? 1 : 0) + (t >= 2 * ns ? 1 : 0), slot = t - dim * ns;   // t < 3 ns
@@ -187,6 +195,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
                 stencil_weights<T, M_, false>(wp, pa, d0, w, dw);
                 using V4 = typename Vec4<T>::type;
                 if (dim == 2) {
+                    smask[slot] = (unsigned char)((unsigned)sb[slot] >> 20);
                     const T q = st[slot * RP + OD + 3];
                     T r16[16];
 #pragma unroll
@@ -210,12 +219,11 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
                 }
             }
             __syncthreads();
-            if (tid == 0) nslot_s = 0;      // every thread has read ns; the next cull starts after a barrier
             // ---- accumulate: each warp visits the staged particles that overlap its 8 x 8 cells
             for (int e0 = 0; e0 < ns; e0 += 64) {                      // 64 staged slots per pass
                 // patch mask from the cull: does slot e0 + lane / e0 + 32 + lane touch this warp's cells?
-                const bool ov0 = e0 + lane < ns && ((sb[e0 + lane] >> (20 + warp)) & 1);
-                const bool ov1 = e0 + 32 + lane < ns && ((sb[e0 + 32 + lane] >> (20 + warp)) & 1);
+                const bool ov0 = e0 + lane < ns && ((smask[e0 + lane] >> warp) & 1);
+                const bool ov1 = e0 + 32 + lane < ns && ((smask[e0 + 32 + lane] >> warp) & 1);
                 const unsigned om0 = __ballot_sync(0xffffffffu, ov0), om1 = __ballot_sync(0xffffffffu, ov1);
                 const int cnt0 = __popc(om0), cnt = cnt0 + __popc(om1);
                 if (cnt == 0) continue;
@@ -254,15 +262,22 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
                 }
                 __syncwarp();                    // the list is rewritten by the next group of 64 slots
             }
+            // ---- next round: the rest of this slab, or the next slab after storing the finished plane
             c0 += span;
-            if (c0 < total) __syncthreads();           // staging buffers are reused by the next chunk
-        }
-        // ---- the lowest plane of the window (s - m, trimmed: s - m + 1) is complete: store it, slide
-        const int zo = s - SHI;
-        if (zo >= z0) *reinterpret_cast<P2*>(gout + (size_t)zo * g.n * g.n) = acc[0];
+            span = 2 * kCullT;
+            if (c0 >= rng_max[rb]) {
+                // the lowest plane of the window (s - m, trimmed: s - m + 1) is complete: store it, slide
+                const int zo = s - SHI;
+                if (zo >= z0) *reinterpret_cast<P2*>(gout + (size_t)zo * g.n * g.n) = acc[0];
 #pragma unroll
-        for (int k = 0; k + 1 < WZ; ++k) acc[k] = acc[k + 1];
-        acc[WZ - 1].x = (T)0; acc[WZ - 1].y = (T)0;
+                for (int k = 0; k + 1 < WZ; ++k) acc[k] = acc[k + 1];
+                acc[WZ - 1].x = (T)0; acc[WZ - 1].y = (T)0;
+                ++s; rb = rb == 2 ? 0 : rb + 1; c0 = 0;
+                if (s >= s_end) break;
+            }
+            kk ^= 1;
+            cull(rb, c0, span, kk);                            // no barrier: see the comment above the loop
+        }
     }
 }
 
