@@ -220,6 +220,8 @@ void free_workspace(enuf_plan* p) {
     p->fft_done = nullptr;
     p->events_valid = false;
     p->partial_ready = false;
+    p->bin_count_clean = false;
+    p->real_count_clean = false;
     p->allocated = false;
     p->workspace_bytes = 0;
     (void)cudaGetLastError();
@@ -642,6 +644,7 @@ int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, in
         if ((rc = dev_alloc(p, (void**)&p->real_cursor, 4 * (size_t)ncells))) return rc;
         if ((rc = dev_alloc(p, (void**)&p->real_scan_total, 4 * (((size_t)ncells + 1023) / 1024)))) return rc;
         p->real_ncells_cap = ncells;
+        p->real_count_clean = false;
     }
     p->real_ncd = ncd; p->real_s = s;
     {

@@ -62,7 +62,8 @@ bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict
 // the scatter's running positions).  Two launches of kScanThreads threads per CTA, each
 // CTA owning kScanChunk = 4 * kScanThreads consecutive bins:
 //   bin_scan_totals: total[b] = sum of chunk b
-//   bin_scan_apply : base = sum of total[< b] (few hundred values at most), then a CTA scan.
+//   bin_scan_apply : base = sum of total[< b] (few hundred values at most), then a CTA scan; it also
+//                    clears count[] behind itself, so only the first evaluation needs a memset.
 constexpr int kScanThreads = 256;
 constexpr int kScanChunk = 4 * kScanThreads;
 
@@ -86,7 +87,7 @@ bin_scan_totals_kernel(const uint32_t* __restrict__ count, int nbins, uint32_t* 
 }
 
 static __global__ void __launch_bounds__(kScanThreads)
-bin_scan_apply_kernel(const uint32_t* __restrict__ count, int nbins, const uint32_t* __restrict__ total,
+bin_scan_apply_kernel(uint32_t* __restrict__ count, int nbins, const uint32_t* __restrict__ total,
                       uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor) {
     __shared__ uint32_t ws[kScanThreads / 32];
     __shared__ uint32_t base_s;
@@ -110,7 +111,11 @@ bin_scan_apply_kernel(const uint32_t* __restrict__ count, int nbins, const uint3
     const int i0 = blockIdx.x * kScanChunk + threadIdx.x * 4;
     uint32_t c[4], sum = 0;
 #pragma unroll
-    for (int e = 0; e < 4; ++e) { c[e] = i0 + e < nbins ? count[i0 + e] : 0u; sum += c[e]; }
+    for (int e = 0; e < 4; ++e) {
+        c[e] = i0 + e < nbins ? count[i0 + e] : 0u;
+        sum += c[e];
+        if (i0 + e < nbins) count[i0 + e] = 0u;      // the histogram is left cleared for the next evaluation
+    }
     uint32_t inc = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {

@@ -94,7 +94,9 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     cudaStream_t s = p->stream;
     const int64_t N = p->N;
     const int nbins = p->tg.nbins;
-    if (cudaMemsetAsync(p->bin_count, 0, sizeof(uint32_t) * nbins, s) != cudaSuccess) return -1;
+    // the scan clears the histogram behind itself: a memset is needed only when that did not happen
+    if (!p->bin_count_clean && cudaMemsetAsync(p->bin_count, 0, sizeof(uint32_t) * nbins, s) != cudaSuccess) return -1;
+    p->bin_count_clean = false;
     const unsigned blocks = (unsigned)((N + 255) / 256);
     const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
     bin_count_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q),
@@ -104,7 +106,9 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
                                                           p->bin_cursor);
     bin_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
                                                  p->tg, p->bin_cursor, static_cast<PSlot<T>*>(p->rec));
-    return cudaGetLastError() == cudaSuccess ? 4 : -1;
+    if (cudaGetLastError() != cudaSuccess) return -1;
+    p->bin_count_clean = true;
+    return 4;
 }
 
 template <typename T>
@@ -262,7 +266,8 @@ int launch_real(enuf_plan* p, const void* r, const void* q, double r_cut, int ac
     const RealGeom g{p->real_ncd, p->real_s, p->L};
     const int ncells = g.ncd * g.ncd * g.ncd;
     using V4 = typename Vec4<T>::type;
-    if (cudaMemsetAsync(p->real_count, 0, sizeof(uint32_t) * ncells, s) != cudaSuccess) return -1;
+    if (!p->real_count_clean && cudaMemsetAsync(p->real_count, 0, sizeof(uint32_t) * ncells, s) != cudaSuccess) return -1;
+    p->real_count_clean = false;
     const unsigned blocks = (unsigned)((N + 255) / 256);
     const unsigned sblocks = (unsigned)((ncells + kScanChunk - 1) / kScanChunk);
     real_count_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), static_cast<T*>(F),
@@ -287,7 +292,9 @@ int launch_real(enuf_plan* p, const void* r, const void* q, double r_cut, int ac
             ef, accumulate, static_cast<T*>(F), p->real_partial);
     real_energy_finish_kernel<<<1, 256, 0, s>>>(p->real_partial, (int)fblocks, 0.5,
                                                p->alpha * 0.56418958354775628694807945156077, p->real_e_dev);
-    return cudaGetLastError() == cudaSuccess ? 6 : -1;
+    if (cudaGetLastError() != cudaSuccess) return -1;
+    p->real_count_clean = true;      // the scan cleared the cell histogram (all real_ncells_cap entries beyond ncells stay 0)
+    return 6;
 }
 
 }  // namespace enuf

@@ -22,6 +22,8 @@ struct enuf_plan {
     enuf::WindowParams wp{};
     int Kxp = 0, Ky = 0;
     bool allocated = false, tables_dirty = true, evaluated = false;
+    bool bin_count_clean = false;  // bin_count is all zero (left so by the last scan)
+    bool real_count_clean = false; // same for real_count
     bool partial_ready = false;    // enuf_spectrum_partial has run and enuf_forces_from_spectrum has not yet
     size_t esize = 4;              // bytes per real
     size_t workspace_bytes = 0;
