@@ -196,7 +196,7 @@ int dev_alloc(enuf_plan* p, void** ptr, size_t bytes) {
 void free_workspace(enuf_plan* p) {
     auto fr = [](void* q) { if (q) cudaFree(q); };
     fr(p->rec); fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
-    fr(p->scan_total);
+    fr(p->scan_total); fr(p->scan_desc); p->scan_desc = nullptr;
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev); fr(p->fft_done);
     fr(p->r_stage); fr(p->q_stage); fr(p->F_stage);
@@ -259,6 +259,7 @@ int ensure_allocated(enuf_plan* p) {
     ALLOC(p->bin_offset, 4 * ((size_t)p->tg.nbins + 1));
     ALLOC(p->bin_cursor, 4 * (size_t)p->tg.nbins);
     ALLOC(p->scan_total, 4 * (((size_t)p->tg.nbins + 1023) / 1024));
+    ALLOC(p->scan_desc, 8 * (((size_t)p->tg.nbins + 1023) / 1024));
     for (int d = 0; d < nfield; ++d) {
         ALLOC(p->grid[d], es * n3);
         ALLOC(p->A1[d], 2 * es * n * n * p->Kxp);
@@ -295,6 +296,8 @@ int ensure_allocated(enuf_plan* p) {
     if (p->spectrum) cudaMemsetAsync(p->spectrum, 0, 2 * es * (size_t)p->Ky * p->Ky * p->Kxp, p->stream);
     cudaMemsetAsync(p->e_dev, 0, 8, p->stream);
     cudaMemsetAsync(p->fft_done, 0, 4, p->stream);
+    cudaMemsetAsync(p->scan_desc, 0, 8 * (((size_t)p->tg.nbins + 1023) / 1024), p->stream);
+    p->scan_epoch = 0;
     rc = p->precision == ENUF_F32 ? enuf::configure_kernels<float>(p) : enuf::configure_kernels<double>(p);
     if (rc) {
         cudaError_t le = cudaGetLastError();

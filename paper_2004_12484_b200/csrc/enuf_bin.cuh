@@ -136,6 +136,70 @@ bin_scan_apply_kernel(uint32_t* __restrict__ count, int nbins, const uint32_t* _
     if (i0 <= nbins - 1 && nbins - 1 < i0 + 4) offset[nbins] = run;   // thread owning the last bin
 }
 
+// Single-launch variant for histograms of at most kScanMaxResident chunks (every CTA is resident at once, so a
+// CTA may wait for its predecessors): chunk b publishes (epoch << 32 | its total) in desc[b] and sums the
+// totals of the chunks before it as they appear (decoupled look-back without the aggregate chain -- with <= 64
+// chunks reading all predecessors is cheaper than chaining).  `epoch` changes with every launch, so desc[] is
+// never reset.
+constexpr int kScanMaxResident = 128;
+static __global__ void __launch_bounds__(kScanThreads)
+bin_scan_single_kernel(uint32_t* __restrict__ count, int nbins, unsigned long long* __restrict__ desc,
+                       uint32_t epoch, uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor) {
+    __shared__ uint32_t ws[kScanThreads / 32];
+    __shared__ uint32_t base_s;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int i0 = blockIdx.x * kScanChunk + threadIdx.x * 4;
+    uint32_t c[4], sum = 0;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        c[e] = i0 + e < nbins ? count[i0 + e] : 0u;
+        sum += c[e];
+        if (i0 + e < nbins) count[i0 + e] = 0u;      // the histogram is left cleared for the next evaluation
+    }
+    // inclusive scan of the per-thread sums inside the CTA
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) ws[wid] = inc;
+    __syncthreads();
+    uint32_t wbase = 0, ctot = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) { if (w < wid) wbase += ws[w]; ctot += ws[w]; }
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicExch(&desc[blockIdx.x], ((unsigned long long)epoch << 32) | ctot);
+    }
+    // totals of the chunks before this one
+    uint32_t part = 0;
+    for (int i = threadIdx.x; i < (int)blockIdx.x; i += kScanThreads) {
+        unsigned long long d;
+        do { d = *reinterpret_cast<volatile unsigned long long*>(&desc[i]); } while ((uint32_t)(d >> 32) != epoch);
+        part += (uint32_t)d;
+    }
+    __syncthreads();                                  // ws is reused
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if (lane == 0) ws[wid] = part;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t b = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) b += ws[w];
+        base_s = b;
+    }
+    __syncthreads();
+    uint32_t run = base_s + wbase + inc - sum;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        if (i0 + e < nbins) { offset[i0 + e] = run; cursor[i0 + e] = run; }
+        run += c[e];
+    }
+    if (i0 <= nbins - 1 && nbins - 1 < i0 + 4) offset[nbins] = run;   // thread owning the last bin
+}
+
 // Scatter into bin order.  The order inside a bin follows the atomic cursor (any order is
 // a valid sort; sums downstream differ only in rounding order, R22).
 template <typename T>

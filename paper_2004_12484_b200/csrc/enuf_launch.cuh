@@ -101,14 +101,22 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
     bin_count_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q),
                                                static_cast<T*>(F), N, p->L, p->tg, p->bin_count);
-    bin_scan_totals_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total);
-    bin_scan_apply_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total, p->bin_offset,
-                                                          p->bin_cursor);
+    int nlaunch = 4;
+    if ((int)sblocks <= kScanMaxResident && (int)sblocks <= p->num_sms) {
+        // every scan CTA is resident at once: one launch, chunk totals exchanged through scan_desc
+        bin_scan_single_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_desc, ++p->scan_epoch,
+                                                                p->bin_offset, p->bin_cursor);
+        nlaunch = 3;
+    } else {
+        bin_scan_totals_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total);
+        bin_scan_apply_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total, p->bin_offset,
+                                                              p->bin_cursor);
+    }
     bin_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
                                                  p->tg, p->bin_cursor, static_cast<PSlot<T>*>(p->rec));
     if (cudaGetLastError() != cudaSuccess) return -1;
     p->bin_count_clean = true;
-    return 4;
+    return nlaunch;
 }
 
 template <typename T>

@@ -35,6 +35,8 @@ struct enuf_plan {
     uint32_t* bin_offset = nullptr;   // [nbins+1]
     uint32_t* bin_cursor = nullptr;   // [nbins]
     uint32_t* scan_total = nullptr;   // [ceil(nbins / kScanChunk)]
+    unsigned long long* scan_desc = nullptr;   // [ceil(nbins / kScanChunk)] (epoch << 32 | chunk total), single-launch scan
+    uint32_t scan_epoch = 0;
     float poly_c[enuf::kPolyMaxDeg + 1][enuf::kMaxM + 1] = {};   // host copy of the polynomial window table
     float poly_d[enuf::kPolyMaxDeg][enuf::kMaxM + 1] = {};       // (fp32 path; packed into PolyArg<m> per launch)
     int zchunk = 0;                   // grid planes per spread CTA
