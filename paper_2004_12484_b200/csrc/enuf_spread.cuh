@@ -141,10 +141,15 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
         auto cull = [&](int rbuf, int c0, int span, int kk) {
             const int my_start = cull_i >= 0 ? rng_start[rbuf][cull_i] : 0;
             const int my_cnt = cull_i >= 0 ? rng_cnt[rbuf][cull_i] : 0;
-            for (int c = c0 + cull_k; c < min(my_cnt, c0 + span); c += kCullT) {
-                const uint32_t pidx = (uint32_t)(my_start + c);
+            // a thread has at most two candidates per chunk (span <= 2 kCullT): both cells are loaded before
+            // either is examined, so the chunk costs one global-load latency, not two
+            const int cend = min(my_cnt, c0 + span);
+            const int ca = c0 + cull_k, cb = ca + kCullT;
+            const uint32_t cell_a = ca < cend ? slots[my_start + ca].cell : 0u;
+            const uint32_t cell_b = cb < cend ? slots[my_start + cb].cell : 0u;
+            auto examine = [&](uint32_t pidx, uint32_t cellv) {
                 int cx, cy, czp;
-                unpack_cell(slots[pidx].cell, cx, cy, czp);
+                unpack_cell(cellv, cx, cy, czp);
                 const int bxm = (cx & (kTile - 1)) + cull_dx;   // bx + m, bx relative to the column
                 const int bym = (cy & (kTile - 1)) + cull_dy;
                 if ((unsigned)bxm < (unsigned)(kTile + 2 * M_) && (unsigned)bym < (unsigned)(kTile + 2 * M_)) {
@@ -167,7 +172,9 @@ spread_kernel(const PSlot<T>* __restrict__ slots,
                         }
                     }
                 }
-            }
+            };
+            if (ca < cend) examine((uint32_t)(my_start + ca), cell_a);
+            if (cb < cend) examine((uint32_t)(my_start + cb), cell_b);
         };
 
         cull(rb, c0, span, kk);                                // round 0
