@@ -54,8 +54,13 @@ enum enuf_option {
     ENUF_OPT_NUM_PARTICLES = 5,  /* lower N for the next calls, 0 <= N <= planned capacity          */
     ENUF_OPT_PROFILE = 6,        /* 1: record per-stage CUDA-event times (enuf_plan_stage_ms)        */
     ENUF_OPT_KEEP_SPECTRUM = 7,  /* 1: also store S~(n) so enuf_plan_structure_factor() can read it  */
-    ENUF_OPT_SPREAD_ZCHUNK = 8   /* tuning: grid planes per spreading CTA (power of two, 8..n);
+    ENUF_OPT_SPREAD_ZCHUNK = 8,  /* tuning: grid planes per spreading CTA (power of two, 8..n);
                                     default fills the SMs several times over                         */
+    ENUF_OPT_CUDA_GRAPH = 9      /* 1: the launches of one evaluation are captured into a CUDA graph
+                                    the second time the same (r, q, F) pointers and N are passed, and
+                                    replayed while they stay the same (an MD loop that updates r in
+                                    place); any enuf_plan_set call drops the graph.  Ignored while
+                                    ENUF_OPT_PROFILE is on.  For the launch-bound small systems.     */
 };
 
 enum { ENUF_F32 = 0, ENUF_F64 = 1 };

@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libenuf_b200.so")
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 OPT_PRECISION, OPT_WINDOW, OPT_FORCE_VARIANT, OPT_SLATER_LAMBDA = 1, 2, 3, 4
 OPT_NUM_PARTICLES, OPT_PROFILE, OPT_KEEP_SPECTRUM, OPT_SPREAD_ZCHUNK = 5, 6, 7, 8
+OPT_CUDA_GRAPH = 9
 F32, F64 = 0, 1
 WINDOWS = {"gaussian": 0, "kaiser_bessel": 1}
 VARIANTS = {"analytic": 0, "ik": 1}
@@ -141,7 +142,7 @@ class Plan:
     """enuf_plan_create / enuf_plan_set / enuf_energy_forces / enuf_plan_destroy."""
 
     def __init__(self, N, L, alpha, k_cut, M, sigma=2.0, m=6, dtype=None, window="kaiser_bessel",
-                 variant="analytic", slater_lambda=0.0, profile=False, keep_spectrum=False):
+                 variant="analytic", slater_lambda=0.0, profile=False, keep_spectrum=False, cuda_graph=False):
         import torch
         self._torch = torch
         self._h = C.c_void_p()
@@ -158,6 +159,8 @@ class Plan:
         self.set(OPT_SLATER_LAMBDA, slater_lambda)
         self.set(OPT_PROFILE, int(profile))
         self.set(OPT_KEEP_SPECTRUM, int(keep_spectrum))
+        if cuda_graph:
+            self.set(OPT_CUDA_GRAPH, 1)
 
     @classmethod
     def from_workload(cls, w, **kw):

@@ -193,10 +193,16 @@ int dev_alloc(enuf_plan* p, void** ptr, size_t bytes) {
     return ENUF_OK;
 }
 
+void drop_graph(enuf_plan* p) {
+    if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }
+    p->g_r = p->g_q = nullptr; p->g_F = nullptr; p->g_N = -1;
+}
+
 void free_workspace(enuf_plan* p) {
+    drop_graph(p);
     auto fr = [](void* q) { if (q) cudaFree(q); };
     fr(p->rec); fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
-    fr(p->scan_total); fr(p->scan_desc); p->scan_desc = nullptr;
+    fr(p->scan_total); fr(p->scan_desc); p->scan_desc = nullptr; fr(p->scan_epoch); p->scan_epoch = nullptr;
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev); fr(p->fft_done);
     fr(p->r_stage); fr(p->q_stage); fr(p->F_stage);
@@ -260,6 +266,7 @@ int ensure_allocated(enuf_plan* p) {
     ALLOC(p->bin_cursor, 4 * (size_t)p->tg.nbins);
     ALLOC(p->scan_total, 4 * (((size_t)p->tg.nbins + 1023) / 1024));
     ALLOC(p->scan_desc, 8 * (((size_t)p->tg.nbins + 1023) / 1024));
+    ALLOC(p->scan_epoch, 4);
     for (int d = 0; d < nfield; ++d) {
         ALLOC(p->grid[d], es * n3);
         ALLOC(p->A1[d], 2 * es * n * n * p->Kxp);
@@ -297,7 +304,7 @@ int ensure_allocated(enuf_plan* p) {
     cudaMemsetAsync(p->e_dev, 0, 8, p->stream);
     cudaMemsetAsync(p->fft_done, 0, 4, p->stream);
     cudaMemsetAsync(p->scan_desc, 0, 8 * (((size_t)p->tg.nbins + 1023) / 1024), p->stream);
-    p->scan_epoch = 0;
+    cudaMemsetAsync(p->scan_epoch, 0, 4, p->stream);
     rc = p->precision == ENUF_F32 ? enuf::configure_kernels<float>(p) : enuf::configure_kernels<double>(p);
     if (rc) {
         cudaError_t le = cudaGetLastError();
@@ -378,7 +385,35 @@ int evaluate_device(enuf_plan* p, const void* r, const void* q, void* F, double*
     if (p->N == 0) {
         CU(cudaMemsetAsync(p->e_dev, 0, 8, p->stream));
         if (p->profile) for (int i = 0; i <= ENUF_NUM_STAGES; ++i) cudaEventRecord(p->ev[i], p->stream);
+    } else if (p->use_graph && !p->profile && p->gexec && r == p->g_r && q == p->g_q && F == p->g_F && p->N == p->g_N) {
+        CU(cudaGraphLaunch(p->gexec, p->stream));
+        p->launches = p->g_launches;
+    } else if (p->use_graph && !p->profile && p->evaluated && r == p->g_r && q == p->g_q && F == p->g_F && p->N == p->g_N) {
+        // second call with the same arguments: capture (nothing runs), instantiate, launch.  The capture is
+        // made on a stream of the plan's own, because the caller's may be the legacy default stream.
+        if (!p->cap_stream) CU(cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+        cudaStream_t user = p->stream;
+        p->stream = p->cap_stream;
+        cudaGraph_t graph = nullptr;
+        cudaError_t ce = cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal);
+        int rc = 0;
+        if (ce == cudaSuccess) {
+            rc = p->precision == ENUF_F32 ? run_all<float>(p, r, q, F) : run_all<double>(p, r, q, F);
+            ce = cudaStreamEndCapture(p->cap_stream, &graph);
+        }
+        p->stream = user;
+        if (ce != cudaSuccess || rc || !graph) {
+            if (graph) cudaGraphDestroy(graph);
+            drop_graph(p);
+            return fail_cuda(ce != cudaSuccess ? ce : cudaGetLastError(), "CUDA graph capture");
+        }
+        ce = cudaGraphInstantiate(&p->gexec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ce != cudaSuccess) { p->gexec = nullptr; drop_graph(p); return fail_cuda(ce, "cudaGraphInstantiate"); }
+        p->g_launches = p->launches;
+        CU(cudaGraphLaunch(p->gexec, p->stream));
     } else {
+        if (p->use_graph) { drop_graph(p); p->g_r = r; p->g_q = q; p->g_F = F; p->g_N = p->N; }
         int rc = p->precision == ENUF_F32 ? run_all<float>(p, r, q, F) : run_all<double>(p, r, q, F);
         if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
     }
@@ -432,6 +467,7 @@ int enuf_plan_create(enuf_plan** out, int64_t N, double L, double alpha, int k_c
 int enuf_plan_set(enuf_plan* p, int key, double value) {
     g_err[0] = 0;
     if (!p) return fail(ENUF_EINVAL, "plan is NULL");
+    drop_graph(p);                 // whatever changes, a captured evaluation no longer describes the plan
     const int iv = (int)value;
     switch (key) {
         case ENUF_OPT_PRECISION:
@@ -466,6 +502,9 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
         case ENUF_OPT_KEEP_SPECTRUM:
             if (p->allocated && (iv != 0) != p->keep_spectrum) { cudaStreamSynchronize(p->stream); free_workspace(p); }
             p->keep_spectrum = iv != 0;
+            return ENUF_OK;
+        case ENUF_OPT_CUDA_GRAPH:
+            p->use_graph = iv != 0;
             return ENUF_OK;
         case ENUF_OPT_SPREAD_ZCHUNK:
             if (iv < 8 || iv > p->n || (iv & (iv - 1))) return fail(ENUF_EINVAL, "zchunk must be a power of two in [8, n]");
@@ -787,6 +826,7 @@ void enuf_plan_destroy(enuf_plan* p) {
     if (!p) return;
     if (p->allocated) cudaStreamSynchronize(p->stream);
     free_workspace(p);
+    if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     delete p;
 }
 

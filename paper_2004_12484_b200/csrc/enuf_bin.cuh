@@ -47,9 +47,11 @@ __device__ __forceinline__ int bin_of(const CellOfParticle& p, const TileGeom& g
 template <typename T>
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict__ F, int64_t N,
-                 double L, TileGeom g, uint32_t* __restrict__ count) {
+                 double L, TileGeom g, uint32_t* __restrict__ count, uint32_t* __restrict__ scan_epoch) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
+    if (j == 0) scan_epoch[0] += 1u;    // the epoch of this evaluation's scan: kept on the device so that a
+                                        // replayed CUDA graph (ENUF_OPT_CUDA_GRAPH) advances it as well
     if (q[j] == (T)0) {
         F[3 * j] = (T)0; F[3 * j + 1] = (T)0; F[3 * j + 2] = (T)0;
         return;
@@ -139,14 +141,16 @@ bin_scan_apply_kernel(uint32_t* __restrict__ count, int nbins, const uint32_t* _
 // Single-launch variant for histograms of at most kScanMaxResident chunks (every CTA is resident at once, so a
 // CTA may wait for its predecessors): chunk b publishes (epoch << 32 | its total) in desc[b] and sums the
 // totals of the chunks before it as they appear (decoupled look-back without the aggregate chain -- with <= 64
-// chunks reading all predecessors is cheaper than chaining).  `epoch` changes with every launch, so desc[] is
+// chunks reading all predecessors is cheaper than chaining).  the epoch changes with every evaluation, so desc[] is
 // never reset.
 constexpr int kScanMaxResident = 128;
 static __global__ void __launch_bounds__(kScanThreads)
 bin_scan_single_kernel(uint32_t* __restrict__ count, int nbins, unsigned long long* __restrict__ desc,
-                       uint32_t epoch, uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor) {
+                       const uint32_t* __restrict__ scan_epoch, uint32_t* __restrict__ offset,
+                       uint32_t* __restrict__ cursor) {
     __shared__ uint32_t ws[kScanThreads / 32];
     __shared__ uint32_t base_s;
+    const uint32_t epoch = scan_epoch[0];             // advanced by bin_count_kernel of this evaluation
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int i0 = blockIdx.x * kScanChunk + threadIdx.x * 4;
     uint32_t c[4], sum = 0;

@@ -100,11 +100,11 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     const unsigned blocks = (unsigned)((N + 255) / 256);
     const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
     bin_count_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q),
-                                               static_cast<T*>(F), N, p->L, p->tg, p->bin_count);
+                                               static_cast<T*>(F), N, p->L, p->tg, p->bin_count, p->scan_epoch);
     int nlaunch = 4;
     if ((int)sblocks <= kScanMaxResident && (int)sblocks <= p->num_sms) {
         // every scan CTA is resident at once: one launch, chunk totals exchanged through scan_desc
-        bin_scan_single_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_desc, ++p->scan_epoch,
+        bin_scan_single_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_desc, p->scan_epoch,
                                                                 p->bin_offset, p->bin_cursor);
         nlaunch = 3;
     } else {

@@ -17,6 +17,13 @@ struct enuf_plan {
     bool profile = false, keep_spectrum = false;
     bool trim = false;             // fp32 Kaiser-Bessel m >= 5: kernels visit 2m stencil points per dimension
     cudaStream_t stream = nullptr;
+    // ENUF_OPT_CUDA_GRAPH: one evaluation's launches, captured on cap_stream, replayed on `stream`
+    bool use_graph = false;
+    cudaGraphExec_t gexec = nullptr;
+    cudaStream_t cap_stream = nullptr;
+    const void* g_r = nullptr; const void* g_q = nullptr; void* g_F = nullptr;   // what the graph was captured for
+    int64_t g_N = -1;
+    int g_launches = 0;
     // derived
     enuf::TileGeom tg{};
     enuf::WindowParams wp{};
@@ -36,7 +43,7 @@ struct enuf_plan {
     uint32_t* bin_cursor = nullptr;   // [nbins]
     uint32_t* scan_total = nullptr;   // [ceil(nbins / kScanChunk)]
     unsigned long long* scan_desc = nullptr;   // [ceil(nbins / kScanChunk)] (epoch << 32 | chunk total), single-launch scan
-    uint32_t scan_epoch = 0;
+    uint32_t* scan_epoch = nullptr;            // [1] device word: evaluation counter, the epoch of scan_desc
     float poly_c[enuf::kPolyMaxDeg + 1][enuf::kMaxM + 1] = {};   // host copy of the polynomial window table
     float poly_d[enuf::kPolyMaxDeg][enuf::kMaxM + 1] = {};       // (fp32 path; packed into PolyArg<m> per launch)
     int zchunk = 0;                   // grid planes per spread CTA

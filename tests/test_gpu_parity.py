@@ -405,3 +405,46 @@ def test_fp32_particles_exactly_on_grid_points(enuf, torch_cuda, oracle):
         assert abs(E - ref["E"]) <= F32_E * abs(ref["E"])
         assert rel_rms(F.cpu().numpy(), ref["F"]) <= F32_F
         plan.close()
+
+
+@pytest.mark.parametrize("name,variant", [("cfg1", "analytic"), ("cfg2", "ik"), ("cfg3", "analytic")])
+def test_cuda_graph_replay_matches_oracle(enuf, torch_cuda, oracle, name, variant):
+    """ENUF_OPT_CUDA_GRAPH (enuf.h): an MD-style loop that updates r in place.  Call 1 runs eagerly, call 2
+    captures and launches, calls 3.. replay; every call is checked against Oracle B on that call's positions,
+    then a different F buffer, a different N and the original arguments again (graph dropped and rebuilt)."""
+    torch = torch_cuda
+    w = make_workload(name)
+    tf, te = tols(w)
+    plan = enuf.Plan.from_workload(w, variant=variant, cuda_graph=True)
+    r = torch.from_numpy(w.r).cuda(); q = torch.from_numpy(w.q).cuda()
+    F = torch.empty_like(r)
+    launches = None
+    for step in range(5):
+        r_host = w.r if step == 0 else displaced_positions(w.r, w.L, 77, step, 0.05)
+        r.copy_(torch.from_numpy(r_host))
+        E, Fo = plan.energy_forces(r, q, F=F)
+        assert Fo.data_ptr() == F.data_ptr()
+        ref = oracle.enuf(r_host, w.q, w.L, w.alpha, w.k_cut, w.n, w.m, w.window, variant=variant,
+                          slater_lambda=w.slater_lambda)
+        assert abs(E - ref["E"]) <= te * abs(ref["E"]), (step, E, ref["E"])
+        assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf, step
+        launches = plan.launch_count() if launches is None else launches
+        assert plan.launch_count() == launches
+    # other output buffer: eager again, same result
+    E2, F2 = plan.energy_forces(r, q)
+    assert abs(E2 - E) <= 1e-6 * abs(E) and rel_rms(F2.cpu().numpy(), F.cpu().numpy()) <= tf
+    # fewer particles, twice eagerly + captured, then the full set again
+    n_low = w.N // 2
+    plan.set_num_particles(n_low)
+    rl = r[:n_low].contiguous(); ql = q[:n_low].contiguous(); Fl = torch.empty_like(rl)
+    ref = oracle.enuf(r_host[:n_low], w.q[:n_low], w.L, w.alpha, w.k_cut, w.n, w.m, w.window, variant=variant,
+                      slater_lambda=w.slater_lambda)
+    for _ in range(3):
+        El, _ = plan.energy_forces(rl, ql, F=Fl)
+        assert abs(El - ref["E"]) <= te * abs(ref["E"])
+        assert rel_rms(Fl.cpu().numpy(), ref["F"]) <= tf
+    plan.set_num_particles(w.N)
+    for _ in range(3):
+        E3, _ = plan.energy_forces(r, q, F=F)
+        assert abs(E3 - E) <= 1e-6 * abs(E)
+    plan.close()
