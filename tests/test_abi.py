@@ -54,6 +54,8 @@ def test_plan_create_validation(lib):
     assert lib.enuf_plan_set(h, enuf.OPT_NUM_PARTICLES, 11.0) == enuf.EINVAL
     assert lib.enuf_plan_set(h, enuf.OPT_NUM_PARTICLES, 7.0) == enuf.OK
     assert lib.enuf_plan_set(h, enuf.OPT_SLATER_LAMBDA, -0.5) == enuf.EINVAL
+    assert lib.enuf_plan_set(h, enuf.OPT_CUDA_GRAPH, 1.0) == enuf.OK   # host flag only: nothing is captured yet
+    assert lib.enuf_plan_set(h, enuf.OPT_CUDA_GRAPH, 0.0) == enuf.OK
     E = C.c_double()
     assert lib.enuf_plan_energy(h, C.byref(E)) == enuf.ESTATE       # nothing evaluated yet
     assert lib.enuf_energy_forces(h, None, None, None, C.byref(E)) == enuf.EINVAL   # NULL pointers, N > 0
