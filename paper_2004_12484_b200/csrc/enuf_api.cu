@@ -454,9 +454,11 @@ int enuf_plan_create(enuf_plan** out, int64_t N, double L, double alpha, int k_c
     p->tg.n = n;
     p->tg.nt = n / enuf::kTile;
     p->tg.nbins = p->tg.nt * p->tg.nt * n;
-    // spread: columns x z-chunks; enough CTAs to fill 148 SMs several times over, chunks >= 16 planes
+    // spread: columns x z-chunks; enough CTAs to fill 148 SMs several times over, chunks >= 8 planes (measured,
+    // spread ms at chunk 16 -> 8: n = 32 0.072 -> 0.051, n = 64 0.188 -> 0.138, n = 128 0.040 -> 0.034; n = 256
+    // stays at 64 planes: 0.176 against 0.197 / 0.239 / 0.322 at 32 / 16 / 8)
     p->zchunk = n;
-    while (p->zchunk > 16 && p->tg.nt * p->tg.nt * (n / p->zchunk) < 592) p->zchunk /= 2;
+    while (p->zchunk > 8 && p->tg.nt * p->tg.nt * (n / p->zchunk) < 592) p->zchunk /= 2;
     p->Kxp = ((k_cut + 1 + enuf::kLinesPerGroup - 1) / enuf::kLinesPerGroup) * enuf::kLinesPerGroup;
     p->Ky = 2 * k_cut + 1;
     fill_window_params(p);
