@@ -124,6 +124,21 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
+    def _lines(self) -> int:
+        try:
+            with open(self.tmp.name) as fh:
+                return sum(1 for line in fh if line.count(",") >= 6)
+        except OSError:
+            return 0
+
+    def wait_first(self, keep_busy, timeout: float = 3.0) -> None:
+        """nvidia-smi takes a few hundred ms to start, longer than a 100-step timed region: keep the GPU
+        under the same (untimed) load until the first sample is there, then mark where the timed region begins."""
+        t0 = time.perf_counter()
+        while self.proc is not None and self._lines() == 0 and time.perf_counter() - t0 < timeout:
+            keep_busy()
+        self.n0 = self._lines()
+
     def stop(self) -> dict:
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
@@ -141,6 +156,9 @@ class ClockSampler:
                 if len(parts) >= 7:
                     rows.append(parts)
         os.unlink(self.tmp.name)
+        n0 = getattr(self, "n0", 0)
+        if len(rows) > n0:
+            rows = rows[n0:]          # samples taken from the start of the timed region on
         if not rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         sm = sorted(float(r[0]) for r in rows if r[0].replace(".", "").isdigit())
@@ -286,10 +304,19 @@ def run_ours(args):
     evaluate = plan.energy_forces_sharded if sharded else plan.energy_forces
     for s in range(W):
         evaluate(pos_dev[s], q_dev, F=F_dev, want_energy=False)
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        def keep_busy():
+            if sharded:                      # its evaluation holds a collective: rank 0 must not run one alone
+                time.sleep(0.05)
+                return
+            for s_ in range(W):
+                evaluate(pos_dev[s_], q_dev, F=F_dev, want_energy=False)
+            torch.cuda.synchronize()
+        sampler.wait_first(keep_busy)
     plan.set(enuf.OPT_PROFILE, 1)                                  # per-stage events from here on
     torch.cuda.synchronize()
     barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
     torch.cuda.synchronize()
