@@ -12,6 +12,8 @@
 // ("forces in 3D packed into a single calculation entity").
 #pragma once
 
+#include <type_traits>
+
 #include "enuf_common.cuh"
 #include "enuf_spread.cuh"   // Pair2, fma_pair
 
@@ -234,24 +236,41 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
             }
             const int base = base_s[slot];
             const T* origin = tile_s + base;
-            T fx = (T)0, fy = (T)0, fz = (T)0;
+            // kWide (fp32, analytic variant, m <= 3): the three sums are formed in fp64.  sum Psi phi' cancels
+            // heavily and the narrow windows have twice the max|phi'| of m >= 4, so the fp32 summation error
+            // alone reaches the 2e-6 bar there; the stencil is small, the fp64 FMAs are cheap.
+            constexpr bool kWide = sizeof(T) == 4 && M_ <= 3 && !kIk;
+            using A = typename std::conditional<kWide, double, T>::type;
+            A fx = (A)0, fy = (A)0, fz = (A)0;
             // one stencil row: s = sum_k (phi, phi')[k] * v[k], then the y, z weights of the row
             auto finish_row = [&](int it, const T (&v)[WE]) {
-                P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
-#pragma unroll
-                for (int k = 0; k < WE; ++k) {
-                    if (k & 1) fma_pair(sb2, wx[k], v[k]);
-                    else fma_pair(sa, wx[k], v[k]);
-                }
-                const P2 s2 = pair_add(sa, sb2);                       // (sum Psi phi_x, sum Psi phi_x')
                 const P2 wy = wt[ryo[it]], wz = wt[rzo[it]];
-                if (kIk) {
-                    fx += s2.x * (wy.x * wz.x);
+                if constexpr (kWide) {
+                    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+                    for (int k = 0; k < WE; ++k) {
+                        s0 = fma((double)wx[k].x, (double)v[k], s0);
+                        s1 = fma((double)wx[k].y, (double)v[k], s1);
+                    }
+                    fx = fma(s1, (double)wy.x * (double)wz.x, fx);
+                    fy = fma(s0, (double)wy.y * (double)wz.x, fy);
+                    fz = fma(s0, (double)wy.x * (double)wz.y, fz);
                 } else {
-                    const P2 yz = pair_scale(wy, wz.x);                // (phi_y phi_z, phi_y' phi_z)
-                    fx += s2.y * yz.x;
-                    fy += s2.x * yz.y;
-                    fz += s2.x * (wy.x * wz.y);
+                    P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
+#pragma unroll
+                    for (int k = 0; k < WE; ++k) {
+                        if (k & 1) fma_pair(sb2, wx[k], v[k]);
+                        else fma_pair(sa, wx[k], v[k]);
+                    }
+                    const P2 s2 = pair_add(sa, sb2);                   // (sum Psi phi_x, sum Psi phi_x')
+                    if (kIk) {
+                        fx += s2.x * (wy.x * wz.x);
+                    } else {
+                        const P2 yz = pair_scale(wy, wz.x);            // (phi_y phi_z, phi_y' phi_z)
+                        fx += s2.y * yz.x;
+                        fy += s2.x * yz.y;
+                        fz += s2.x * (wy.x * wz.y);
+                    }
                 }
             };
             if constexpr (C::kPair && sizeof(T) == 4) {
@@ -305,13 +324,13 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
                 // lane over bit 3, then a plain butterfly: 6 shuffles instead of 15.  The totals of x, y, z
                 // end in the lanes with (lane >> 3) = 0, 1, 2.
                 const bool b4 = (lane & 16) != 0, b3 = (lane & 8) != 0;
-                T k0 = (b4 ? fz : fx) + __shfl_xor_sync(0xffffffffu, b4 ? fx : fz, 16);
-                T k1 = (b4 ? (T)0 : fy) + __shfl_xor_sync(0xffffffffu, b4 ? fy : (T)0, 16);
-                T k = (b3 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, b3 ? k0 : k1, 8);
+                A k0 = (b4 ? fz : fx) + __shfl_xor_sync(0xffffffffu, b4 ? fx : fz, 16);
+                A k1 = (b4 ? (A)0 : fy) + __shfl_xor_sync(0xffffffffu, b4 ? fy : (A)0, 16);
+                A k = (b3 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, b3 ? k0 : k1, 8);
                 k += __shfl_xor_sync(0xffffffffu, k, 4);
                 k += __shfl_xor_sync(0xffffffffu, k, 2);
                 k += __shfl_xor_sync(0xffffffffu, k, 1);
-                if ((lane & 7) == 0 && lane < 24) F[3 * j + (lane >> 3)] = sc * k;
+                if ((lane & 7) == 0 && lane < 24) F[3 * j + (lane >> 3)] = (T)((A)sc * k);
             }
         }
         __syncwarp();

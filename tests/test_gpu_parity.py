@@ -182,8 +182,47 @@ def test_cfg4_sampled(enuf, torch_cuda, oracle):
     _sampled_check(enuf, torch_cuda, oracle, w, w.r)
 
 
+def _full_check(enuf, torch, oracle, w, variant="analytic"):
+    """Every particle of a large config against Oracle B: the relative RMS bar AND a per-particle bound.
+    A bug in a rare path of the spread / gather (staging overflow, chunk or column boundary, trimmed
+    stencils, the producer's ring) hits a handful of particles in 1e5..1e6 and hides under an RMS; the
+    per-particle bound max_i |dF_i| <= PER_PARTICLE_C * RMS|F| cannot be met with
+    one stencil point, one slab or one particle dropped (that costs >= 1e-3 RMS|F| on that particle)."""
+    ref = oracle.enuf_workload(w, variant=variant)
+    plan, E, F = gpu_eval(enuf, torch, w, variant)
+    tf, te = tols(w)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"]), (E, ref["E"])
+    assert np.isfinite(F).all()
+    err = rel_rms(F, ref["F"])
+    assert err <= tf, err
+    d = np.sqrt(((F.astype(np.float64) - ref["F"]) ** 2).sum(1))
+    rms_f = math.sqrt((ref["F"] ** 2).sum() / w.N)
+    worst = d.max() / rms_f
+    assert worst <= PER_PARTICLE_C[w.dtype], (worst, int(d.argmax()))
+    plan.close()
+    return err, worst
+
+
+# max over particles of |F_i(gpu) - F_i(oracle)| in units of RMS|F|.  fp32: the error of a single force is
+# ~ the RMS error (1e-6 RMS|F|) times a tail factor; 2e-5 = ten times the 2e-6 RMS bar leaves room for the
+# 5-sigma tail of 1e6 particles and is still 50x below the smallest structural error (one dropped stencil
+# point of a m = 6 Kaiser-Bessel window moves that particle's force by >= 1e-3 RMS|F|).
+PER_PARTICLE_C = {"f32": 2e-5, "f64": 1e-10}
+
+
 @pytest.mark.slow
-@pytest.mark.parametrize("step", [0, 1, 99])
+def test_cfg4_full(enuf, torch_cuda, oracle):
+    _full_check(enuf, torch_cuda, oracle, make_workload("cfg4"))
+
+
+@pytest.mark.slow
+def test_cfg5_full_step0(enuf, torch_cuda, oracle):
+    """All 1e6 particles of config 5 (Oracle B: ~15 s on the GPU box's host cores)."""
+    _full_check(enuf, torch_cuda, oracle, make_workload("cfg5"))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("step", [0, 1, 50, 99])
 def test_cfg5_sampled_steps(enuf, torch_cuda, oracle, step):
     """Config 5 in the launch configuration bench.py times; positions after `step` displacements."""
     w = make_workload("cfg5")
@@ -252,12 +291,8 @@ def test_all_grid_sizes_and_supports(enuf, torch_cuda, oracle, n, m, window, dty
                      dtype=torch.float64 if dtype == "f64" else torch.float32)
     E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
     tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
-    if dtype == "f32" and variant == "analytic" and m <= 2:
-        # the analytic-derivative gather differences the fp32-rounded field Psi
-        # with phi'; for the narrow m <= 2 windows max|phi'| is ~2x that of m >= 4 and the measured
-        # error sits at 1.95e-6..2.01e-6 (it moves with the summation order, R22).  The five
-        # configs (m = 4, 6) keep the 2e-6 bar.
-        tf = 2 * F32_F
+    # fp32, analytic variant, m <= 3: the gather forms its three sums in fp64 (narrow windows have twice the
+    # max|phi'| of m >= 4; with fp32 sums this case sat at 1.95e-6..2.01e-6) -- the 2e-6 bar holds for every m
     assert abs(E - ref["E"]) <= te * abs(ref["E"])
     assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
     plan.close()

@@ -341,6 +341,23 @@ def test_enuf_invariances(oracle):
     assert d["E"] == a["E"] and np.array_equal(d["F"][:-1], a["F"]) and not d["F"][-1].any()
 
 
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+@pytest.mark.parametrize("window,m", [("kaiser_bessel", 6), ("gaussian", 4)])
+def test_enuf_sampled_forces_match_full(oracle, variant, window, m):
+    """The `sample` branch of orc_gather / orc_enuf (the one the config 4 / 5 parity tests rely on): forces on a
+    sample of particles are the rows of the full result, in the sample's order, bit for bit (same E too)."""
+    L, alpha, kc, n = 6.0, 1.0, 8, 32
+    r, q = random_neutral_gas(40, L, seed=12)
+    q[5] = 0.0                                  # a neutral particle in the sample
+    sample = [5, 39, 0, 17, 18]
+    full = oracle.enuf(r, q, L, alpha, kc, n, m, window, variant=variant, slater_lambda=0.3)
+    part = oracle.enuf(r, q, L, alpha, kc, n, m, window, variant=variant, slater_lambda=0.3, sample=sample)
+    assert part["F"].shape == (5, 3)
+    assert np.array_equal(part["F"], full["F"][sample])
+    assert part["E"] == full["E"]
+    assert not part["F"][0].any()
+
+
 def test_slater_factor_against_direct_and_limit(oracle):
     """R19 (unpinned against the paper): Oracle B with the factor vs Oracle A with the factor."""
     L, alpha, kc, n, m, lam = 6.0, 1.0, 8, 32, 6, 0.4
