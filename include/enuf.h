@@ -54,7 +54,7 @@ enum enuf_option {
     ENUF_OPT_NUM_PARTICLES = 5,  /* lower N for the next calls, 0 <= N <= planned capacity          */
     ENUF_OPT_PROFILE = 6,        /* 1: record per-stage CUDA-event times (enuf_plan_stage_ms)        */
     ENUF_OPT_KEEP_SPECTRUM = 7,  /* 1: also store S~(n) so enuf_plan_structure_factor() can read it  */
-    ENUF_OPT_SPREAD_ZCHUNK = 8,  /* tuning: grid planes per spreading CTA (power of two, 8..n);
+    ENUF_OPT_SPREAD_ZCHUNK = 8,  /* tuning: grid planes per spreading CTA (integer, 1..n);
                                     default fills the SMs several times over                         */
     ENUF_OPT_CUDA_GRAPH = 9      /* 1: the launches of one evaluation are captured into a CUDA graph
                                     the second time the same (r, q, F) pointers and N are passed, and

@@ -201,7 +201,7 @@ void drop_graph(enuf_plan* p) {
 void free_workspace(enuf_plan* p) {
     drop_graph(p);
     auto fr = [](void* q) { if (q) cudaFree(q); };
-    fr(p->rec); fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
+    fr(p->rec); fr(p->rows); p->rows = nullptr; fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
     fr(p->scan_total); fr(p->scan_desc); p->scan_desc = nullptr; fr(p->scan_epoch); p->scan_epoch = nullptr;
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev); fr(p->fft_done);
@@ -256,11 +256,23 @@ int ensure_allocated(enuf_plan* p) {
     // b m / sinh(b m) (<= 2.7e-9 for m >= 5): the fp32 kernels then skip that point
     p->trim = p->precision == ENUF_F32 && p->window == ENUF_WINDOW_KAISER_BESSEL && p->m >= 5;
     p->tg.trim = p->trim ? 1 : 0;
+    if (!p->zchunk_user) {
+        // spread: columns x z-chunks, all CTAs resident at once (one wave): as many chunks as the device has
+        // room for, but chunks of >= 8 planes (every chunk walks 2m extra slabs)
+        const int per_sm = p->precision == ENUF_F32 ? enuf::spread_ctas_per_sm<float>(p->spread_npx)
+                                                    : enuf::spread_ctas_per_sm<double>(p->spread_npx);
+        const int ncol = (p->n / (8 * p->spread_npx)) * (p->n / 16);
+        int chunks = p->num_sms * per_sm / ncol;
+        if (chunks < 1) chunks = 1;
+        p->zchunk = (p->n + chunks - 1) / chunks;
+        if (p->zchunk < 8) p->zchunk = 8;
+    }
     const size_t es = p->esize, n = p->n, n3 = n * n * n, cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1);
     const int nfield = p->variant == ENUF_FORCE_IK ? 3 : 1;
     int rc;
 #define ALLOC(ptr, bytes) if ((rc = dev_alloc(p, (void**)&(ptr), (bytes)))) { free_workspace(p); return rc; }
     ALLOC(p->rec, (es == 4 ? sizeof(enuf::PSlot<float>) : sizeof(enuf::PSlot<double>)) * cap);
+    ALLOC(p->rows, es * 48 * cap);
     ALLOC(p->bin_count, 4 * (size_t)p->tg.nbins);
     ALLOC(p->bin_offset, 4 * ((size_t)p->tg.nbins + 1));
     ALLOC(p->bin_cursor, 4 * (size_t)p->tg.nbins);
@@ -454,11 +466,8 @@ int enuf_plan_create(enuf_plan** out, int64_t N, double L, double alpha, int k_c
     p->tg.n = n;
     p->tg.nt = n / enuf::kTile;
     p->tg.nbins = p->tg.nt * p->tg.nt * n;
-    // spread: columns x z-chunks; enough CTAs to fill 148 SMs several times over, chunks >= 8 planes (measured,
-    // spread ms at chunk 16 -> 8: n = 32 0.072 -> 0.051, n = 64 0.188 -> 0.138, n = 128 0.040 -> 0.034; n = 256
-    // stays at 64 planes: 0.176 against 0.197 / 0.239 / 0.322 at 32 / 16 / 8)
-    p->zchunk = n;
-    while (p->zchunk > 8 && p->tg.nt * p->tg.nt * (n / p->zchunk) < 592) p->zchunk /= 2;
+    p->spread_npx = n >= 128 ? 4 : 2;
+    p->zchunk = n;                 // derived in ensure_allocated (depends on the precision and the SM count)
     p->Kxp = ((k_cut + 1 + enuf::kLinesPerGroup - 1) / enuf::kLinesPerGroup) * enuf::kLinesPerGroup;
     p->Ky = 2 * k_cut + 1;
     fill_window_params(p);
@@ -509,8 +518,8 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
             p->use_graph = iv != 0;
             return ENUF_OK;
         case ENUF_OPT_SPREAD_ZCHUNK:
-            if (iv < 8 || iv > p->n || (iv & (iv - 1))) return fail(ENUF_EINVAL, "zchunk must be a power of two in [8, n]");
-            p->zchunk = iv;
+            if (iv < 1 || iv > p->n) return fail(ENUF_EINVAL, "zchunk must be an integer in [1, n]");
+            p->zchunk = iv; p->zchunk_user = true;
             return ENUF_OK;
         default:
             return fail(ENUF_EINVAL, "unknown option key %d", key);

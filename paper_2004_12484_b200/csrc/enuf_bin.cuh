@@ -8,6 +8,7 @@
 #pragma once
 
 #include "enuf_common.cuh"
+#include "enuf_spread.cuh"   // write_window_rows
 
 namespace enuf {
 
@@ -205,11 +206,15 @@ bin_scan_single_kernel(uint32_t* __restrict__ count, int nbins, unsigned long lo
 }
 
 // Scatter into bin order.  The order inside a bin follows the atomic cursor (any order is
-// a valid sort; sums downstream differ only in rounding order, R22).
-template <typename T>
+// a valid sort; sums downstream differ only in rounding order, R22).  The scatter also evaluates the
+// particle's 3 x (2m+1) window values -- once per particle and evaluation -- and stores them as the three
+// 16-element rows the spreading kernel stages (enuf_spread.cuh, write_window_rows); bits 30 / 31 of the
+// packed cell carry ks_x / ks_y of the trimmed stencils.
+template <typename T, int M_, bool kTrim>
 __global__ void __launch_bounds__(256)
 bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, double L, TileGeom g,
-                   uint32_t* __restrict__ cursor, PSlot<T>* __restrict__ slots) {
+                   WindowParams wp, const __grid_constant__ PolyArg<M_> pa,
+                   uint32_t* __restrict__ cursor, PSlot<T>* __restrict__ slots, T* __restrict__ rows) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     T qj = q[j];
@@ -218,9 +223,14 @@ bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, 
     uint32_t pos = atomicAdd(&cursor[bin_of<T>(p, g)], 1u);
     PSlot<T> o;
     o.rec.dx = (T)p.d0[0]; o.rec.dy = (T)p.d0[1]; o.rec.dz = (T)p.d0[2]; o.rec.q = qj;
-    o.cell = pack_cell(p.c[0], p.c[1], p.c[2]);
+    const int ksx = (kTrim && o.rec.dx > (T)0) ? 1 : 0, ksy = (kTrim && o.rec.dy > (T)0) ? 1 : 0;
+    o.cell = pack_cell(p.c[0], p.c[1], p.c[2]) | ((uint32_t)ksx << 30) | ((uint32_t)ksy << 31);
     o.idx = (uint32_t)j;
     slots[pos] = o;
+    // parity of the first x stencil point (grid index c_x - m + ks_x; n is even, so wrapping keeps it)
+    const int parx = (p.c[0] + M_ + ksx) & 1;
+    write_window_rows<T, M_, kTrim>(wp, pa, o.rec.dx, o.rec.dy, o.rec.dz, qj, parx,
+                                    rows + (size_t)pos * (kRowsPerParticle * kRowElems));
 }
 
 }  // namespace enuf

@@ -3,6 +3,7 @@
 
 namespace enuf {
 template int configure_kernels<float>(enuf_plan*);
+template int spread_ctas_per_sm<float>(int);
 template int launch_bin<float>(enuf_plan*, const void*, const void*, void*);
 template int launch_spread<float>(enuf_plan*);
 template int launch_fft<float>(enuf_plan*);

@@ -3,6 +3,7 @@
 
 namespace enuf {
 template int configure_kernels<double>(enuf_plan*);
+template int spread_ctas_per_sm<double>(int);
 template int launch_bin<double>(enuf_plan*, const void*, const void*, void*);
 template int launch_spread<double>(enuf_plan*);
 template int launch_fft<double>(enuf_plan*);

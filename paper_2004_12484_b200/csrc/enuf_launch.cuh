@@ -62,12 +62,29 @@ static inline bool set_smem(K kernel, size_t bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
 }
 
+// f(IntC<npx>) -> int: patches per column row of the spreading kernel (column = 8 npx x 16 cells)
+template <typename F>
+static inline int dispatch_npx(int npx, F&& f) {
+    return npx == 4 ? f(IntC<4>{}) : f(IntC<2>{});
+}
+
+// spread: CTAs the device holds at once for this plan's kernel variant (enuf_spread.cuh)
+template <typename T>
+int spread_ctas_per_sm(int npx) {
+    return npx == 4 ? SpreadCfg<T, 1, false, 4>::CTAS_PER_SM : SpreadCfg<T, 1, false, 2>::CTAS_PER_SM;
+}
+
 template <typename T>
 int configure_kernels(enuf_plan* p) {
     int rc = dispatch_m(p, [&](auto mc) -> int {
         constexpr int M_ = decltype(mc)::value;
-        bool ok = set_smem(spread_kernel<T, M_>, spread_smem_bytes<T, M_>());
-        if constexpr (M_ >= 5 && sizeof(T) == 4) ok = ok && set_smem(spread_kernel<T, M_, true>, spread_smem_bytes<T, M_>());
+        bool ok = dispatch_npx(p->spread_npx, [&](auto xc) -> int {
+            constexpr int NPX = decltype(xc)::value;
+            bool k = set_smem(spread_kernel<T, M_, false, NPX>, spread_smem_bytes<T, M_, false, NPX>());
+            if constexpr (M_ >= 5 && sizeof(T) == 4)
+                k = k && set_smem(spread_kernel<T, M_, true, NPX>, spread_smem_bytes<T, M_, true, NPX>());
+            return k ? 0 : -1;
+        }) == 0;
         ok = ok && set_smem(gather_kernel<T, M_, false>, gather_smem_bytes<T, M_>());
         ok = ok && set_smem(gather_kernel<T, M_, true>, gather_smem_bytes<T, M_>());
         if constexpr (M_ >= 5 && sizeof(T) == 4) {
@@ -112,9 +129,23 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
         bin_scan_apply_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total, p->bin_offset,
                                                               p->bin_cursor);
     }
-    bin_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
-                                                 p->tg, p->bin_cursor, static_cast<PSlot<T>*>(p->rec));
-    if (cudaGetLastError() != cudaSuccess) return -1;
+    const int rc = dispatch_m(p, [&](auto mc) -> int {
+        constexpr int M_ = decltype(mc)::value;
+        const PolyArg<M_> pa = make_poly_arg<M_>(p);
+        if constexpr (M_ >= 5 && sizeof(T) == 4) {
+            if (p->trim) {
+                bin_scatter_kernel<T, M_, true><<<blocks, 256, 0, s>>>(
+                    static_cast<const T*>(r), static_cast<const T*>(q), N, p->L, p->tg, p->wp, pa, p->bin_cursor,
+                    static_cast<PSlot<T>*>(p->rec), static_cast<T*>(p->rows));
+                return 0;
+            }
+        }
+        bin_scatter_kernel<T, M_, false><<<blocks, 256, 0, s>>>(
+            static_cast<const T*>(r), static_cast<const T*>(q), N, p->L, p->tg, p->wp, pa, p->bin_cursor,
+            static_cast<PSlot<T>*>(p->rec), static_cast<T*>(p->rows));
+        return 0;
+    });
+    if (rc || cudaGetLastError() != cudaSuccess) return -1;
     p->bin_count_clean = true;
     return nlaunch;
 }
@@ -124,21 +155,22 @@ int launch_spread(enuf_plan* p) {
     cudaStream_t s = p->stream;
     int rc = dispatch_m(p, [&](auto mc) -> int {
         constexpr int M_ = decltype(mc)::value;
-        using C = SpreadCfg<M_>;
-        const dim3 grid((unsigned)(p->tg.nt * p->tg.nt), (unsigned)((p->n + p->zchunk - 1) / p->zchunk));
-        const PolyArg<M_> pa = make_poly_arg<M_>(p);
-        if constexpr (M_ >= 5 && sizeof(T) == 4) {
-            if (p->trim) {
-                spread_kernel<T, M_, true><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
-                    static_cast<const PSlot<T>*>(p->rec), p->bin_offset, p->tg, p->wp, pa, p->zchunk,
-                    static_cast<T*>(p->grid[0]));
+        return dispatch_npx(p->spread_npx, [&](auto xc) -> int {
+            constexpr int NPX = decltype(xc)::value;
+            auto run = [&](auto trim_c) -> int {
+                constexpr bool kTrim = decltype(trim_c)::value != 0;
+                using C = SpreadCfg<T, M_, kTrim, NPX>;
+                const dim3 grid((unsigned)((p->n / C::CX) * (p->n / C::CY)), (unsigned)((p->n + p->zchunk - 1) / p->zchunk));
+                spread_kernel<T, M_, kTrim, NPX><<<grid, C::NT, spread_smem_bytes<T, M_, kTrim, NPX>(), s>>>(
+                    static_cast<const PSlot<T>*>(p->rec), static_cast<const T*>(p->rows), p->bin_offset, p->tg,
+                    p->zchunk, static_cast<T*>(p->grid[0]));
                 return 0;
+            };
+            if constexpr (M_ >= 5 && sizeof(T) == 4) {
+                if (p->trim) return run(IntC<1>{});
             }
-        }
-        spread_kernel<T, M_, false><<<grid, C::NT, spread_smem_bytes<T, M_>(), s>>>(
-            static_cast<const PSlot<T>*>(p->rec), p->bin_offset, p->tg, p->wp, pa, p->zchunk,
-            static_cast<T*>(p->grid[0]));
-        return 0;
+            return run(IntC<0>{});
+        });
     });
     if (rc) return -1;
     return cudaGetLastError() == cudaSuccess ? 1 : -1;

@@ -38,6 +38,7 @@ struct enuf_plan {
     int num_sms = 148;             // multiProcessorCount of the current device (persistent FFT grids)
     // device workspace
     void* rec = nullptr;           // PSlot<T>[N_cap]: record, packed cell, caller index (bin order)
+    void* rows = nullptr;          // T[N_cap][3][16]: window rows of the spreading kernel (bin order)
     uint32_t* bin_count = nullptr;    // [nbins]
     uint32_t* bin_offset = nullptr;   // [nbins+1]
     uint32_t* bin_cursor = nullptr;   // [nbins]
@@ -47,6 +48,8 @@ struct enuf_plan {
     float poly_c[enuf::kPolyMaxDeg + 1][enuf::kMaxM + 1] = {};   // host copy of the polynomial window table
     float poly_d[enuf::kPolyMaxDeg][enuf::kMaxM + 1] = {};       // (fp32 path; packed into PolyArg<m> per launch)
     int zchunk = 0;                   // grid planes per spread CTA
+    bool zchunk_user = false;         // set through ENUF_OPT_SPREAD_ZCHUNK: not re-derived
+    int spread_npx = 4;               // spread column = 8 spread_npx x 16 cells (4 for n >= 128, 2 below)
     void* grid[3] = {nullptr, nullptr, nullptr};   // real n^3 (1 for analytic, 3 for ik)
     void* A1[3] = {nullptr, nullptr, nullptr};     // complex [n][n][Kxp]
     void* A2[3] = {nullptr, nullptr, nullptr};     // complex [n][Ky][Kxp]
@@ -98,6 +101,7 @@ template <typename T> int launch_fft_forward(enuf_plan* p);    // X, Y forward p
 template <typename T> int launch_fft_backward(enuf_plan* p);   // Z fused + inverse passes + energy
 template <typename T> int launch_gather(enuf_plan* p, void* F);
 template <typename T> int configure_kernels(enuf_plan* p);   // opt-in shared memory sizes
+template <typename T> int spread_ctas_per_sm(int npx);       // resident spreading CTAs per SM
 // real-space part: cell sort + pair kernel + energy reduction (enuf_real.cuh)
 template <typename T> int launch_real(enuf_plan* p, const void* r, const void* q, double r_cut, int accumulate, void* F);
 
