@@ -1,6 +1,7 @@
 // Step a1 -- wrap positions (x = r/L; R10) and counting-sort the charged
 // particles by bin (16 x 16 column in x, y and grid plane in z; TileGeom in enuf_common.cuh):
-// histogram -> exclusive scan (two launches, any number of bins) -> scatter.  The cell index c and
+// histogram -> exclusive scan (one launch, or two for histograms of more chunks than SMs) -> scatter ->
+// window rows of the sorted particles.  The cell index c and
 // the fractional offset d0 = u - c are formed in fp64 in the order
 //   x = r/L;  x -= floor(x);  u = n*x;  c = floor(u + 1/2)
 // for both precisions (an fp32 u would lose the offset: ulp(256) ~ 1.5e-5 cells), so the
@@ -41,7 +42,7 @@ __device__ __forceinline__ int bin_of(const CellOfParticle& p, const TileGeom& g
         bz += ((T)p.d0[2] > (T)0 ? 1 : 0) - 1;
         bz += bz < 0 ? g.n : 0;
     }
-    return ((p.c[1] / kTile) * g.nt + (p.c[0] / kTile)) * g.n + bz;
+    return bin_index(g, p.c[0] / kTile, p.c[1] / kTile, bz);
 }
 
 // Histogram of charged particles per bin; neutral particles get F = 0 here and are dropped.
@@ -206,15 +207,12 @@ bin_scan_single_kernel(uint32_t* __restrict__ count, int nbins, unsigned long lo
 }
 
 // Scatter into bin order.  The order inside a bin follows the atomic cursor (any order is
-// a valid sort; sums downstream differ only in rounding order, R22).  The scatter also evaluates the
-// particle's 3 x (2m+1) window values -- once per particle and evaluation -- and stores them as the three
-// 16-element rows the spreading kernel stages (enuf_spread.cuh, write_window_rows); bits 30 / 31 of the
-// packed cell carry ks_x / ks_y of the trimmed stencils.
-template <typename T, int M_, bool kTrim>
+// a valid sort; sums downstream differ only in rounding order, R22).  Bits 30 / 31 of the packed cell carry
+// ks_x / ks_y = (d0 > 0) of the trimmed stencils (the spreading producer culls on the cell word alone).
+template <typename T>
 __global__ void __launch_bounds__(256)
 bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, double L, TileGeom g,
-                   WindowParams wp, const __grid_constant__ PolyArg<M_> pa,
-                   uint32_t* __restrict__ cursor, PSlot<T>* __restrict__ slots, T* __restrict__ rows) {
+                   uint32_t* __restrict__ cursor, PSlot<T>* __restrict__ slots) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     T qj = q[j];
@@ -223,14 +221,47 @@ bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, 
     uint32_t pos = atomicAdd(&cursor[bin_of<T>(p, g)], 1u);
     PSlot<T> o;
     o.rec.dx = (T)p.d0[0]; o.rec.dy = (T)p.d0[1]; o.rec.dz = (T)p.d0[2]; o.rec.q = qj;
-    const int ksx = (kTrim && o.rec.dx > (T)0) ? 1 : 0, ksy = (kTrim && o.rec.dy > (T)0) ? 1 : 0;
-    o.cell = pack_cell(p.c[0], p.c[1], p.c[2]) | ((uint32_t)ksx << 30) | ((uint32_t)ksy << 31);
+    const uint32_t ksx = (g.trim && o.rec.dx > (T)0) ? 1u : 0u, ksy = (g.trim && o.rec.dy > (T)0) ? 1u : 0u;
+    o.cell = pack_cell(p.c[0], p.c[1], p.c[2]) | (ksx << 30) | (ksy << 31);
     o.idx = (uint32_t)j;
     slots[pos] = o;
-    // parity of the first x stencil point (grid index c_x - m + ks_x; n is even, so wrapping keeps it)
-    const int parx = (p.c[0] + M_ + ksx) & 1;
-    write_window_rows<T, M_, kTrim>(wp, pa, o.rec.dx, o.rec.dy, o.rec.dz, qj, parx,
-                                    rows + (size_t)pos * (kRowsPerParticle * kRowElems));
+}
+
+// The window rows of the sorted particles (enuf_spread.cuh, WindowRows): the 3 x (2m+1) window values of a
+// particle are evaluated ONCE per evaluation here ("window values ... kept") and read by every
+// spreading CTA whose halo holds the particle.  A warp takes 32 consecutive sorted particles, one lane per
+// particle for the evaluation, and writes their rows -- one contiguous block -- with coalesced 16-byte stores
+// through a shared-memory transpose.
+template <typename T> constexpr int rows_warps() { return sizeof(T) == 4 ? 4 : 2; }   // static shared memory <= 48 KB
+template <typename T, int M_, bool kTrim>
+__global__ void __launch_bounds__(32 * rows_warps<T>())
+window_rows_kernel(const PSlot<T>* __restrict__ slots, const uint32_t* __restrict__ offset, int nbins, WindowParams wp,
+                   const __grid_constant__ PolyArg<M_> pa, T* __restrict__ rows) {
+    using R = WindowRows<M_, kTrim>;
+    using V4 = typename Vec4<T>::type;
+    constexpr int SP = R::RP + 4;                                  // 44 / 52 elements: conflict-free 16-byte accesses
+    constexpr int kRowsWarps = rows_warps<T>();
+    __shared__ __align__(16) T tile[kRowsWarps][32 * SP];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t n_charged = offset[nbins];
+    const uint32_t base = (uint32_t)(blockIdx.x * kRowsWarps + warp) * 32u;
+    if (base >= n_charged) return;
+    const uint32_t nv = min(32u, n_charged - base);
+    T* mine = tile[warp] + lane * SP;
+    if ((uint32_t)lane < nv) {
+        const PSlot<T> sl = slots[base + lane];
+        const int ksx = (int)((sl.cell >> 30) & 1u);
+        // parity of the first x stencil point (grid index c_x - m + ks_x; n is even, so wrapping keeps it)
+        const int parx = ((int)(sl.cell & 1023u) + M_ + ksx) & 1;
+        write_window_rows<T, M_, kTrim>(wp, pa, sl.rec.dx, sl.rec.dy, sl.rec.dz, sl.rec.q, parx, mine);
+    }
+    __syncwarp();
+    T* out = rows + (size_t)base * R::RP;
+    constexpr int CH = R::RP / 4;                                  // 16-byte (fp32) / 32-byte (fp64) chunks per particle
+    for (int c = lane; c < (int)nv * CH; c += 32) {
+        const int pp = c / CH, cc = c - pp * CH;
+        reinterpret_cast<V4*>(out)[c] = reinterpret_cast<const V4*>(tile[warp] + pp * SP)[cc];
+    }
 }
 
 }  // namespace enuf

@@ -44,10 +44,11 @@ template <typename T> struct alignas(4 * sizeof(T)) PRec { T dx, dy, dz, q; };
 template <typename T> struct alignas(sizeof(T) == 4 ? 32 : 16) PSlot { PRec<T> rec; uint32_t cell, idx; };
 
 // Geometry shared by bin / spread / gather.  Particles are counting-sorted into bins
-//   bin = (Ty * nt + Tx) * n + cz,   Tx = cx / 16, Ty = cy / 16
-// (a column of 16 x 16 cells in x, y; one grid plane in z), so that
-//   - the particles of a z-slab of a column are one contiguous range (spread walks z), and
-//   - the particles of a 16^3 tile are one contiguous range of 16 bins (gather).
+//   bin = (Ty * n + bz) * nt + Tx,   Tx = cx / 16, Ty = cy / 16, bz = the particle's grid plane
+// (a column of 16 x 16 cells in x, y; one grid plane in z; x-neighbouring columns adjacent), so that
+//   - the particles of plane bz in a run of x-neighbouring columns are ONE contiguous range: the spreading
+//     producer reads the halo of its column, slab by slab, as three such ranges (one per row of columns), and
+//   - the particles of a 16^3 tile are 16 ranges, one per plane (gather).
 constexpr int kTile = 16;
 struct TileGeom {
     int n;        // grid points per dimension
@@ -84,6 +85,8 @@ struct PolyArg {
     float2 dp[NP][M_ + 1];
 };
 
+__host__ __device__ inline int bin_index(const TileGeom& g, int tx, int ty, int bz) { return (ty * g.n + bz) * g.nt + tx; }
+
 __host__ __device__ inline uint32_t pack_cell(int cx, int cy, int cz) {
     return (uint32_t)cx | ((uint32_t)cy << 10) | ((uint32_t)cz << 20);
 }
@@ -109,6 +112,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// same for waits that can be long (another warp's work): sleep between tries, with a growing interval, instead of
+// spinning through issue slots that the working warps of the SM need
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity) {
+    uint32_t done, ns = 32;
+    for (;;) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(ns);
+        ns = ns < 512u ? 2u * ns : ns;
+    }
 }
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");

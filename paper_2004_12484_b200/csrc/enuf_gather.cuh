@@ -1,7 +1,7 @@
 // Step a6 -- interpolating (forward NFFT, last part; Eq. 42 :340).
 //
-// One CTA per 16^3 grid tile, working on the tile's particles (a contiguous range of 16
-// bins, TileGeom), with the tile plus a halo of m cells per side ((16+2m)^3 values) held in
+// One CTA per 16^3 grid tile, working on the tile's particles (16 ranges of the sorted array, one
+// per plane; TileGeom), with the tile plus a halo of m cells per side ((16+2m)^3 values) held in
 // shared memory (staged with cp.async).  Every warp takes a contiguous share of the tile's
 // particles (shares differ by at most one), five at a time: first the 3 W window values and derivatives of those particles are computed once
 // (one lane per particle and dimension) and kept on chip, then the warp
@@ -87,14 +87,40 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
     using P2 = typename Pair2<T>::type;
     constexpr int W = C::W, WE = C::WE, TP = C::TP, SX = C::SX, SPL = C::SPL, PBW = C::PBW, ITER = C::ITER, WP = C::WP;
 
-    // tile (Tx, Ty, Tz): bins (Ty*nt + Tx)*n + 16 Tz .. + 16
+    // tile (Tx, Ty, Tz): the particles of its 16 planes are 16 ranges of the sorted array, bins
+    // bin_index(Tx, Ty, 16 Tz + zl) (TileGeom); pre_s[zl] = particles of the planes before zl
     const int ntz = g.n / kTile;
     const int Tz = blockIdx.x % ntz, col = blockIdx.x / ntz;
     const int Tx = col % g.nt, Ty = col / g.nt;
-    const int bin0 = col * g.n + Tz * kTile;
-    const uint32_t start = offset[bin0];
-    const int cnt = (int)(offset[bin0 + kTile] - start);
+    __shared__ uint32_t st_s[kTile];
+    __shared__ int pre_s[kTile + 1];
+    if (threadIdx.x < 32) {
+        const int zl = threadIdx.x & (kTile - 1);
+        const int b = bin_index(g, Tx, Ty, Tz * kTile + zl);
+        const uint32_t st = offset[b];
+        int c = (int)(offset[b + 1] - st), inc = c;
+#pragma unroll
+        for (int o = 1; o < kTile; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o, kTile);
+            if (zl >= o) inc += t;
+        }
+        if (threadIdx.x < kTile) {
+            st_s[zl] = st; pre_s[zl] = inc - c;
+            if (zl == kTile - 1) pre_s[kTile] = inc;
+        }
+    }
+    __syncthreads();
+    const int cnt = pre_s[kTile];
     if (cnt == 0) return;
+    // sorted-array index of the tile's p-th particle
+    auto slot_of = [&](int p) -> uint32_t {
+        int lo = 0;
+        if (pre_s[lo + 8] <= p) lo += 8;
+        if (pre_s[lo + 4] <= p) lo += 4;
+        if (pre_s[lo + 2] <= p) lo += 2;
+        if (pre_s[lo + 1] <= p) lo += 1;
+        return st_s[lo] + (uint32_t)(p - pre_s[lo]);
+    };
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* tile_s = reinterpret_cast<T*>(smem_raw);
@@ -171,7 +197,8 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
     auto batch_weights = [&](int p0, int nb) {
         if (lane < 3 * nb) {
             const int dim = lane / nb, slot = lane - dim * nb;
-            const PRec<T> pr = slots[start + p0 + slot].rec;
+            const uint32_t gi = slot_of(p0 + slot);
+            const PRec<T> pr = slots[gi].rec;
             const T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
             T w[W], dw[W];
             stencil_weights<T, M_, !kIk, true>(wp, pa, d0, w, dw);   // packed Horner chains
@@ -186,7 +213,7 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
             }
             if (dim == 0) {
                 int cx, cy, cz;
-                unpack_cell(slots[start + p0 + slot].cell, cx, cy, cz);
+                unpack_cell(slots[gi].cell, cx, cy, cz);
                 int zrel = cz - tz0;                  // trimmed bins: c_z may be the first plane of the next tile
                 zrel += zrel < 0 ? g.n : 0;
                 if (kTrim) {
@@ -194,7 +221,7 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
                 }
                 base_s[slot] = zrel * SPL + (cy - ty0) * SX + (cx - tx0) + (C::XS - M_);
                 q_s[slot] = pre * pr.q;
-                idx_s[slot] = (int)slots[start + p0 + slot].idx;
+                idx_s[slot] = (int)slots[gi].idx;
             }
         }
     };
@@ -204,13 +231,6 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
     // batches of PBW: the CTA ends within one particle of perfect balance
     const int share = cnt / C::WARPS, extra = cnt - share * C::WARPS;
     const int wbeg = warp * share + min(warp, extra), wend = wbeg + share + (warp < extra ? 1 : 0);
-    // the warp's whole share of sorted slots (~20 x 32 B) is started towards L2 now: the load that opens each
-    // later batch_weights then waits for an L2 hit instead of a DRAM access
-    {
-        const char* sh0 = reinterpret_cast<const char*>(slots + start + wbeg);
-        const int bytes = (wend - wbeg) * (int)sizeof(PSlot<T>);
-        for (int o = 128 * lane; o < bytes + 127; o += 128 * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(sh0 + o));
-    }
     if (wbeg < wend) batch_weights(wbeg, min(PBW, wend - wbeg));
     cp_async_wait_all();
     __syncthreads();

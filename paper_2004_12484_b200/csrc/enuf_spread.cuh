@@ -9,7 +9,7 @@
 //     acc[k] += (a0, a1) * (q wz[k]) with (a0, a1) = wx[cells] * wy[cell].  After slab s the lowest plane
 //     of the window is complete: one coalesced store, and the window slides.  Every grid value is written
 //     exactly once -- no atomics, no clearing of the grid, no shared-memory read-modify-write;
-//   - two PRODUCER warps, one per stage of a two-stage buffer in shared memory, taking the slabs in turn:
+//   - four PRODUCER warps taking the slabs in turn, two sharing each stage of a two-stage buffer in shared memory:
 //     a producer culls the particles of the neighbouring bins against the column's halo, copies the three
 //     window rows of the accepted ones (3 x 16 values, evaluated ONCE per particle by the bin scatter --
 //     "window values computed [once and kept]") into slots of its stage with cp.async, builds
@@ -60,11 +60,12 @@ struct SpreadCfg {
     static constexpr int WZ = W - (kTrim ? 1 : 0);               // stencil points per dimension = planes in the window
     static constexpr int SLO = M_, SHI = kTrim ? M_ - 1 : M_;    // slab s reaches the planes s - SHI .. s + SLO
     static constexpr int NPX = NPX_, NPY = 2, NCONS = NPX * NPY; // 8 x 8 patches = consumer warps
-    static constexpr int NPROD = 2;                              // producer warps = stages: producer k fills stage k
+    static constexpr int NPROD = 4;                              // producer warps: producer k takes the slabs k, k + 4, .. of the chunk
+    static constexpr int NSTAGE = 3;                             //   slab i of the chunk is staged in stage i % 3
     static constexpr int CX = 8 * NPX, CY = 8 * NPY;             // column
     static constexpr int NT = 32 * (NCONS + NPROD);
     static constexpr int NBX = CX / kTile + 2, NBY = CY / kTile + 2;   // bins (16 x 16, enuf_common.cuh) the halo touches
-    static constexpr int NBIN = NBX * NBY, NPAIR = (NBIN + 1) / 2;
+    static constexpr int NSEG = 2 * NBY;                         // ranges of the sorted array per slab (<= 2 per row of bin columns)
     // slot layout (elements of T): zeros | x row | zeros | y row | zeros | z row ; the largest index a lane reads is
     // x: 8 + 1 + (WZ-1) + 7, y: OYF + (WZ-1) + 7 (header comment)
     static constexpr int OXF = 8;
@@ -73,13 +74,14 @@ struct SpreadCfg {
     static constexpr int PITCH = OZF + 16 <= 68 ? 68 : 76;       // = 4 / 12 mod 32: 16-byte row chunks of 8 slots hit 32 banks
     static constexpr int CAP = sizeof(T) == 4 ? (NPX == 4 ? (PITCH == 68 ? 96 : 88) : 56) : (NPX == 4 ? 48 : 40);   // staged particles per round
     static constexpr int LCAP = CAP + 4;                         // visit-list entries per patch (even padding + prefetch)
-    static constexpr int NSTAGE = NPROD;
     static constexpr int kBlk = 16;                              // slabs (of one producer) whose bin ranges are loaded at once
-    static constexpr int CTAS_PER_SM = sizeof(T) == 4 ? (NPX == 4 ? 3 : 5) : (NPX == 4 ? 1 : 2);
+    static constexpr int CTAS_PER_SM = sizeof(T) == 4 ? (NPX == 4 ? 2 : 3) : (NPX == 4 ? 1 : 2);
     static constexpr size_t SLOT_BYTES = sizeof(T) * (size_t)(CAP + 1) * PITCH;   // slot CAP is all zero
     static constexpr size_t LIST_BYTES = sizeof(uint2) * (size_t)NCONS * LCAP;
-    static constexpr size_t STAGE_BYTES = ((SLOT_BYTES + LIST_BYTES + sizeof(int) * CAP + 15) / 16) * 16;
-    static_assert(CAP >= 32, "a cull step stages up to 32 particles");
+    static constexpr size_t STAGE_BYTES = ((SLOT_BYTES + LIST_BYTES + 15) / 16) * 16;
+    static_assert(CAP >= 32 && CAP + 1 < 256 && NCONS <= 8, "a cull step stages up to 32 particles; packed list lengths");
+    static_assert(NSEG <= 32 && kBlk == 16, "one lane per segment; lanes = 16 slabs x (start, end)");
+    static_assert(NPROD == 4 && NSTAGE == 3, "barrier protocol: slab i - 3 held the stage, its producer is (k + 1) & 3");
     static_assert(SLOT_BYTES < 65536, "visit-list entries are 16-bit byte offsets");
     static_assert(OZF + 16 <= PITCH, "slot layout");
 };
@@ -90,16 +92,24 @@ constexpr size_t spread_smem_bytes() {
     return C::STAGE_BYTES * C::NSTAGE;
 }
 
-// The three 16-element window rows of one particle, as the spreading kernel stages them (written once per
-// particle by the bin scatter, enuf_bin.cuh, read by every CTA whose halo the particle is in):
-//   x row: element j = phi_x at stencil point j - parx (parx = parity of the first stencil point's grid index),
-//   y row: element j = phi_y at stencil point j,   z row: element j = q phi_z at stencil point j,
+// The three window rows of one particle, as the spreading kernel stages them (evaluated once per particle by
+// window_rows_kernel, enuf_bin.cuh, read by every CTA whose halo the particle is in): RP elements per particle,
+//   x row [0, 16):        element j = phi_x at stencil point j - parx (parx = parity of the first stencil point's grid index),
+//   y row [16, 16 + RY):  element j = phi_y at stencil point j,
+//   z row [16 + RY, RP):  element j = q phi_z at stencil point j,
 // zero beyond the WZ stencil points.  kTrim: stencil point k is point k + ks of the 2m+1 (ks = d0 > 0).
-constexpr int kRowElems = 16, kRowsPerParticle = 3;
+template <int M_, bool kTrim>
+struct WindowRows {
+    static constexpr int W = 2 * M_ + 1, WZ = W - (kTrim ? 1 : 0);
+    static constexpr int RX = 16, RY = (WZ + 3) / 4 * 4, OY = RX, OZ = RX + RY, RP = RX + 2 * RY;
+    static_assert(WZ + 1 <= RX, "x row: WZ points + one parity element");
+};
+
 template <typename T, int M_, bool kTrim>
 __device__ __forceinline__ void write_window_rows(const WindowParams& wp, const PolyArg<M_>& pa, T dx, T dy, T dz, T q,
                                                   int parx, T* __restrict__ dst) {
-    constexpr int W = 2 * M_ + 1, WZ = W - (kTrim ? 1 : 0);
+    using R = WindowRows<M_, kTrim>;
+    constexpr int W = R::W, WZ = R::WZ;
     using V4 = typename Vec4<T>::type;
 #pragma unroll
     for (int dim = 0; dim < 3; ++dim) {
@@ -109,9 +119,11 @@ __device__ __forceinline__ void write_window_rows(const WindowParams& wp, const 
         const int sh = (kTrim && d0 > (T)0) ? 1 : 0;
         const int par = dim == 0 ? parx : 0;
         const T mult = dim == 2 ? q : (T)1;
-        T r16[kRowElems];
+        constexpr int RMAX = R::RX;
+        const int len = dim == 0 ? R::RX : R::RY;                 // compile-time per unrolled dim
+        T rr[RMAX];
 #pragma unroll
-        for (int j = 0; j < kRowElems; ++j) {
+        for (int j = 0; j < RMAX; ++j) {
             // element j holds stencil point k = j - par, i.e. w[k + sh]
             T v = (T)0;
             if (kTrim) {
@@ -125,15 +137,46 @@ __device__ __forceinline__ void write_window_rows(const WindowParams& wp, const 
                 const T b0 = (j >= 1 && j - 1 < WZ) ? w[j >= 1 ? j - 1 : 0] : (T)0;
                 v = par ? b0 : a0;
             }
-            r16[j] = v * mult;
+            rr[j] = v * mult;
         }
-        V4* row4 = reinterpret_cast<V4*>(dst + dim * kRowElems);
+        V4* row4 = reinterpret_cast<V4*>(dst + (dim == 0 ? 0 : (dim == 1 ? R::OY : R::OZ)));
 #pragma unroll
-        for (int v = 0; v < kRowElems / 4; ++v) {
-            V4 o; o.x = r16[4 * v]; o.y = r16[4 * v + 1]; o.z = r16[4 * v + 2]; o.w = r16[4 * v + 3];
-            row4[v] = o;
+        for (int v = 0; v < RMAX / 4; ++v) {
+            if (4 * v < len) {
+                V4 o; o.x = rr[4 * v]; o.y = rr[4 * v + 1]; o.z = rr[4 * v + 2]; o.w = rr[4 * v + 3];
+                row4[v] = o;
+            }
         }
     }
+}
+
+// explicit shared-space loads (32-bit shared addresses: no generic-to-shared conversion inside the visit loop)
+template <typename T> __device__ __forceinline__ typename Pair2<T>::type lds_pair(uint32_t a);
+template <> __device__ __forceinline__ float2 lds_pair<float>(uint32_t a) {
+    float2 v; asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a)); return v;
+}
+template <> __device__ __forceinline__ double2 lds_pair<double>(uint32_t a) {
+    double2 v; asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a)); return v;
+}
+template <typename T> __device__ __forceinline__ T lds_one(uint32_t a);
+template <> __device__ __forceinline__ float lds_one<float>(uint32_t a) {
+    float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v;
+}
+template <> __device__ __forceinline__ double lds_one<double>(uint32_t a) {
+    double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v;
+}
+template <typename T> __device__ __forceinline__ typename Vec4<T>::type lds_quad(uint32_t a);
+template <> __device__ __forceinline__ float4 lds_quad<float>(uint32_t a) {
+    float4 v; asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a)); return v;
+}
+template <> __device__ __forceinline__ double4 lds_quad<double>(uint32_t a) {
+    double4 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.z), "=d"(v.w) : "r"(a + 16u));
+    return v;
+}
+__device__ __forceinline__ uint2 lds_u2(uint32_t a) {
+    uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v;
 }
 
 __device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void* gmem_src) {
@@ -144,149 +187,197 @@ __device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
+#ifdef ENUF_TRACE
+// debugging aid (never defined in the product build): time stamps of one CTA's producers and two of its consumers
+__device__ long long g_spread_trace[16384];
+__device__ __forceinline__ long long trace_clock() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define ENUF_TR(slot, val) do { if (tr_on && lane == 0) g_spread_trace[(slot)] = (val); } while (0)
+#else
+#define ENUF_TR(slot, val) do { } while (0)
+#endif
+
 // slots[].cell: bits 0..29 the packed nearest cell, bits 30 / 31 = ks_x / ks_y (trimmed plans; enuf_bin.cuh)
-// rows: [N][3][16] window rows in bin order (write_window_rows)
+// rows: [N][RP] window rows in bin order (WindowRows)
 template <typename T, int M_, bool kTrim, int NPX>
 __global__ void __launch_bounds__((SpreadCfg<T, M_, kTrim, NPX>::NT), (SpreadCfg<T, M_, kTrim, NPX>::CTAS_PER_SM))
 spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
               const uint32_t* __restrict__ offset, TileGeom g, int zchunk, T* __restrict__ grid) {
     using C = SpreadCfg<T, M_, kTrim, NPX>;
+    using R = WindowRows<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
     using V4 = typename Vec4<T>::type;
     constexpr int WZ = C::WZ, NCONS = C::NCONS, CX = C::CX, CY = C::CY, CAP = C::CAP, LCAP = C::LCAP;
     constexpr int PITCH = C::PITCH, OXF = C::OXF, OYF = C::OYF, OZF = C::OZF;
-    constexpr int NBX = C::NBX, NBIN = C::NBIN, NPAIR = C::NPAIR, NSTAGE = C::NSTAGE, kBlk = C::kBlk;
+    constexpr int NSTAGE = C::NSTAGE, kBlk = C::kBlk, NSEG = C::NSEG;
     constexpr unsigned ES = (unsigned)sizeof(T);
     constexpr unsigned FULL = 0xffffffffu;
-    constexpr int NCH = (int)(kRowElems * sizeof(T) / 16);        // 16-byte chunks per row
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ uint64_t full_bar[NSTAGE], empty_bar[NSTAGE];
-    __shared__ int cnt_s[NSTAGE][NCONS];        // visits of each patch in the stage (even, zero-record padded)
+    // per producer k: full_bar[k]  -- a round of one of its slabs is staged (consumers wait),
+    //                 again_bar[k] -- every consumer is done with a round that was not the slab's last (producer k waits),
+    //                 empty_bar[k] -- every consumer is done with the last round of a slab of producer k: its stage is
+    //                                 free for the slab three further on, i.e. for producer (k + 3) & 3 (only that one waits on it).
+    // Every barrier has one waiting party that sees each of its phases in turn, so one parity bit per party suffices.
+    __shared__ uint64_t full_bar[C::NPROD], empty_bar[C::NPROD], again_bar[C::NPROD];
+    __shared__ int cnt_s[NSTAGE][NCONS];        // visits of each patch in the stage
     __shared__ int last_s[NSTAGE];              // 1: the stage is the last round of its slab
-    __shared__ uint32_t rng[C::NPROD][NBIN][2 * kBlk];   // [..][0..kBlk): range starts of kBlk slabs, [kBlk..): ends
+    __shared__ uint32_t rng[C::NPROD][NSEG][2 * kBlk];   // [..][0..kBlk): range starts of kBlk slabs, [kBlk..): ends
+    __shared__ uint2 acc_rec[C::NPROD][CAP];            // producer's side buffer: accepted particles of the round,
+                                                        //   (sorted-array index, (X0 + 32) | (Y0 + 32) << 8)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int ncx_per = CX / kTile, ncy_per = CY / kTile;
     const int ncolx = g.n / CX;
     const int Tx = blockIdx.x % ncolx, Ty = blockIdx.x / ncolx;
     const int z0 = blockIdx.y * zchunk, z1 = min(g.n, z0 + zchunk);
     const int s_begin = z0 - C::SLO, s_end = z1 + C::SHI;
+#ifdef ENUF_TRACE
+    const bool tr_on = blockIdx.x == 37 && blockIdx.y == 1;
+#endif
 
     // the zero padding of every slot (and the all-zero slot CAP) is written once; rows are rewritten per round
     for (int i = tid; i < (int)(C::STAGE_BYTES * NSTAGE / 16); i += C::NT)
         reinterpret_cast<uint4*>(smem_raw)[i] = make_uint4(0u, 0u, 0u, 0u);
     if (tid == 0) {
 #pragma unroll
-        for (int st = 0; st < NSTAGE; ++st) {
+        for (int st = 0; st < C::NPROD; ++st) {
             // full: one arrival per producer lane when its row copies have landed + one after the lists are written
             mbar_init(&full_bar[st], 33);
             mbar_init(&empty_bar[st], NCONS);
+            mbar_init(&again_bar[st], NCONS);
         }
     }
     __syncthreads();
 
     if (warp >= NCONS) {
         // =========================================================== producers
-        // producer k fills stage k with the slabs s_begin + k, s_begin + k + 2, ..
-        const int k = warp - NCONS, stage = k;
+        // producer k stages the slabs s_begin + k, s_begin + k + 4, ..; slab i of the chunk goes to stage i % 3
+        const int k = warp - NCONS;
         const int half = lane >> 4, l16 = lane & 15;
         const unsigned below = (1u << lane) - 1u;
-        int bin0 = 0;                            // lane b < NBIN: first bin (plane 0) of neighbouring bin column b
-        if (lane < NBIN) {
-            int tbx = Tx * ncx_per - 1 + lane % NBX, tby = Ty * ncy_per - 1 + lane / NBX;
-            tbx += tbx < 0 ? g.nt : 0; tbx -= tbx >= g.nt ? g.nt : 0;
-            tby += tby < 0 ? g.nt : 0; tby -= tby >= g.nt ? g.nt : 0;
-            bin0 = (tby * g.nt + tbx) * g.n;
+        // The halo of the column touches NBY rows of NBX bin columns; in bin order (TileGeom) the NBX bins of one
+        // row and plane are adjacent, so a slab is NBY ranges of the sorted array, each split in two where the
+        // row of columns wraps around the box (segments 2 jy, 2 jy + 1).  Lane sg < NSEG: (first bin of plane 0,
+        // number of bins) of segment sg.  Rows / columns the periodic box holds only once are taken once.
+        int seg_bin0 = 0, seg_nb = 0;
+        if (lane < NSEG) {
+            const int jy = lane >> 1, second = lane & 1;
+            const int nrow = C::NBY < g.nt ? C::NBY : g.nt, nbx = C::NBX < g.nt ? C::NBX : g.nt;
+            int ty = Ty * (CY / kTile) - 1 + jy;
+            ty += ty < 0 ? g.nt : 0; ty -= ty >= g.nt ? g.nt : 0;
+            int txlo = Tx * (CX / kTile) - 1;
+            txlo += txlo < 0 ? g.nt : 0;
+            if (nbx == g.nt) txlo = 0;
+            const int na = min(nbx, g.nt - txlo);        // bins before the wrap
+            const int tx = second ? 0 : txlo;
+            seg_nb = jy < nrow ? (second ? nbx - na : na) : 0;
+            seg_bin0 = bin_index(g, tx, ty, 0);
         }
-        unsigned char* sbase = smem_raw + (size_t)stage * C::STAGE_BYTES;
-        const uint32_t sl32 = smem_u32(sbase);
-        uint2* lists = reinterpret_cast<uint2*>(sbase + C::SLOT_BYTES);
-        int* pk = reinterpret_cast<int*>(sbase + C::SLOT_BYTES + C::LIST_BYTES);
+        // first stencil point in column coordinates from the packed cell: the periodic image that can overlap the column
+        const int offx = -M_ - CX * Tx + (WZ - 1), offy = -M_ - CY * Ty + (WZ - 1), nmask = g.n - 1;
         uint32_t (*rg)[2 * kBlk] = rng[k];
-        unsigned pe = 0;                         // phase of empty_bar[stage] this producer waits for next, flipped
-        int blk0 = s_begin + k - 2 * kBlk;
+        unsigned pe = 0, pa = 0;                 // parities of the next phase of empty_bar[(k + 1) & 3] / again_bar[k] to wait for
+        int blk0 = s_begin + k - C::NPROD * kBlk;
         for (int s = s_begin + k; s < s_end; s += C::NPROD) {
-            if (s - blk0 >= 2 * kBlk) {
+            if (s - blk0 >= C::NPROD * kBlk) {
                 // ranges of this producer's next kBlk slabs: lane & 15 = slab, lanes 0..15 load the starts, 16..31 the ends
                 blk0 = s;
                 __syncwarp();
-                const int cz = (blk0 + 2 * l16) & (g.n - 1);
+                const int cz = (blk0 + C::NPROD * l16) & nmask;
 #pragma unroll
-                for (int b = 0; b < NBIN; ++b) {
-                    const int bb = __shfl_sync(FULL, bin0, b);
-                    rg[b][lane] = offset[bb + cz + half];
+                for (int sg = 0; sg < NSEG; ++sg) {
+                    const int b0 = __shfl_sync(FULL, seg_bin0, sg), nb = __shfl_sync(FULL, seg_nb, sg);
+                    rg[sg][lane] = offset[b0 + cz * g.nt + half * nb];
                 }
                 __syncwarp();
             }
-            const int js = (s - blk0) >> 1;
-            int c0 = 0, p0 = 0;                  // next candidates: index c0 + (0..15) of the bins of pairs p0..
-            bool slab_done = false;
-            while (!slab_done) {
-                mbar_wait(&empty_bar[stage], pe ^ 1u);
-                pe ^= 1u;
-                int ns = 0;
-                // ---- cull: 16 candidates of two bins per step (half-warp each); all cell loads of a sweep over
-                //      the bins are issued before the first is examined.  An accepted particle's three window
-                //      rows are copied from global memory into its slot by cp.async.
-                for (;;) {
-                    uint32_t cellw[NPAIR], pidx[NPAIR];
-                    int cmax = 0;
+            const int js = (s - blk0) / C::NPROD;
+            const int stage = (s - s_begin) % NSTAGE;
+            unsigned char* sbase = smem_raw + (size_t)stage * C::STAGE_BYTES;
+            const uint32_t sl32 = smem_u32(sbase);
+            uint2* lists = reinterpret_cast<uint2*>(sbase + C::SLOT_BYTES);
+            // candidates: the ranges of the NSEG segments, 32 per step.  The cell words of up to kSteps steps are
+            // loaded together (one global-load latency per slab, not one per step), then examined in order.
+            constexpr int kSteps = 8;
+            int sg = 0;
+            uint32_t gs = 0, ge = 0;
+            uint32_t cw[kSteps], cbase[kSteps];
+            int nst = 0;                         // steps loaded (consumed ones are marked invalid)
+            auto load_steps = [&]() {
+                nst = 0;
 #pragma unroll
-                    for (int p = 0; p < NPAIR; ++p) {
-                        const int b = 2 * p + half;
-                        uint32_t st = 0; int cn = 0;
-                        if (b < NBIN) { st = rg[b][js]; cn = (int)(rg[b][kBlk + js] - st); }
-                        cmax = max(cmax, cn);
-                        const int kk = c0 + l16;
-                        pidx[p] = st + (uint32_t)kk;
-                        cellw[p] = (p >= p0 && kk < cn) ? slots[pidx[p]].cell : 0xffffffffu;
+                for (int j = 0; j < kSteps; ++j) {
+                    while (gs >= ge && sg < NSEG) { gs = rg[sg][js]; ge = rg[sg][kBlk + js]; ++sg; }
+                    cbase[j] = gs;
+                    cw[j] = 0xffffffffu;
+                    if (gs < ge) {
+                        if (gs + (uint32_t)lane < ge) cw[j] = slots[gs + (uint32_t)lane].cell;
+                        gs += 32u;
+                        nst = j + 1;
                     }
-                    cmax = max(cmax, __shfl_xor_sync(FULL, cmax, 16));
-                    bool stop = false;
-#pragma unroll
-                    for (int p = 0; p < NPAIR; ++p) {
-                        if (p < p0) continue;
-                        const uint32_t cw = cellw[p];
-                        const unsigned vb = __ballot_sync(FULL, cw != 0xffffffffu);
-                        if (vb == 0u) continue;                       // both bins exhausted
-                        if (ns + __popc(vb) > CAP) { p0 = p; stop = true; break; }
-                        const int b = 2 * p + half;
-                        // first stencil point, column coords: nearest cell - m (+ ks when trimmed)
-                        const int X0 = (int)(cw & 15u) + (b % NBX - 1) * kTile - M_ + (kTrim ? (int)((cw >> 30) & 1u) : 0);
-                        const int Y0 = (int)((cw >> 10) & 15u) + (b / NBX - 1) * kTile - M_ + (kTrim ? (int)(cw >> 31) : 0);
-                        const bool ok = cw != 0xffffffffu && X0 <= CX - 1 && X0 + WZ - 1 >= 0 && Y0 <= CY - 1 && Y0 + WZ - 1 >= 0;
-                        const unsigned bal = __ballot_sync(FULL, ok);
-                        if (ok) {
-                            const int pos = ns + __popc(bal & below);
-                            pk[pos] = (X0 + 32) | ((Y0 + 32) << 8);
-                            const char* src = reinterpret_cast<const char*>(rows + (size_t)pidx[p] * (kRowsPerParticle * kRowElems));
-                            const uint32_t dst = sl32 + (uint32_t)(pos * PITCH) * ES;
-#pragma unroll
-                            for (int c = 0; c < NCH; ++c) cp_async_16(dst + OXF * ES + 16 * c, src + 16 * c);
-#pragma unroll
-                            for (int c = 0; c < NCH; ++c) cp_async_16(dst + OYF * ES + 16 * c, src + 16 * (NCH + c));
-#pragma unroll
-                            for (int c = 0; c < NCH; ++c) cp_async_16(dst + OZF * ES + 16 * c, src + 16 * (2 * NCH + c));
-                        }
-                        ns += __popc(bal);
-                    }
-                    if (stop) break;
-                    p0 = 0; c0 += 16;
-                    if (c0 >= cmax) { slab_done = true; break; }
                 }
-                cp_async_mbar_arrive(&full_bar[stage]);
+            };
+            load_steps();
+            bool slab_done = false, first_round = true;
+            while (!slab_done) {
+                // ---- cull (before the stage is free: it needs only this producer's side buffer): accepted particles'
+                //      sorted-array index and packed stencil origin; their rows are started towards L2
+                int ns = 0;
+                ENUF_TR((s - s_begin) * 16 + 0, trace_clock());
+                for (;;) {
+                    // all loaded steps at once, branch-free (the steps are independent up to the running slot count)
+                    int pkv[kSteps]; unsigned bal[kSteps];
+#pragma unroll
+                    for (int j = 0; j < kSteps; ++j) {
+                        const uint32_t cwj = cw[j];
+                        const int X0 = (((int)(cwj & 1023u) + (int)((cwj >> 30) & 1u) + offx) & nmask) - (WZ - 1);
+                        const int Y0 = (((int)((cwj >> 10) & 1023u) + (int)(cwj >> 31) + offy) & nmask) - (WZ - 1);
+                        const bool ok = cwj != 0xffffffffu && X0 <= CX - 1 && Y0 <= CY - 1;
+                        bal[j] = __ballot_sync(FULL, ok);
+                        pkv[j] = ok ? ((X0 + 32) | ((Y0 + 32) << 8)) : -1;
+                    }
+                    // steps are taken while their accepted particles fit into the round (CAP slots)
+                    int jl = kSteps, base = ns, pb[kSteps];
+#pragma unroll
+                    for (int j = 0; j < kSteps; ++j) {
+                        const int c = __popc(bal[j]);
+                        if (jl == kSteps && base + c > CAP) jl = j;
+                        pb[j] = base;
+                        if (j < jl) base += c;
+                    }
+#pragma unroll
+                    for (int j = 0; j < kSteps; ++j) {
+                        if (j < jl) {
+                            if (pkv[j] >= 0)
+                                acc_rec[k][pb[j] + __popc(bal[j] & below)] = make_uint2(cbase[j] + (uint32_t)lane, (unsigned)pkv[j]);
+                            cw[j] = 0xffffffffu;                        // consumed
+                        }
+                    }
+                    ns = base;
+                    if (jl < kSteps) break;                            // step jl opens the next round of this slab
+                    if (nst < kSteps) { slab_done = true; break; }     // the ranges are exhausted
+                    load_steps();                                      // a long slab: the next kSteps steps
+                    if (nst == 0) { slab_done = true; break; }
+                }
+                __syncwarp();
+                ENUF_TR((s - s_begin) * 16 + 1, trace_clock());
+                if (first_round) {
+                    // the slab that held the stage before (s - 3, staged by producer (k + 1) & 3) must be finished
+                    if (s - NSTAGE >= s_begin) { mbar_wait_backoff(&empty_bar[(k + 1) & 3], pe); pe ^= 1u; }
+                    first_round = false;
+                } else {
+                    mbar_wait_backoff(&again_bar[k], pa); pa ^= 1u;     // the previous round of this slab
+                }
+                ENUF_TR((s - s_begin) * 16 + 2, trace_clock());
                 __syncwarp();
                 // ---- visit lists: for every patch the staged particles whose stencil overlaps it, as ready-made
                 //      byte offsets (x row | z row << 16, y row) into the stage
-                int lc[NCONS];
-#pragma unroll
-                for (int w8 = 0; w8 < NCONS; ++w8) lc[w8] = 0;
+                // (the NCONS running list lengths are bytes of two packed words: a round stages at most CAP + 1 < 256 entries per list)
+                unsigned lcp[2] = {0u, 0u};
                 for (int g0 = 0; g0 < ns; g0 += 32) {
                     const int slot = g0 + lane;
                     const bool v = slot < ns;
                     int X0 = 64, Y0 = 64;
-                    if (v) { const int pkv = pk[slot]; X0 = (pkv & 255) - 32; Y0 = ((pkv >> 8) & 255) - 32; }
+                    if (v) { const int pkv = (int)acc_rec[k][slot].y; X0 = (pkv & 255) - 32; Y0 = ((pkv >> 8) & 255) - 32; }
                     const unsigned sb = (unsigned)(slot * PITCH) * ES;
                     const unsigned xb = sb + (unsigned)(OXF + (X0 & 1) - X0) * ES;
                     const unsigned yb = sb + (unsigned)(OYF - Y0) * ES;
@@ -296,24 +387,47 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                         const int px0 = 8 * (w8 % NPX), py0 = 8 * (w8 / NPX);
                         const bool ov = v && X0 <= px0 + 7 && X0 + WZ - 1 >= px0 && Y0 <= py0 + 7 && Y0 + WZ - 1 >= py0;
                         const unsigned bal = __ballot_sync(FULL, ov);
-                        if (ov) lists[w8 * LCAP + lc[w8] + __popc(bal & below)] =
+                        const unsigned cur = (lcp[w8 >> 2] >> (8 * (w8 & 3))) & 255u;
+                        if (ov) lists[w8 * LCAP + cur + __popc(bal & below)] =
                                     make_uint2((xb + (unsigned)px0 * ES) | (zb << 16), yb + (unsigned)py0 * ES);
-                        lc[w8] += __popc(bal);
+                        lcp[w8 >> 2] += (unsigned)__popc(bal) << (8 * (w8 & 3));
                     }
                 }
+                ENUF_TR((s - s_begin) * 16 + 13, trace_clock());
                 if (lane == 0) {
                     const unsigned zs = (unsigned)(CAP * PITCH) * ES;      // the all-zero slot
 #pragma unroll
                     for (int w8 = 0; w8 < NCONS; ++w8) {
-                        int c = lc[w8];
-                        if (c & 1) { lists[w8 * LCAP + c] = make_uint2((zs + OXF * ES) | ((zs + OZF * ES) << 16), zs + OYF * ES); ++c; }
-                        cnt_s[stage][w8] = c;
+                        const int c = (int)((lcp[w8 >> 2] >> (8 * (w8 & 3))) & 255u);
+                        // even length, and the consumer loads its operands one visit ahead: entries that point at the zero slot
+                        lists[w8 * LCAP + c] = lists[w8 * LCAP + c + 1] = lists[w8 * LCAP + c + 2] =
+                            make_uint2((zs + OXF * ES) | ((zs + OZF * ES) << 16), zs + OYF * ES);
+                        cnt_s[stage][w8] = c + (c & 1);
                     }
                     last_s[stage] = slab_done ? 1 : 0;
                 }
-                __threadfence_block();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&full_bar[stage]);
+                // ---- copy the window rows of the accepted particles into the slots (cp.async; they arrive on full_bar themselves)
+                for (int g0 = 0; g0 < ns; g0 += 32) {
+                    const int pos = g0 + lane;
+                    if (pos < ns) {
+                        const char* src = reinterpret_cast<const char*>(rows + (size_t)acc_rec[k][pos].x * R::RP);
+                        const uint32_t dst = sl32 + (uint32_t)(pos * PITCH) * ES;
+                        constexpr int CHX = (int)(R::RX * sizeof(T) / 16), CHY = (int)(R::RY * sizeof(T) / 16);
+#pragma unroll
+                        for (int c = 0; c < CHX; ++c) cp_async_16(dst + OXF * ES + 16 * c, src + 16 * c);
+#pragma unroll
+                        for (int c = 0; c < CHY; ++c) cp_async_16(dst + OYF * ES + 16 * c, src + R::OY * ES + 16 * c);
+#pragma unroll
+                        for (int c = 0; c < CHY; ++c) cp_async_16(dst + OZF * ES + 16 * c, src + R::OZ * ES + 16 * c);
+                    }
+                }
+                cp_async_mbar_arrive(&full_bar[k]);
+                ENUF_TR((s - s_begin) * 16 + 3, trace_clock());
+                ENUF_TR((s - s_begin) * 16 + 8, (long long)ns);
+                ENUF_TR((s - s_begin) * 16 + 14, trace_clock());
+                __syncwarp();                                       // lane 0's arrive (release) publishes every lane's list entries
+                if (lane == 0) mbar_arrive(&full_bar[k]);
+                ENUF_TR((s - s_begin) * 16 + 4, trace_clock());
             }
         }
         return;
@@ -324,55 +438,76 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     const int lxl = (lane & 3) * 2, lyl = lane >> 2;              // this lane's two cells (lxl, lyl), (lxl + 1, lyl) of the patch
     T* gout = grid + ((size_t)(Ty * CY + py0 + lyl)) * g.n + Tx * CX + px0 + lxl;
     const size_t plane = (size_t)g.n * g.n;
+    constexpr int NV = (WZ + 3) / 4;
 
     P2 acc[WZ];
 #pragma unroll
-    for (int k = 0; k < WZ; ++k) { acc[k].x = (T)0; acc[k].y = (T)0; }
+    for (int kk = 0; kk < WZ; ++kk) { acc[kk].x = (T)0; acc[kk].y = (T)0; }
 
-    unsigned pf = 0;                                              // phase bits of full_bar[0], full_bar[1]
+    // operands of one visit: this lane's (wx pair, wy) and the particle's q * z row
+    struct Ops { P2 wx; T wy; V4 z[NV]; };
+    auto load_ops = [&](uint32_t sbx, uint32_t sby, uint32_t sbz, uint2 e) {
+        Ops o;
+        o.wx = lds_pair<T>(sbx + (e.x & 0xffffu));
+        o.wy = lds_one<T>(sby + e.y);
+        const uint32_t za = sbz + (e.x >> 16);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) o.z[v] = lds_quad<T>(za + v * (uint32_t)sizeof(V4));
+        return o;
+    };
+
+    unsigned pf = 0;                                              // parity bits of the next phase of full_bar[0..3]
+    const uint32_t smem32 = smem_u32(smem_raw);
     for (int s = s_begin; s < s_end; ++s) {
-        const int stage = (s - s_begin) & 1;
-        const unsigned char* sbase = smem_raw + (size_t)stage * C::STAGE_BYTES;
-        const char* sbx = reinterpret_cast<const char*>(sbase) + lxl * ES;
-        const char* sby = reinterpret_cast<const char*>(sbase) + lyl * ES;
-        const char* sbz = reinterpret_cast<const char*>(sbase);
-        const uint4* lp = reinterpret_cast<const uint4*>(sbase + C::SLOT_BYTES) + warp * (LCAP / 2);
+        const int stage = (s - s_begin) % NSTAGE, prod = (s - s_begin) & 3;
+        const uint32_t sbz = smem32 + (uint32_t)(stage * C::STAGE_BYTES);
+        const uint32_t sbx = sbz + lxl * ES, sby = sbz + lyl * ES;
+        const uint32_t lp = sbz + (uint32_t)C::SLOT_BYTES + (uint32_t)(warp * LCAP * sizeof(uint2));
         int lastf;
         do {
-            mbar_wait(&full_bar[stage], (pf >> stage) & 1u);
-            pf ^= 1u << stage;
+            mbar_wait_backoff(&full_bar[prod], (pf >> prod) & 1u);
+            pf ^= 1u << prod;
             const int cnt = cnt_s[stage][warp];
             lastf = last_s[stage];
-            uint4 ee = lp[0];
+#ifdef ENUF_TRACE
+            if (warp == 0) { ENUF_TR((s - s_begin) * 16 + 5, trace_clock()); ENUF_TR((s - s_begin) * 16 + 9, (long long)cnt); }
+            if (warp == 5) { ENUF_TR((s - s_begin) * 16 + 10, trace_clock()); ENUF_TR((s - s_begin) * 16 + 12, (long long)cnt); }
+#endif
+            // one visit ahead: while visit i is accumulated, the operands of visit i + 1 and the entry of visit i + 2 are
+            // in flight.  Two visits per trip (A, B alternate, no register moves); the list is padded with entries that
+            // point at the all-zero slot: to an even length, and two more for the loads that run ahead.
+            Ops A = load_ops(sbx, sby, sbz, lds_u2(lp));
+            uint2 en = lds_u2(lp + 8);
             for (int i = 0; i < cnt; i += 2) {
-                const uint4 e = ee;
-                ee = lp[(i >> 1) + 1];                                   // next trip (the list has spare entries)
-                const P2 wx1 = *reinterpret_cast<const P2*>(sbx + (e.x & 0xffffu));
-                const T wy1 = *reinterpret_cast<const T*>(sby + e.y);
-                const P2 wx2 = *reinterpret_cast<const P2*>(sbx + (e.z & 0xffffu));
-                const T wy2 = *reinterpret_cast<const T*>(sby + e.w);
-                constexpr int NV = (WZ + 3) / 4;
-                V4 zv1[NV], zv2[NV];
+                const Ops B = load_ops(sbx, sby, sbz, en);
+                en = lds_u2(lp + 8 * (uint32_t)(i + 2));
+                {
+                    const P2 a = pair_scale(A.wx, A.wy);
+                    const T* wz = reinterpret_cast<const T*>(A.z);
 #pragma unroll
-                for (int v = 0; v < NV; ++v) zv1[v] = reinterpret_cast<const V4*>(sbz + (e.x >> 16))[v];
+                    for (int kk = 0; kk < WZ; ++kk) fma_pair(acc[kk], a, wz[kk]);
+                }
+                A = load_ops(sbx, sby, sbz, en);
+                en = lds_u2(lp + 8 * (uint32_t)(i + 3));
+                {
+                    const P2 a = pair_scale(B.wx, B.wy);
+                    const T* wz = reinterpret_cast<const T*>(B.z);
 #pragma unroll
-                for (int v = 0; v < NV; ++v) zv2[v] = reinterpret_cast<const V4*>(sbz + (e.z >> 16))[v];
-                const P2 a1 = pair_scale(wx1, wy1), a2 = pair_scale(wx2, wy2);
-                const T* wz1 = reinterpret_cast<const T*>(zv1);
-                const T* wz2 = reinterpret_cast<const T*>(zv2);
-#pragma unroll
-                for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a1, wz1[k]);
-#pragma unroll
-                for (int k = 0; k < WZ; ++k) fma_pair(acc[k], a2, wz2[k]);
+                    for (int kk = 0; kk < WZ; ++kk) fma_pair(acc[kk], a, wz[kk]);
+                }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_bar[stage]);
+            if (lane == 0) mbar_arrive(lastf ? &empty_bar[prod] : &again_bar[prod]);
+#ifdef ENUF_TRACE
+            if (warp == 0) ENUF_TR((s - s_begin) * 16 + 6, trace_clock());
+            if (warp == 5) ENUF_TR((s - s_begin) * 16 + 11, trace_clock());
+#endif
         } while (!lastf);
         // the lowest plane of the window (s - SHI) is complete: store it, slide
         const int zo = s - C::SHI;
         if (zo >= z0) *reinterpret_cast<P2*>(gout + (size_t)zo * plane) = acc[0];
 #pragma unroll
-        for (int k = 0; k + 1 < WZ; ++k) acc[k] = acc[k + 1];
+        for (int kk = 0; kk + 1 < WZ; ++kk) acc[kk] = acc[kk + 1];
         acc[WZ - 1].x = (T)0; acc[WZ - 1].y = (T)0;
     }
 }
