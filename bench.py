@@ -7,9 +7,10 @@
 A "step" is one pass of the whole hot path (bin, spread, FFT+scale+energy, inverse FFT,
 gather) over BASELINE.json config 5 (N = 1e6, n = 256, Kaiser-Bessel m = 6, fp32); every
 step sees positions displaced by a fresh random 0.05 per coordinate (the config's 100-step
-loop), so every step re-bins.  For N > 1 GPUs each rank runs an independent replica of
-the system (weak scaling, no data-path collective).  One JSON line
-is printed by rank 0.
+loop), so every step re-bins.  For N > 1 GPUs ONE system is sharded by particle over the ranks
+(HP-ENUF: every rank spreads and transforms its own particles, one all-reduce of the
+partial spectra, every rank finishes for its own particles; strong scaling; DESIGN.md section 9);
+`--parallel replicas` runs independent copies instead.  One JSON line is printed by rank 0.
 """
 from __future__ import annotations
 
@@ -40,10 +41,10 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--variant", default="analytic", choices=["analytic", "ik"])
-    ap.add_argument("--parallel", default="replicas", choices=["replicas", "sharded"],
-                    help="N > 1: independent replicas (weak scaling, no data-path collective; default) or ONE "
-                         "system sharded by particle with an all-reduce of the partial spectra (strong scaling; "
-                         "DESIGN.md section 9)")
+    ap.add_argument("--parallel", default=None, choices=["replicas", "sharded"],
+                    help="N > 1: ONE system sharded by particle with an all-reduce of the partial spectra (strong "
+                         "scaling; the default, DESIGN.md section 9) or independent replicas (weak scaling, no "
+                         "data-path collective)")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-comparisons", action="store_true",
@@ -217,8 +218,11 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "variant": args.variant, "N": int(w.N), "n": int(w.n),
-                   "m": int(w.m), "window": w.window, "sample": sample},
+        # what was timed: the sub-box, not the full workload (same density, cell size, alpha and window)
+        "config": {"workload": args.workload, "variant": args.variant, "N": int(q.shape[0]), "L": float(L), "n": int(n),
+                   "k_cut": int(kc), "m": int(w.m), "window": w.window, "same_config": scale == 1,
+                   "full_workload": {"N": int(w.N), "L": float(w.L), "n": int(w.n), "k_cut": int(w.k_cut)},
+                   "sample": sample},
         "evals_per_sec": 1.0 / t_step,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -277,7 +281,7 @@ def run_ours(args):
     w = make_workload(args.workload)
     K, W = args.steps, args.warmup
     tdtype = torch.float64 if w.dtype == "f64" else torch.float32
-    sharded = args.parallel == "sharded"
+    sharded = args.parallel == "sharded" or (args.parallel is None and world > 1)
     N_sys = w.N
     if sharded:
         # ONE system, the same on every rank; this rank owns the particles [lo, hi)
@@ -371,6 +375,37 @@ def run_ours(args):
     e2e = {"value": (N_sys if sharded else w.N * world) / t_e2e, "unit": UNIT, "ms_per_step": 1e3 * t_e2e, "steps": Ke,
            "h2d_bytes_per_step": int(N_loc * 4 * esz), "d2h_bytes_per_step": int(N_loc * 3 * esz + 8),
            "api": api}
+    if not sharded:
+        # the same call with q = NULL: the charges of the previous host call stay resident on the device
+        # (an MD loop moves positions, not charges); r in, F and E out every step
+        plan.set(enuf.OPT_CUDA_GRAPH, 1)
+        for s in range(3):
+            plan.energy_forces_host(pos_pinned[s], q_pinned if s == 0 else None, F=F_host)
+        torch.cuda.synchronize()
+        barrier()
+        t0 = time.perf_counter()
+        for s in range(Ke):
+            plan.energy_forces_host(pos_pinned[W + s], None, F=F_host)
+        torch.cuda.synchronize()
+        t_res = max_over_ranks((time.perf_counter() - t0) / Ke)
+        barrier()
+        plan.set(enuf.OPT_CUDA_GRAPH, 0)
+        e2e["q_resident"] = {"value": w.N * world / t_res, "unit": UNIT, "ms_per_step": 1e3 * t_res,
+                             "h2d_bytes_per_step": int(N_loc * 3 * esz), "d2h_bytes_per_step": int(N_loc * 3 * esz + 8)}
+    exchange = None
+    if sharded:
+        # the one exchange step of the sharded path, timed alone: all-reduce (sum) of the partial spectrum buffer
+        buf = plan.spectrum_tensor()
+        for _ in range(3):
+            enuf.all_reduce_sum_(buf)
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); barrier(); c0.record()
+        for _ in range(10):
+            enuf.all_reduce_sum_(buf)
+        c1.record(); torch.cuda.synchronize()
+        exchange = {"collective": "all_reduce(SUM) of the partial spectrum [z][ky'][kx] after the Y pass (NCCL)",
+                    "bytes_per_rank": int(buf.numel() * buf.element_size()),
+                    "ms": max_over_ranks(c0.elapsed_time(c1) / 10), "ranks": world}
 
     if rank != 0:
         plan.close()
@@ -468,6 +503,25 @@ def run_ours(args):
         cpu_baseline = {"value": w.N / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
                         "sample": f"1 full evaluation of {args.workload} (N={w.N}, forces on all particles), {dt:.1f} s",
                         "seconds": dt}
+        # single-thread leg on a bounded sample: the 1/4^3 sub-box (same density, cell size, alpha)
+        cores = O.num_threads()
+        sc = 4 if w.n // 4 >= 32 else (2 if w.n // 2 >= 32 else 1)
+        rs, qs, Ls, kcs, ns_ = sub_box_sample(w, sc)
+        O.set_threads(1)
+        dt1, _ = oracle_step(O, w, rs, qs, Ls, kcs, ns_, args.variant)
+        O.set_threads(cores)
+        dtm, _ = oracle_step(O, w, rs, qs, Ls, kcs, ns_, args.variant)
+        cpu_baseline["single_thread"] = {"value": qs.shape[0] / dt1, "unit": UNIT, "seconds": dt1,
+                                         "all_cores_same_sample": {"value": qs.shape[0] / dtm, "seconds": dtm, "cores": cores},
+                                         "sample": f"sub-box 1/{sc}^3 of the volume: N={qs.shape[0]}, n={ns_}, k_cut={kcs}"}
+        # Oracle A (direct Ewald sum, the definition) on configs 1-3, all cores
+        oa = {}
+        for name in ("cfg1", "cfg2", "cfg3"):
+            wa = make_workload(name)
+            t0 = time.perf_counter()
+            O.direct(wa.r, wa.q, wa.L, wa.alpha, wa.k_cut, slater_lambda=wa.slater_lambda)
+            oa[name] = {"seconds": time.perf_counter() - t0, "N": int(wa.N), "k_cut": int(wa.k_cut)}
+        cpu_baseline["oracle_a_direct_sum"] = oa
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -483,6 +537,7 @@ def run_ours(args):
         "energy_last_step": E_last,
         "clocks": clocks, "e2e": e2e, "gpu_launches": total_launches,
         "roofline": roofline, "stages": stages, "cpu_baseline": cpu_baseline, "comparisons": comparisons,
+        "exchange": exchange,
     }
     print(json.dumps(line), flush=True)
     plan.close()

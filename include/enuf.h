@@ -69,8 +69,8 @@ enum { ENUF_FORCE_ANALYTIC = 0, ENUF_FORCE_IK = 1 };
 
 /* stage indices of enuf_plan_stage_ms() */
 enum enuf_stage {
-    ENUF_STAGE_BIN = 0,     /* a1 */
-    ENUF_STAGE_SPREAD = 1,  /* a2 (includes clearing the grid) */
+    ENUF_STAGE_BIN = 0,     /* a1: histogram, scan, scatter, window rows of the sorted particles */
+    ENUF_STAGE_SPREAD = 1,  /* a2: every grid value is written exactly once (no clearing pass) */
     ENUF_STAGE_FFT = 2,     /* a3 + a4 + a5 */
     ENUF_STAGE_GATHER = 3,  /* a6 */
     ENUF_STAGE_ENERGY = 4,  /* a7 */
@@ -114,7 +114,10 @@ int enuf_plan_set_stream(enuf_plan *plan, void *cuda_stream);
 int enuf_energy_forces(enuf_plan *plan, const void *r, const void *q, void *F, double *E);
 
 /* Same, with HOST buffers: copies r, q to plan-owned device staging, evaluates, copies F
- * back, synchronises.  E may be NULL.  (The end-to-end path bench.py times.) */
+ * back, synchronises.  E may be NULL.  (The end-to-end path bench.py times.)
+ * q_host may be NULL: the charges of the previous host call on this plan stay resident on the
+ * device and are reused (an MD loop moves positions, not charges); ENUF_ESTATE if there was no
+ * previous host call, or the workspace was re-allocated since. */
 int enuf_energy_forces_host(enuf_plan *plan, const void *r_host, const void *q_host,
                             void *F_host, double *E);
 
@@ -189,7 +192,7 @@ int enuf_plan_stage_ms_mean(enuf_plan *plan, float *ms, int count, int *n_evals)
 int enuf_plan_launch_count(const enuf_plan *plan);
 
 /* Test / multi-GPU taps (valid after an evaluation; each synchronises the stream).
- *   enuf_plan_copy_grid: spread grid g (after a2) is NOT kept -- this returns the real-space
+ *   enuf_plan_copy_field: the spread grid g (after a2) is NOT kept -- this returns the real-space
  *     field Psi (analytic variant) or B_x (ik) that the gather read, n^3 values [z][y][x],
  *     to a HOST buffer of the plan's precision.
  *   enuf_plan_structure_factor: S~(n) for `count` modes (nx, ny, nz triples, each within

@@ -203,20 +203,24 @@ class Plan:
                                         self._dev(F, (N, 3), "F"), C.byref(E) if want_energy else None))
         return (E.value if want_energy else None), F
 
-    def energy_forces_host(self, r, q, F=None):
-        """One evaluation on HOST tensors / numpy arrays (H2D and D2H inside the call)."""
+    def energy_forces_host(self, r, q=None, F=None):
+        """One evaluation on HOST tensors / numpy arrays (H2D and D2H inside the call).  q=None reuses the
+        charges of the previous host call, which stay resident on the device."""
         torch = self._torch
         N = self.N
         r_t = r if isinstance(r, torch.Tensor) else torch.from_numpy(r)
-        q_t = q if isinstance(q, torch.Tensor) else torch.from_numpy(q)
+        q_t = None if q is None else (q if isinstance(q, torch.Tensor) else torch.from_numpy(q))
         if F is None:
             F = torch.empty((N, 3), dtype=self.dtype)
         for t, shape, name in ((r_t, (N, 3), "r"), (q_t, (N,), "q"), (F, (N, 3), "F")):
+            if t is None:
+                continue
             if t.is_cuda or t.dtype != self.dtype or tuple(t.shape) != shape or not t.is_contiguous():
                 raise ValueError(f"{name} must be a contiguous host {self.dtype} tensor of shape {shape}")
         self._use_current_stream()
         E = C.c_double(0.0)
-        _check(lib().enuf_energy_forces_host(self._h, C.c_void_p(r_t.data_ptr()), C.c_void_p(q_t.data_ptr()),
+        _check(lib().enuf_energy_forces_host(self._h, C.c_void_p(r_t.data_ptr()),
+                                             C.c_void_p(q_t.data_ptr()) if q_t is not None else None,
                                              C.c_void_p(F.data_ptr()), C.byref(E)))
         return E.value, F
 

@@ -22,6 +22,14 @@ int fail(int code, const char* fmt, ...) {
     return code;
 }
 
+int fail_cuda(cudaError_t e, const char* what);
+// a launch_* helper returned -1: its CUDA error was stored in the plan (launch_ok, enuf_launch.cuh)
+int fail_launch(enuf_plan* p) {
+    const cudaError_t e = p->launch_error != cudaSuccess ? p->launch_error : cudaErrorUnknown;
+    p->launch_error = cudaSuccess;
+    return fail_cuda(e, "kernel launch");
+}
+
 int fail_cuda(cudaError_t e, const char* what) {
     snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
     (void)cudaGetLastError();
@@ -226,6 +234,8 @@ void free_workspace(enuf_plan* p) {
     p->fft_done = nullptr;
     p->events_valid = false;
     p->partial_ready = false;
+    p->evaluated = false;          // e_dev, grid, spectrum are gone
+    p->q_stage_valid = false;
     p->bin_count_clean = false;
     p->real_count_clean = false;
     p->allocated = false;
@@ -417,7 +427,8 @@ int evaluate_device(enuf_plan* p, const void* r, const void* q, void* F, double*
         if (ce != cudaSuccess || rc || !graph) {
             if (graph) cudaGraphDestroy(graph);
             drop_graph(p);
-            return fail_cuda(ce != cudaSuccess ? ce : cudaGetLastError(), "CUDA graph capture");
+            return fail_cuda(ce != cudaSuccess ? ce : (p->launch_error != cudaSuccess ? p->launch_error : cudaErrorUnknown),
+                             "CUDA graph capture");
         }
         ce = cudaGraphInstantiate(&p->gexec, graph, 0);
         cudaGraphDestroy(graph);
@@ -427,7 +438,7 @@ int evaluate_device(enuf_plan* p, const void* r, const void* q, void* F, double*
     } else {
         if (p->use_graph) { drop_graph(p); p->g_r = r; p->g_q = q; p->g_F = F; p->g_N = p->N; }
         int rc = p->precision == ENUF_F32 ? run_all<float>(p, r, q, F) : run_all<double>(p, r, q, F);
-        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+        if (rc) return fail_launch(p);
     }
     p->evaluated = true;
     if (E) {
@@ -479,6 +490,7 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
     g_err[0] = 0;
     if (!p) return fail(ENUF_EINVAL, "plan is NULL");
     drop_graph(p);                 // whatever changes, a captured evaluation no longer describes the plan
+    p->partial_ready = false;      // ... nor does a partial spectrum: enuf_forces_from_spectrum needs a fresh first half
     const int iv = (int)value;
     switch (key) {
         case ENUF_OPT_PRECISION:
@@ -545,19 +557,30 @@ int enuf_energy_forces(enuf_plan* p, const void* r, const void* q, void* F, doub
 int enuf_energy_forces_host(enuf_plan* p, const void* r_host, const void* q_host, void* F_host, double* E) {
     g_err[0] = 0;
     if (!p) return fail(ENUF_EINVAL, "plan is NULL");
-    if (p->N > 0 && (!r_host || !q_host || !F_host)) return fail(ENUF_EINVAL, "r, q and F must be non-NULL when N > 0");
+    if (p->N > 0 && (!r_host || !F_host)) return fail(ENUF_EINVAL, "r and F must be non-NULL when N > 0");
     int rc = prepare(p);
     if (rc) return rc;
+    if (p->N > 0 && !q_host && !p->q_stage_valid)
+        return fail(ENUF_ESTATE, "q_host = NULL reuses the charges of the previous host call: there is none");
     const size_t es = p->esize, cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1);
     if (!p->r_stage) {
-        if ((rc = dev_alloc(p, &p->r_stage, 3 * es * cap))) return rc;
-        if ((rc = dev_alloc(p, &p->q_stage, es * cap))) return rc;
-        if ((rc = dev_alloc(p, &p->F_stage, 3 * es * cap))) return rc;
+        // the three staging buffers are allocated as a group: all or none
+        if ((rc = dev_alloc(p, &p->r_stage, 3 * es * cap)) || (rc = dev_alloc(p, &p->q_stage, es * cap)) ||
+            (rc = dev_alloc(p, &p->F_stage, 3 * es * cap))) {
+            if (p->r_stage) cudaFree(p->r_stage);
+            if (p->q_stage) cudaFree(p->q_stage);
+            if (p->F_stage) cudaFree(p->F_stage);
+            p->r_stage = p->q_stage = p->F_stage = nullptr;
+            return rc;
+        }
     }
     const size_t N = (size_t)p->N;
     if (N > 0) {
         CU(cudaMemcpyAsync(p->r_stage, r_host, 3 * es * N, cudaMemcpyHostToDevice, p->stream));
-        CU(cudaMemcpyAsync(p->q_stage, q_host, es * N, cudaMemcpyHostToDevice, p->stream));
+        if (q_host) {
+            CU(cudaMemcpyAsync(p->q_stage, q_host, es * N, cudaMemcpyHostToDevice, p->stream));
+            p->q_stage_valid = true;
+        }
     }
     rc = evaluate_device(p, p->r_stage, p->q_stage, p->F_stage, nullptr);
     if (rc) return rc;
@@ -586,7 +609,7 @@ int enuf_spectrum_partial(enuf_plan* p, const void* r, const void* q, void* F) {
         if (p->profile) for (int i = 0; i <= 2; ++i) cudaEventRecord(p->ev[i], p->stream);
     } else {
         rc = p->precision == ENUF_F32 ? run_partial<float>(p, r, q, F) : run_partial<double>(p, r, q, F);
-        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+        if (rc) return fail_launch(p);
     }
     p->partial_ready = true;
     return ENUF_OK;
@@ -605,8 +628,8 @@ int enuf_plan_spectrum_buffer(enuf_plan* p, void** dev_ptr, size_t* count) {
 int enuf_forces_from_spectrum(enuf_plan* p, void* F, double* E) {
     g_err[0] = 0;
     if (!p) return fail(ENUF_EINVAL, "plan is NULL");
-    if (!p->allocated || !p->partial_ready)
-        return fail(ENUF_ESTATE, "enuf_forces_from_spectrum needs a preceding enuf_spectrum_partial");
+    if (!p->allocated || p->tables_dirty || !p->partial_ready)
+        return fail(ENUF_ESTATE, "enuf_forces_from_spectrum needs a preceding enuf_spectrum_partial (and no enuf_plan_set since)");
     if (p->N > 0 && !F) return fail(ENUF_EINVAL, "F must be non-NULL when N > 0");
     p->partial_ready = false;
     const int before = p->launches;
@@ -614,12 +637,12 @@ int enuf_forces_from_spectrum(enuf_plan* p, void* F, double* E) {
     if (p->N == 0) {
         // no particles to interpolate onto, but the energy of the summed spectrum is still produced
         rc = p->precision == ENUF_F32 ? enuf::launch_fft_backward<float>(p) : enuf::launch_fft_backward<double>(p);
-        if (rc < 0) return fail_cuda(cudaGetLastError(), "kernel launch");
+        if (rc < 0) return fail_launch(p);
         p->launches = before + rc;
         if (p->profile) for (int i = 3; i <= ENUF_NUM_STAGES; ++i) cudaEventRecord(p->ev[i], p->stream);
     } else {
         rc = p->precision == ENUF_F32 ? run_finish<float>(p, F) : run_finish<double>(p, F);
-        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+        if (rc) return fail_launch(p);
     }
     p->evaluated = true;
     if (E) {
@@ -678,24 +701,41 @@ int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, in
     const int ncells = ncd * ncd * ncd;
     const size_t cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1), es = p->esize;
     if (!p->real_pos) {
-        if ((rc = dev_alloc(p, &p->real_pos, 4 * es * cap))) return rc;
-        if ((rc = dev_alloc(p, (void**)&p->real_idx, 4 * cap))) return rc;
-        if ((rc = dev_alloc(p, (void**)&p->real_partial, 16 * ((cap + 127) / 128)))) return rc;
-        if ((rc = dev_alloc(p, (void**)&p->real_e_dev, 16))) return rc;
-        if (cudaMallocHost((void**)&p->real_e_pinned, 16) != cudaSuccess) {
+        // allocated as a group: all or none
+        rc = dev_alloc(p, &p->real_pos, 4 * es * cap);
+        if (!rc) rc = dev_alloc(p, (void**)&p->real_idx, 4 * cap);
+        if (!rc) rc = dev_alloc(p, (void**)&p->real_partial, 16 * ((cap + 127) / 128));
+        if (!rc) rc = dev_alloc(p, (void**)&p->real_e_dev, 16);
+        if (!rc && cudaMallocHost((void**)&p->real_e_pinned, 16) != cudaSuccess) {
             (void)cudaGetLastError();
-            return fail(ENUF_ENOMEM, "cudaMallocHost failed");
+            p->real_e_pinned = nullptr;
+            rc = fail(ENUF_ENOMEM, "cudaMallocHost failed");
+        }
+        if (rc) {
+            if (p->real_pos) cudaFree(p->real_pos);
+            if (p->real_idx) cudaFree(p->real_idx);
+            if (p->real_partial) cudaFree(p->real_partial);
+            if (p->real_e_dev) cudaFree(p->real_e_dev);
+            p->real_pos = nullptr; p->real_idx = nullptr; p->real_partial = nullptr; p->real_e_dev = nullptr;
+            return rc;
         }
     }
     if (ncells > p->real_ncells_cap) {
         CU(cudaStreamSynchronize(p->stream));
-        if (p->real_count) { cudaFree(p->real_count); cudaFree(p->real_offset); cudaFree(p->real_cursor); cudaFree(p->real_scan_total); }
-        p->real_count = p->real_offset = p->real_cursor = p->real_scan_total = nullptr;
-        p->real_ncells_cap = 0;
-        if ((rc = dev_alloc(p, (void**)&p->real_count, 4 * (size_t)ncells))) return rc;
-        if ((rc = dev_alloc(p, (void**)&p->real_offset, 4 * ((size_t)ncells + 1)))) return rc;
-        if ((rc = dev_alloc(p, (void**)&p->real_cursor, 4 * (size_t)ncells))) return rc;
-        if ((rc = dev_alloc(p, (void**)&p->real_scan_total, 4 * (((size_t)ncells + 1023) / 1024)))) return rc;
+        auto drop_cells = [&]() {
+            if (p->real_count) cudaFree(p->real_count);
+            if (p->real_offset) cudaFree(p->real_offset);
+            if (p->real_cursor) cudaFree(p->real_cursor);
+            if (p->real_scan_total) cudaFree(p->real_scan_total);
+            p->real_count = p->real_offset = p->real_cursor = p->real_scan_total = nullptr;
+            p->real_ncells_cap = 0;
+        };
+        drop_cells();
+        rc = dev_alloc(p, (void**)&p->real_count, 4 * (size_t)ncells);
+        if (!rc) rc = dev_alloc(p, (void**)&p->real_offset, 4 * ((size_t)ncells + 1));
+        if (!rc) rc = dev_alloc(p, (void**)&p->real_cursor, 4 * (size_t)ncells);
+        if (!rc) rc = dev_alloc(p, (void**)&p->real_scan_total, 4 * (((size_t)ncells + 1023) / 1024));
+        if (rc) { drop_cells(); return rc; }
         p->real_ncells_cap = ncells;
         p->real_count_clean = false;
     }
@@ -710,7 +750,7 @@ int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, in
     } else {
         const int l = p->precision == ENUF_F32 ? enuf::launch_real<float>(p, r, q, r_cut, accumulate, F)
                                                : enuf::launch_real<double>(p, r, q, r_cut, accumulate, F);
-        if (l < 0) return fail_cuda(cudaGetLastError(), "kernel launch");
+        if (l < 0) return fail_launch(p);
         p->launches = l;
     }
     if (E_real || E_self) {
@@ -725,7 +765,7 @@ int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, in
 int enuf_plan_energy(enuf_plan* p, double* E) {
     g_err[0] = 0;
     if (!p || !E) return fail(ENUF_EINVAL, "plan or E is NULL");
-    if (!p->evaluated) return fail(ENUF_ESTATE, "no evaluation has been run");
+    if (!p->evaluated || !p->allocated || !p->e_dev) return fail(ENUF_ESTATE, "no evaluation has been run");
     CU(cudaMemcpyAsync(p->e_pinned, p->e_dev, 8, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));
     *E = *p->e_pinned;
@@ -824,7 +864,7 @@ int enuf_spread_only(enuf_plan* p, const void* r, const void* q, void* grid_host
         if ((size_t)p->N * 3 * p->esize > 2 * p->esize * n * n * p->Kxp)
             return fail(ENUF_EINVAL, "enuf_spread_only: N too large for the scratch buffer");
         rc = p->precision == ENUF_F32 ? run_bin_spread<float>(p, r, q, scratch) : run_bin_spread<double>(p, r, q, scratch);
-        if (rc) return fail_cuda(cudaGetLastError(), "kernel launch");
+        if (rc) return fail_launch(p);
     }
     CU(cudaMemcpyAsync(grid_host, p->grid[0], bytes, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));

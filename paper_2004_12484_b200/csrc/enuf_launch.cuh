@@ -57,6 +57,14 @@ static inline PolyArg<M_> make_poly_arg(const enuf_plan* p) {
     return a;
 }
 
+// After a group of launches: the CUDA error, if any, is taken out of the runtime (cudaGetLastError clears it) and
+// kept in the plan, where the C-ABI entry point finds it for enuf_last_error().
+static inline bool launch_ok(enuf_plan* p) {
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) p->launch_error = e;
+    return e == cudaSuccess;
+}
+
 template <typename K>
 static inline bool set_smem(K kernel, size_t bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
@@ -148,7 +156,7 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
             static_cast<const PSlot<T>*>(p->rec), p->bin_offset, nbins, p->wp, pa, static_cast<T*>(p->rows));
         return 0;
     });
-    if (rc || cudaGetLastError() != cudaSuccess) return -1;
+    if (rc || !launch_ok(p)) return -1;
     ++nlaunch;
     p->bin_count_clean = true;
     return nlaunch;
@@ -177,7 +185,7 @@ int launch_spread(enuf_plan* p) {
         });
     });
     if (rc) return -1;
-    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+    return launch_ok(p) ? 1 : -1;
 }
 
 // Forward half of the FFT stage (a3): X real-to-complex and Y passes; leaves the partial spectrum
@@ -208,7 +216,7 @@ int launch_fft_forward(enuf_plan* p) {
         return 2;
     });
     if (launches < 0) return -1;
-    return cudaGetLastError() == cudaSuccess ? launches : -1;
+    return launch_ok(p) ? launches : -1;
 }
 
 // Backward half (a4 + a5 + a7): Z forward . scale . energy . Z inverse on A2[0] (in place; the ik
@@ -257,7 +265,7 @@ int launch_fft_backward(enuf_plan* p) {
         return launches;
     });
     if (launches < 0) return -1;
-    return cudaGetLastError() == cudaSuccess ? launches : -1;
+    return launch_ok(p) ? launches : -1;
 }
 
 template <typename T>
@@ -300,7 +308,7 @@ int launch_gather(enuf_plan* p, void* F) {
         return run(IntC<0>{});
     });
     if (launches < 0) return -1;
-    return cudaGetLastError() == cudaSuccess ? launches : -1;
+    return launch_ok(p) ? launches : -1;
 }
 
 template <typename T>
@@ -336,7 +344,7 @@ int launch_real(enuf_plan* p, const void* r, const void* q, double r_cut, int ac
             ef, accumulate, static_cast<T*>(F), p->real_partial);
     real_energy_finish_kernel<<<1, 256, 0, s>>>(p->real_partial, (int)fblocks, 0.5,
                                                p->alpha * 0.56418958354775628694807945156077, p->real_e_dev);
-    if (cudaGetLastError() != cudaSuccess) return -1;
+    if (!launch_ok(p)) return -1;
     p->real_count_clean = true;      // the scan cleared the cell histogram (all real_ncells_cap entries beyond ncells stay 0)
     return 6;
 }

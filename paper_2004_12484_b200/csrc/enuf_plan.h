@@ -35,6 +35,8 @@ struct enuf_plan {
     size_t esize = 4;              // bytes per real
     size_t workspace_bytes = 0;
     int launches = 0;
+    cudaError_t launch_error = cudaSuccess;   // error of the last failed kernel launch (launch_ok, enuf_launch.cuh)
+    bool q_stage_valid = false;    // the host-API staging buffer holds the charges of the previous host call
     int num_sms = 148;             // multiProcessorCount of the current device (persistent FFT grids)
     // device workspace
     void* rec = nullptr;           // PSlot<T>[N_cap]: record, packed cell, caller index (bin order)
@@ -92,8 +94,8 @@ struct enuf_plan {
 namespace enuf {
 
 // Implemented once per precision in enuf_kernels_f32.cu / enuf_kernels_f64.cu.
-// Each returns the number of kernel launches it issued, or -1 with the CUDA error left
-// in cudaGetLastError().
+// Each returns the number of kernel launches it issued, or -1 with the CUDA error stored
+// in plan->launch_error.
 template <typename T> int launch_bin(enuf_plan* p, const void* r, const void* q, void* F);
 template <typename T> int launch_spread(enuf_plan* p);
 template <typename T> int launch_fft(enuf_plan* p);            // = forward + backward

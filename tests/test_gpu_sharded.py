@@ -4,12 +4,16 @@ HP-ENUF: every rank spreads and forward-transforms its own pa
 spectra are summed over ranks (Eq. 61, :533-540), and every rank finishes (scale, energy, inverse
 transform, gather onto its own particles).  Here the "ranks" are plans on the same device and the sum
 is a tensor add of the plans' spectrum buffers, so the arithmetic of the N-GPU path is exercised
-exactly; the NCCL collective itself is covered with a one-rank process group, and the host logic
-with two gloo ranks in tests/test_multirank_gloo.py.
+exactly.  The collective is exercised by the two-rank tests at the end: two processes, one plan and one
+shard each, Plan.energy_forces_sharded through torch.distributed -- over gloo with both ranks on cuda:0
+(runs on a one-GPU box) and over NCCL when the box has two GPUs (skipped otherwise).  The one-rank NCCL
+test only checks the call sequence (with one rank all_reduce_sum_ returns before the collective).
 """
 import math
 import os
 import socket
+import subprocess
+import sys
 
 import numpy as np
 import pytest
@@ -146,3 +150,41 @@ def test_finish_without_partial_is_a_state_error(enuf, torch_cuda):
     with pytest.raises(enuf.EnufError):
         plan.forces_from_spectrum(F)      # a full evaluation does not arm the second half either
     plan.close()
+
+
+# ------------------------------------------------------------------ two ranks, a real collective
+
+def _two_ranks(backend, case, tmp_path, oracle, tol_f, tol_e):
+    """Spawn two ranks (tests/sharded_worker.py), each evaluating its half through Plan.energy_forces_sharded;
+    both must report the same E, and the concatenated forces must match Oracle B on the whole system."""
+    from sharded_worker import case_inputs
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]
+    worker = os.path.join(os.path.dirname(os.path.abspath(__file__)), "sharded_worker.py")
+    procs = [subprocess.Popen([sys.executable, worker, str(rk), "2", backend, str(port), case, str(tmp_path)],
+                              stdout=subprocess.PIPE, stderr=subprocess.STDOUT) for rk in range(2)]
+    outs = [p.communicate(timeout=600)[0].decode(errors="replace") for p in procs]
+    assert all(p.returncode == 0 for p in procs), "\n".join(outs)
+    r, q, pk = case_inputs(case)
+    ref = oracle.enuf(r, q, pk["L"], pk["alpha"], pk["k_cut"], int(round(pk["sigma"] * pk["M"])), pk["m"], pk["window"],
+                      pk["sigma"])
+    parts = [np.load(os.path.join(str(tmp_path), f"rank{rk}.npz")) for rk in range(2)]
+    assert float(parts[0]["E"]) == float(parts[1]["E"])                   # identical on both ranks
+    assert abs(float(parts[0]["E"]) - ref["E"]) <= tol_e * abs(ref["E"])
+    assert int(parts[0]["hi"]) == int(parts[1]["lo"])
+    F = np.concatenate([parts[0]["F"], parts[1]["F"]], axis=0)
+    assert rel_rms(F, ref["F"]) <= tol_f
+
+
+@pytest.mark.parametrize("case,tol_f,tol_e", [("cfg1", 1e-11, 1e-12), ("gas20k", 2e-6, 1e-6)])
+def test_two_ranks_gloo_one_gpu(torch_cuda, oracle, tmp_path, case, tol_f, tol_e):
+    """Two processes on the same GPU, all-reduce of the partial spectra over gloo (CUDA tensors)."""
+    _two_ranks("gloo", case, tmp_path, oracle, tol_f, tol_e)
+
+
+@pytest.mark.parametrize("case,tol_f,tol_e", [("cfg1", 1e-11, 1e-12), ("gas20k", 2e-6, 1e-6)])
+def test_two_ranks_nccl(torch_cuda, oracle, tmp_path, case, tol_f, tol_e):
+    """Two GPUs, the all-reduce over NCCL: the path `bench.py --gpus 2` measures."""
+    if torch_cuda.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    _two_ranks("nccl", case, tmp_path, oracle, tol_f, tol_e)
