@@ -51,9 +51,14 @@ struct GatherCfg {
     static constexpr int CELLS = ((TP * SPL + 3) / 4) * 4;      // shared tile size in elements (16 B multiple)
     static constexpr int WARPS = 12;
     static constexpr int NT = WARPS * 32;
-    static constexpr int PBW = 5;                               // particles per warp batch (15 lanes compute weights)
+    // kPairWarp (trimmed stencils of 4 k points, i.e. fp32 Kaiser-Bessel m = 6): a warp contracts TWO particles at a
+    // time, 16 lanes each; a lane owns the (WE/4)^2 rows (y, z) = (ya + 4 i, zb + 4 j) of the stencil and keeps their
+    // y and z weights in registers
+    static constexpr bool kPairWarp = kPair && WE % 4 == 0;
+    static constexpr int PBW = kPairWarp ? 4 : 5;               // particles per warp batch (3 lanes per particle compute weights); shared memory: 2 CTAs per SM
     static constexpr int ITER = (WE * WE + 31) / 32;            // stencil rows per lane
-    static constexpr int WP = 14;                               // pitch of a (phi, phi') weight row: >= W + 1, 16-byte aligned
+    static constexpr int WP = kPairWarp ? WE : 14;              // pitch of a (phi, phi') weight row: >= WE, 16-byte aligned
+    static constexpr int PERM = 64;                             // kPairWarp: particles a warp sorts by row parity at a time
 };
 
 template <typename T, int M_, bool kTrim = false>
@@ -61,7 +66,7 @@ constexpr size_t gather_smem_bytes() {
     using C = GatherCfg<M_, kTrim>;
     // tile + per warp and batch particle: (phi, phi') pairs [3][WP], pre*q, tile offset, caller index
     return sizeof(T) * ((size_t)C::CELLS + (size_t)C::WARPS * C::PBW * (3 * C::WP * 2 + 1))
-           + sizeof(int) * 2 * C::WARPS * C::PBW;
+           + sizeof(int) * 2 * C::WARPS * C::PBW + (C::kPairWarp ? sizeof(uint32_t) * C::WARPS * C::PERM : 0);
 }
 
 __device__ __forceinline__ void cp_async_4(void* smem_dst, const void* gmem_src) {
@@ -176,6 +181,173 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
                 }
             }
         }
+    }
+
+    if constexpr (C::kPairWarp && sizeof(T) == 4) {
+        // ================================================= two particles per warp (header of GatherCfg)
+        constexpr int NR = WE / 4;                               // rows per lane and direction
+        uint32_t* perm = reinterpret_cast<uint32_t*>(idx_all + C::WARPS * PBW) + warp * C::PERM;
+        P2* wtab = wtab_all + warp * PBW * 3 * WP;
+        T* q_s = q_all + warp * PBW;
+        int* base_s = base_all + warp * PBW;
+        int* idx_s = idx_all + warp * PBW;
+        const int half = lane >> 4, l16 = lane & 15, ya = l16 & 3, zb = l16 >> 2;
+        const int rowbase = zb * SPL + ya * SX;                  // row (i, j) of the lane: + 4 i SX + 4 j SPL
+        const unsigned below = (1u << lane) - 1u;
+        const int share = cnt / C::WARPS, extra = cnt - share * C::WARPS;
+        const int wbeg = warp * share + min(warp, extra), wend = wbeg + share + (warp < extra ? 1 : 0);
+        bool tile_ready = false;
+        for (int c0 = wbeg; c0 < wend; c0 += C::PERM) {
+            const int n = min(C::PERM, wend - c0);
+            // ---- particles whose stencil rows start on an even tile column first, the odd ones after: the two
+            //      particles of a pair then take the same (aligned / unaligned) row-load path, except one pair per chunk
+            {
+                uint32_t gi[2]; bool ev[2], od[2];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int pl = 32 * h + lane;
+                    gi[h] = 0; ev[h] = od[h] = false;
+                    if (pl < n) {
+                        gi[h] = slot_of(c0 + pl);
+                        const uint32_t cw = slots[gi[h]].cell;
+                        const bool odd = (((cw & 1023u) + ((cw >> 30) & 1u) + (unsigned)(C::XS - M_)) & 1u) != 0u;
+                        ev[h] = !odd; od[h] = odd;
+                    }
+                }
+                const unsigned e0 = __ballot_sync(0xffffffffu, ev[0]), e1 = __ballot_sync(0xffffffffu, ev[1]);
+                const unsigned o0 = __ballot_sync(0xffffffffu, od[0]), o1 = __ballot_sync(0xffffffffu, od[1]);
+                const int ne = __popc(e0) + __popc(e1);
+                __syncwarp();
+                if (ev[0]) perm[__popc(e0 & below)] = gi[0];
+                if (ev[1]) perm[__popc(e0) + __popc(e1 & below)] = gi[1];
+                if (od[0]) perm[ne + __popc(o0 & below)] = gi[0];
+                if (od[1]) perm[ne + __popc(o0) + __popc(o1 & below)] = gi[1];
+                __syncwarp();
+            }
+            for (int b0 = 0; b0 < n; b0 += PBW) {
+                const int nb = min(PBW, n - b0);
+                // ---- window values of the batch: one lane per (dimension, particle)
+                if (lane < 3 * nb) {
+                    const int dim = lane / nb, slot = lane - dim * nb;
+                    const uint32_t gi = perm[b0 + slot];
+                    const PSlot<T> sl = slots[gi];
+                    const PRec<T> pr = sl.rec;
+                    const T d0 = dim == 0 ? pr.dx : (dim == 1 ? pr.dy : pr.dz);
+                    T w[W], dw[W];
+                    stencil_weights<T, M_, !kIk, true>(wp, pa, d0, w, dw);   // packed Horner chains
+                    P2* row = wtab + (slot * 3 + dim) * WP;
+                    const bool sh = d0 > (T)0;                  // ks = 1: the k = 0 point is the zero one
+#pragma unroll
+                    for (int k = 0; k < WE; k += 2) {
+                        typename Vec4<T>::type v4;
+                        v4.x = sh ? w[k + 1] : w[k];      v4.y = sh ? dw[k + 1] : dw[k];
+                        v4.z = sh ? w[k + 2] : w[k + 1];  v4.w = sh ? dw[k + 2] : dw[k + 1];
+                        reinterpret_cast<typename Vec4<T>::type*>(row)[k / 2] = v4;
+                    }
+                    if (dim == 0) {
+                        int cx, cy, cz;
+                        unpack_cell(sl.cell, cx, cy, cz);
+                        int zrel = cz - tz0;              // trimmed bins: c_z may be the first plane of the next tile
+                        zrel += zrel < 0 ? g.n : 0;
+                        cx += pr.dx > (T)0 ? 1 : 0; cy += pr.dy > (T)0 ? 1 : 0; zrel += pr.dz > (T)0 ? 1 : 0;
+                        base_s[slot] = zrel * SPL + (cy - ty0) * SX + (cx - tx0) + (C::XS - M_);
+                        q_s[slot] = pre * pr.q;
+                        idx_s[slot] = (int)sl.idx;
+                    }
+                }
+                if (!tile_ready) {                   // the first batch's weights overlapped the tile copy
+                    cp_async_wait_all();
+                    __syncthreads();
+                    tile_ready = true;
+                } else {
+                    __syncwarp();
+                }
+                // ---- pairs: half-warp h contracts particle pr + h
+                for (int pr2 = 0; pr2 < nb; pr2 += 2) {
+                    const bool act = pr2 + half < nb;
+                    const int slot = act ? pr2 + half : pr2;     // an idle half repeats its neighbour's particle, result dropped
+                    const P2* wt = wtab + slot * 3 * WP;
+                    P2 wx[WE], wy[NR], wz[NR];
+                    {
+                        using V4 = typename Vec4<T>::type;
+                        const V4* w4 = reinterpret_cast<const V4*>(wt);
+#pragma unroll
+                        for (int v = 0; v < WE / 2; ++v) {
+                            const V4 t4 = w4[v];
+                            wx[2 * v].x = t4.x; wx[2 * v].y = t4.y; wx[2 * v + 1].x = t4.z; wx[2 * v + 1].y = t4.w;
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < NR; ++i) { wy[i] = wt[WP + ya + 4 * i]; wz[i] = wt[2 * WP + zb + 4 * i]; }
+                    const int base = base_s[slot];
+                    const T* origin = tile_s + base + rowbase;
+                    T fx = (T)0, fy = (T)0, fz = (T)0;
+                    auto finish_row = [&](int i, int j, const T (&v)[WE]) {
+                        P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
+#pragma unroll
+                        for (int k = 0; k < WE; ++k) {
+                            if (k & 1) fma_pair(sb2, wx[k], v[k]);
+                            else fma_pair(sa, wx[k], v[k]);
+                        }
+                        const P2 s2 = pair_add(sa, sb2);                   // (sum Psi phi_x, sum Psi phi_x')
+                        if (kIk) {
+                            fx += s2.x * (wy[i].x * wz[j].x);
+                        } else {
+                            const P2 yz = pair_scale(wy[i], wz[j].x);      // (phi_y phi_z, phi_y' phi_z)
+                            fx += s2.y * yz.x;
+                            fy += s2.x * yz.y;
+                            fz += s2.x * (wy[i].x * wz[j].y);
+                        }
+                    };
+                    if ((base & 1) == 0) {
+#pragma unroll
+                        for (int j = 0; j < NR; ++j)
+#pragma unroll
+                            for (int i = 0; i < NR; ++i) {
+                                const P2* row = reinterpret_cast<const P2*>(origin + 4 * i * SX + 4 * j * SPL);
+                                T v[WE];
+#pragma unroll
+                                for (int k = 0; k < WE / 2; ++k) { const P2 t2 = row[k]; v[2 * k] = t2.x; v[2 * k + 1] = t2.y; }
+                                finish_row(i, j, v);
+                            }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < NR; ++j)
+#pragma unroll
+                            for (int i = 0; i < NR; ++i) {
+                                const T* rowf = origin + 4 * i * SX + 4 * j * SPL;
+                                const P2* row = reinterpret_cast<const P2*>(rowf + 1);
+                                T v[WE];
+                                v[0] = rowf[0];
+#pragma unroll
+                                for (int k = 0; k < WE / 2 - 1; ++k) { const P2 t2 = row[k]; v[2 * k + 1] = t2.x; v[2 * k + 2] = t2.y; }
+                                v[WE - 1] = rowf[WE - 1];
+                                finish_row(i, j, v);
+                            }
+                    }
+                    const size_t jp = (size_t)(uint32_t)idx_s[slot];
+                    const T sc = q_s[slot];
+                    if (kIk) {
+#pragma unroll
+                        for (int o = 8; o > 0; o >>= 1) fx += __shfl_xor_sync(0xffffffffu, fx, o);
+                        if (act && l16 == 0) F[3 * jp + component] = sc * fx;
+                    } else {
+                        // the three sums over the 16 lanes of the half by recursive halving (5 shuffles); the totals of
+                        // x, y, z end in the lanes l16 = 0, 4, 8
+                        const bool b3 = (l16 & 8) != 0, b2 = (l16 & 4) != 0;
+                        const T k0 = (b3 ? fz : fx) + __shfl_xor_sync(0xffffffffu, b3 ? fx : fz, 8);
+                        const T k1 = (b3 ? (T)0 : fy) + __shfl_xor_sync(0xffffffffu, b3 ? fy : (T)0, 8);
+                        T kk = (b2 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, b2 ? k0 : k1, 4);
+                        kk += __shfl_xor_sync(0xffffffffu, kk, 2);
+                        kk += __shfl_xor_sync(0xffffffffu, kk, 1);
+                        if (act && (l16 & 3) == 0 && l16 < 12) F[3 * jp + (l16 >> 2)] = sc * kk;
+                    }
+                }
+                __syncwarp();                        // the batch's weight rows are rewritten next
+            }
+        }
+        if (!tile_ready) { cp_async_wait_all(); __syncthreads(); }   // (a warp without particles still joins the barrier)
+        return;
     }
 
     // stencil rows owned by this lane: rr = lane + 32 it -> (rz, ry)
