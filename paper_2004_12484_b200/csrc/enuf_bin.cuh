@@ -9,7 +9,7 @@
 #pragma once
 
 #include "enuf_common.cuh"
-#include "enuf_spread.cuh"   // write_window_rows
+#include "enuf_spread.cuh"   // WindowRows, write_window_row
 
 namespace enuf {
 
@@ -229,38 +229,37 @@ bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, 
 
 // The window rows of the sorted particles (enuf_spread.cuh, WindowRows): the 3 x (2m+1) window values of a
 // particle are evaluated ONCE per evaluation here ("window values ... kept") and read by every
-// spreading CTA whose halo holds the particle.  A warp takes 32 consecutive sorted particles, one lane per
-// particle for the evaluation, and writes their rows -- one contiguous block -- with coalesced 16-byte stores
-// through a shared-memory transpose.
-template <typename T> constexpr int rows_warps() { return sizeof(T) == 4 ? 4 : 2; }   // static shared memory <= 48 KB
+// spreading CTA whose halo holds the particle.  A CTA of three warps takes 32 consecutive sorted particles --
+// warp d evaluates dimension d, one lane per particle -- and writes their rows, one contiguous block, with
+// coalesced 16-byte stores through a shared-memory transpose.
+constexpr int kRowsThreads = 96;
 template <typename T, int M_, bool kTrim>
-__global__ void __launch_bounds__(32 * rows_warps<T>())
+__global__ void __launch_bounds__(kRowsThreads)
 window_rows_kernel(const PSlot<T>* __restrict__ slots, const uint32_t* __restrict__ offset, int nbins, WindowParams wp,
                    const __grid_constant__ PolyArg<M_> pa, T* __restrict__ rows) {
     using R = WindowRows<M_, kTrim>;
     using V4 = typename Vec4<T>::type;
     constexpr int SP = R::RP + 4;                                  // 44 / 52 elements: conflict-free 16-byte accesses
-    constexpr int kRowsWarps = rows_warps<T>();
-    __shared__ __align__(16) T tile[kRowsWarps][32 * SP];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __shared__ __align__(16) T tile[32 * SP];
+    const int lane = threadIdx.x & 31, dim = threadIdx.x >> 5;
     const uint32_t n_charged = offset[nbins];
-    const uint32_t base = (uint32_t)(blockIdx.x * kRowsWarps + warp) * 32u;
+    const uint32_t base = (uint32_t)blockIdx.x * 32u;
     if (base >= n_charged) return;
     const uint32_t nv = min(32u, n_charged - base);
-    T* mine = tile[warp] + lane * SP;
     if ((uint32_t)lane < nv) {
         const PSlot<T> sl = slots[base + lane];
         const int ksx = (int)((sl.cell >> 30) & 1u);
         // parity of the first x stencil point (grid index c_x - m + ks_x; n is even, so wrapping keeps it)
         const int parx = ((int)(sl.cell & 1023u) + M_ + ksx) & 1;
-        write_window_rows<T, M_, kTrim>(wp, pa, sl.rec.dx, sl.rec.dy, sl.rec.dz, sl.rec.q, parx, mine);
+        const T d0 = dim == 0 ? sl.rec.dx : (dim == 1 ? sl.rec.dy : sl.rec.dz);
+        write_window_row<T, M_, kTrim>(wp, pa, dim, d0, sl.rec.q, parx, tile + lane * SP);
     }
-    __syncwarp();
+    __syncthreads();
     T* out = rows + (size_t)base * R::RP;
     constexpr int CH = R::RP / 4;                                  // 16-byte (fp32) / 32-byte (fp64) chunks per particle
-    for (int c = lane; c < (int)nv * CH; c += 32) {
+    for (int c = threadIdx.x; c < (int)nv * CH; c += kRowsThreads) {
         const int pp = c / CH, cc = c - pp * CH;
-        reinterpret_cast<V4*>(out)[c] = reinterpret_cast<const V4*>(tile[warp] + pp * SP)[cc];
+        reinterpret_cast<V4*>(out)[c] = reinterpret_cast<const V4*>(tile + pp * SP)[cc];
     }
 }
 

@@ -201,7 +201,11 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
             const int n = min(C::PERM, wend - c0);
             // ---- particles whose stencil rows start on an even tile column first, the odd ones after: the two
             //      particles of a pair then take the same (aligned / unaligned) row-load path, except one pair per chunk
-            {
+            if (n <= 2) {
+                // one pair: nothing to sort (and no global-load round trip for the cell words)
+                if (lane < n) perm[lane] = slot_of(c0 + lane);
+                __syncwarp();
+            } else {
                 uint32_t gi[2]; bool ev[2], od[2];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {

@@ -140,19 +140,18 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     bin_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
                                                  p->tg, p->bin_cursor, static_cast<PSlot<T>*>(p->rec));
     // window rows of the sorted particles (read by the spreading kernel); N bounds the number of charged particles
-    constexpr int kRowsWarps = rows_warps<T>();
-    const unsigned rblocks = (unsigned)((N + 32 * kRowsWarps - 1) / (32 * kRowsWarps));
+    const unsigned rblocks = (unsigned)((N + 31) / 32);
     const int rc = dispatch_m(p, [&](auto mc) -> int {
         constexpr int M_ = decltype(mc)::value;
         const PolyArg<M_> pa = make_poly_arg<M_>(p);
         if constexpr (M_ >= 5 && sizeof(T) == 4) {
             if (p->trim) {
-                window_rows_kernel<T, M_, true><<<rblocks, 32 * kRowsWarps, 0, s>>>(
+                window_rows_kernel<T, M_, true><<<rblocks, kRowsThreads, 0, s>>>(
                     static_cast<const PSlot<T>*>(p->rec), p->bin_offset, nbins, p->wp, pa, static_cast<T*>(p->rows));
                 return 0;
             }
         }
-        window_rows_kernel<T, M_, false><<<rblocks, 32 * kRowsWarps, 0, s>>>(
+        window_rows_kernel<T, M_, false><<<rblocks, kRowsThreads, 0, s>>>(
             static_cast<const PSlot<T>*>(p->rec), p->bin_offset, nbins, p->wp, pa, static_cast<T*>(p->rows));
         return 0;
     });

@@ -106,46 +106,42 @@ struct WindowRows {
 };
 
 template <typename T, int M_, bool kTrim>
-__device__ __forceinline__ void write_window_rows(const WindowParams& wp, const PolyArg<M_>& pa, T dx, T dy, T dz, T q,
-                                                  int parx, T* __restrict__ dst) {
+__device__ __forceinline__ void write_window_row(const WindowParams& wp, const PolyArg<M_>& pa, int dim, T d0, T q,
+                                                 int parx, T* __restrict__ dst) {
     using R = WindowRows<M_, kTrim>;
     constexpr int W = R::W, WZ = R::WZ;
     using V4 = typename Vec4<T>::type;
+    T w[W], dw[W];
+    stencil_weights<T, M_, false>(wp, pa, d0, w, dw);
+    const int sh = (kTrim && d0 > (T)0) ? 1 : 0;
+    const int par = dim == 0 ? parx : 0;
+    const T mult = dim == 2 ? q : (T)1;
+    constexpr int RMAX = R::RX;
+    T rr[RMAX];
 #pragma unroll
-    for (int dim = 0; dim < 3; ++dim) {
-        const T d0 = dim == 0 ? dx : (dim == 1 ? dy : dz);
-        T w[W], dw[W];
-        stencil_weights<T, M_, false>(wp, pa, d0, w, dw);
-        const int sh = (kTrim && d0 > (T)0) ? 1 : 0;
-        const int par = dim == 0 ? parx : 0;
-        const T mult = dim == 2 ? q : (T)1;
-        constexpr int RMAX = R::RX;
-        const int len = dim == 0 ? R::RX : R::RY;                 // compile-time per unrolled dim
-        T rr[RMAX];
-#pragma unroll
-        for (int j = 0; j < RMAX; ++j) {
-            // element j holds stencil point k = j - par, i.e. w[k + sh]
-            T v = (T)0;
-            if (kTrim) {
-                const T a0 = (j < WZ) ? w[j < W ? j : 0] : (T)0;                          // par 0, sh 0
-                const T a1 = (j + 1 < W && j < WZ) ? w[j + 1 < W ? j + 1 : 0] : (T)0;      // par 0, sh 1
-                const T b0 = (j >= 1 && j - 1 < WZ) ? w[j >= 1 ? j - 1 : 0] : (T)0;        // par 1, sh 0
-                const T b1 = (j >= 1 && j - 1 < WZ) ? w[j < W ? j : 0] : (T)0;             // par 1, sh 1
-                v = par ? (sh ? b1 : b0) : (sh ? a1 : a0);
-            } else {
-                const T a0 = (j < WZ) ? w[j < W ? j : 0] : (T)0;
-                const T b0 = (j >= 1 && j - 1 < WZ) ? w[j >= 1 ? j - 1 : 0] : (T)0;
-                v = par ? b0 : a0;
-            }
-            rr[j] = v * mult;
+    for (int j = 0; j < RMAX; ++j) {
+        // element j holds stencil point k = j - par, i.e. w[k + sh]
+        T v = (T)0;
+        if (kTrim) {
+            const T a0 = (j < WZ) ? w[j < W ? j : 0] : (T)0;                          // par 0, sh 0
+            const T a1 = (j + 1 < W && j < WZ) ? w[j + 1 < W ? j + 1 : 0] : (T)0;      // par 0, sh 1
+            const T b0 = (j >= 1 && j - 1 < WZ) ? w[j >= 1 ? j - 1 : 0] : (T)0;        // par 1, sh 0
+            const T b1 = (j >= 1 && j - 1 < WZ) ? w[j < W ? j : 0] : (T)0;             // par 1, sh 1
+            v = par ? (sh ? b1 : b0) : (sh ? a1 : a0);
+        } else {
+            const T a0 = (j < WZ) ? w[j < W ? j : 0] : (T)0;
+            const T b0 = (j >= 1 && j - 1 < WZ) ? w[j >= 1 ? j - 1 : 0] : (T)0;
+            v = par ? b0 : a0;
         }
-        V4* row4 = reinterpret_cast<V4*>(dst + (dim == 0 ? 0 : (dim == 1 ? R::OY : R::OZ)));
+        rr[j] = v * mult;
+    }
+    const int len = dim == 0 ? R::RX : R::RY;
+    V4* row4 = reinterpret_cast<V4*>(dst + (dim == 0 ? 0 : (dim == 1 ? R::OY : R::OZ)));
 #pragma unroll
-        for (int v = 0; v < RMAX / 4; ++v) {
-            if (4 * v < len) {
-                V4 o; o.x = rr[4 * v]; o.y = rr[4 * v + 1]; o.z = rr[4 * v + 2]; o.w = rr[4 * v + 3];
-                row4[v] = o;
-            }
+    for (int v = 0; v < RMAX / 4; ++v) {
+        if (4 * v < len) {
+            V4 o; o.x = rr[4 * v]; o.y = rr[4 * v + 1]; o.z = rr[4 * v + 2]; o.w = rr[4 * v + 3];
+            row4[v] = o;
         }
     }
 }
@@ -324,16 +320,24 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 int ns = 0;
                 ENUF_TR((s - s_begin) * 16 + 0, trace_clock());
                 for (;;) {
-                    // all loaded steps at once, branch-free (the steps are independent up to the running slot count)
+                    // all loaded steps at once, branch-free (the steps are independent up to the running slot count);
+                    // in halves, so that sparse slabs (few steps) skip the unused half
                     int pkv[kSteps]; unsigned bal[kSteps];
 #pragma unroll
-                    for (int j = 0; j < kSteps; ++j) {
-                        const uint32_t cwj = cw[j];
-                        const int X0 = (((int)(cwj & 1023u) + (int)((cwj >> 30) & 1u) + offx) & nmask) - (WZ - 1);
-                        const int Y0 = (((int)((cwj >> 10) & 1023u) + (int)(cwj >> 31) + offy) & nmask) - (WZ - 1);
-                        const bool ok = cwj != 0xffffffffu && X0 <= CX - 1 && Y0 <= CY - 1;
-                        bal[j] = __ballot_sync(FULL, ok);
-                        pkv[j] = ok ? ((X0 + 32) | ((Y0 + 32) << 8)) : -1;
+                    for (int j = 0; j < kSteps; ++j) { pkv[j] = -1; bal[j] = 0u; }
+#pragma unroll
+                    for (int hh = 0; hh < 2; ++hh) {
+                        if (hh * (kSteps / 2) < nst) {
+#pragma unroll
+                            for (int j = hh * (kSteps / 2); j < (hh + 1) * (kSteps / 2); ++j) {
+                                const uint32_t cwj = cw[j];
+                                const int X0 = (((int)(cwj & 1023u) + (int)((cwj >> 30) & 1u) + offx) & nmask) - (WZ - 1);
+                                const int Y0 = (((int)((cwj >> 10) & 1023u) + (int)(cwj >> 31) + offy) & nmask) - (WZ - 1);
+                                const bool ok = cwj != 0xffffffffu && X0 <= CX - 1 && Y0 <= CY - 1;
+                                bal[j] = __ballot_sync(FULL, ok);
+                                pkv[j] = ok ? ((X0 + 32) | ((Y0 + 32) << 8)) : -1;
+                            }
+                        }
                     }
                     // steps are taken while their accepted particles fit into the round (CAP slots)
                     int jl = kSteps, base = ns, pb[kSteps];
@@ -345,11 +349,16 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                         if (j < jl) base += c;
                     }
 #pragma unroll
-                    for (int j = 0; j < kSteps; ++j) {
-                        if (j < jl) {
-                            if (pkv[j] >= 0)
-                                acc_rec[k][pb[j] + __popc(bal[j] & below)] = make_uint2(cbase[j] + (uint32_t)lane, (unsigned)pkv[j]);
-                            cw[j] = 0xffffffffu;                        // consumed
+                    for (int hh = 0; hh < 2; ++hh) {
+                        if (hh * (kSteps / 2) < nst) {
+#pragma unroll
+                            for (int j = hh * (kSteps / 2); j < (hh + 1) * (kSteps / 2); ++j) {
+                                if (j < jl) {
+                                    if (pkv[j] >= 0)
+                                        acc_rec[k][pb[j] + __popc(bal[j] & below)] = make_uint2(cbase[j] + (uint32_t)lane, (unsigned)pkv[j]);
+                                    cw[j] = 0xffffffffu;                // consumed
+                                }
+                            }
                         }
                     }
                     ns = base;
