@@ -25,7 +25,9 @@
  * alpha-independence of the total energy, forces = -dE/dr by central differences,
  * sum_i F_i = 0, two-particle antisymmetry, window transform by quadrature, window
  * derivative by differences, DFT == radix-2 FFT == numpy.fft, additivity Eq. 61,
- * S~(n) vs S(n) mode by mode, error falls with m.
+ * S~(n) vs S(n) mode by mode, error falls with m; B-spline window: m = 1 hat
+ * function in closed form, partition of unity, transform by quadrature, derivative by differences,
+ * brute force against Oracle A.
  * Parity unpinned against the paper: the Slater form factor in k-space (R19) -- it is
  * BASELINE.json's variant, pinned only against quadrature of Eq. 51 and Oracle A.
  *
@@ -43,7 +45,7 @@
 
 #define ORC_PI 3.14159265358979323846264338327950288
 
-enum { ORC_WIN_GAUSSIAN = 0, ORC_WIN_KAISER_BESSEL = 1 };
+enum { ORC_WIN_GAUSSIAN = 0, ORC_WIN_KAISER_BESSEL = 1, ORC_WIN_BSPLINE = 2 };
 enum { ORC_FORCE_ANALYTIC = 0, ORC_FORCE_IK = 1 };
 
 int orc_num_threads(void)
@@ -79,9 +81,22 @@ static double kb_b(double sigma)
     return ORC_PI * (2.0 - 1.0 / sigma);
 }
 
+/* Centred cardinal B-spline of order p (degree p - 1, support [-p/2, p/2]) by its defining recursion
+ * (Cox-de Boor for uniform knots): B_1 = indicator of [-1/2, 1/2),
+ * B_p(x) = [(x + p/2) B_{p-1}(x + 1/2) + (p/2 - x) B_{p-1}(x - 1/2)] / (p - 1).
+ * Slow (2^p leaves) and obviously the definition.  PAPER.md:266 names the B-spline among the NFFT
+ * windows without a formula; the NFFT literature it cites uses order 2m, normalised here to phi(0) = 1 (R7). */
+static double bspline_rec(int p, double x)
+{
+    if (p == 1) return (x >= -0.5 && x < 0.5) ? 1.0 : 0.0;
+    return ((x + 0.5 * p) * bspline_rec(p - 1, x + 0.5) + (0.5 * p - x) * bspline_rec(p - 1, x - 0.5)) / (p - 1);
+}
+
 double orc_phi(int window, int m, double sigma, double d)
 {
-    if (window == ORC_WIN_GAUSSIAN) {
+    if (window == ORC_WIN_BSPLINE) {
+        return bspline_rec(2 * m, d) / bspline_rec(2 * m, 0.0);
+    } else if (window == ORC_WIN_GAUSSIAN) {
         return exp(-d * d / gauss_b(m, sigma));
     } else {
         double b = kb_b(sigma);
@@ -99,7 +114,10 @@ double orc_phi(int window, int m, double sigma, double d)
 /* d phi / d d (used by the analytic-derivative force variant). */
 double orc_dphi(int window, int m, double sigma, double d)
 {
-    if (window == ORC_WIN_GAUSSIAN) {
+    if (window == ORC_WIN_BSPLINE) {
+        /* B_p' (x) = B_{p-1}(x + 1/2) - B_{p-1}(x - 1/2) */
+        return (bspline_rec(2 * m - 1, d + 0.5) - bspline_rec(2 * m - 1, d - 0.5)) / bspline_rec(2 * m, 0.0);
+    } else if (window == ORC_WIN_GAUSSIAN) {
         double b = gauss_b(m, sigma);
         return -(2.0 * d / b) * exp(-d * d / b);
     } else {
@@ -136,7 +154,11 @@ static double bessel_i0(double x)
  * Phi(k) = int phi(d) exp(-2 pi i k d / n) dd.                                   */
 double orc_Phi(int window, int m, double sigma, int n, int k)
 {
-    if (window == ORC_WIN_GAUSSIAN) {
+    if (window == ORC_WIN_BSPLINE) {
+        /* B_p is the p-fold convolution of the unit box, whose transform at frequency k/n is sinc(pi k/n) */
+        double t = ORC_PI * k / n, sc = k == 0 ? 1.0 : sin(t) / t;
+        return pow(sc, 2 * m) / bspline_rec(2 * m, 0.0);
+    } else if (window == ORC_WIN_GAUSSIAN) {
         double b = gauss_b(m, sigma);
         double t = ORC_PI * k / n;
         return sqrt(ORC_PI * b) * exp(-b * t * t);

@@ -131,6 +131,66 @@ def test_window_transform_by_quadrature(oracle, window, m, tol):
         assert abs(val - ref) < tol * abs(oracle.Phi(window, m, sigma, n, 0)), (k, val, ref)
 
 
+# ----------------------------------------------------------------- B-spline window
+
+def test_bspline_m1_is_the_hat_function(oracle):
+    """Order 2 (m = 1): phi(d) = 1 - |d| on [-1, 1] -- a closed form the recursion must reproduce."""
+    for d in (-1.3, -1.0, -0.75, -0.2, 0.0, 0.4, 0.999, 1.0, 2.0):
+        want = max(0.0, 1.0 - abs(d))
+        assert abs(oracle.phi("bspline", 1, 2.0, d) - want) < 1e-15
+    assert oracle.dphi("bspline", 1, 2.0, 0.3) == -1.0 and oracle.dphi("bspline", 1, 2.0, -0.3) == 1.0
+
+
+@pytest.mark.parametrize("m", [2, 3, 4, 6])
+def test_bspline_partition_of_unity_and_support(oracle, m):
+    """sum_j B_p(x - j) = 1 for every x (the classic B-spline identity), phi(0) = 1 (R7), support [-m, m],
+    central value of the cubic spline 2/3 (phi = B_4 / B_4(0), so phi(1) = (1/6)/(2/3) = 1/4)."""
+    B0 = 1.0 / sum(oracle.phi("bspline", m, 2.0, j) for j in range(-m, m + 1))     # = B_2m(0)
+    for x in (0.0, 0.17, 0.5, 0.93):
+        total = sum(oracle.phi("bspline", m, 2.0, x - j) for j in range(-m - 1, m + 2)) * B0
+        assert abs(total - 1.0) < 1e-14
+    assert abs(oracle.phi("bspline", m, 2.0, 0.0) - 1.0) < 1e-15
+    assert oracle.phi("bspline", m, 2.0, m) == 0.0 and oracle.phi("bspline", m, 2.0, m + 0.3) == 0.0
+    assert oracle.phi("bspline", m, 2.0, m - 1e-3) > 0.0
+    if m == 2:
+        assert abs(B0 - 2.0 / 3.0) < 1e-15 and abs(oracle.phi("bspline", 2, 2.0, 1.0) - 0.25) < 1e-15
+
+
+@pytest.mark.parametrize("m", [2, 4, 6])
+def test_bspline_transform_and_derivative(oracle, m):
+    n = 64
+    for k in (0, 1, 5, 16):
+        f = lambda d: oracle.phi("bspline", m, 2.0, d) * math.cos(2 * math.pi * k * d / n)
+        val, _ = integrate.quad(f, -m, m, limit=400, epsabs=1e-13, epsrel=1e-13, points=list(range(-m + 1, m)))
+        assert abs(val - oracle.Phi("bspline", m, 2.0, n, k)) < 1e-11 * oracle.Phi("bspline", m, 2.0, n, 0)
+    h = 1e-6
+    for d in (-m + 0.4, -0.7, 0.0, 0.3, 1.5, m - 0.2):
+        fd = (oracle.phi("bspline", m, 2.0, d + h) - oracle.phi("bspline", m, 2.0, d - h)) / (2 * h)
+        assert abs(fd - oracle.dphi("bspline", m, 2.0, d)) < 1e-8
+
+
+@pytest.mark.parametrize("variant,bound", [("analytic", 2e-2), ("ik", 2e-3)])
+def test_bspline_enuf_against_direct_ewald(oracle, variant, bound):
+    """Brute force: Oracle B with the B-spline window (m = 6, sigma = 2) against Oracle A on 64 particles.
+    The B-spline is the least accurate of the NFFT windows at equal m (error ~ (1/(2 sigma - 1))^{2m} ~ 2e-6 per
+    dimension at the band edge)."""
+    L, alpha, kc, n, m = 6.0, 1.0, 8, 32, 6
+    r, q = random_neutral_gas(64, L, seed=21)
+    Ea, Fa = oracle.direct(r, q, L, alpha, kc)
+    b = oracle.enuf(r, q, L, alpha, kc, n, m, "bspline", variant=variant)
+    assert abs(b["E"] - Ea) < 1e-3 * abs(Ea)
+    err = math.sqrt(((b["F"] - Fa) ** 2).sum() / (Fa ** 2).sum())
+    assert err < bound, err
+    if variant == "analytic":       # exact gradient of the ENUF energy (R17)
+        h = 1e-5
+        for i, d in ((3, 0), (40, 2)):
+            rp = r.copy(); rp[i, d] += h
+            rm = r.copy(); rm[i, d] -= h
+            ep = oracle.enuf(rp, q, L, alpha, kc, n, m, "bspline", forces=False)["E"]
+            em = oracle.enuf(rm, q, L, alpha, kc, n, m, "bspline", forces=False)["E"]
+            assert abs(b["F"][i, d] + (ep - em) / (2 * h)) < 1e-7 * np.abs(b["F"]).max()
+
+
 @pytest.mark.parametrize("window,m", [("kaiser_bessel", 4), ("kaiser_bessel", 6), ("gaussian", 4)])
 def test_window_normalisation_symmetry_support(oracle, window, m):
     assert abs(oracle.phi(window, m, 2.0, 0.0) - 1.0) < 1e-15           # R7
