@@ -48,7 +48,8 @@ enum enuf_status {
 /* keys of enuf_plan_set(); values are passed as double */
 enum enuf_option {
     ENUF_OPT_PRECISION = 1,      /* ENUF_F32 (default) | ENUF_F64; only before the first evaluation */
-    ENUF_OPT_WINDOW = 2,         /* ENUF_WINDOW_KAISER_BESSEL (default) | ENUF_WINDOW_GAUSSIAN (R6) */
+    ENUF_OPT_WINDOW = 2,         /* ENUF_WINDOW_KAISER_BESSEL (default) | ENUF_WINDOW_GAUSSIAN (R6) |
+                                    ENUF_WINDOW_BSPLINE: centred cardinal B-spline of order 2m (:266)  */
     ENUF_OPT_FORCE_VARIANT = 3,  /* ENUF_FORCE_ANALYTIC (default) | ENUF_FORCE_IK (paper, Eq. 41)   */
     ENUF_OPT_SLATER_LAMBDA = 4,  /* decay length of the Slater density Eq. 51 (:407); 0 = point (R19) */
     ENUF_OPT_NUM_PARTICLES = 5,  /* lower N for the next calls, 0 <= N <= planned capacity          */
@@ -64,7 +65,7 @@ enum enuf_option {
 };
 
 enum { ENUF_F32 = 0, ENUF_F64 = 1 };
-enum { ENUF_WINDOW_GAUSSIAN = 0, ENUF_WINDOW_KAISER_BESSEL = 1 };
+enum { ENUF_WINDOW_GAUSSIAN = 0, ENUF_WINDOW_KAISER_BESSEL = 1, ENUF_WINDOW_BSPLINE = 2 };
 enum { ENUF_FORCE_ANALYTIC = 0, ENUF_FORCE_IK = 1 };
 
 /* stage indices of enuf_plan_stage_ms() */
@@ -222,6 +223,18 @@ const char *enuf_last_error(void);
 int enuf_ncut(double alpha, double L, double delta);
 double enuf_alpha_from_rc(double r_c, double delta);
 double enuf_rc_from_ncut(int n_c, double alpha, double L);
+
+/*
+ * The parameter loop of the paper ("for a given accuracy delta and real-space cutoff r_c, alpha and
+ * n_c follow from Eq. 31-32"; :254-262) as a plan constructor: alpha = sqrt(-ln delta) / r_c (R15),
+ * k_cut = n_c = ceil((alpha L / pi) sqrt(-ln delta)) (R14), M = the smallest power of two >= 2 k_cut (R5; all five
+ * BASELINE configs follow this rule), then enuf_plan_create(N, L, alpha, k_cut, M, sigma, m).
+ * ENUF_EINVAL if delta is not in (0, 1), r_c <= 0, or sigma * M leaves {32, 64, 128, 256}.
+ * enuf_plan_get reads back what was chosen: key = ENUF_GET_ALPHA / K_CUT / M / GRID (n = sigma M) / SUPPORT (m).
+ */
+enum { ENUF_GET_ALPHA = 1, ENUF_GET_K_CUT = 2, ENUF_GET_M = 3, ENUF_GET_GRID = 4, ENUF_GET_SUPPORT = 5 };
+int enuf_plan_create_auto(enuf_plan **out, int64_t N, double L, double delta, double r_c, double sigma, int m);
+int enuf_plan_get(const enuf_plan *plan, int key, double *value);
 
 #ifdef __cplusplus
 }

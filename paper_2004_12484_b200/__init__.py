@@ -22,7 +22,7 @@ OPT_PRECISION, OPT_WINDOW, OPT_FORCE_VARIANT, OPT_SLATER_LAMBDA = 1, 2, 3, 4
 OPT_NUM_PARTICLES, OPT_PROFILE, OPT_KEEP_SPECTRUM, OPT_SPREAD_ZCHUNK = 5, 6, 7, 8
 OPT_CUDA_GRAPH = 9
 F32, F64 = 0, 1
-WINDOWS = {"gaussian": 0, "kaiser_bessel": 1}
+WINDOWS = {"gaussian": 0, "kaiser_bessel": 1, "bspline": 2}
 VARIANTS = {"analytic": 0, "ik": 1}
 STAGES = ("bin", "spread", "fft", "gather", "energy")
 
@@ -36,7 +36,9 @@ SYMBOLS = (
     "enuf_plan_copy_field", "enuf_plan_structure_factor", "enuf_spread_only",
     "enuf_plan_workspace_bytes", "enuf_plan_destroy", "enuf_last_error",
     "enuf_ncut", "enuf_alpha_from_rc", "enuf_rc_from_ncut",
+    "enuf_plan_create_auto", "enuf_plan_get",
 )
+GET_ALPHA, GET_K_CUT, GET_M, GET_GRID, GET_SUPPORT = 1, 2, 3, 4, 5
 
 
 class EnufError(RuntimeError):
@@ -87,6 +89,9 @@ def lib():
         L.enuf_ncut.restype = i; L.enuf_ncut.argtypes = [d, d, d]
         L.enuf_alpha_from_rc.restype = d; L.enuf_alpha_from_rc.argtypes = [d, d]
         L.enuf_rc_from_ncut.restype = d; L.enuf_rc_from_ncut.argtypes = [i, d, d]
+        L.enuf_plan_create_auto.restype = i
+        L.enuf_plan_create_auto.argtypes = [C.POINTER(vp), i64, d, d, d, d, i]
+        L.enuf_plan_get.restype = i; L.enuf_plan_get.argtypes = [vp, i, C.POINTER(d)]
         _lib = L
     return _lib
 
@@ -161,6 +166,25 @@ class Plan:
         self.set(OPT_KEEP_SPECTRUM, int(keep_spectrum))
         if cuda_graph:
             self.set(OPT_CUDA_GRAPH, 1)
+
+    @classmethod
+    def auto(cls, N, L, delta, r_c, sigma=2.0, m=6, **kw):
+        """enuf_plan_create_auto: alpha, k_cut and M from the accuracy delta and the real-space cutoff r_c by the
+        parameter rule Eq. 31-32.  Other keyword arguments as for Plan()."""
+        h = C.c_void_p()
+        _check(lib().enuf_plan_create_auto(C.byref(h), int(N), float(L), float(delta), float(r_c), float(sigma), int(m)))
+        v = C.c_double(0.0)
+        got = {}
+        for name, key in (("alpha", GET_ALPHA), ("k_cut", GET_K_CUT), ("M", GET_M)):
+            _check(lib().enuf_plan_get(h, key, C.byref(v)))
+            got[name] = v.value
+        lib().enuf_plan_destroy(h)
+        return cls(N, L, got["alpha"], int(got["k_cut"]), int(got["M"]), sigma=sigma, m=m, **kw)
+
+    def get(self, key: int) -> float:
+        v = C.c_double(0.0)
+        _check(lib().enuf_plan_get(self._h, int(key), C.byref(v)))
+        return v.value
 
     @classmethod
     def from_workload(cls, w, **kw):

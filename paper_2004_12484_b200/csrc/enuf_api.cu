@@ -56,9 +56,34 @@ double bessel_i0_series(double x) {
     return sum;
 }
 
+// B_p(x) and its i-th derivative from the right, B_p^(i)(x) = sum_l (-1)^l C(i, l) B_{p-i}(x + i/2 - l)
+// (B_p' = B_{p-1}(. + 1/2) - B_{p-1}(. - 1/2) applied i times); host, fp64, p <= 12
+double bspline_host(int p, double x) {
+    const double t = x + 0.5 * p;
+    if (!(t >= 0.0) || !(t < p)) return 0.0;
+    double a[16] = {0};
+    a[(int)t] = 1.0;                                   // right-continuous at the knots
+    for (int k = 2; k <= p; ++k)
+        for (int j = 0; j + k <= p; ++j) a[j] = ((t - j) * a[j] + (k - t + j) * a[j + 1]) / (k - 1);
+    return a[0];
+}
+double bspline_deriv_host(int p, int i, double x) {
+    double s = 0.0, binom = 1.0;
+    for (int l = 0; l <= i; ++l) {
+        s += ((l & 1) ? -1.0 : 1.0) * binom * bspline_host(p - i, x + 0.5 * i - l);
+        binom = binom * (i - l) / (l + 1);
+    }
+    return s;
+}
+
 // Window transform Phi(k) = int phi(d) exp(-2 pi i k d/n) dd for the phi(0)=1 windows (R6, R7)
 double window_transform(const enuf_plan* p, int k) {
     const double m = p->m, sg = p->sigma, n = p->n;
+    if (p->window == ENUF_WINDOW_BSPLINE) {
+        // the order-2m B-spline is the 2m-fold convolution of the unit box: sinc(pi k/n)^(2m), over B_2m(0)
+        const double t = kPi * k / n, sc = k == 0 ? 1.0 : std::sin(t) / t;
+        return std::pow(sc, 2 * p->m) / bspline_host(2 * p->m, 0.0);
+    }
     if (p->window == ENUF_WINDOW_GAUSSIAN) {
         const double b = 2.0 * sg * m / ((2.0 * sg - 1.0) * kPi);
         const double t = kPi * k / n;
@@ -74,7 +99,10 @@ void fill_window_params(enuf_plan* p) {
     enuf::WindowParams& w = p->wp;
     w.kind = p->window;
     w.m = p->m;
-    if (p->window == ENUF_WINDOW_GAUSSIAN) {
+    if (p->window == ENUF_WINDOW_BSPLINE) {
+        w.b = w.inv_b = w.bm = w.inv1m = 0.0;
+        w.A = 1.0 / bspline_host(2 * p->m, 0.0);       // phi = A B_2m
+    } else if (p->window == ENUF_WINDOW_GAUSSIAN) {
         w.b = 2.0 * p->sigma * p->m / ((2.0 * p->sigma - 1.0) * kPi);
         w.inv_b = 1.0 / w.b;
         w.bm = w.b * p->m;
@@ -111,6 +139,24 @@ double window_smooth(const enuf_plan* p, double d) {
 // D = poly_degree(m) of d0 -> phi(d0 - j) on [-1/2, 1/2], converted to monomials in d0, and
 // its exact derivative (enuf_common.cuh, PolyArg).
 void build_poly_table(enuf_plan* p) {
+    if (p->window == ENUF_WINDOW_BSPLINE) {
+        // exact pieces: phi(t - j) = sum_i B^(i)(-j from the right) / i! t^i on t in [0, 1/2], degree 2m - 1
+        const int P = 2 * p->m;
+        const double A = 1.0 / bspline_host(P, 0.0);
+        for (int jj = 0; jj <= 2 * p->m; ++jj) {
+            const int j = jj - p->m;
+            double fact = 1.0, c[16] = {0};
+            for (int i = 0; i < P; ++i) {
+                if (i > 0) fact *= i;
+                c[i] = A * bspline_deriv_host(P, i, (double)-j) / fact;
+            }
+            for (int i = 0; i < P; ++i) {
+                p->bs_c[i][jj] = (float)c[i];
+                p->bs_d[i][jj] = i + 1 < P ? (float)((i + 1) * c[i + 1]) : 0.f;
+            }
+        }
+        return;
+    }
     constexpr int NCMAX = enuf::kPolyMaxDeg + 1;
     const int D = enuf::poly_degree(p->m), NC = D + 1;
     for (int j = 0; j <= p->m; ++j) {
@@ -499,7 +545,8 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
             p->precision = iv;
             return ENUF_OK;
         case ENUF_OPT_WINDOW:
-            if (iv != ENUF_WINDOW_GAUSSIAN && iv != ENUF_WINDOW_KAISER_BESSEL) return fail(ENUF_EINVAL, "unknown window");
+            if (iv != ENUF_WINDOW_GAUSSIAN && iv != ENUF_WINDOW_KAISER_BESSEL && iv != ENUF_WINDOW_BSPLINE)
+                return fail(ENUF_EINVAL, "unknown window");
             p->window = iv; p->tables_dirty = true; fill_window_params(p);
             p->trim = p->precision == ENUF_F32 && p->window == ENUF_WINDOW_KAISER_BESSEL && p->m >= 5;
             p->tg.trim = p->trim ? 1 : 0;
@@ -879,6 +926,34 @@ void enuf_plan_destroy(enuf_plan* p) {
     free_workspace(p);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     delete p;
+}
+
+int enuf_plan_create_auto(enuf_plan** out, int64_t N, double L, double delta, double r_c, double sigma, int m) {
+    g_err[0] = 0;
+    if (!out) return fail(ENUF_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!(delta > 0) || !(delta < 1)) return fail(ENUF_EINVAL, "delta must be in (0, 1)");
+    if (!(r_c > 0) || !std::isfinite(r_c)) return fail(ENUF_EINVAL, "r_c must be positive and finite");
+    if (!(L > 0) || !std::isfinite(L)) return fail(ENUF_EINVAL, "L must be positive and finite");
+    const double alpha = std::sqrt(-std::log(delta)) / r_c;                                   // Eq. 32 (R15)
+    const int k_cut = (int)std::ceil(alpha * L / kPi * std::sqrt(-std::log(delta)));          // Eq. 31 (R14)
+    if (k_cut < 1 || k_cut > 4096) return fail(ENUF_EINVAL, "Eq. 31 gives k_cut = %d: out of range", k_cut);
+    int M = 2;
+    while (M < 2 * k_cut) M *= 2;                                                             // R5: k_cut <= M/2
+    return enuf_plan_create(out, N, L, alpha, k_cut, M, sigma, m);
+}
+
+int enuf_plan_get(const enuf_plan* p, int key, double* value) {
+    g_err[0] = 0;
+    if (!p || !value) return fail(ENUF_EINVAL, "plan or value is NULL");
+    switch (key) {
+        case ENUF_GET_ALPHA: *value = p->alpha; return ENUF_OK;
+        case ENUF_GET_K_CUT: *value = p->k_cut; return ENUF_OK;
+        case ENUF_GET_M: *value = p->M; return ENUF_OK;
+        case ENUF_GET_GRID: *value = p->n; return ENUF_OK;
+        case ENUF_GET_SUPPORT: *value = p->m; return ENUF_OK;
+        default: return fail(ENUF_EINVAL, "unknown key %d", key);
+    }
 }
 
 int enuf_ncut(double alpha, double L, double delta) {

@@ -83,6 +83,11 @@ struct PolyArg {
     alignas(8) float top[M_ + 1 + ((M_ + 1) & 1)];
     float2 vp[NP][M_ + 1];
     float2 dp[NP][M_ + 1];
+    // B-spline window (order 2m): for d0 in [0, 1/2] the weight phi(d0 - j), j = -m..m, is ONE polynomial piece of
+    // degree 2m - 1 in d0 (the knots are the integers), stored exactly: bc[i][j + m] t^i; bd = its derivative.
+    // For d0 < 0 the evenness of phi gives w_j(d0) = w_{-j}(-d0).
+    float bc[2 * M_][2 * M_ + 1];
+    float bd[2 * M_][2 * M_ + 1];
 };
 
 __host__ __device__ inline int bin_index(const TileGeom& g, int tx, int ty, int bz) { return (ty * g.n + bz) * g.nt + tx; }
@@ -150,12 +155,41 @@ __device__ __forceinline__ double r_sqrt(double x) { return sqrt(x); }
 // integer stencil offset.  d^2 is formed as j^2 + d0 (d0 - 2j) and the Kaiser-Bessel exponent
 // b (s - m) as -b d^2/(s + m): in fp32 the direct forms lose ~ulp(m) = 5e-7 in s - m, i.e. a
 // relative error of b*5e-7 = 2e-6 on the CENTRAL weights (fp32 error budget).
-template <typename T, bool kDeriv>
+// Centred cardinal B-spline of order P and its derivative (de Boor's triangle on uniform knots; all terms positive).
+// M_k(t) on [0, k], t = x + P/2:  M_k(t - j) = [(t - j) M_{k-1}(t - j) + (k - t + j) M_{k-1}(t - j - 1)] / (k - 1),
+// M_P'(t) = M_{P-1}(t) - M_{P-1}(t - 1).
+template <typename T, int P>
+__host__ __device__ inline void bspline_eval(T x, T& val, T& dval) {
+    const T t = x + (T)(0.5 * P);
+    val = (T)0; dval = (T)0;
+    if (!(t > (T)0) || !(t < (T)P)) return;
+    T a[P + 1];
+    const int i0 = (int)t;
+#pragma unroll
+    for (int j = 0; j <= P; ++j) a[j] = j == i0 ? (T)1 : (T)0;
+    if (P == 2) dval = a[0] - a[1];
+#pragma unroll
+    for (int k = 2; k <= P; ++k) {
+#pragma unroll
+        for (int j = 0; j + k <= P; ++j) a[j] = ((t - (T)j) * a[j] + ((T)k - t + (T)j) * a[j + 1]) / (T)(k - 1);
+        if (k == P - 1) dval = a[0] - a[1];
+    }
+    val = a[0];
+}
+
+template <typename T, bool kDeriv, int M_ = 0>
 __device__ __forceinline__ void window_eval(const WindowParams& wp, T d0, int j, T& phi, T& dphi) {
     const T jf = (T)j;
     const T d = d0 - jf;
     const T d2 = d0 * (d0 - (T)2 * jf) + jf * jf;
-    if (wp.kind == ENUF_WINDOW_GAUSSIAN) {
+    if (wp.kind == ENUF_WINDOW_BSPLINE) {
+        if constexpr (M_ > 0) {
+            T v, dv;
+            bspline_eval<T, 2 * M_>(d, v, dv);
+            phi = v * (T)wp.A;                       // A = 1 / B_2m(0)
+            if (kDeriv) dphi = dv * (T)wp.A;
+        }
+    } else if (wp.kind == ENUF_WINDOW_GAUSSIAN) {
         T ib = (T)wp.inv_b;
         phi = r_exp(-d2 * ib);
         if (kDeriv) dphi = -(T)2 * d * ib * phi;
@@ -204,11 +238,34 @@ __device__ __forceinline__ void stencil_weights(const WindowParams& wp, const Po
 #pragma unroll
         for (int k = 0; k < W; ++k) {
             dw[k] = (T)0;
-            window_eval<T, kDeriv>(wp, d0, k - M_, w[k], dw[k]);
+            window_eval<T, kDeriv, M_>(wp, d0, k - M_, w[k], dw[k]);
         }
     } else {
         const float x = (float)d0, y = x * x;
         float v[W], dv[W];
+        if (wp.kind == ENUF_WINDOW_BSPLINE) {
+            // one exact polynomial piece per stencil offset on d0 in [0, 1/2]; d0 < 0 by symmetry
+            const float t = fabsf(x);
+            float u[W], du[W];
+#pragma unroll
+            for (int jj = 0; jj < W; ++jj) {
+                float s = pa.bc[2 * M_ - 1][jj];
+#pragma unroll
+                for (int i = 2 * M_ - 2; i >= 0; --i) s = fmaf(s, t, pa.bc[i][jj]);
+                u[jj] = s;
+                float ds = 0.f;
+                if (kDeriv) {
+                    ds = pa.bd[2 * M_ - 2][jj];
+#pragma unroll
+                    for (int i = 2 * M_ - 3; i >= 0; --i) ds = fmaf(ds, t, pa.bd[i][jj]);
+                }
+                du[jj] = ds;
+            }
+            const bool neg = x < 0.f;
+#pragma unroll
+            for (int k = 0; k < W; ++k) { w[k] = (T)(neg ? u[W - 1 - k] : u[k]); dw[k] = (T)(neg ? -du[W - 1 - k] : du[k]); }
+            return;
+        }
         if constexpr (kPacked) {
             const float2 yy = make_float2(y, y);
             constexpr int NP = PolyArg<M_>::NP;

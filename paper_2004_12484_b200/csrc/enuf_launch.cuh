@@ -54,6 +54,8 @@ static inline PolyArg<M_> make_poly_arg(const enuf_plan* p) {
             a.dp[k][j] = make_float2(p->poly_d[D - 2 - 2 * k][j], p->poly_d[D - 1 - 2 * k][j]);
         }
     }
+    for (int i = 0; i < 2 * M_; ++i)
+        for (int jj = 0; jj <= 2 * M_; ++jj) { a.bc[i][jj] = p->bs_c[i][jj]; a.bd[i][jj] = p->bs_d[i][jj]; }
     return a;
 }
 

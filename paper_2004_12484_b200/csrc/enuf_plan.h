@@ -49,6 +49,8 @@ struct enuf_plan {
     uint32_t* scan_epoch = nullptr;            // [1] device word: evaluation counter, the epoch of scan_desc
     float poly_c[enuf::kPolyMaxDeg + 1][enuf::kMaxM + 1] = {};   // host copy of the polynomial window table
     float poly_d[enuf::kPolyMaxDeg][enuf::kMaxM + 1] = {};       // (fp32 path; packed into PolyArg<m> per launch)
+    float bs_c[2 * enuf::kMaxM][2 * enuf::kMaxM + 1] = {};       // B-spline window: exact pieces on d0 in [0, 1/2] (PolyArg::bc, bd)
+    float bs_d[2 * enuf::kMaxM][2 * enuf::kMaxM + 1] = {};
     int zchunk = 0;                   // grid planes per spread CTA
     bool zchunk_user = false;         // set through ENUF_OPT_SPREAD_ZCHUNK: not re-derived
     int spread_npx = 4;               // spread column = 8 spread_npx x 16 cells (4 for n >= 128, 2 below)

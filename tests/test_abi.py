@@ -92,3 +92,38 @@ def test_parameter_rule_literals(lib):
     assert enuf.ncut(a, 215.0, 1e-4) == 64
     assert abs(enuf.rc_from_ncut(64, a, 215.0) - math.pi * 64 / (a * a * 215.0)) < 1e-12
     assert enuf.ncut(-1.0, 1.0, 0.5) < 0 and math.isnan(enuf.alpha_from_rc(0.0, 0.5))
+
+
+def test_plan_create_auto_reproduces_the_config_literals(lib):
+    """enuf_plan_create_auto (the parameter loop of PAPER.md:350, Eq. 31-32 :254-262) against the literal plan
+    parameters BASELINE.json / DESIGN.md section 2 give for configs 3, 4 and 5 (no GPU needed: plans are host objects)."""
+    from enuf_inputs import make_workload
+    v = C.c_double()
+
+    def get(h, key):
+        assert lib.enuf_plan_get(h, key, C.byref(v)) == enuf.OK
+        return v.value
+
+    for name in ("cfg3", "cfg4", "cfg5"):
+        w = make_workload(name)
+        delta = w.meta["delta"]
+        r_c = math.sqrt(-math.log(delta)) / w.alpha          # Eq. 32 (R15), the cutoff the config's alpha belongs to
+        h = C.c_void_p()
+        assert lib.enuf_plan_create_auto(C.byref(h), w.N, w.L, delta, r_c, w.sigma, w.m) == enuf.OK
+        assert abs(get(h, enuf.GET_ALPHA) - w.alpha) <= 1e-14 * w.alpha
+        assert get(h, enuf.GET_K_CUT) == w.k_cut and get(h, enuf.GET_M) == w.M
+        assert get(h, enuf.GET_GRID) == w.n and get(h, enuf.GET_SUPPORT) == w.m
+        lib.enuf_plan_destroy(h)
+    # config 5 from its own literals: r_c = 10, delta = 1e-4, L = 215
+    h = C.c_void_p()
+    assert lib.enuf_plan_create_auto(C.byref(h), 1000000, 215.0, 1e-4, 10.0, 2.0, 6) == enuf.OK
+    assert abs(get(h, enuf.GET_ALPHA) - 0.30348542587702925) < 1e-15 and get(h, enuf.GET_K_CUT) == 64
+    assert get(h, enuf.GET_M) == 128 and get(h, enuf.GET_GRID) == 256
+    lib.enuf_plan_destroy(h)
+    # bad arguments, and a grid the library does not have (sigma M = 512)
+    h = C.c_void_p()
+    assert lib.enuf_plan_create_auto(C.byref(h), 10, 215.0, 1.5, 10.0, 2.0, 6) == enuf.EINVAL
+    assert lib.enuf_plan_create_auto(C.byref(h), 10, 215.0, 1e-4, 0.0, 2.0, 6) == enuf.EINVAL
+    assert lib.enuf_plan_create_auto(C.byref(h), 10, 430.0, 1e-4, 10.0, 2.0, 6) == enuf.EINVAL
+    assert b"sigma*M" in lib.enuf_last_error()
+    assert lib.enuf_plan_get(None, enuf.GET_ALPHA, C.byref(v)) == enuf.EINVAL

@@ -298,6 +298,43 @@ def test_all_grid_sizes_and_supports(enuf, torch_cuda, oracle, n, m, window, dty
     plan.close()
 
 
+@pytest.mark.parametrize("n,m,dtype", [(32, 1, "f64"), (32, 3, "f64"), (64, 6, "f64"), (32, 2, "f32"), (64, 4, "f32"),
+                                       (128, 6, "f32")])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_bspline_window_matches_oracle(enuf, torch_cuda, oracle, n, m, dtype, variant):
+    """ENUF_WINDOW_BSPLINE: order-2m B-spline, Phi(k) = sinc^2m / B_2m(0).  fp64: de Boor's triangle
+    on the device; fp32: the exact polynomial pieces.  Against Oracle B, which evaluates the defining recursion."""
+    torch = torch_cuda
+    N, L = 333, 7.5
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = random_neutral_gas(N, L, seed=500 + n + m, dtype=npdt)
+    M = n // 2
+    k_cut = M // 2
+    alpha = 0.9 * math.pi * k_cut / (L * 3.0)
+    ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, "bspline", 2.0, variant=variant)
+    plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=2.0, m=m, window="bspline", variant=variant,
+                     dtype=torch.float64 if dtype == "f64" else torch.float32)
+    E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+    tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+    plan.close()
+
+
+def test_plan_auto_runs_config3(enuf, torch_cuda, oracle):
+    """Plan.auto (enuf_plan_create_auto): config 3 planned from (delta, r_c) evaluates like the literal plan."""
+    torch = torch_cuda
+    w = make_workload("cfg3")
+    r_c = math.sqrt(-math.log(w.meta["delta"])) / w.alpha
+    plan = enuf.Plan.auto(w.N, w.L, w.meta["delta"], r_c, sigma=w.sigma, m=w.m, window=w.window,
+                          slater_lambda=w.slater_lambda, dtype=torch.float32)
+    assert plan.get(enuf.GET_K_CUT) == w.k_cut and plan.get(enuf.GET_M) == w.M
+    E, F = plan.energy_forces(torch.from_numpy(w.r).cuda(), torch.from_numpy(w.q).cuda())
+    ref = oracle.enuf_workload(w)
+    assert abs(E - ref["E"]) <= F32_E * abs(ref["E"]) and rel_rms(F.cpu().numpy(), ref["F"]) <= F32_F
+    plan.close()
+
+
 # ------------------------------------------------------------------ edge cases
 
 def test_empty_and_neutral_inputs(enuf, torch_cuda):
