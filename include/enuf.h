@@ -57,6 +57,10 @@ enum enuf_option {
     ENUF_OPT_KEEP_SPECTRUM = 7,  /* 1: also store S~(n) so enuf_plan_structure_factor() can read it  */
     ENUF_OPT_SPREAD_ZCHUNK = 8,  /* tuning: grid planes per spreading CTA (integer, 1..n);
                                     default fills the SMs several times over                         */
+    ENUF_OPT_PDL = 10,           /* 1 (default): the kernels of an evaluation are launched with programmatic
+                                    dependent launch -- each may be scheduled while its predecessor still runs
+                                    and waits for it on the device (griddepcontrol), which hides the launch
+                                    latency between the 11 kernels; 0: plain stream order                  */
     ENUF_OPT_CUDA_GRAPH = 9      /* 1: the launches of one evaluation are captured into a CUDA graph
                                     the second time the same (r, q, F) pointers and N are passed, and
                                     replayed while they stay the same (an MD loop that updates r in

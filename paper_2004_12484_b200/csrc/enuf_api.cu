@@ -576,6 +576,9 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
         case ENUF_OPT_CUDA_GRAPH:
             p->use_graph = iv != 0;
             return ENUF_OK;
+        case ENUF_OPT_PDL:
+            p->pdl = iv != 0;
+            return ENUF_OK;
         case ENUF_OPT_SPREAD_ZCHUNK:
             if (iv < 1 || iv > p->n) return fail(ENUF_EINVAL, "zchunk must be an integer in [1, n]");
             p->zchunk = iv; p->zchunk_user = true;

@@ -50,6 +50,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict__ F, int64_t N,
                  double L, TileGeom g, uint32_t* __restrict__ count, uint32_t* __restrict__ scan_epoch) {
+    pdl_prologue();
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     if (j == 0) scan_epoch[0] += 1u;    // the epoch of this evaluation's scan: kept on the device so that a
@@ -73,6 +74,7 @@ constexpr int kScanChunk = 4 * kScanThreads;
 
 static __global__ void __launch_bounds__(kScanThreads)
 bin_scan_totals_kernel(const uint32_t* __restrict__ count, int nbins, uint32_t* __restrict__ total) {
+    pdl_prologue();
     __shared__ uint32_t ws[kScanThreads / 32];
     const int i0 = blockIdx.x * kScanChunk + threadIdx.x * 4;
     uint32_t v = 0;
@@ -93,6 +95,7 @@ bin_scan_totals_kernel(const uint32_t* __restrict__ count, int nbins, uint32_t* 
 static __global__ void __launch_bounds__(kScanThreads)
 bin_scan_apply_kernel(uint32_t* __restrict__ count, int nbins, const uint32_t* __restrict__ total,
                       uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor) {
+    pdl_prologue();
     __shared__ uint32_t ws[kScanThreads / 32];
     __shared__ uint32_t base_s;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -150,6 +153,7 @@ static __global__ void __launch_bounds__(kScanThreads)
 bin_scan_single_kernel(uint32_t* __restrict__ count, int nbins, unsigned long long* __restrict__ desc,
                        const uint32_t* __restrict__ scan_epoch, uint32_t* __restrict__ offset,
                        uint32_t* __restrict__ cursor) {
+    pdl_prologue();
     __shared__ uint32_t ws[kScanThreads / 32];
     __shared__ uint32_t base_s;
     const uint32_t epoch = scan_epoch[0];             // advanced by bin_count_kernel of this evaluation
@@ -213,6 +217,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, double L, TileGeom g,
                    uint32_t* __restrict__ cursor, PSlot<T>* __restrict__ slots) {
+    pdl_prologue();
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     T qj = q[j];
@@ -237,6 +242,7 @@ template <typename T, int M_, bool kTrim>
 __global__ void __launch_bounds__(kRowsThreads)
 window_rows_kernel(const PSlot<T>* __restrict__ slots, const uint32_t* __restrict__ offset, int nbins, WindowParams wp,
                    const __grid_constant__ PolyArg<M_> pa, T* __restrict__ rows) {
+    pdl_prologue();
     using R = WindowRows<M_, kTrim>;
     using V4 = typename Vec4<T>::type;
     constexpr int SP = R::RP + 4;                                  // 44 / 52 elements: conflict-free 16-byte accesses

@@ -99,6 +99,19 @@ __host__ __device__ inline void unpack_cell(uint32_t p, int& cx, int& cy, int& c
     cx = p & 1023u; cy = (p >> 10) & 1023u; cz = (p >> 20) & 1023u;
 }
 
+// ---------------------------------------------------------------- programmatic dependent launch
+// First statement of every hot-path kernel.  When the kernel was launched with the programmatic-stream-serialization
+// attribute (enuf_launch.cuh, pdl_launch) its CTAs may be scheduled while the preceding kernel still runs: `wait` then
+// blocks until that kernel has completed and its memory is visible, so nothing of this kernel's reads or writes moves
+// ahead of it -- only the launch latency and the CTA start-up overlap.  `launch_dependents` lets the NEXT kernel in the
+// stream do the same with this one; that kernel starts only once every CTA of this one has issued it (i.e. is resident
+// or done), so a waiting dependent never keeps a CTA of this grid off the machine (the single-launch scan relies on
+// all of its CTAs being resident).  Without the attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_prologue() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // ---------------------------------------------------------------- mbarrier (shared::cta) wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {

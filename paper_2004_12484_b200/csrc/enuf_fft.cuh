@@ -170,6 +170,7 @@ struct FftGeom {
 template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_x_forward_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    pdl_prologue();
     using S = FftShape<N, -1>;
     static_assert(S::TPL <= 32, "a line must fit in one warp");
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
@@ -222,6 +223,7 @@ fft_x_forward_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg
 template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_x_inverse_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    pdl_prologue();
     using S = FftShape<N, +1>;
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -279,6 +281,7 @@ template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_x_forward_tma_kernel(const T* __restrict__ G, Cx<T>* __restrict__ A1, FftGeom fg, const Cx<T>* __restrict__ tw,
                          int ntiles) {
+    pdl_prologue();
     using S = FftShape<N, -1>;
     static_assert(S::TPL <= 32, "a line must fit in one warp");
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>(), SP = fft_xf_stage_pitch<T, N>();
@@ -359,6 +362,7 @@ template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_x_inverse_tma_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeom fg, const Cx<T>* __restrict__ tw,
                          int ntiles) {
+    pdl_prologue();
     using S = FftShape<N, +1>;
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -423,6 +427,7 @@ fft_x_inverse_tma_kernel(const Cx<T>* __restrict__ A1, T* __restrict__ G, FftGeo
 template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_y_forward_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    pdl_prologue();
     using S = FftShape<N, -1>;
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -458,6 +463,7 @@ fft_y_forward_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, FftGe
 template <typename T, int N>
 __global__ void __launch_bounds__(kFftThreads)
 fft_y_inverse_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, FftGeom fg, const Cx<T>* __restrict__ tw) {
+    pdl_prologue();
     using S = FftShape<N, +1>;
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -536,6 +542,7 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
                    const Cx<T>* __restrict__ tw, ScaleTables st, double* __restrict__ e_partial,
                    Cx<T>* __restrict__ spectrum, unsigned* __restrict__ done_count, double e_scale,
                    double* __restrict__ e_out) {
+    pdl_prologue();
     using SF = FftShape<N, -1>;
     using SI = FftShape<N, +1>;
     constexpr int LPC = fft_lines_per_cta<N>(), PITCH = fft_line_pitch<N>();

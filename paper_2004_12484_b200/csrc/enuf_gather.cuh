@@ -88,6 +88,7 @@ __global__ void __launch_bounds__(GatherCfg<M_, kTrim>::NT)
 gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
               const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F) {
+    pdl_prologue();
     using C = GatherCfg<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
     constexpr int W = C::W, WE = C::WE, TP = C::TP, SX = C::SX, SPL = C::SPL, PBW = C::PBW, ITER = C::ITER, WP = C::WP;

@@ -67,6 +67,20 @@ static inline bool launch_ok(enuf_plan* p) {
     return e == cudaSuccess;
 }
 
+// Launch with the programmatic-stream-serialization attribute (unless the plan has it switched off): the kernel's CTAs
+// may be scheduled while the preceding kernel of the stream still runs and wait in pdl_prologue() (enuf_common.cuh).
+template <typename... KArgs, typename... Args>
+static inline void pdl_launch(const enuf_plan* p, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                              cudaStream_t s, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = p->pdl ? 1 : 0;
+    (void)cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 template <typename K>
 static inline bool set_smem(K kernel, size_t bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
@@ -126,20 +140,20 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     p->bin_count_clean = false;
     const unsigned blocks = (unsigned)((N + 255) / 256);
     const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
-    bin_count_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q),
+    pdl_launch(p, bin_count_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q),
                                                static_cast<T*>(F), N, p->L, p->tg, p->bin_count, p->scan_epoch);
     int nlaunch = 4;
     if ((int)sblocks <= kScanMaxResident && (int)sblocks <= p->num_sms) {
         // every scan CTA is resident at once: one launch, chunk totals exchanged through scan_desc
-        bin_scan_single_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_desc, p->scan_epoch,
+        pdl_launch(p, bin_scan_single_kernel, sblocks, kScanThreads, 0, s, p->bin_count, nbins, p->scan_desc, p->scan_epoch,
                                                                 p->bin_offset, p->bin_cursor);
         nlaunch = 3;
     } else {
-        bin_scan_totals_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total);
-        bin_scan_apply_kernel<<<sblocks, kScanThreads, 0, s>>>(p->bin_count, nbins, p->scan_total, p->bin_offset,
+        pdl_launch(p, bin_scan_totals_kernel, sblocks, kScanThreads, 0, s, p->bin_count, nbins, p->scan_total);
+        pdl_launch(p, bin_scan_apply_kernel, sblocks, kScanThreads, 0, s, p->bin_count, nbins, p->scan_total, p->bin_offset,
                                                               p->bin_cursor);
     }
-    bin_scatter_kernel<T><<<blocks, 256, 0, s>>>(static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
+    pdl_launch(p, bin_scatter_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
                                                  p->tg, p->bin_cursor, static_cast<PSlot<T>*>(p->rec));
     // window rows of the sorted particles (read by the spreading kernel); N bounds the number of charged particles
     const unsigned rblocks = (unsigned)((N + 31) / 32);
@@ -148,12 +162,12 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
         const PolyArg<M_> pa = make_poly_arg<M_>(p);
         if constexpr (M_ >= 5 && sizeof(T) == 4) {
             if (p->trim) {
-                window_rows_kernel<T, M_, true><<<rblocks, kRowsThreads, 0, s>>>(
+                pdl_launch(p, window_rows_kernel<T, M_, true>, rblocks, kRowsThreads, 0, s, 
                     static_cast<const PSlot<T>*>(p->rec), p->bin_offset, nbins, p->wp, pa, static_cast<T*>(p->rows));
                 return 0;
             }
         }
-        window_rows_kernel<T, M_, false><<<rblocks, kRowsThreads, 0, s>>>(
+        pdl_launch(p, window_rows_kernel<T, M_, false>, rblocks, kRowsThreads, 0, s, 
             static_cast<const PSlot<T>*>(p->rec), p->bin_offset, nbins, p->wp, pa, static_cast<T*>(p->rows));
         return 0;
     });
@@ -174,7 +188,7 @@ int launch_spread(enuf_plan* p) {
                 constexpr bool kTrim = decltype(trim_c)::value != 0;
                 using C = SpreadCfg<T, M_, kTrim, NPX>;
                 const dim3 grid((unsigned)((p->n / C::CX) * (p->n / C::CY)), (unsigned)((p->n + p->zchunk - 1) / p->zchunk));
-                spread_kernel<T, M_, kTrim, NPX><<<grid, C::NT, spread_smem_bytes<T, M_, kTrim, NPX>(), s>>>(
+                pdl_launch(p, spread_kernel<T, M_, kTrim, NPX>, grid, C::NT, spread_smem_bytes<T, M_, kTrim, NPX>(), s, 
                     static_cast<const PSlot<T>*>(p->rec), static_cast<const T*>(p->rows), p->bin_offset, p->tg,
                     p->zchunk, static_cast<T*>(p->grid[0]));
                 return 0;
@@ -209,10 +223,10 @@ int launch_fft_forward(enuf_plan* p) {
             const int per_sm = (int)((size_t)(227 * 1024) / (sbt + 1024));
             const int ntiles = (int)(bx / 2);
             const int gridx = ntiles < p->num_sms * per_sm ? ntiles : p->num_sms * per_sm;
-            fft_x_forward_tma_kernel<T, N_><<<gridx, kFftThreads, sbt, s>>>(static_cast<const T*>(p->grid[0]),
+            pdl_launch(p, fft_x_forward_tma_kernel<T, N_>, gridx, kFftThreads, sbt, s, static_cast<const T*>(p->grid[0]),
                                                                            static_cast<Cx<T>*>(p->A1[0]), fg, tw, ntiles);
         }
-        fft_y_forward_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A1[0]),
+        pdl_launch(p, fft_y_forward_kernel<T, N_>, by, kFftThreads, sb, s, static_cast<const Cx<T>*>(p->A1[0]),
                                                                static_cast<Cx<T>*>(p->A2[0]), fg, tw);
         return 2;
     });
@@ -241,24 +255,24 @@ int launch_fft_backward(enuf_plan* p) {
         Cx<T>* spec = p->keep_spectrum ? static_cast<Cx<T>*>(p->spectrum) : nullptr;
         const double e_scale = 1.0 / (2.0 * 3.14159265358979323846 * p->L);   // Eq. 38: C/(2 pi L), C = 1
         if (nout == 1)
-            fft_z_fused_kernel<T, N_, 1><<<bz, kFftThreads, sb, s>>>(static_cast<Cx<T>*>(p->A2[0]), nullptr, nullptr,
+            pdl_launch(p, fft_z_fused_kernel<T, N_, 1>, bz, kFftThreads, sb, s, static_cast<Cx<T>*>(p->A2[0]), nullptr, nullptr,
                                                                     fg, tw, st, p->e_partial, spec, p->fft_done,
                                                                     e_scale, p->e_dev);
         else
-            fft_z_fused_kernel<T, N_, 3><<<bz, kFftThreads, sb, s>>>(static_cast<Cx<T>*>(p->A2[0]),
+            pdl_launch(p, fft_z_fused_kernel<T, N_, 3>, bz, kFftThreads, sb, s, static_cast<Cx<T>*>(p->A2[0]),
                                                                     static_cast<Cx<T>*>(p->A2[1]),
                                                                     static_cast<Cx<T>*>(p->A2[2]), fg, tw, st,
                                                                     p->e_partial, spec, p->fft_done, e_scale, p->e_dev);
         launches = 1;
         for (int d = 0; d < nout; ++d) {
-            fft_y_inverse_kernel<T, N_><<<by, kFftThreads, sb, s>>>(static_cast<const Cx<T>*>(p->A2[d]),
+            pdl_launch(p, fft_y_inverse_kernel<T, N_>, by, kFftThreads, sb, s, static_cast<const Cx<T>*>(p->A2[d]),
                                                                    static_cast<Cx<T>*>(p->A1[d]), fg, tw);
             {
                 const size_t sbt = fft_xi_tma_smem_bytes<T, N_>(p->Kxp);
                 const int per_sm = (int)((size_t)(227 * 1024) / (sbt + 1024));
                 const int ntiles = (int)(bx / 2);
                 const int cap = p->num_sms * (per_sm < 4 ? per_sm : 4);
-                fft_x_inverse_tma_kernel<T, N_><<<ntiles < cap ? ntiles : cap, kFftThreads, sbt, s>>>(
+                pdl_launch(p, fft_x_inverse_tma_kernel<T, N_>, ntiles < cap ? ntiles : cap, kFftThreads, sbt, s, 
                     static_cast<const Cx<T>*>(p->A1[d]), static_cast<T*>(p->grid[d]), fg, tw, ntiles);
             }
             launches += 2;
@@ -291,14 +305,14 @@ int launch_gather(enuf_plan* p, void* F) {
             const size_t sb = gather_smem_bytes<T, M_, kTrim>();
             if (p->variant == ENUF_FORCE_ANALYTIC) {
                 const T pre = (T)(-(double)p->n / (PI * p->L * p->L));
-                gather_kernel<T, M_, false, kTrim><<<ntiles, C::NT, sb, s>>>(
+                pdl_launch(p, gather_kernel<T, M_, false, kTrim>, ntiles, C::NT, sb, s, 
                     static_cast<const T*>(p->grid[0]), static_cast<const PSlot<T>*>(p->rec),
                     p->bin_offset, p->tg, p->wp, pa, pre, 0, static_cast<T*>(F));
                 return 1;
             }
             const T pre = (T)(2.0 / (p->L * p->L));
             for (int d = 0; d < 3; ++d)
-                gather_kernel<T, M_, true, kTrim><<<ntiles, C::NT, sb, s>>>(
+                pdl_launch(p, gather_kernel<T, M_, true, kTrim>, ntiles, C::NT, sb, s, 
                     static_cast<const T*>(p->grid[d]), static_cast<const PSlot<T>*>(p->rec),
                     p->bin_offset, p->tg, p->wp, pa, pre, d, static_cast<T*>(F));
             return 3;

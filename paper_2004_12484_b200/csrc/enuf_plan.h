@@ -15,6 +15,7 @@ struct enuf_plan {
     int precision = ENUF_F32, window = ENUF_WINDOW_KAISER_BESSEL, variant = ENUF_FORCE_ANALYTIC;
     double lambda = 0.0;
     bool profile = false, keep_spectrum = false;
+    bool pdl = true;               // ENUF_OPT_PDL: programmatic dependent launch of the hot-path kernels
     bool trim = false;             // fp32 Kaiser-Bessel m >= 5: kernels visit 2m stencil points per dimension
     cudaStream_t stream = nullptr;
     // ENUF_OPT_CUDA_GRAPH: one evaluation's launches, captured on cap_stream, replayed on `stream`

@@ -198,6 +198,7 @@ template <typename T, int M_, bool kTrim, int NPX>
 __global__ void __launch_bounds__((SpreadCfg<T, M_, kTrim, NPX>::NT), (SpreadCfg<T, M_, kTrim, NPX>::CTAS_PER_SM))
 spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
               const uint32_t* __restrict__ offset, TileGeom g, int zchunk, T* __restrict__ grid) {
+    pdl_prologue();
     using C = SpreadCfg<T, M_, kTrim, NPX>;
     using R = WindowRows<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
