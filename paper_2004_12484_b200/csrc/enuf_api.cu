@@ -255,7 +255,7 @@ void drop_graph(enuf_plan* p) {
 void free_workspace(enuf_plan* p) {
     drop_graph(p);
     auto fr = [](void* q) { if (q) cudaFree(q); };
-    fr(p->rec); fr(p->rows); p->rows = nullptr; fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
+    fr(p->rec); fr(p->rows); p->rows = nullptr; fr(p->binrank); p->binrank = nullptr; fr(p->bin_count); fr(p->bin_offset); fr(p->bin_cursor);
     fr(p->scan_total); fr(p->scan_desc); p->scan_desc = nullptr; fr(p->scan_epoch); p->scan_epoch = nullptr;
     for (int d = 0; d < 3; ++d) { fr(p->grid[d]); fr(p->A1[d]); fr(p->A2[d]); p->grid[d] = p->A1[d] = p->A2[d] = nullptr; }
     fr(p->spectrum); fr(p->tw); fr(p->iphi); fr(p->wf); fr(p->e_partial); fr(p->e_dev); fr(p->fft_done);
@@ -332,6 +332,7 @@ int ensure_allocated(enuf_plan* p) {
     ALLOC(p->bin_count, 4 * (size_t)p->tg.nbins);
     ALLOC(p->bin_offset, 4 * ((size_t)p->tg.nbins + 1));
     ALLOC(p->bin_cursor, 4 * (size_t)p->tg.nbins);
+    ALLOC(p->binrank, 8 * cap);
     ALLOC(p->scan_total, 4 * (((size_t)p->tg.nbins + 1023) / 1024));
     ALLOC(p->scan_desc, 8 * (((size_t)p->tg.nbins + 1023) / 1024));
     ALLOC(p->scan_epoch, 4);

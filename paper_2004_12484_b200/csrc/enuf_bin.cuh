@@ -45,11 +45,14 @@ __device__ __forceinline__ int bin_of(const CellOfParticle& p, const TileGeom& g
     return bin_index(g, p.c[0] / kTile, p.c[1] / kTile, bz);
 }
 
-// Histogram of charged particles per bin; neutral particles get F = 0 here and are dropped.
+// Histogram of charged particles per bin; neutral particles get F = 0 here and are dropped.  The histogram atomic
+// returns the particle's rank inside its bin: (bin, rank) is kept per particle, so that the scatter needs no atomic.
+constexpr uint32_t kNoBin = 0xffffffffu;
 template <typename T>
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict__ F, int64_t N,
-                 double L, TileGeom g, uint32_t* __restrict__ count, uint32_t* __restrict__ scan_epoch) {
+                 double L, TileGeom g, uint32_t* __restrict__ count, uint32_t* __restrict__ scan_epoch,
+                 uint2* __restrict__ binrank) {
     pdl_prologue();
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
@@ -57,10 +60,12 @@ bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict
                                         // replayed CUDA graph (ENUF_OPT_CUDA_GRAPH) advances it as well
     if (q[j] == (T)0) {
         F[3 * j] = (T)0; F[3 * j + 1] = (T)0; F[3 * j + 2] = (T)0;
+        binrank[j] = make_uint2(kNoBin, 0u);
         return;
     }
     CellOfParticle p = locate(r, j, L, g.n);
-    atomicAdd(&count[bin_of<T>(p, g)], 1u);
+    const uint32_t b = (uint32_t)bin_of<T>(p, g);
+    binrank[j] = make_uint2(b, atomicAdd(&count[b], 1u));
 }
 
 // Exclusive scan of count[0..nbins) into offset[0..nbins] (and a copy in cursor[0..nbins),
@@ -210,20 +215,22 @@ bin_scan_single_kernel(uint32_t* __restrict__ count, int nbins, unsigned long lo
     if (i0 <= nbins - 1 && nbins - 1 < i0 + 4) offset[nbins] = run;   // thread owning the last bin
 }
 
-// Scatter into bin order.  The order inside a bin follows the atomic cursor (any order is
-// a valid sort; sums downstream differ only in rounding order, R22).  Bits 30 / 31 of the packed cell carry
+// Scatter into bin order: position = offset[bin] + rank, both from the count pass (no atomic here).  The order inside
+// a bin is the arrival order at the histogram (any order is a valid sort; sums downstream differ only in rounding
+// order, R22).  Bits 30 / 31 of the packed cell carry
 // ks_x / ks_y = (d0 > 0) of the trimmed stencils (the spreading producer culls on the cell word alone).
 template <typename T>
 __global__ void __launch_bounds__(256)
 bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, double L, TileGeom g,
-                   uint32_t* __restrict__ cursor, PSlot<T>* __restrict__ slots) {
+                   const uint32_t* __restrict__ offset, const uint2* __restrict__ binrank, PSlot<T>* __restrict__ slots) {
     pdl_prologue();
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
-    T qj = q[j];
-    if (qj == (T)0) return;
+    const uint2 br = binrank[j];
+    if (br.x == kNoBin) return;
+    const T qj = q[j];
     CellOfParticle p = locate(r, j, L, g.n);
-    uint32_t pos = atomicAdd(&cursor[bin_of<T>(p, g)], 1u);
+    const uint32_t pos = offset[br.x] + br.y;
     PSlot<T> o;
     o.rec.dx = (T)p.d0[0]; o.rec.dy = (T)p.d0[1]; o.rec.dz = (T)p.d0[2]; o.rec.q = qj;
     const uint32_t ksx = (g.trim && o.rec.dx > (T)0) ? 1u : 0u, ksy = (g.trim && o.rec.dy > (T)0) ? 1u : 0u;

@@ -141,7 +141,7 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     const unsigned blocks = (unsigned)((N + 255) / 256);
     const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
     pdl_launch(p, bin_count_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q),
-                                               static_cast<T*>(F), N, p->L, p->tg, p->bin_count, p->scan_epoch);
+                                               static_cast<T*>(F), N, p->L, p->tg, p->bin_count, p->scan_epoch, p->binrank);
     int nlaunch = 4;
     if ((int)sblocks <= kScanMaxResident && (int)sblocks <= p->num_sms) {
         // every scan CTA is resident at once: one launch, chunk totals exchanged through scan_desc
@@ -154,7 +154,7 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
                                                               p->bin_cursor);
     }
     pdl_launch(p, bin_scatter_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
-                                                 p->tg, p->bin_cursor, static_cast<PSlot<T>*>(p->rec));
+                                                 p->tg, p->bin_offset, p->binrank, static_cast<PSlot<T>*>(p->rec));
     // window rows of the sorted particles (read by the spreading kernel); N bounds the number of charged particles
     const unsigned rblocks = (unsigned)((N + 31) / 32);
     const int rc = dispatch_m(p, [&](auto mc) -> int {

@@ -45,6 +45,7 @@ struct enuf_plan {
     uint32_t* bin_count = nullptr;    // [nbins]
     uint32_t* bin_offset = nullptr;   // [nbins+1]
     uint32_t* bin_cursor = nullptr;   // [nbins]
+    uint2* binrank = nullptr;         // [N_cap] (bin, rank inside the bin) of every particle, from the count pass
     uint32_t* scan_total = nullptr;   // [ceil(nbins / kScanChunk)]
     unsigned long long* scan_desc = nullptr;   // [ceil(nbins / kScanChunk)] (epoch << 32 | chunk total), single-launch scan
     uint32_t* scan_epoch = nullptr;            // [1] device word: evaluation counter, the epoch of scan_desc

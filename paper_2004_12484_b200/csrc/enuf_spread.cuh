@@ -486,24 +486,26 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             // one visit ahead: while visit i is accumulated, the operands of visit i + 1 and the entry of visit i + 2 are
             // in flight.  Two visits per trip (A, B alternate, no register moves); the list is padded with entries that
             // point at the all-zero slot: to an even length, and two more for the loads that run ahead.
-            Ops A = load_ops(sbx, sby, sbz, lds_u2(lp));
-            uint2 en = lds_u2(lp + 8);
-            for (int i = 0; i < cnt; i += 2) {
-                const Ops B = load_ops(sbx, sby, sbz, en);
-                en = lds_u2(lp + 8 * (uint32_t)(i + 2));
-                {
-                    const P2 a = pair_scale(A.wx, A.wy);
-                    const T* wz = reinterpret_cast<const T*>(A.z);
+            if (cnt > 0) {                                          // (sparse systems: most patches see no particle in a slab)
+                Ops A = load_ops(sbx, sby, sbz, lds_u2(lp));
+                uint2 en = lds_u2(lp + 8);
+                for (int i = 0; i < cnt; i += 2) {
+                    const Ops B = load_ops(sbx, sby, sbz, en);
+                    en = lds_u2(lp + 8 * (uint32_t)(i + 2));
+                    {
+                        const P2 a = pair_scale(A.wx, A.wy);
+                        const T* wz = reinterpret_cast<const T*>(A.z);
 #pragma unroll
-                    for (int kk = 0; kk < WZ; ++kk) fma_pair(acc[kk], a, wz[kk]);
-                }
-                A = load_ops(sbx, sby, sbz, en);
-                en = lds_u2(lp + 8 * (uint32_t)(i + 3));
-                {
-                    const P2 a = pair_scale(B.wx, B.wy);
-                    const T* wz = reinterpret_cast<const T*>(B.z);
+                        for (int kk = 0; kk < WZ; ++kk) fma_pair(acc[kk], a, wz[kk]);
+                    }
+                    A = load_ops(sbx, sby, sbz, en);
+                    en = lds_u2(lp + 8 * (uint32_t)(i + 3));
+                    {
+                        const P2 a = pair_scale(B.wx, B.wy);
+                        const T* wz = reinterpret_cast<const T*>(B.z);
 #pragma unroll
-                    for (int kk = 0; kk < WZ; ++kk) fma_pair(acc[kk], a, wz[kk]);
+                        for (int kk = 0; kk < WZ; ++kk) fma_pair(acc[kk], a, wz[kk]);
+                    }
                 }
             }
             __syncwarp();
