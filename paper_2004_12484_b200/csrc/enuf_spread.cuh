@@ -9,12 +9,12 @@
 //     acc[k] += (a0, a1) * (q wz[k]) with (a0, a1) = wx[cells] * wy[cell].  After slab s the lowest plane
 //     of the window is complete: one coalesced store, and the window slides.  Every grid value is written
 //     exactly once -- no atomics, no clearing of the grid, no shared-memory read-modify-write;
-//   - four PRODUCER warps taking the slabs in turn, two sharing each stage of a two-stage buffer in shared memory:
+//   - four PRODUCER warps taking the slabs in turn (slab i of the chunk goes to stage i % 3 of a three-stage ring):
 //     a producer culls the particles of the neighbouring bins against the column's halo, copies the three
-//     window rows of the accepted ones (3 x 16 values, evaluated ONCE per particle by the bin scatter --
+//     window rows of the accepted ones (evaluated ONCE per particle by window_rows_kernel, enuf_bin.cuh --
 //     "window values computed [once and kept]") into slots of its stage with cp.async, builds
 //     for every patch the list of staged particles whose stencil overlaps it, and hands the stage over
-//     through an mbarrier (full / empty pair per stage; the copies arrive on the full barrier themselves).
+//     through mbarriers (full / empty / again per producer; the copies arrive on the full barrier themselves).
 //     The consumers never meet at a CTA-wide barrier: each waits only for the producers, and hands a
 //     stage back when its own visits are done.
 //
