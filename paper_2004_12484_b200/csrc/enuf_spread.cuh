@@ -274,6 +274,30 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
         uint32_t (*rg)[2 * kBlk] = rng[k];
         unsigned pe = 0, pa = 0;                 // parities of the next phase of empty_bar[(k + 1) & 3] / again_bar[k] to wait for
         int blk0 = s_begin + k - C::NPROD * kBlk;
+        // candidates of a slab: the ranges of the NSEG segments, 32 per step.  The cell words of up to kSteps steps are
+        // loaded together (one global-load latency per slab, not one per step), then examined in order; those of the
+        // producer's NEXT slab are started as soon as the current slab is culled, so that they arrive during the
+        // hand-over, the lists and the copies.
+        constexpr int kSteps = 8;
+        int sg = 0;
+        uint32_t gs = 0, ge = 0;
+        uint32_t cw[kSteps], cbase[kSteps];
+        int nst = 0;                             // steps loaded (consumed ones are marked invalid)
+        bool preloaded = false;                  // cw / cbase already hold the first steps of this slab
+        auto load_steps = [&](int js) {
+            nst = 0;
+#pragma unroll
+            for (int j = 0; j < kSteps; ++j) {
+                while (gs >= ge && sg < NSEG) { gs = rg[sg][js]; ge = rg[sg][kBlk + js]; ++sg; }
+                cbase[j] = gs;
+                cw[j] = 0xffffffffu;
+                if (gs < ge) {
+                    if (gs + (uint32_t)lane < ge) cw[j] = slots[gs + (uint32_t)lane].cell;
+                    gs += 32u;
+                    nst = j + 1;
+                }
+            }
+        };
         for (int s = s_begin + k; s < s_end; s += C::NPROD) {
             if (s - blk0 >= C::NPROD * kBlk) {
                 // ranges of this producer's next kBlk slabs: lane & 15 = slab, lanes 0..15 load the starts, 16..31 the ends
@@ -292,28 +316,8 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             unsigned char* sbase = smem_raw + (size_t)stage * C::STAGE_BYTES;
             const uint32_t sl32 = smem_u32(sbase);
             uint2* lists = reinterpret_cast<uint2*>(sbase + C::SLOT_BYTES);
-            // candidates: the ranges of the NSEG segments, 32 per step.  The cell words of up to kSteps steps are
-            // loaded together (one global-load latency per slab, not one per step), then examined in order.
-            constexpr int kSteps = 8;
-            int sg = 0;
-            uint32_t gs = 0, ge = 0;
-            uint32_t cw[kSteps], cbase[kSteps];
-            int nst = 0;                         // steps loaded (consumed ones are marked invalid)
-            auto load_steps = [&]() {
-                nst = 0;
-#pragma unroll
-                for (int j = 0; j < kSteps; ++j) {
-                    while (gs >= ge && sg < NSEG) { gs = rg[sg][js]; ge = rg[sg][kBlk + js]; ++sg; }
-                    cbase[j] = gs;
-                    cw[j] = 0xffffffffu;
-                    if (gs < ge) {
-                        if (gs + (uint32_t)lane < ge) cw[j] = slots[gs + (uint32_t)lane].cell;
-                        gs += 32u;
-                        nst = j + 1;
-                    }
-                }
-            };
-            load_steps();
+            if (!preloaded) { sg = 0; gs = 0; ge = 0; load_steps(js); }
+            preloaded = false;
             bool slab_done = false, first_round = true;
             while (!slab_done) {
                 // ---- cull (before the stage is free: it needs only this producer's side buffer): accepted particles'
@@ -365,8 +369,13 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     ns = base;
                     if (jl < kSteps) break;                            // step jl opens the next round of this slab
                     if (nst < kSteps) { slab_done = true; break; }     // the ranges are exhausted
-                    load_steps();                                      // a long slab: the next kSteps steps
+                    load_steps(js);                                    // a long slab: the next kSteps steps
                     if (nst == 0) { slab_done = true; break; }
+                }
+                if (slab_done && s + C::NPROD < s_end && js + 1 < kBlk) {
+                    sg = 0; gs = 0; ge = 0;
+                    load_steps(js + 1);                                // the next slab of this producer (same block of ranges)
+                    preloaded = true;
                 }
                 __syncwarp();
                 ENUF_TR((s - s_begin) * 16 + 1, trace_clock());
@@ -404,17 +413,14 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     }
                 }
                 ENUF_TR((s - s_begin) * 16 + 13, trace_clock());
-                if (lane == 0) {
+                if (lane < NCONS) {                                        // lane w8 closes list w8
                     const unsigned zs = (unsigned)(CAP * PITCH) * ES;      // the all-zero slot
-#pragma unroll
-                    for (int w8 = 0; w8 < NCONS; ++w8) {
-                        const int c = (int)((lcp[w8 >> 2] >> (8 * (w8 & 3))) & 255u);
-                        // even length, and the consumer loads its operands one visit ahead: entries that point at the zero slot
-                        lists[w8 * LCAP + c] = lists[w8 * LCAP + c + 1] = lists[w8 * LCAP + c + 2] =
-                            make_uint2((zs + OXF * ES) | ((zs + OZF * ES) << 16), zs + OYF * ES);
-                        cnt_s[stage][w8] = c + (c & 1);
-                    }
-                    last_s[stage] = slab_done ? 1 : 0;
+                    const int c = (int)(((lane < 4 ? lcp[0] : lcp[1]) >> (8 * (lane & 3))) & 255u);
+                    // even length, and the consumer loads its operands one visit ahead: entries that point at the zero slot
+                    lists[lane * LCAP + c] = lists[lane * LCAP + c + 1] = lists[lane * LCAP + c + 2] =
+                        make_uint2((zs + OXF * ES) | ((zs + OZF * ES) << 16), zs + OYF * ES);
+                    cnt_s[stage][lane] = c + (c & 1);
+                    if (lane == 0) last_s[stage] = slab_done ? 1 : 0;
                 }
                 // ---- copy the window rows of the accepted particles into the slots (cp.async; they arrive on full_bar themselves)
                 for (int g0 = 0; g0 < ns; g0 += 32) {
