@@ -444,6 +444,15 @@ def run_ours(args):
                     "algorithmic_flops": flops, "events_averaged": n_prof,
                     "hbm": {"achieved": stages[dom]["GBps"], "peak": peak, "unit": "GB/s",
                             "frac": stages[dom]["hbm_frac"], "peak_source": peak_src}}
+        # what binds both kernels in practice is the shared-memory data pipe (one 128-byte wavefront per SM and clock;
+        # ncu l1tex 67-79 %).  Algorithmic wavefronts: every stencil value of every particle crosses
+        # it once -- the gather reads (2m+1)^3 field values per particle (32 words per wavefront); the spread's
+        # register accumulation needs its window values: (2m+1)^2 (x, y) products + (2m+1) z values per particle.
+        smem_peak = 148 * sm_max * 1e6
+        wf = n_charged * (W3 / 32.0 if dom == "gather" else ((2 * w.m + 1) ** 2 + (2 * w.m + 1)) / 32.0)
+        roofline["smem_pipe"] = {"algorithmic_wavefronts": wf, "achieved": wf / (stages[dom]["ms"] * 1e-3),
+                                 "peak": smem_peak, "unit": "wavefronts/s", "frac": wf / (stages[dom]["ms"] * 1e-3) / smem_peak,
+                                 "peak_source": "148 SMs x 1 wavefront per clock x clocks.max.sm (B300_MICROARCH.md: 128 B/clk/SM)"}
     else:
         roofline = {"bound": "hbm", "kernel": dom, "achieved": stages[dom]["GBps"], "peak": peak, "unit": "GB/s",
                     "frac": stages[dom]["hbm_frac"], "traffic": recorded_traffic(dom), "peak_source": peak_src,
