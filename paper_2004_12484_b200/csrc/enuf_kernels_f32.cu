@@ -12,9 +12,3 @@ template int launch_fft_backward<float>(enuf_plan*);
 template int launch_gather<float>(enuf_plan*, void*);
 template int launch_real<float>(enuf_plan*, const void*, const void*, double, int, void*);
 }  // namespace enuf
-
-#ifdef ENUF_TRACE
-extern "C" int enuf_debug_spread_trace(long long* out, int n) {
-    return (int)cudaMemcpyFromSymbol(out, enuf::g_spread_trace, sizeof(long long) * (size_t)n);
-}
-#endif

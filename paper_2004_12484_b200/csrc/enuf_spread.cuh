@@ -183,15 +183,6 @@ __device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-#ifdef ENUF_TRACE
-// debugging aid (never defined in the product build): time stamps of one CTA's producers and two of its consumers
-__device__ long long g_spread_trace[16384];
-__device__ __forceinline__ long long trace_clock() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define ENUF_TR(slot, val) do { if (tr_on && lane == 0) g_spread_trace[(slot)] = (val); } while (0)
-#else
-#define ENUF_TR(slot, val) do { } while (0)
-#endif
-
 // slots[].cell: bits 0..29 the packed nearest cell, bits 30 / 31 = ks_x / ks_y (trimmed plans; enuf_bin.cuh)
 // rows: [N][RP] window rows in bin order (WindowRows)
 template <typename T, int M_, bool kTrim, int NPX>
@@ -227,9 +218,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     const int Tx = blockIdx.x % ncolx, Ty = blockIdx.x / ncolx;
     const int z0 = blockIdx.y * zchunk, z1 = min(g.n, z0 + zchunk);
     const int s_begin = z0 - C::SLO, s_end = z1 + C::SHI;
-#ifdef ENUF_TRACE
-    const bool tr_on = blockIdx.x == 37 && blockIdx.y == 1;
-#endif
 
     // the zero padding of every slot (and the all-zero slot CAP) is written once; rows are rewritten per round
     for (int i = tid; i < (int)(C::STAGE_BYTES * NSTAGE / 16); i += C::NT)
@@ -323,7 +311,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 // ---- cull (before the stage is free: it needs only this producer's side buffer): accepted particles'
                 //      sorted-array index and packed stencil origin; their rows are started towards L2
                 int ns = 0;
-                ENUF_TR((s - s_begin) * 16 + 0, trace_clock());
                 for (;;) {
                     // all loaded steps at once, branch-free (the steps are independent up to the running slot count);
                     // in halves, so that sparse slabs (few steps) skip the unused half
@@ -378,7 +365,35 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     preloaded = true;
                 }
                 __syncwarp();
-                ENUF_TR((s - s_begin) * 16 + 1, trace_clock());
+                // ---- visit lists, first half (still before the hand-over): for every patch the staged particles whose
+                //      stencil overlaps it (ballot + popc compaction), kept in registers -- per group of 32 slots the patch
+                //      mask, the 8 list positions (bytes of two words) and the ready-made byte offsets of the x and y rows.
+                //      (A round stages at most CAP + 1 < 256 entries per list, so list lengths are bytes of lcp[].)
+                constexpr int NGRP = (CAP + 31) / 32;
+                unsigned lcp[2] = {0u, 0u}, lmask[NGRP], lpos[NGRP][2], lxb[NGRP], lyb[NGRP];
+#pragma unroll
+                for (int gq = 0; gq < NGRP; ++gq) {
+                    lmask[gq] = 0u; lpos[gq][0] = lpos[gq][1] = 0u; lxb[gq] = lyb[gq] = 0u;
+                    if (32 * gq < ns) {
+                        const int slot = 32 * gq + lane;
+                        const bool v = slot < ns;
+                        int X0 = 64, Y0 = 64;
+                        if (v) { const int pkv = (int)acc_rec[k][slot].y; X0 = (pkv & 255) - 32; Y0 = ((pkv >> 8) & 255) - 32; }
+                        const unsigned sb = (unsigned)(slot * PITCH) * ES;
+                        lxb[gq] = sb + (unsigned)(OXF + (X0 & 1) - X0) * ES;
+                        lyb[gq] = sb + (unsigned)(OYF - Y0) * ES;
+#pragma unroll
+                        for (int w8 = 0; w8 < NCONS; ++w8) {
+                            const int px0 = 8 * (w8 % NPX), py0 = 8 * (w8 / NPX);
+                            const bool ov = v && X0 <= px0 + 7 && X0 + WZ - 1 >= px0 && Y0 <= py0 + 7 && Y0 + WZ - 1 >= py0;
+                            const unsigned bal = __ballot_sync(FULL, ov);
+                            const unsigned cur = (lcp[w8 >> 2] >> (8 * (w8 & 3))) & 255u;
+                            lmask[gq] |= ov ? (1u << w8) : 0u;
+                            lpos[gq][w8 >> 2] |= (cur + (unsigned)__popc(bal & below)) << (8 * (w8 & 3));
+                            lcp[w8 >> 2] += (unsigned)__popc(bal) << (8 * (w8 & 3));
+                        }
+                    }
+                }
                 if (first_round) {
                     // the slab that held the stage before (s - 3, staged by producer (k + 1) & 3) must be finished
                     if (s - NSTAGE >= s_begin) { mbar_wait_backoff(&empty_bar[(k + 1) & 3], pe); pe ^= 1u; }
@@ -386,33 +401,21 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 } else {
                     mbar_wait_backoff(&again_bar[k], pa); pa ^= 1u;     // the previous round of this slab
                 }
-                ENUF_TR((s - s_begin) * 16 + 2, trace_clock());
                 __syncwarp();
-                // ---- visit lists: for every patch the staged particles whose stencil overlaps it, as ready-made
-                //      byte offsets (x row | z row << 16, y row) into the stage
-                // (the NCONS running list lengths are bytes of two packed words: a round stages at most CAP + 1 < 256 entries per list)
-                unsigned lcp[2] = {0u, 0u};
-                for (int g0 = 0; g0 < ns; g0 += 32) {
-                    const int slot = g0 + lane;
-                    const bool v = slot < ns;
-                    int X0 = 64, Y0 = 64;
-                    if (v) { const int pkv = (int)acc_rec[k][slot].y; X0 = (pkv & 255) - 32; Y0 = ((pkv >> 8) & 255) - 32; }
-                    const unsigned sb = (unsigned)(slot * PITCH) * ES;
-                    const unsigned xb = sb + (unsigned)(OXF + (X0 & 1) - X0) * ES;
-                    const unsigned yb = sb + (unsigned)(OYF - Y0) * ES;
-                    const unsigned zb = sb + (unsigned)OZF * ES;
+                // ---- visit lists, second half: the entries worked out before the hand-over are stored into the stage
 #pragma unroll
-                    for (int w8 = 0; w8 < NCONS; ++w8) {
-                        const int px0 = 8 * (w8 % NPX), py0 = 8 * (w8 / NPX);
-                        const bool ov = v && X0 <= px0 + 7 && X0 + WZ - 1 >= px0 && Y0 <= py0 + 7 && Y0 + WZ - 1 >= py0;
-                        const unsigned bal = __ballot_sync(FULL, ov);
-                        const unsigned cur = (lcp[w8 >> 2] >> (8 * (w8 & 3))) & 255u;
-                        if (ov) lists[w8 * LCAP + cur + __popc(bal & below)] =
-                                    make_uint2((xb + (unsigned)px0 * ES) | (zb << 16), yb + (unsigned)py0 * ES);
-                        lcp[w8 >> 2] += (unsigned)__popc(bal) << (8 * (w8 & 3));
+                for (int gq = 0; gq < NGRP; ++gq) {
+                    if (32 * gq < ns) {
+                        const unsigned zb = (unsigned)((32 * gq + lane) * PITCH + OZF) * ES;
+#pragma unroll
+                        for (int w8 = 0; w8 < NCONS; ++w8) {
+                            const int px0 = 8 * (w8 % NPX), py0 = 8 * (w8 / NPX);
+                            if ((lmask[gq] >> w8) & 1u)
+                                lists[w8 * LCAP + ((lpos[gq][w8 >> 2] >> (8 * (w8 & 3))) & 255u)] =
+                                    make_uint2((lxb[gq] + (unsigned)px0 * ES) | (zb << 16), lyb[gq] + (unsigned)py0 * ES);
+                        }
                     }
                 }
-                ENUF_TR((s - s_begin) * 16 + 13, trace_clock());
                 if (lane < NCONS) {                                        // lane w8 closes list w8
                     const unsigned zs = (unsigned)(CAP * PITCH) * ES;      // the all-zero slot
                     const int c = (int)(((lane < 4 ? lcp[0] : lcp[1]) >> (8 * (lane & 3))) & 255u);
@@ -438,12 +441,8 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     }
                 }
                 cp_async_mbar_arrive(&full_bar[k]);
-                ENUF_TR((s - s_begin) * 16 + 3, trace_clock());
-                ENUF_TR((s - s_begin) * 16 + 8, (long long)ns);
-                ENUF_TR((s - s_begin) * 16 + 14, trace_clock());
                 __syncwarp();                                       // lane 0's arrive (release) publishes every lane's list entries
                 if (lane == 0) mbar_arrive(&full_bar[k]);
-                ENUF_TR((s - s_begin) * 16 + 4, trace_clock());
             }
         }
         return;
@@ -485,10 +484,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             pf ^= 1u << prod;
             const int cnt = cnt_s[stage][warp];
             lastf = last_s[stage];
-#ifdef ENUF_TRACE
-            if (warp == 0) { ENUF_TR((s - s_begin) * 16 + 5, trace_clock()); ENUF_TR((s - s_begin) * 16 + 9, (long long)cnt); }
-            if (warp == 5) { ENUF_TR((s - s_begin) * 16 + 10, trace_clock()); ENUF_TR((s - s_begin) * 16 + 12, (long long)cnt); }
-#endif
             // one visit ahead: while visit i is accumulated, the operands of visit i + 1 and the entry of visit i + 2 are
             // in flight.  Two visits per trip (A, B alternate, no register moves); the list is padded with entries that
             // point at the all-zero slot: to an even length, and two more for the loads that run ahead.
@@ -516,10 +511,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(lastf ? &empty_bar[prod] : &again_bar[prod]);
-#ifdef ENUF_TRACE
-            if (warp == 0) ENUF_TR((s - s_begin) * 16 + 6, trace_clock());
-            if (warp == 5) ENUF_TR((s - s_begin) * 16 + 11, trace_clock());
-#endif
         } while (!lastf);
         // the lowest plane of the window (s - SHI) is complete: store it, slide
         const int zo = s - C::SHI;
