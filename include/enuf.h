@@ -61,6 +61,9 @@ enum enuf_option {
                                     dependent launch -- each may be scheduled while its predecessor still runs
                                     and waits for it on the device (griddepcontrol), which hides the launch
                                     latency between the 11 kernels; 0: plain stream order                  */
+    ENUF_OPT_SPREAD_SPARSE = 11, /* tuning, fp32: -1 (default) the plan picks per evaluation, 1 / 0 force the
+                                    spreading kernel's eight-stage ring of 32-particle rounds (made for < ~12
+                                    staged particles per slab and column) on / off; results are the same   */
     ENUF_OPT_CUDA_GRAPH = 9      /* 1: the launches of one evaluation are captured into a CUDA graph
                                     the second time the same (r, q, F) pointers and N are passed, and
                                     replayed while they stay the same (an MD loop that updates r in

@@ -21,6 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 OPT_PRECISION, OPT_WINDOW, OPT_FORCE_VARIANT, OPT_SLATER_LAMBDA = 1, 2, 3, 4
 OPT_NUM_PARTICLES, OPT_PROFILE, OPT_KEEP_SPECTRUM, OPT_SPREAD_ZCHUNK = 5, 6, 7, 8
 OPT_PDL = 10
+OPT_SPREAD_SPARSE = 11
 OPT_CUDA_GRAPH = 9
 F32, F64 = 0, 1
 WINDOWS = {"gaussian": 0, "kaiser_bessel": 1, "bspline": 2}

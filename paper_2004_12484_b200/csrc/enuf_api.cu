@@ -398,6 +398,12 @@ int run_bin_spread(enuf_plan* p, const void* r, const void* q, void* F) {
     if (l < 0) return -1;
     p->launches += l;
     if (p->profile) cudaEventRecord(p->ev[1], p->stream);
+    {
+        // mean number of particles a spreading CTA stages per slab: N (column + stencil margin) / n^3
+        const int w = 2 * p->m - (p->trim ? 1 : 0), cx = 8 * p->spread_npx + w, cy = 16 + w;
+        const double per_slab = (double)p->N * cx * cy / ((double)p->n * p->n * p->n);
+        p->spread_sparse = sizeof(T) == 4 && (p->spread_sparse_user < 0 ? per_slab <= 12.0 : p->spread_sparse_user == 1);
+    }
     l = enuf::launch_spread<T>(p);
     if (l < 0) return -1;
     p->launches += l;
@@ -579,6 +585,10 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
             return ENUF_OK;
         case ENUF_OPT_PDL:
             p->pdl = iv != 0;
+            return ENUF_OK;
+        case ENUF_OPT_SPREAD_SPARSE:
+            if (iv < -1 || iv > 1) return fail(ENUF_EINVAL, "spread_sparse must be -1 (auto), 0 or 1");
+            p->spread_sparse_user = iv;
             return ENUF_OK;
         case ENUF_OPT_SPREAD_ZCHUNK:
             if (iv < 1 || iv > p->n) return fail(ENUF_EINVAL, "zchunk must be an integer in [1, n]");

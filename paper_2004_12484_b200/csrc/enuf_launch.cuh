@@ -105,8 +105,12 @@ int configure_kernels(enuf_plan* p) {
         bool ok = dispatch_npx(p->spread_npx, [&](auto xc) -> int {
             constexpr int NPX = decltype(xc)::value;
             bool k = set_smem(spread_kernel<T, M_, false, NPX>, spread_smem_bytes<T, M_, false, NPX>());
-            if constexpr (M_ >= 5 && sizeof(T) == 4)
+            if constexpr (sizeof(T) == 4)
+                k = k && set_smem(spread_kernel<T, M_, false, NPX, true>, spread_smem_bytes<T, M_, false, NPX, true>());
+            if constexpr (M_ >= 5 && sizeof(T) == 4) {
                 k = k && set_smem(spread_kernel<T, M_, true, NPX>, spread_smem_bytes<T, M_, true, NPX>());
+                k = k && set_smem(spread_kernel<T, M_, true, NPX, true>, spread_smem_bytes<T, M_, true, NPX, true>());
+            }
             return k ? 0 : -1;
         }) == 0;
         ok = ok && set_smem(gather_kernel<T, M_, false>, gather_smem_bytes<T, M_>());
@@ -188,6 +192,15 @@ int launch_spread(enuf_plan* p) {
                 constexpr bool kTrim = decltype(trim_c)::value != 0;
                 using C = SpreadCfg<T, M_, kTrim, NPX>;
                 const dim3 grid((unsigned)((p->n / C::CX) * (p->n / C::CY)), (unsigned)((p->n + p->zchunk - 1) / p->zchunk));
+                if constexpr (sizeof(T) == 4) {
+                    if (p->spread_sparse) {      // few particles per slab: 8 stages of 32 slots (SpreadCfg)
+                        pdl_launch(p, spread_kernel<T, M_, kTrim, NPX, true>, grid, C::NT,
+                                   spread_smem_bytes<T, M_, kTrim, NPX, true>(), s,
+                                   static_cast<const PSlot<T>*>(p->rec), static_cast<const T*>(p->rows), p->bin_offset, p->tg,
+                                   p->zchunk, static_cast<T*>(p->grid[0]));
+                        return 0;
+                    }
+                }
                 pdl_launch(p, spread_kernel<T, M_, kTrim, NPX>, grid, C::NT, spread_smem_bytes<T, M_, kTrim, NPX>(), s, 
                     static_cast<const PSlot<T>*>(p->rec), static_cast<const T*>(p->rows), p->bin_offset, p->tg,
                     p->zchunk, static_cast<T*>(p->grid[0]));

@@ -56,6 +56,8 @@ struct enuf_plan {
     int zchunk = 0;                   // grid planes per spread CTA
     bool zchunk_user = false;         // set through ENUF_OPT_SPREAD_ZCHUNK: not re-derived
     int spread_npx = 4;               // spread column = 8 spread_npx x 16 cells (4 for n >= 128, 2 below)
+    int spread_sparse_user = -1;      // ENUF_OPT_SPREAD_SPARSE: -1 auto, 0 / 1 forced
+    bool spread_sparse = false;       // fp32: eight-stage ring of 32-slot rounds (few particles per slab and column)
     void* grid[3] = {nullptr, nullptr, nullptr};   // real n^3 (1 for analytic, 3 for ik)
     void* A1[3] = {nullptr, nullptr, nullptr};     // complex [n][n][Kxp]
     void* A2[3] = {nullptr, nullptr, nullptr};     // complex [n][Ky][Kxp]

@@ -54,14 +54,17 @@ __device__ __forceinline__ double2 pair_scale(double2 a, const double f) { a.x *
 // kTrim (fp32 Kaiser-Bessel, m >= 5): particles are binned by the plane s = c_z - 1 + ks_z, ks = (d0 > 0),
 // so that every particle of slab s has its 2m non-zero z weights on the planes s-m+1 .. s+m: the window
 // is WZ = 2m planes and the x / y stencils are the 2m points from c - m + ks on.
-template <typename T, int M_, bool kTrim, int NPX_>
+// kSparse: few particles per slab and column (the plan decides, enuf_api.cu): rounds of 32 slots in an eight-stage ring
+// instead of 96 in three -- the same shared memory, but the flight time of the row copies after a hand-over (which is
+// what bounds a sparse slab) is spread over eight slabs.  Correct for any density (a denser slab takes several rounds).
+template <typename T, int M_, bool kTrim, int NPX_, bool kSparse = false>
 struct SpreadCfg {
     static constexpr int W = 2 * M_ + 1;
     static constexpr int WZ = W - (kTrim ? 1 : 0);               // stencil points per dimension = planes in the window
     static constexpr int SLO = M_, SHI = kTrim ? M_ - 1 : M_;    // slab s reaches the planes s - SHI .. s + SLO
     static constexpr int NPX = NPX_, NPY = 2, NCONS = NPX * NPY; // 8 x 8 patches = consumer warps
     static constexpr int NPROD = 4;                              // producer warps: producer k takes the slabs k, k + 4, .. of the chunk
-    static constexpr int NSTAGE = 3;                             //   slab i of the chunk is staged in stage i % 3
+    static constexpr int NSTAGE = kSparse ? 8 : 3;               //   slab i of the chunk is staged in stage i % NSTAGE
     static constexpr int CX = 8 * NPX, CY = 8 * NPY;             // column
     static constexpr int NT = 32 * (NCONS + NPROD);
     static constexpr int NBX = CX / kTile + 2, NBY = CY / kTile + 2;   // bins (16 x 16, enuf_common.cuh) the halo touches
@@ -72,7 +75,8 @@ struct SpreadCfg {
     static constexpr int OYF = (16 + WZ + 3) / 4 * 4 > 24 ? (16 + WZ + 3) / 4 * 4 : 24;
     static constexpr int OZF = (OYF + WZ + 7 + 3) / 4 * 4 > OYF + 16 ? (OYF + WZ + 7 + 3) / 4 * 4 : OYF + 16;
     static constexpr int PITCH = OZF + 16 <= 68 ? 68 : 76;       // = 4 / 12 mod 32: 16-byte row chunks of 8 slots hit 32 banks
-    static constexpr int CAP = sizeof(T) == 4 ? (NPX == 4 ? (PITCH == 68 ? 96 : 88) : 56) : (NPX == 4 ? 48 : 40);   // staged particles per round
+    static constexpr int CAP = kSparse ? 32 :
+        (sizeof(T) == 4 ? (NPX == 4 ? (PITCH == 68 ? 96 : 88) : 56) : (NPX == 4 ? 48 : 40));   // staged particles per round
     static constexpr int LCAP = CAP + 4;                         // visit-list entries per patch (even padding + prefetch)
     static constexpr int kBlk = 16;                              // slabs (of one producer) whose bin ranges are loaded at once
     static constexpr int CTAS_PER_SM = sizeof(T) == 4 ? (NPX == 4 ? 2 : 3) : (NPX == 4 ? 1 : 2);
@@ -81,14 +85,19 @@ struct SpreadCfg {
     static constexpr size_t STAGE_BYTES = ((SLOT_BYTES + LIST_BYTES + 15) / 16) * 16;
     static_assert(CAP >= 32 && CAP + 1 < 256 && NCONS <= 8, "a cull step stages up to 32 particles; packed list lengths");
     static_assert(NSEG <= 32 && kBlk == 16, "one lane per segment; lanes = 16 slabs x (start, end)");
-    static_assert(NPROD == 4 && NSTAGE == 3, "barrier protocol: slab i - 3 held the stage, its producer is (k + 1) & 3");
+    static_assert(NPROD == 4, "barrier protocol: slab i - NSTAGE held the stage, its producer is (k - NSTAGE) & 3");
+    // A barrier may run at most one phase ahead of its waiter.  With full / empty barriers per PRODUCER that holds as
+    // long as NSTAGE <= NPROD (slab i + 4 can be staged / finished only after slab i was consumed / its stage re-staged);
+    // the eight-stage ring keeps them per STAGE instead, where it holds for any depth.
+    static constexpr bool kStageBars = NSTAGE > NPROD;
+    static constexpr int NBAR = kStageBars ? NSTAGE : NPROD;
     static_assert(SLOT_BYTES < 65536, "visit-list entries are 16-bit byte offsets");
     static_assert(OZF + 16 <= PITCH, "slot layout");
 };
 
-template <typename T, int M_, bool kTrim, int NPX>
+template <typename T, int M_, bool kTrim, int NPX, bool kSparse = false>
 constexpr size_t spread_smem_bytes() {
-    using C = SpreadCfg<T, M_, kTrim, NPX>;
+    using C = SpreadCfg<T, M_, kTrim, NPX, kSparse>;
     return C::STAGE_BYTES * C::NSTAGE;
 }
 
@@ -185,12 +194,12 @@ __device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar) {
 
 // slots[].cell: bits 0..29 the packed nearest cell, bits 30 / 31 = ks_x / ks_y (trimmed plans; enuf_bin.cuh)
 // rows: [N][RP] window rows in bin order (WindowRows)
-template <typename T, int M_, bool kTrim, int NPX>
-__global__ void __launch_bounds__((SpreadCfg<T, M_, kTrim, NPX>::NT), (SpreadCfg<T, M_, kTrim, NPX>::CTAS_PER_SM))
+template <typename T, int M_, bool kTrim, int NPX, bool kSparse = false>
+__global__ void __launch_bounds__((SpreadCfg<T, M_, kTrim, NPX, kSparse>::NT), (SpreadCfg<T, M_, kTrim, NPX, kSparse>::CTAS_PER_SM))
 spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
               const uint32_t* __restrict__ offset, TileGeom g, int zchunk, T* __restrict__ grid) {
     pdl_prologue();
-    using C = SpreadCfg<T, M_, kTrim, NPX>;
+    using C = SpreadCfg<T, M_, kTrim, NPX, kSparse>;
     using R = WindowRows<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
     using V4 = typename Vec4<T>::type;
@@ -204,9 +213,11 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     // per producer k: full_bar[k]  -- a round of one of its slabs is staged (consumers wait),
     //                 again_bar[k] -- every consumer is done with a round that was not the slab's last (producer k waits),
     //                 empty_bar[k] -- every consumer is done with the last round of a slab of producer k: its stage is
-    //                                 free for the slab three further on, i.e. for producer (k + 3) & 3 (only that one waits on it).
+    //                                 free for the slab NSTAGE further on, i.e. for producer (k + NSTAGE) & 3 (only that one waits on it).
     // Every barrier has one waiting party that sees each of its phases in turn, so one parity bit per party suffices.
-    __shared__ uint64_t full_bar[C::NPROD], empty_bar[C::NPROD], again_bar[C::NPROD];
+    // (kStageBars: full_bar / empty_bar are indexed by the stage instead, the phases of empty_bar[stage] are the slabs
+    //  stage, stage + NSTAGE, .. of the chunk, so the waiter's parity follows from the slab index.)
+    __shared__ uint64_t full_bar[C::NBAR], empty_bar[C::NBAR], again_bar[C::NPROD];
     __shared__ int cnt_s[NSTAGE][NCONS];        // visits of each patch in the stage
     __shared__ int last_s[NSTAGE];              // 1: the stage is the last round of its slab
     __shared__ uint32_t rng[C::NPROD][NSEG][2 * kBlk];   // [..][0..kBlk): range starts of kBlk slabs, [kBlk..): ends
@@ -224,12 +235,13 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
         reinterpret_cast<uint4*>(smem_raw)[i] = make_uint4(0u, 0u, 0u, 0u);
     if (tid == 0) {
 #pragma unroll
-        for (int st = 0; st < C::NPROD; ++st) {
+        for (int st = 0; st < C::NBAR; ++st) {
             // full: one arrival per producer lane when its row copies have landed + one after the lists are written
             mbar_init(&full_bar[st], 33);
             mbar_init(&empty_bar[st], NCONS);
-            mbar_init(&again_bar[st], NCONS);
         }
+#pragma unroll
+        for (int st = 0; st < C::NPROD; ++st) mbar_init(&again_bar[st], NCONS);
     }
     __syncthreads();
 
@@ -260,7 +272,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
         // first stencil point in column coordinates from the packed cell: the periodic image that can overlap the column
         const int offx = -M_ - CX * Tx + (WZ - 1), offy = -M_ - CY * Ty + (WZ - 1), nmask = g.n - 1;
         uint32_t (*rg)[2 * kBlk] = rng[k];
-        unsigned pe = 0, pa = 0;                 // parities of the next phase of empty_bar[(k + 1) & 3] / again_bar[k] to wait for
+        unsigned pe = 0, pa = 0;                 // parities of the next phase of empty_bar[(k - NSTAGE) & 3] / again_bar[k] to wait for
         int blk0 = s_begin + k - C::NPROD * kBlk;
         // candidates of a slab: the ranges of the NSEG segments, 32 per step.  The cell words of up to kSteps steps are
         // loaded together (one global-load latency per slab, not one per step), then examined in order; those of the
@@ -395,8 +407,14 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     }
                 }
                 if (first_round) {
-                    // the slab that held the stage before (s - 3, staged by producer (k + 1) & 3) must be finished
-                    if (s - NSTAGE >= s_begin) { mbar_wait_backoff(&empty_bar[(k + 1) & 3], pe); pe ^= 1u; }
+                    // the slab that held the stage before (s - NSTAGE, staged by producer (k - NSTAGE) & 3) must be finished
+                    if (s - NSTAGE >= s_begin) {
+                        if constexpr (C::kStageBars) {
+                            mbar_wait_backoff(&empty_bar[stage], (unsigned)(((s - s_begin) / NSTAGE - 1) & 1));
+                        } else {
+                            mbar_wait_backoff(&empty_bar[(k - NSTAGE) & 3], pe); pe ^= 1u;
+                        }
+                    }
                     first_round = false;
                 } else {
                     mbar_wait_backoff(&again_bar[k], pa); pa ^= 1u;     // the previous round of this slab
@@ -440,9 +458,10 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                         for (int c = 0; c < CHY; ++c) cp_async_16(dst + OZF * ES + 16 * c, src + R::OZ * ES + 16 * c);
                     }
                 }
-                cp_async_mbar_arrive(&full_bar[k]);
+                uint64_t* fb = &full_bar[C::kStageBars ? stage : k];
+                cp_async_mbar_arrive(fb);
                 __syncwarp();                                       // lane 0's arrive (release) publishes every lane's list entries
-                if (lane == 0) mbar_arrive(&full_bar[k]);
+                if (lane == 0) mbar_arrive(fb);
             }
         }
         return;
@@ -471,17 +490,18 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
         return o;
     };
 
-    unsigned pf = 0;                                              // parity bits of the next phase of full_bar[0..3]
+    unsigned pf = 0;                                              // parity bits of the next phase of full_bar[..]
     const uint32_t smem32 = smem_u32(smem_raw);
     for (int s = s_begin; s < s_end; ++s) {
         const int stage = (s - s_begin) % NSTAGE, prod = (s - s_begin) & 3;
+        const int bar = C::kStageBars ? stage : prod;
         const uint32_t sbz = smem32 + (uint32_t)(stage * C::STAGE_BYTES);
         const uint32_t sbx = sbz + lxl * ES, sby = sbz + lyl * ES;
         const uint32_t lp = sbz + (uint32_t)C::SLOT_BYTES + (uint32_t)(warp * LCAP * sizeof(uint2));
         int lastf;
         do {
-            mbar_wait_backoff(&full_bar[prod], (pf >> prod) & 1u);
-            pf ^= 1u << prod;
+            mbar_wait_backoff(&full_bar[bar], (pf >> bar) & 1u);
+            pf ^= 1u << bar;
             const int cnt = cnt_s[stage][warp];
             lastf = last_s[stage];
             // one visit ahead: while visit i is accumulated, the operands of visit i + 1 and the entry of visit i + 2 are
@@ -510,7 +530,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(lastf ? &empty_bar[prod] : &again_bar[prod]);
+            if (lane == 0) mbar_arrive(lastf ? &empty_bar[bar] : &again_bar[prod]);
         } while (!lastf);
         // the lowest plane of the window (s - SHI) is complete: store it, slide
         const int zo = s - C::SHI;

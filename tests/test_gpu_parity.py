@@ -455,6 +455,26 @@ def test_dense_cluster_many_particles_per_bin(enuf, torch_cuda, oracle):
         plan.close()
 
 
+@pytest.mark.parametrize("n,m,N", [(64, 4, 40000), (128, 5, 60000), (128, 2, 3000), (256, 4, 20000)])
+@pytest.mark.parametrize("sparse", [0, 1])
+def test_spread_rings_give_the_same_grid(enuf, torch_cuda, oracle, n, m, N, sparse):
+    """ENUF_OPT_SPREAD_SPARSE forces the spreading kernel's ring (three stages of 96-particle rounds, or eight of 32)
+    against the plan's own choice: dense inputs through the eight-stage ring take several rounds per slab, dilute
+    ones through the three-stage ring leave most rounds empty; the spread grid must match the oracle either way."""
+    torch = torch_cuda
+    rng = np.random.default_rng(1000 + n + N)
+    L = 7.0
+    r = rng.uniform(-L, 2 * L, size=(N, 3)).astype(np.float32)
+    r[: N // 3] = (np.array([0.02, 6.99, 3.5]) + rng.normal(0, 0.4, size=(N // 3, 3))).astype(np.float32)   # a dense lump on a face
+    q = rng.uniform(-1, 1, size=N).astype(np.float32)
+    plan = enuf.Plan(N, L, 1.1, n // 4, n // 2, sigma=2.0, m=m, window="kaiser_bessel", dtype=torch.float32)
+    plan.set(enuf.OPT_SPREAD_SPARSE, sparse)
+    g = plan.spread_only(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda()).numpy()
+    ref = oracle.spread(r, q, L, n, m, "kaiser_bessel", 2.0)
+    assert np.abs(g - ref).max() <= 2e-6 * np.abs(ref).max()
+    plan.close()
+
+
 def test_fp32_particles_exactly_on_grid_points(enuf, torch_cuda, oracle):
     """fp32 Kaiser-Bessel m = 6 visits 2m stencil points per dimension (the far outermost one is an
     exact zero) -- except for a particle exactly on a grid point, where both ends carry
