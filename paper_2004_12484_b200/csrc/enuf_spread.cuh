@@ -84,7 +84,7 @@ struct SpreadCfg {
     static constexpr size_t LIST_BYTES = sizeof(uint2) * (size_t)NCONS * LCAP;
     static constexpr size_t STAGE_BYTES = ((SLOT_BYTES + LIST_BYTES + 15) / 16) * 16;
     static_assert(CAP >= 32 && CAP + 1 < 256 && NCONS <= 8, "a cull step stages up to 32 particles; packed list lengths");
-    static_assert(NSEG <= 32 && kBlk == 16, "one lane per segment; lanes = 16 slabs x (start, end)");
+    static_assert(NSEG <= 8 && kBlk == 16, "segment table: 8 packed ends + 8 offsets per slab; lanes = 16 slabs x (start, end)");
     static_assert(NPROD == 4, "barrier protocol: slab i - NSTAGE held the stage, its producer is (k - NSTAGE) & 3");
     // A barrier may run at most one phase ahead of its waiter.  With full / empty barriers per PRODUCER that holds as
     // long as NSTAGE <= NPROD (slab i + 4 can be staged / finished only after slab i was consumed / its stage re-staged);
@@ -220,7 +220,10 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     __shared__ uint64_t full_bar[C::NBAR], empty_bar[C::NBAR], again_bar[C::NPROD];
     __shared__ int cnt_s[NSTAGE][NCONS];        // visits of each patch in the stage
     __shared__ int last_s[NSTAGE];              // 1: the stage is the last round of its slab
-    __shared__ uint32_t rng[C::NPROD][NSEG][2 * kBlk];   // [..][0..kBlk): range starts of kBlk slabs, [kBlk..): ends
+    // candidates of a slab = its NSEG ranges of the sorted array laid end to end ("packed" numbering e = 0 .. total - 1);
+    // per slab: [0..6] packed end of segment 0..6 (total from segment NSEG - 1 on), [7] total, [8 + i] = start of
+    // segment i - its packed start, so that candidate e of segment i is slots[e + [8 + i]]
+    __shared__ __align__(16) uint32_t segtab[C::NPROD][kBlk][16];
     __shared__ uint2 acc_rec[C::NPROD][CAP];            // producer's side buffer: accepted particles of the round,
                                                         //   (sorted-array index, (X0 + 32) | (Y0 + 32) << 8)
 
@@ -271,32 +274,40 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
         }
         // first stencil point in column coordinates from the packed cell: the periodic image that can overlap the column
         const int offx = -M_ - CX * Tx + (WZ - 1), offy = -M_ - CY * Ty + (WZ - 1), nmask = g.n - 1;
-        uint32_t (*rg)[2 * kBlk] = rng[k];
+        const uint4* tb = reinterpret_cast<const uint4*>(segtab[k]);
         unsigned pe = 0, pa = 0;                 // parities of the next phase of empty_bar[(k - NSTAGE) & 3] / again_bar[k] to wait for
         int blk0 = s_begin + k - C::NPROD * kBlk;
-        // candidates of a slab: the ranges of the NSEG segments, 32 per step.  The cell words of up to kSteps steps are
-        // loaded together (one global-load latency per slab, not one per step), then examined in order; those of the
-        // producer's NEXT slab are started as soon as the current slab is culled, so that they arrive during the
-        // hand-over, the lists and the copies.
+        // candidates of a slab, 32 per step, in packed numbering (segtab): a sparse slab is ONE step however its
+        // particles are spread over the segments.  The cell words of up to kSteps steps are loaded together (one
+        // global-load latency per slab, not one per step), then examined in order; those of the producer's NEXT slab
+        // are started as soon as the current slab is culled, so that they arrive during the hand-over, the lists and
+        // the copies.
         constexpr int kSteps = 8;
-        int sg = 0;
-        uint32_t gs = 0, ge = 0;
-        uint32_t cw[kSteps], cbase[kSteps];
+        uint32_t ebase = 0, total = 0;           // first candidate of the next load, candidates of the slab
+        uint32_t cw[kSteps], cidx[kSteps];
         int nst = 0;                             // steps loaded (consumed ones are marked invalid)
-        bool preloaded = false;                  // cw / cbase already hold the first steps of this slab
+        bool preloaded = false;                  // cw / cidx already hold the first steps of this slab
         auto load_steps = [&](int js) {
+            const uint4 e0 = tb[4 * js], e1 = tb[4 * js + 1], d0 = tb[4 * js + 2], d1 = tb[4 * js + 3];
+            const uint32_t pe_[7] = {e0.x, e0.y, e0.z, e0.w, e1.x, e1.y, e1.z};
+            const uint32_t dl_[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+            total = e1.w;
             nst = 0;
 #pragma unroll
             for (int j = 0; j < kSteps; ++j) {
-                while (gs >= ge && sg < NSEG) { gs = rg[sg][js]; ge = rg[sg][kBlk + js]; ++sg; }
-                cbase[j] = gs;
                 cw[j] = 0xffffffffu;
-                if (gs < ge) {
-                    if (gs + (uint32_t)lane < ge) cw[j] = slots[gs + (uint32_t)lane].cell;
-                    gs += 32u;
+                cidx[j] = 0u;
+                if (ebase + 32u * j < total) {
+                    const uint32_t e = ebase + 32u * j + (uint32_t)lane;
+                    uint32_t dl = dl_[0];
+#pragma unroll
+                    for (int i = 0; i + 1 < NSEG; ++i) dl = e >= pe_[i] ? dl_[i + 1] : dl;
+                    cidx[j] = e + dl;
+                    if (e < total) cw[j] = slots[cidx[j]].cell;
                     nst = j + 1;
                 }
             }
+            ebase += 32u * kSteps;
         };
         for (int s = s_begin + k; s < s_end; s += C::NPROD) {
             if (s - blk0 >= C::NPROD * kBlk) {
@@ -304,10 +315,26 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 blk0 = s;
                 __syncwarp();
                 const int cz = (blk0 + C::NPROD * l16) & nmask;
+                uint32_t pend[8], pdel[8], run = 0u;
+#pragma unroll
+                for (int sg = 0; sg < 8; ++sg) { pend[sg] = 0u; pdel[sg] = 0u; }
 #pragma unroll
                 for (int sg = 0; sg < NSEG; ++sg) {
                     const int b0 = __shfl_sync(FULL, seg_bin0, sg), nb = __shfl_sync(FULL, seg_nb, sg);
-                    rg[sg][lane] = offset[b0 + cz * g.nt + half * nb];
+                    const uint32_t v = offset[b0 + cz * g.nt + half * nb];
+                    const uint32_t ve = __shfl_down_sync(FULL, v, 16);      // lanes < 16: the end of the range
+                    pdel[sg] = v - run;
+                    run += ve - v;
+                    pend[sg] = run;
+                }
+#pragma unroll
+                for (int sg = NSEG - 1; sg < 8; ++sg) pend[sg] = run;       // [NSEG - 1 .. 7] = total
+                if (lane < kBlk) {
+                    uint4* t4 = reinterpret_cast<uint4*>(segtab[k][lane]);
+                    t4[0] = make_uint4(pend[0], pend[1], pend[2], pend[3]);
+                    t4[1] = make_uint4(pend[4], pend[5], pend[6], pend[7]);
+                    t4[2] = make_uint4(pdel[0], pdel[1], pdel[2], pdel[3]);
+                    t4[3] = make_uint4(pdel[4], pdel[5], pdel[6], pdel[7]);
                 }
                 __syncwarp();
             }
@@ -316,7 +343,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             unsigned char* sbase = smem_raw + (size_t)stage * C::STAGE_BYTES;
             const uint32_t sl32 = smem_u32(sbase);
             uint2* lists = reinterpret_cast<uint2*>(sbase + C::SLOT_BYTES);
-            if (!preloaded) { sg = 0; gs = 0; ge = 0; load_steps(js); }
+            if (!preloaded) { ebase = 0u; load_steps(js); }
             preloaded = false;
             bool slab_done = false, first_round = true;
             while (!slab_done) {
@@ -324,23 +351,19 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 //      sorted-array index and packed stencil origin; their rows are started towards L2
                 int ns = 0;
                 for (;;) {
-                    // all loaded steps at once, branch-free (the steps are independent up to the running slot count);
-                    // in halves, so that sparse slabs (few steps) skip the unused half
+                    // all loaded steps at once (the steps are independent up to the running slot count)
                     int pkv[kSteps]; unsigned bal[kSteps];
 #pragma unroll
                     for (int j = 0; j < kSteps; ++j) { pkv[j] = -1; bal[j] = 0u; }
 #pragma unroll
-                    for (int hh = 0; hh < 2; ++hh) {
-                        if (hh * (kSteps / 2) < nst) {
-#pragma unroll
-                            for (int j = hh * (kSteps / 2); j < (hh + 1) * (kSteps / 2); ++j) {
-                                const uint32_t cwj = cw[j];
-                                const int X0 = (((int)(cwj & 1023u) + (int)((cwj >> 30) & 1u) + offx) & nmask) - (WZ - 1);
-                                const int Y0 = (((int)((cwj >> 10) & 1023u) + (int)(cwj >> 31) + offy) & nmask) - (WZ - 1);
-                                const bool ok = cwj != 0xffffffffu && X0 <= CX - 1 && Y0 <= CY - 1;
-                                bal[j] = __ballot_sync(FULL, ok);
-                                pkv[j] = ok ? ((X0 + 32) | ((Y0 + 32) << 8)) : -1;
-                            }
+                    for (int j = 0; j < kSteps; ++j) {
+                        if (j < nst) {                                  // (uniform)
+                            const uint32_t cwj = cw[j];
+                            const int X0 = (((int)(cwj & 1023u) + (int)((cwj >> 30) & 1u) + offx) & nmask) - (WZ - 1);
+                            const int Y0 = (((int)((cwj >> 10) & 1023u) + (int)(cwj >> 31) + offy) & nmask) - (WZ - 1);
+                            const bool ok = cwj != 0xffffffffu && X0 <= CX - 1 && Y0 <= CY - 1;
+                            bal[j] = __ballot_sync(FULL, ok);
+                            pkv[j] = ok ? ((X0 + 32) | ((Y0 + 32) << 8)) : -1;
                         }
                     }
                     // steps are taken while their accepted particles fit into the round (CAP slots)
@@ -353,26 +376,20 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                         if (j < jl) base += c;
                     }
 #pragma unroll
-                    for (int hh = 0; hh < 2; ++hh) {
-                        if (hh * (kSteps / 2) < nst) {
-#pragma unroll
-                            for (int j = hh * (kSteps / 2); j < (hh + 1) * (kSteps / 2); ++j) {
-                                if (j < jl) {
-                                    if (pkv[j] >= 0)
-                                        acc_rec[k][pb[j] + __popc(bal[j] & below)] = make_uint2(cbase[j] + (uint32_t)lane, (unsigned)pkv[j]);
-                                    cw[j] = 0xffffffffu;                // consumed
-                                }
-                            }
+                    for (int j = 0; j < kSteps; ++j) {
+                        if (j < nst && j < jl) {
+                            if (pkv[j] >= 0)
+                                acc_rec[k][pb[j] + __popc(bal[j] & below)] = make_uint2(cidx[j], (unsigned)pkv[j]);
+                            cw[j] = 0xffffffffu;                        // consumed
                         }
                     }
                     ns = base;
                     if (jl < kSteps) break;                            // step jl opens the next round of this slab
-                    if (nst < kSteps) { slab_done = true; break; }     // the ranges are exhausted
+                    if (ebase >= total) { slab_done = true; break; }   // the ranges are exhausted
                     load_steps(js);                                    // a long slab: the next kSteps steps
-                    if (nst == 0) { slab_done = true; break; }
                 }
                 if (slab_done && s + C::NPROD < s_end && js + 1 < kBlk) {
-                    sg = 0; gs = 0; ge = 0;
+                    ebase = 0u;
                     load_steps(js + 1);                                // the next slab of this producer (same block of ranges)
                     preloaded = true;
                 }

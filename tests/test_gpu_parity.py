@@ -471,7 +471,10 @@ def test_spread_rings_give_the_same_grid(enuf, torch_cuda, oracle, n, m, N, spar
     plan.set(enuf.OPT_SPREAD_SPARSE, sparse)
     g = plan.spread_only(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda()).numpy()
     ref = oracle.spread(r, q, L, n, m, "kaiser_bessel", 2.0)
-    assert np.abs(g - ref).max() <= 2e-6 * np.abs(ref).max()
+    # a cell inside the lump sums K ~ 1e3..1e4 terms of random sign in fp32, in an order that changes from run to
+    # run (the counting sort's ranks are atomics): error ~ sqrt(K) eps |term| against a maximum ~ sqrt(K) |term|,
+    # with a constant of a few -- measured 2.0e-6..2.7e-6 over 40 runs at n = 64; one lost particle would be ~1e-2
+    assert np.abs(g - ref).max() <= 1e-5 * np.abs(ref).max()
     plan.close()
 
 
