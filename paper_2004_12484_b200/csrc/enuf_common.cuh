@@ -150,6 +150,24 @@ __device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// the same on a shared-window address the caller keeps (inner loops: no generic-to-shared conversion per call)
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar32, uint32_t parity) {
+    uint32_t done, ns = 32;
+    for (;;) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(bar32), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(ns);
+        ns = ns < 512u ? 2u * ns : ns;
+    }
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar32) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar32) : "memory");
+}
 
 // ---------------------------------------------------------------- math wrappers
 __device__ __forceinline__ float r_exp(float x) { return expf(x); }

@@ -180,6 +180,11 @@ template <> __device__ __forceinline__ double4 lds_quad<double>(uint32_t a) {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.z), "=d"(v.w) : "r"(a + 16u));
     return v;
 }
+__device__ __forceinline__ int lds_s32(uint32_t a) {
+    int v;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
 __device__ __forceinline__ uint2 lds_u2(uint32_t a) {
     uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v;
 }
@@ -218,8 +223,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     // (kStageBars: full_bar / empty_bar are indexed by the stage instead, the phases of empty_bar[stage] are the slabs
     //  stage, stage + NSTAGE, .. of the chunk, so the waiter's parity follows from the slab index.)
     __shared__ uint64_t full_bar[C::NBAR], empty_bar[C::NBAR], again_bar[C::NPROD];
-    __shared__ int cnt_s[NSTAGE][NCONS];        // visits of each patch in the stage
-    __shared__ int last_s[NSTAGE];              // 1: the stage is the last round of its slab
+    __shared__ int cl_s[NSTAGE][NCONS];         // visits of each patch in the stage | 0x10000 if it is the slab's last round
     // candidates of a slab = its NSEG ranges of the sorted array laid end to end ("packed" numbering e = 0 .. total - 1);
     // per slab: [0..6] packed end of segment 0..6 (total from segment NSEG - 1 on), [7] total, [8 + i] = start of
     // segment i - its packed start, so that candidate e of segment i is slots[e + [8 + i]]
@@ -457,8 +461,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     // even length, and the consumer loads its operands one visit ahead: entries that point at the zero slot
                     lists[lane * LCAP + c] = lists[lane * LCAP + c + 1] = lists[lane * LCAP + c + 2] =
                         make_uint2((zs + OXF * ES) | ((zs + OZF * ES) << 16), zs + OYF * ES);
-                    cnt_s[stage][lane] = c + (c & 1);
-                    if (lane == 0) last_s[stage] = slab_done ? 1 : 0;
+                    cl_s[stage][lane] = (c + (c & 1)) | (slab_done ? 0x10000 : 0);
                 }
                 // ---- copy the window rows of the accepted particles into the slots (cp.async; they arrive on full_bar themselves)
                 for (int g0 = 0; g0 < ns; g0 += 32) {
@@ -508,19 +511,25 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     };
 
     unsigned pf = 0;                                              // parity bits of the next phase of full_bar[..]
+    // everything a slab needs is kept as a shared-window address or stepped along, so that an empty slab costs a
+    // wait, one load, one arrive, the store and the slide (dilute systems are bound by exactly that)
     const uint32_t smem32 = smem_u32(smem_raw);
+    const uint32_t fb32 = smem_u32(full_bar), eb32 = smem_u32(empty_bar), ab32 = smem_u32(again_bar);
+    const uint32_t cl32 = smem_u32(cl_s) + (uint32_t)warp * 4u;
+    const uint32_t lpw = (uint32_t)C::SLOT_BYTES + (uint32_t)(warp * LCAP * sizeof(uint2));
+    int stage = 0, prod = 0;
+    gout += (ptrdiff_t)(s_begin - C::SHI) * (ptrdiff_t)plane;     // plane s - SHI; first dereferenced at plane z0
     for (int s = s_begin; s < s_end; ++s) {
-        const int stage = (s - s_begin) % NSTAGE, prod = (s - s_begin) & 3;
         const int bar = C::kStageBars ? stage : prod;
-        const uint32_t sbz = smem32 + (uint32_t)(stage * C::STAGE_BYTES);
+        const uint32_t sbz = smem32 + (uint32_t)stage * (uint32_t)C::STAGE_BYTES;
         const uint32_t sbx = sbz + lxl * ES, sby = sbz + lyl * ES;
-        const uint32_t lp = sbz + (uint32_t)C::SLOT_BYTES + (uint32_t)(warp * LCAP * sizeof(uint2));
-        int lastf;
+        const uint32_t lp = sbz + lpw;
+        int cl;
         do {
-            mbar_wait_backoff(&full_bar[bar], (pf >> bar) & 1u);
+            mbar_wait_backoff(fb32 + 8u * (uint32_t)bar, (pf >> bar) & 1u);
             pf ^= 1u << bar;
-            const int cnt = cnt_s[stage][warp];
-            lastf = last_s[stage];
+            cl = lds_s32(cl32 + (uint32_t)stage * (uint32_t)(NCONS * 4));
+            const int cnt = cl & 0xffff;
             // one visit ahead: while visit i is accumulated, the operands of visit i + 1 and the entry of visit i + 2 are
             // in flight.  Two visits per trip (A, B alternate, no register moves); the list is padded with entries that
             // point at the all-zero slot: to an even length, and two more for the loads that run ahead.
@@ -547,14 +556,16 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(lastf ? &empty_bar[bar] : &again_bar[prod]);
-        } while (!lastf);
+            if (lane == 0) mbar_arrive((cl >> 16) ? eb32 + 8u * (uint32_t)bar : ab32 + 8u * (uint32_t)prod);
+        } while (!(cl >> 16));
         // the lowest plane of the window (s - SHI) is complete: store it, slide
-        const int zo = s - C::SHI;
-        if (zo >= z0) *reinterpret_cast<P2*>(gout + (size_t)zo * plane) = acc[0];
+        if (s >= z0 + C::SHI) *reinterpret_cast<P2*>(gout) = acc[0];
+        gout += plane;
 #pragma unroll
         for (int kk = 0; kk + 1 < WZ; ++kk) acc[kk] = acc[kk + 1];
         acc[WZ - 1].x = (T)0; acc[WZ - 1].y = (T)0;
+        stage = stage + 1 == NSTAGE ? 0 : stage + 1;
+        prod = (prod + 1) & 3;
     }
 }
 
