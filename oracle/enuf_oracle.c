@@ -659,3 +659,272 @@ int orc_enuf(int64_t N, const double *r, const double *q, double L, double alpha
     free(g_re); free(g_im); free(p_re); free(p_im);
     return 0;
 }
+
+/* =================================================================== orthorhombic boxes
+ * SURVEY.md section 8(f).4.  The paper treats the cubic box only and names non-cubic
+ * boxes as motivation (:35, :609); this is the textbook Ewald sum of a cell with edges
+ * Lb = (Lx, Ly, Lz), volume V = Lx Ly Lz, written out the same way (reading R20):
+ *   x_d = r_d / L_d,  wave vector k = 2 pi h,  h = (nx/Lx, ny/Ly, nz/Lz),  n integer,
+ *   S(n)  = sum_j q_j exp(-2 pi i n.x_j)                                         (Eq. 37)
+ *   E_rec = (1/(2 pi V)) sum_K f^2(h) exp(-pi^2 |h|^2/alpha^2)/|h|^2 |S(n)|^2    (Eq. 38 with n/L -> h)
+ *   F_i,d = (2 q_i/V) sum_K h_d f^2 exp(..)/|h|^2 Im{S e^{+2 pi i n.x_i}}        (Eq. 41 likewise)
+ *   K     = { n != 0 : |h| Lmax <= k_cut },  Lmax = max(Lx, Ly, Lz)              (R20: a sphere of wave
+ *           vectors; every |n_d| <= k_cut L_d/Lmax <= k_cut; the cubic K of R4 when the edges are equal)
+ * With Lx = Ly = Lz all of this is the cubic case above term by term.  The ENUF steps keep ONE grid size n
+ * in all three directions (grid spacing L_d/n differs per direction); only u_d = n x_d, the weights and the
+ * prefactors change:  E~ = (1/(2 pi V)) sum_K f^2 w |S~|^2,
+ *   analytic forces F_i,d = -(q_i n/(pi V L_d)) sum_stencil Psi[l] phi'(d_d) phi phi,
+ *   ik forces       b^_d = -i h_d f^2 w S~/D,  F_i,d = (2 q_i/V) sum_stencil B_d[l] phi phi phi.
+ * Pins (tests/test_oracle_pins.py): equal edges reproduce the cubic functions; a cubic system repeated
+ * along one axis (box 2L x L x L, k_cut doubled) has exactly twice the energy and the same forces; forces
+ * are -dE/dr by central differences per direction; Oracle B against Oracle A within the NFFT error.    */
+
+static double box_lmax(const double *Lb)
+{
+    double a = Lb[0] > Lb[1] ? Lb[0] : Lb[1];
+    return a > Lb[2] ? a : Lb[2];
+}
+
+/* |h|^2 Lmax^2 = nx^2 (Lmax/Lx)^2 + ny^2 (Lmax/Ly)^2 + nz^2 (Lmax/Lz)^2, in this order, fp64
+ * (the membership n in K is decided on this number: <= k_cut^2)                              */
+double orc_box_s(const double *Lb, int nx, int ny, int nz)
+{
+    double lm = box_lmax(Lb);
+    double ax = (lm / Lb[0]) * (lm / Lb[0]), ay = (lm / Lb[1]) * (lm / Lb[1]), az = (lm / Lb[2]) * (lm / Lb[2]);
+    return ((double)(nx * nx) * ax + (double)(ny * ny) * ay) + (double)(nz * nz) * az;
+}
+
+/* f^2(h) exp(-pi^2 |h|^2/alpha^2)/|h|^2 with |h|^2 = s/Lmax^2;  f = (1 + k^2 lambda^2/4)^-2, k = 2 pi |h| (Eq. 51, R19) */
+double orc_box_fw(const double *Lb, double s, double alpha, double lambda)
+{
+    double lm = box_lmax(Lb);
+    double h2 = s / (lm * lm);
+    double w = exp(-ORC_PI * ORC_PI * h2 / (alpha * alpha)) / h2;
+    if (lambda != 0.0) {
+        double g = 1.0 + ORC_PI * ORC_PI * lambda * lambda * h2;
+        w /= g * g * g * g;
+    }
+    return w;
+}
+
+int64_t orc_modes_box(int k_cut, const double *Lb, int *modes)
+{
+    int64_t c = 0;
+    for (int nz = -k_cut; nz <= k_cut; ++nz)
+        for (int ny = -k_cut; ny <= k_cut; ++ny)
+            for (int nx = -k_cut; nx <= k_cut; ++nx) {
+                if (nx == 0 && ny == 0 && nz == 0) continue;
+                if (orc_box_s(Lb, nx, ny, nz) > (double)(k_cut * k_cut)) continue;
+                if (modes) { modes[3 * c] = nx; modes[3 * c + 1] = ny; modes[3 * c + 2] = nz; }
+                ++c;
+            }
+    return c;
+}
+
+/* Oracle A for a box.  Same contract as orc_direct. */
+int orc_direct_box(int64_t N, const double *r, const double *q, const double *Lb, double alpha,
+                   int k_cut, double lambda, double *E, double *F,
+                   int64_t nsample, const int64_t *sample)
+{
+    int64_t nK = orc_modes_box(k_cut, Lb, NULL);
+    int *modes = (int *)malloc(sizeof(int) * 3 * (size_t)(nK > 0 ? nK : 1));
+    double *Sr = (double *)malloc(sizeof(double) * (size_t)(nK > 0 ? nK : 1));
+    double *Si = (double *)malloc(sizeof(double) * (size_t)(nK > 0 ? nK : 1));
+    double *x = (double *)malloc(sizeof(double) * 3 * (size_t)(N > 0 ? N : 1));
+    if (!modes || !Sr || !Si || !x) { free(modes); free(Sr); free(Si); free(x); return -1; }
+    orc_modes_box(k_cut, Lb, modes);
+    for (int64_t j = 0; j < N; ++j)
+        for (int d = 0; d < 3; ++d) x[3 * j + d] = frac_pos(r[3 * j + d], Lb[d]);
+    double V = Lb[0] * Lb[1] * Lb[2];
+#pragma omp parallel for schedule(static)
+    for (int64_t t = 0; t < nK; ++t) {
+        double sr = 0.0, si = 0.0;
+        int nx = modes[3 * t], ny = modes[3 * t + 1], nz = modes[3 * t + 2];
+        for (int64_t j = 0; j < N; ++j) {
+            double ph = 2.0 * ORC_PI * (nx * x[3 * j] + ny * x[3 * j + 1] + nz * x[3 * j + 2]);
+            sr += q[j] * cos(ph);
+            si -= q[j] * sin(ph);
+        }
+        Sr[t] = sr; Si[t] = si;
+    }
+    double e = 0.0;
+    for (int64_t t = 0; t < nK; ++t) {
+        double s = orc_box_s(Lb, modes[3 * t], modes[3 * t + 1], modes[3 * t + 2]);
+        e += orc_box_fw(Lb, s, alpha, lambda) * (Sr[t] * Sr[t] + Si[t] * Si[t]);
+    }
+    *E = e / (2.0 * ORC_PI * V);
+    if (F) {
+        int64_t nf = nsample > 0 ? nsample : N;
+#pragma omp parallel for schedule(static)
+        for (int64_t sI = 0; sI < nf; ++sI) {
+            int64_t i = nsample > 0 ? sample[sI] : sI;
+            double fx = 0.0, fy = 0.0, fz = 0.0;
+            for (int64_t t = 0; t < nK; ++t) {
+                int nx = modes[3 * t], ny = modes[3 * t + 1], nz = modes[3 * t + 2];
+                double ph = 2.0 * ORC_PI * (nx * x[3 * i] + ny * x[3 * i + 1] + nz * x[3 * i + 2]);
+                double im = Sr[t] * sin(ph) + Si[t] * cos(ph);
+                double c = orc_box_fw(Lb, orc_box_s(Lb, nx, ny, nz), alpha, lambda) * im;
+                fx += (nx / Lb[0]) * c; fy += (ny / Lb[1]) * c; fz += (nz / Lb[2]) * c;
+            }
+            double pre = 2.0 * q[i] / V;
+            F[3 * sI] = pre * fx; F[3 * sI + 1] = pre * fy; F[3 * sI + 2] = pre * fz;
+        }
+    }
+    free(modes); free(Sr); free(Si); free(x);
+    return 0;
+}
+
+/* Step 1 with one edge per direction: u_d = n frac(r_d/L_d). */
+static void stencil_weights_box(const double *rj, const double *Lb, int n, int m, int window, double sigma,
+                                int *c, double *wt, double *dwt)
+{
+    for (int t = 0; t < 3; ++t) {
+        double u = n * frac_pos(rj[t], Lb[t]);
+        c[t] = (int)floor(u + 0.5);
+        for (int k = 0; k <= 2 * m; ++k) {
+            double d = u - (double)(c[t] - m + k);
+            wt[t * (2 * m + 1) + k] = orc_phi(window, m, sigma, d);
+            if (dwt) dwt[t * (2 * m + 1) + k] = orc_dphi(window, m, sigma, d);
+        }
+    }
+}
+
+/* Step 3 for a box (same triple loop as orc_spread). */
+void orc_spread_box(int64_t N, const double *r, const double *q, const double *Lb, int n, int m,
+                    int window, double sigma, double *g)
+{
+    int W = 2 * m + 1;
+    double wt[3 * 64];
+    int c[3];
+    for (int64_t j = 0; j < N; ++j) {
+        if (q[j] == 0.0) continue;
+        stencil_weights_box(&r[3 * j], Lb, n, m, window, sigma, c, wt, NULL);
+        for (int kz = 0; kz < W; ++kz) {
+            int lz = wrap_index(c[2] - m + kz, n);
+            for (int ky = 0; ky < W; ++ky) {
+                int ly = wrap_index(c[1] - m + ky, n);
+                double wyz = q[j] * wt[2 * W + kz] * wt[W + ky];
+                for (int kx = 0; kx < W; ++kx) {
+                    int lx = wrap_index(c[0] - m + kx, n);
+                    g[((size_t)lz * n + ly) * n + lx] += wyz * wt[kx];
+                }
+            }
+        }
+    }
+}
+
+/* Step 5 and the subdividing of step 6/7 for a box; same contract as orc_scale, S~ in orc_modes_box order. */
+double orc_scale_box(int n, int k_cut, const double *Lb, double alpha, double lambda, int window, int m,
+                     double sigma, const double *gh_re, const double *gh_im, int component,
+                     double *out_re, double *out_im, double *S_out_re, double *S_out_im)
+{
+    size_t n3 = (size_t)n * n * n;
+    if (out_re) { memset(out_re, 0, sizeof(double) * n3); memset(out_im, 0, sizeof(double) * n3); }
+    double e = 0.0;
+    int64_t c = 0;
+    for (int nz = -k_cut; nz <= k_cut; ++nz)
+        for (int ny = -k_cut; ny <= k_cut; ++ny)
+            for (int nx = -k_cut; nx <= k_cut; ++nx) {
+                if (nx == 0 && ny == 0 && nz == 0) continue;
+                double s = orc_box_s(Lb, nx, ny, nz);
+                if (s > (double)(k_cut * k_cut)) continue;
+                size_t idx = ((size_t)freq_index(nz, n) * n + freq_index(ny, n)) * n + freq_index(nx, n);
+                double D = orc_Phi(window, m, sigma, n, nx) * orc_Phi(window, m, sigma, n, ny)
+                         * orc_Phi(window, m, sigma, n, nz);
+                double sr = gh_re[idx] / D, si = gh_im[idx] / D;
+                double fw = orc_box_fw(Lb, s, alpha, lambda);
+                e += fw * (sr * sr + si * si);
+                if (S_out_re) { S_out_re[c] = sr; S_out_im[c] = si; }
+                if (out_re) {
+                    double pr = fw * sr / D, pi = fw * si / D;
+                    if (component < 0) {
+                        out_re[idx] = pr; out_im[idx] = pi;
+                    } else {
+                        double hd = component == 0 ? nx / Lb[0] : (component == 1 ? ny / Lb[1] : nz / Lb[2]);
+                        out_re[idx] = hd * pi; out_im[idx] = -hd * pr;      /* -i h_d (pr + i pi) */
+                    }
+                }
+                ++c;
+            }
+    return e / (2.0 * ORC_PI * Lb[0] * Lb[1] * Lb[2]);
+}
+
+/* Step 6/7 interpolation for a box; same contract as orc_gather. */
+void orc_gather_box(int64_t N, const double *r, const double *q, const double *Lb, int n, int m, int window,
+                    double sigma, int component, const double *field, double *F,
+                    int64_t nsample, const int64_t *sample)
+{
+    int W = 2 * m + 1;
+    int64_t nf = nsample > 0 ? nsample : N;
+    double V = Lb[0] * Lb[1] * Lb[2];
+#pragma omp parallel for schedule(static)
+    for (int64_t s = 0; s < nf; ++s) {
+        int64_t j = nsample > 0 ? sample[s] : s;
+        double wt[3 * 64], dwt[3 * 64];
+        int c[3];
+        stencil_weights_box(&r[3 * j], Lb, n, m, window, sigma, c, wt, dwt);
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+        for (int kz = 0; kz < W; ++kz) {
+            int lz = wrap_index(c[2] - m + kz, n);
+            for (int ky = 0; ky < W; ++ky) {
+                int ly = wrap_index(c[1] - m + ky, n);
+                for (int kx = 0; kx < W; ++kx) {
+                    int lx = wrap_index(c[0] - m + kx, n);
+                    double v = field[((size_t)lz * n + ly) * n + lx];
+                    if (component < 0) {
+                        a0 += v * dwt[kx] * wt[W + ky] * wt[2 * W + kz];
+                        a1 += v * wt[kx] * dwt[W + ky] * wt[2 * W + kz];
+                        a2 += v * wt[kx] * wt[W + ky] * dwt[2 * W + kz];
+                    } else {
+                        a0 += v * wt[kx] * wt[W + ky] * wt[2 * W + kz];
+                    }
+                }
+            }
+        }
+        if (component < 0) {
+            double pre = -q[j] * n / (ORC_PI * V);
+            F[3 * s] = pre / Lb[0] * a0; F[3 * s + 1] = pre / Lb[1] * a1; F[3 * s + 2] = pre / Lb[2] * a2;
+        } else {
+            F[3 * s + component] = 2.0 * q[j] / V * a0;
+        }
+    }
+}
+
+/* Whole Oracle B for a box; same contract as orc_enuf. */
+int orc_enuf_box(int64_t N, const double *r, const double *q, const double *Lb, double alpha, int k_cut,
+                 int n, int m, int window, double sigma, int variant, double lambda, int use_dft,
+                 double *E, double *F, int64_t nsample, const int64_t *sample,
+                 double *grid_out, double *S_out_re, double *S_out_im)
+{
+    if (n < 2 * m + 1 || (n & (n - 1)) || k_cut < 1 || 2 * k_cut > n || m < 1 || m > 20) return -2;
+    size_t n3 = (size_t)n * n * n;
+    double *g_re = (double *)calloc(n3, sizeof(double));
+    double *g_im = (double *)calloc(n3, sizeof(double));
+    double *p_re = (double *)malloc(sizeof(double) * n3);
+    double *p_im = (double *)malloc(sizeof(double) * n3);
+    if (!g_re || !g_im || !p_re || !p_im) { free(g_re); free(g_im); free(p_re); free(p_im); return -1; }
+
+    orc_spread_box(N, r, q, Lb, n, m, window, sigma, g_re);
+    if (grid_out) memcpy(grid_out, g_re, sizeof(double) * n3);
+    orc_fft3d(n, -1, use_dft, g_re, g_im);
+
+    if (variant == ORC_FORCE_ANALYTIC) {
+        *E = orc_scale_box(n, k_cut, Lb, alpha, lambda, window, m, sigma, g_re, g_im, -1,
+                           F ? p_re : NULL, p_im, S_out_re, S_out_im);
+        if (F) {
+            orc_fft3d(n, +1, use_dft, p_re, p_im);
+            orc_gather_box(N, r, q, Lb, n, m, window, sigma, -1, p_re, F, nsample, sample);
+        }
+    } else {
+        *E = orc_scale_box(n, k_cut, Lb, alpha, lambda, window, m, sigma, g_re, g_im, 0,
+                           NULL, NULL, S_out_re, S_out_im);
+        for (int d = 0; F && d < 3; ++d) {
+            orc_scale_box(n, k_cut, Lb, alpha, lambda, window, m, sigma, g_re, g_im, d,
+                          p_re, p_im, NULL, NULL);
+            orc_fft3d(n, +1, use_dft, p_re, p_im);
+            orc_gather_box(N, r, q, Lb, n, m, window, sigma, d, p_re, F, nsample, sample);
+        }
+    }
+    free(g_re); free(g_im); free(p_re); free(p_im);
+    return 0;
+}

@@ -77,6 +77,15 @@ def lib():
         L.orc_gather.argtypes = [i64, p, p, d, i, i, i, d, i, p, p, i64, pi64]
         L.orc_enuf.restype = i
         L.orc_enuf.argtypes = [i64, p, p, d, d, i, i, i, i, d, i, d, i, p, p, i64, pi64, p, p, p]
+        # orthorhombic boxes (Lb = three edges)
+        L.orc_box_s.restype = d; L.orc_box_s.argtypes = [p, i, i, i]
+        L.orc_box_fw.restype = d; L.orc_box_fw.argtypes = [p, d, d, d]
+        L.orc_modes_box.restype = i64; L.orc_modes_box.argtypes = [i, p, pi32]
+        L.orc_direct_box.restype = i
+        L.orc_direct_box.argtypes = [i64, p, p, p, d, i, d, p, p, i64, pi64]
+        L.orc_spread_box.restype = None; L.orc_spread_box.argtypes = [i64, p, p, p, i, i, i, d, p]
+        L.orc_enuf_box.restype = i
+        L.orc_enuf_box.argtypes = [i64, p, p, p, d, i, i, i, i, d, i, d, i, p, p, i64, pi64, p, p, p]
         _lib = L
     return _lib
 
@@ -241,3 +250,69 @@ def enuf_workload(w, variant="analytic", **kw):
     """Oracle B on an enuf_inputs.Workload (inputs promoted exactly to fp64)."""
     return enuf(w.r, w.q, w.L, w.alpha, w.k_cut, w.n, w.m, w.window, w.sigma,
                 variant=variant, slater_lambda=w.slater_lambda, **kw)
+
+
+# ------------------------------------------------------------------ orthorhombic boxes (SURVEY.md 8(f).4)
+
+def _box(Lb):
+    Lb = _f64(Lb).reshape(3)
+    return Lb
+
+
+def modes_box(k_cut, Lb):
+    """All n in K = {n != 0 : |h| Lmax <= k_cut}, h = n / Lb, as an (|K|, 3) int32 array (fixed order)."""
+    Lb = _box(Lb)
+    nk = lib().orc_modes_box(k_cut, _dp(Lb), None)
+    out = np.empty((nk, 3), dtype=np.int32)
+    lib().orc_modes_box(k_cut, _dp(Lb), out.ctypes.data_as(C.POINTER(C.c_int)))
+    return out
+
+
+def direct_box(r, q, Lb, alpha, k_cut, slater_lambda=0.0, forces=True, sample=None):
+    """Oracle A for a box with edges Lb: (E_rec, F)."""
+    r, q, Lb = _f64(r), _f64(q), _box(Lb)
+    N = q.shape[0]
+    E = C.c_double(0.0)
+    F = None
+    ns, sp = 0, None
+    if sample is not None:
+        sample = np.ascontiguousarray(np.asarray(sample, dtype=np.int64))
+        ns, sp = sample.shape[0], sample.ctypes.data_as(C.POINTER(C.c_int64))
+    if forces:
+        F = np.zeros((ns if ns else N, 3))
+    rc = lib().orc_direct_box(N, _dp(r), _dp(q), _dp(Lb), alpha, k_cut, slater_lambda, C.byref(E),
+                              _dp(F), ns, sp)
+    if rc:
+        raise MemoryError("orc_direct_box failed")
+    return E.value, F
+
+
+def spread_box(r, q, Lb, n, m, window, sigma=2.0):
+    r, q, Lb = _f64(r), _f64(q), _box(Lb)
+    g = np.zeros((n, n, n))
+    lib().orc_spread_box(q.shape[0], _dp(r), _dp(q), _dp(Lb), n, m, WINDOWS[window], sigma, _dp(g))
+    return g
+
+
+def enuf_box(r, q, Lb, alpha, k_cut, n, m, window, sigma=2.0, variant="analytic",
+             slater_lambda=0.0, use_dft=False, forces=True, sample=None, want_grid=False, want_S=False):
+    """Oracle B for a box with edges Lb; same returns as enuf(), S over modes_box(k_cut, Lb)."""
+    r, q, Lb = _f64(r), _f64(q), _box(Lb)
+    N = q.shape[0]
+    E = C.c_double(0.0)
+    ns, sp = 0, None
+    if sample is not None:
+        sample = np.ascontiguousarray(np.asarray(sample, dtype=np.int64))
+        ns, sp = sample.shape[0], sample.ctypes.data_as(C.POINTER(C.c_int64))
+    F = np.zeros((ns if ns else N, 3)) if forces else None
+    grid = np.zeros((n, n, n)) if want_grid else None
+    sr = si = None
+    if want_S:
+        nk = lib().orc_modes_box(k_cut, _dp(Lb), None)
+        sr = np.empty(nk); si = np.empty(nk)
+    rc = lib().orc_enuf_box(N, _dp(r), _dp(q), _dp(Lb), alpha, k_cut, n, m, WINDOWS[window], sigma,
+                            VARIANTS[variant], slater_lambda, int(use_dft), C.byref(E), _dp(F),
+                            ns, sp, _dp(grid), _dp(sr), _dp(si))
+    if rc:
+        raise RuntimeError(f"orc_enuf_box failed with code {rc}")
+    return {"E": E.value, "F": F, "grid": grid, "S": (sr + 1j * si) if want_S else None}

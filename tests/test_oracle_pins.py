@@ -502,3 +502,119 @@ def test_slater_real_space_factors(oracle):
     e2, F2 = oracle.real_forces(r2, q2, 50.0, 1e-9, 1.0, slater_lambda=lam)
     assert e2.sum() == pytest.approx(oracle.slater_BU(0.3, lam) / 0.3, rel=1e-8)
     assert F2[1, 0] == pytest.approx(oracle.slater_BF(0.3, lam) / 0.09, rel=1e-8)
+
+
+# ----------------------------------------------------------------- orthorhombic boxes
+
+def _box_gas(N, Lb, seed):
+    rng = np.random.default_rng(seed)
+    r = rng.uniform(0.0, 1.0, size=(N, 3)) * np.asarray(Lb)
+    q = np.where(np.arange(N) % 2 == 0, 1.0, -1.0) * (1.0 + 0.2 * rng.uniform(size=N))
+    q -= q.mean()
+    return r, q
+
+
+def test_box_with_equal_edges_is_the_cubic_case(oracle):
+    L, alpha, kc, n, m = 5.0, 1.2, 7, 32, 3
+    r, q = random_neutral_gas(20, L, seed=11)
+    Lb = [L, L, L]
+    assert np.array_equal(oracle.modes_box(kc, Lb), oracle.modes(kc))
+    Ea, Fa = oracle.direct(r, q, L, alpha, kc, slater_lambda=0.3)
+    Eb, Fb = oracle.direct_box(r, q, Lb, alpha, kc, slater_lambda=0.3)
+    assert abs(Ea - Eb) <= 1e-13 * abs(Ea) and np.abs(Fa - Fb).max() <= 1e-13 * np.abs(Fa).max()
+    for variant in ("analytic", "ik"):
+        a = oracle.enuf(r, q, L, alpha, kc, n, m, "kaiser_bessel", variant=variant, want_S=True)
+        b = oracle.enuf_box(r, q, Lb, alpha, kc, n, m, "kaiser_bessel", variant=variant, want_S=True)
+        assert abs(a["E"] - b["E"]) <= 1e-13 * abs(a["E"])
+        assert np.abs(a["F"] - b["F"]).max() <= 1e-13 * np.abs(a["F"]).max()
+        assert np.abs(a["S"] - b["S"]).max() <= 1e-13 * np.abs(a["S"]).max()
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_box_supercell_doubles_the_energy(oracle, axis):
+    """A cubic cell repeated once along one axis is the same crystal: the box (2L, L, L) with k_cut doubled
+    holds exactly the cubic wave vectors (odd indices along the long axis have S = 0), so E doubles and
+    every copy feels the cubic forces.  Fixes the per-direction scaling of h, V and the cutoff set."""
+    L, alpha, kc = 4.0, 1.3, 5
+    r, q = random_neutral_gas(14, L, seed=21 + axis)
+    Ec, Fc = oracle.direct(r, q, L, alpha, kc)
+    Lb = [L, L, L]; Lb[axis] = 2 * L
+    shift = np.zeros(3); shift[axis] = L
+    r2 = np.concatenate([r, r + shift]); q2 = np.concatenate([q, q])
+    Eb, Fb = oracle.direct_box(r2, q2, Lb, alpha, 2 * kc)
+    assert abs(Eb - 2 * Ec) <= 1e-12 * abs(Ec)
+    assert np.abs(Fb[:14] - Fc).max() <= 1e-12 * np.abs(Fc).max()
+    assert np.abs(Fb[14:] - Fc).max() <= 1e-12 * np.abs(Fc).max()
+    # the mode set: n_axis even <-> a cubic mode; the count of modes with S != 0 is the cubic count
+    mb = oracle.modes_box(2 * kc, Lb)
+    even = mb[mb[:, axis] % 2 == 0].copy(); even[:, axis] //= 2
+    assert sorted(map(tuple, even)) == sorted(map(tuple, oracle.modes(kc)))
+
+
+def test_box_direct_forces_are_minus_gradient(oracle):
+    Lb = [3.0, 4.5, 6.1]
+    r, q = _box_gas(12, Lb, seed=3)
+    alpha, kc = 1.4, 9
+    _, F = oracle.direct_box(r, q, Lb, alpha, kc, slater_lambda=0.2)
+    h = 1e-5
+    for i in (0, 4, 11):
+        for d in range(3):
+            rp = r.copy(); rp[i, d] += h
+            rm = r.copy(); rm[i, d] -= h
+            ep, _ = oracle.direct_box(rp, q, Lb, alpha, kc, slater_lambda=0.2, forces=False)
+            em, _ = oracle.direct_box(rm, q, Lb, alpha, kc, slater_lambda=0.2, forces=False)
+            assert abs(F[i, d] + (ep - em) / (2 * h)) < 2e-9 * np.abs(F).max()
+    assert np.abs(F.sum(axis=0)).max() < 1e-12 * np.abs(F).max()
+
+
+def test_box_total_energy_independent_of_alpha(oracle):
+    """Real + reciprocal - self of a box does not depend on the splitting parameter: the real-space sum is done
+    here in numpy over image shells (erfc(alpha d)/d, Eq. 17) -- pins exp(-pi^2 h^2/alpha^2)/h^2 and 1/(2 pi V)."""
+    from scipy.special import erfc
+    Lb = np.array([3.0, 3.6, 4.4])
+    r, q = _box_gas(8, Lb, seed=9)
+    tot = []
+    for alpha, kc in ((1.6, 14), (2.0, 17)):
+        e_rec, _ = oracle.direct_box(r, q, Lb, alpha, kc, forces=False)
+        e_real = 0.0
+        for ix in range(-2, 3):
+            for iy in range(-2, 3):
+                for iz in range(-2, 3):
+                    sh = np.array([ix, iy, iz]) * Lb
+                    d = np.linalg.norm(r[:, None, :] - r[None, :, :] + sh, axis=2)
+                    qq = q[:, None] * q[None, :]
+                    if ix == iy == iz == 0:
+                        np.fill_diagonal(d, np.inf)
+                    e_real += 0.5 * (qq * erfc(alpha * d) / d).sum()
+        tot.append(e_real + e_rec - alpha / math.sqrt(math.pi) * (q ** 2).sum())
+    assert abs(tot[0] - tot[1]) < 1e-9 * abs(tot[0])
+
+
+@pytest.mark.parametrize("variant,bound", [("analytic", 2e-7), ("ik", 2e-7)])
+def test_box_enuf_against_direct(oracle, variant, bound):
+    Lb = [5.0, 6.5, 8.0]
+    r, q = _box_gas(40, Lb, seed=17)
+    alpha, kc, n, m = 1.0, 8, 32, 6
+    Ea, Fa = oracle.direct_box(r, q, Lb, alpha, kc)
+    b = oracle.enuf_box(r, q, Lb, alpha, kc, n, m, "kaiser_bessel", variant=variant, want_S=True)
+    assert abs(b["E"] - Ea) <= bound * abs(Ea)
+    assert np.abs(b["F"] - Fa).max() <= bound * np.abs(Fa).max()
+    # S~ mode by mode in modes_box order
+    ml = oracle.modes_box(kc, Lb)
+    x = r / np.asarray(Lb)
+    S = (q[None, :] * np.exp(-2j * np.pi * (ml @ x.T))).sum(axis=1)
+    assert np.abs(b["S"] - S).max() <= bound * np.abs(S).max()
+
+
+def test_box_analytic_variant_is_exact_gradient(oracle):
+    Lb = [4.0, 5.0, 7.0]
+    r, q = _box_gas(10, Lb, seed=5)
+    alpha, kc, n, m = 1.1, 7, 32, 3
+    F = oracle.enuf_box(r, q, Lb, alpha, kc, n, m, "gaussian", variant="analytic")["F"]
+    h = 1e-5
+    for i, d in ((0, 0), (3, 1), (9, 2), (5, 0), (5, 2)):
+        rp = r.copy(); rp[i, d] += h
+        rm = r.copy(); rm[i, d] -= h
+        ep = oracle.enuf_box(rp, q, Lb, alpha, kc, n, m, "gaussian", forces=False)["E"]
+        em = oracle.enuf_box(rm, q, Lb, alpha, kc, n, m, "gaussian", forces=False)["E"]
+        assert abs(F[i, d] + (ep - em) / (2 * h)) < 5e-9 * np.abs(F).max(), (i, d)
