@@ -102,6 +102,21 @@ enum enuf_stage {
 int enuf_plan_create(enuf_plan **out, int64_t N, double L, double alpha, int k_cut, int M,
                      double sigma, int m);
 
+/*
+ * The same for an orthorhombic periodic box with edges Lb[0..2] = (Lx, Ly, Lz) (host pointer, copied).  The
+ * paper treats the cubic box and names other boxes as motivation (:35, :609); this is the Ewald
+ * sum of such a cell written the same way (reading R26): x_d = r_d / L_d, wave vectors
+ * k = 2 pi h with h = (nx/Lx, ny/Ly, nz/Lz), V = Lx Ly Lz,
+ *   E~    = (1/(2 pi V)) sum_K f^2 exp(-pi^2 |h|^2/alpha^2)/|h|^2 |S~(n)|^2,
+ *   K     = { n != 0 : |h| Lmax <= k_cut }, Lmax = max(Lx, Ly, Lz)  (every |n_d| <= k_cut L_d/Lmax <= k_cut),
+ * ONE grid size n = sigma*M in all three directions (grid spacing L_d/n), forces -(q n/(pi V L_d)) sum Psi phi' phi phi
+ * (analytic) or (2 q/V) sum B_d phi phi phi with b^_d = -i h_d psi^ (ik).  Equal edges give enuf_plan_create
+ * exactly.  Everything else (options, evaluation calls, sharded halves, layouts) is the same;
+ * enuf_plan_structure_factor takes modes of this K; enuf_real_space returns ENUF_EINVAL (cubic only).
+ */
+int enuf_plan_create_box(enuf_plan **out, int64_t N, const double *Lb, double alpha, int k_cut, int M,
+                         double sigma, int m);
+
 /* Change an option (see enuf_option).  Tables are rebuilt lazily at the next evaluation. */
 int enuf_plan_set(enuf_plan *plan, int key, double value);
 

@@ -663,12 +663,12 @@ int orc_enuf(int64_t N, const double *r, const double *q, double L, double alpha
 /* =================================================================== orthorhombic boxes
  * SURVEY.md section 8(f).4.  The paper treats the cubic box only and names non-cubic
  * boxes as motivation (:35, :609); this is the textbook Ewald sum of a cell with edges
- * Lb = (Lx, Ly, Lz), volume V = Lx Ly Lz, written out the same way (reading R20):
+ * Lb = (Lx, Ly, Lz), volume V = Lx Ly Lz, written out the same way (reading R26):
  *   x_d = r_d / L_d,  wave vector k = 2 pi h,  h = (nx/Lx, ny/Ly, nz/Lz),  n integer,
  *   S(n)  = sum_j q_j exp(-2 pi i n.x_j)                                         (Eq. 37)
  *   E_rec = (1/(2 pi V)) sum_K f^2(h) exp(-pi^2 |h|^2/alpha^2)/|h|^2 |S(n)|^2    (Eq. 38 with n/L -> h)
  *   F_i,d = (2 q_i/V) sum_K h_d f^2 exp(..)/|h|^2 Im{S e^{+2 pi i n.x_i}}        (Eq. 41 likewise)
- *   K     = { n != 0 : |h| Lmax <= k_cut },  Lmax = max(Lx, Ly, Lz)              (R20: a sphere of wave
+ *   K     = { n != 0 : |h| Lmax <= k_cut },  Lmax = max(Lx, Ly, Lz)              (R26: a sphere of wave
  *           vectors; every |n_d| <= k_cut L_d/Lmax <= k_cut; the cubic K of R4 when the edges are equal)
  * With Lx = Ly = Lz all of this is the cubic case above term by term.  The ENUF steps keep ONE grid size n
  * in all three directions (grid spacing L_d/n differs per direction); only u_d = n x_d, the weights and the

@@ -38,7 +38,7 @@ SYMBOLS = (
     "enuf_plan_copy_field", "enuf_plan_structure_factor", "enuf_spread_only",
     "enuf_plan_workspace_bytes", "enuf_plan_destroy", "enuf_last_error",
     "enuf_ncut", "enuf_alpha_from_rc", "enuf_rc_from_ncut",
-    "enuf_plan_create_auto", "enuf_plan_get",
+    "enuf_plan_create_auto", "enuf_plan_get", "enuf_plan_create_box",
 )
 GET_ALPHA, GET_K_CUT, GET_M, GET_GRID, GET_SUPPORT = 1, 2, 3, 4, 5
 
@@ -91,6 +91,8 @@ def lib():
         L.enuf_ncut.restype = i; L.enuf_ncut.argtypes = [d, d, d]
         L.enuf_alpha_from_rc.restype = d; L.enuf_alpha_from_rc.argtypes = [d, d]
         L.enuf_rc_from_ncut.restype = d; L.enuf_rc_from_ncut.argtypes = [i, d, d]
+        L.enuf_plan_create_box.restype = i
+        L.enuf_plan_create_box.argtypes = [C.POINTER(vp), i64, C.POINTER(d), d, i, i, d, i]
         L.enuf_plan_create_auto.restype = i
         L.enuf_plan_create_auto.argtypes = [C.POINTER(vp), i64, d, d, d, d, i]
         L.enuf_plan_get.restype = i; L.enuf_plan_get.argtypes = [vp, i, C.POINTER(d)]
@@ -146,7 +148,8 @@ class _DeviceBuffer:
 
 
 class Plan:
-    """enuf_plan_create / enuf_plan_set / enuf_energy_forces / enuf_plan_destroy."""
+    """enuf_plan_create (L a number) or enuf_plan_create_box (L = three edges) / enuf_plan_set /
+    enuf_energy_forces / enuf_plan_destroy."""
 
     def __init__(self, N, L, alpha, k_cut, M, sigma=2.0, m=6, dtype=None, window="kaiser_bessel",
                  variant="analytic", slater_lambda=0.0, profile=False, keep_spectrum=False, cuda_graph=False):
@@ -158,8 +161,15 @@ class Plan:
             raise ValueError("dtype must be torch.float32 or torch.float64")
         self.N, self.n = int(N), int(round(sigma * M))
         self.k_cut = int(k_cut)
-        _check(lib().enuf_plan_create(C.byref(self._h), int(N), float(L), float(alpha), int(k_cut),
-                                      int(M), float(sigma), int(m)))
+        if hasattr(L, "__len__"):      # (Lx, Ly, Lz): orthorhombic box, enuf_plan_create_box
+            if len(L) != 3:
+                raise ValueError("L must be a number or three box edges")
+            Lb = (C.c_double * 3)(*[float(v) for v in L])
+            _check(lib().enuf_plan_create_box(C.byref(self._h), int(N), Lb, float(alpha), int(k_cut),
+                                              int(M), float(sigma), int(m)))
+        else:
+            _check(lib().enuf_plan_create(C.byref(self._h), int(N), float(L), float(alpha), int(k_cut),
+                                          int(M), float(sigma), int(m)))
         self.set(OPT_PRECISION, F32 if self.dtype == torch.float32 else F64)
         self.set(OPT_WINDOW, WINDOWS[window])
         self.set(OPT_FORCE_VARIANT, VARIANTS[variant])

@@ -509,11 +509,20 @@ extern "C" {
 const char* enuf_last_error(void) { return g_err; }
 
 int enuf_plan_create(enuf_plan** out, int64_t N, double L, double alpha, int k_cut, int M, double sigma, int m) {
+    const double Lb[3] = {L, L, L};
+    return enuf_plan_create_box(out, N, Lb, alpha, k_cut, M, sigma, m);
+}
+
+int enuf_plan_create_box(enuf_plan** out, int64_t N, const double* Lb, double alpha, int k_cut, int M, double sigma,
+                         int m) {
     g_err[0] = 0;
     if (!out) return fail(ENUF_EINVAL, "out is NULL");
     *out = nullptr;
+    if (!Lb) return fail(ENUF_EINVAL, "Lb is NULL");
     if (N < 0 || N > 0xFFFFFFFFll) return fail(ENUF_EINVAL, "N = %lld out of range [0, 2^32)", (long long)N);
-    if (!(L > 0) || !std::isfinite(L)) return fail(ENUF_EINVAL, "L must be positive and finite");
+    for (int d = 0; d < 3; ++d)
+        if (!(Lb[d] > 0) || !std::isfinite(Lb[d])) return fail(ENUF_EINVAL, "L must be positive and finite");
+    const double L = Lb[0];
     if (!(alpha > 0) || !std::isfinite(alpha)) return fail(ENUF_EINVAL, "alpha must be positive and finite");
     if (M < 2) return fail(ENUF_EINVAL, "M must be >= 2");
     if (!(sigma > 1.0) || !std::isfinite(sigma)) return fail(ENUF_EINVAL, "sigma must be > 1");
@@ -527,6 +536,8 @@ int enuf_plan_create(enuf_plan** out, int64_t N, double L, double alpha, int k_c
     if (!p) return fail(ENUF_ENOMEM, "out of host memory");
     p->N_cap = p->N = N;
     p->L = L; p->alpha = alpha; p->sigma = sigma; p->k_cut = k_cut; p->M = M; p->n = n; p->m = m;
+    for (int d = 0; d < 3; ++d) p->Lb[d] = Lb[d];
+    p->box = !(Lb[0] == Lb[1] && Lb[1] == Lb[2]);
     p->tg.n = n;
     p->tg.nt = n / enuf::kTile;
     p->tg.nbins = p->tg.nt * p->tg.nt * n;
@@ -749,6 +760,7 @@ int enuf_real_space(enuf_plan* p, const void* r, const void* q, double r_cut, in
     g_err[0] = 0;
     if (!p) return fail(ENUF_EINVAL, "plan is NULL");
     if (p->N > 0 && (!r || !q || !F)) return fail(ENUF_EINVAL, "r, q and F must be non-NULL when N > 0");
+    if (p->box) return fail(ENUF_EINVAL, "the real-space part is built for cubic boxes only (DESIGN.md section 11)");
     if (!(r_cut > 0) || !(r_cut <= 0.5 * p->L))
         return fail(ENUF_EINVAL, "r_cut = %g must satisfy 0 < r_cut <= L/2 = %g (minimum image)", r_cut, 0.5 * p->L);
     int rc = prepare(p);
@@ -895,7 +907,18 @@ int enuf_plan_structure_factor(enuf_plan* p, int64_t count, const int* modes, do
     for (int64_t i = 0; i < count; ++i) {
         int nx = modes[3 * i], ny = modes[3 * i + 1], nz = modes[3 * i + 2];
         const int s = nx * nx + ny * ny + nz * nz;
-        if (s == 0 || s > kc * kc) return fail(ENUF_EINVAL, "mode %lld is outside 0 < |n|^2 <= k_cut^2", (long long)i);
+        bool in_k = s != 0 && s <= kc * kc;
+        if (p->box) {
+            // R26: |h|^2 Lmax^2 <= k_cut^2, the number fft_z_fused_kernel decides on (same products, same order)
+            double lm = p->Lb[0] > p->Lb[1] ? p->Lb[0] : p->Lb[1];
+            lm = lm > p->Lb[2] ? lm : p->Lb[2];
+            const volatile double tx = (double)(nx * nx) * ((lm / p->Lb[0]) * (lm / p->Lb[0]));
+            const volatile double ty = (double)(ny * ny) * ((lm / p->Lb[1]) * (lm / p->Lb[1]));
+            const volatile double tz = (double)(nz * nz) * ((lm / p->Lb[2]) * (lm / p->Lb[2]));
+            const volatile double txy = tx + ty;
+            in_k = s != 0 && std::abs(nx) <= kc && std::abs(ny) <= kc && std::abs(nz) <= kc && txy + tz <= (double)(kc * kc);
+        }
+        if (!in_k) return fail(ENUF_EINVAL, "mode %lld is outside the cutoff set K (0 < |n|^2 <= k_cut^2)", (long long)i);
         const bool conj = nx < 0;            // S~(-n) = conj S~(n): only kx >= 0 is stored
         if (conj) { nx = -nx; ny = -ny; nz = -nz; }
         const int kyp = ny >= 0 ? ny : ny + p->Ky, kzp = nz >= 0 ? nz : nz + p->Ky;

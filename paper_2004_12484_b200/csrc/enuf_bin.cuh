@@ -19,11 +19,11 @@ struct CellOfParticle {
 };
 
 template <typename T>
-__device__ __forceinline__ CellOfParticle locate(const T* __restrict__ r, int64_t j, double L, int n) {
+__device__ __forceinline__ CellOfParticle locate(const T* __restrict__ r, int64_t j, const Edges& L, int n) {
     CellOfParticle o;
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
-        double x = __ddiv_rn((double)r[3 * j + t], L);
+        double x = __ddiv_rn((double)r[3 * j + t], L.l[t]);
         x -= floor(x);
         if (x >= 1.0) x = 0.0;
         double u = __dmul_rn((double)n, x);
@@ -51,7 +51,7 @@ constexpr uint32_t kNoBin = 0xffffffffu;
 template <typename T>
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict__ F, int64_t N,
-                 double L, TileGeom g, uint32_t* __restrict__ count, uint32_t* __restrict__ scan_epoch,
+                 Edges L, TileGeom g, uint32_t* __restrict__ count, uint32_t* __restrict__ scan_epoch,
                  uint2* __restrict__ binrank) {
     pdl_prologue();
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -221,7 +221,7 @@ bin_scan_single_kernel(uint32_t* __restrict__ count, int nbins, unsigned long lo
 // ks_x / ks_y = (d0 > 0) of the trimmed stencils (the spreading producer culls on the cell word alone).
 template <typename T>
 __global__ void __launch_bounds__(256)
-bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, double L, TileGeom g,
+bin_scatter_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, Edges L, TileGeom g,
                    const uint32_t* __restrict__ offset, const uint2* __restrict__ binrank, PSlot<T>* __restrict__ slots) {
     pdl_prologue();
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

@@ -113,6 +113,10 @@ __device__ __forceinline__ void pdl_prologue() {
 }
 
 // ---------------------------------------------------------------- mbarrier (shared::cta) wrappers
+// Box edges per direction (cubic: three times L).  Orthorhombic boxes keep ONE grid size n in all directions
+// (R26); only x_d = r_d / L_d, the k-space weight and the force prefactors know the edges.
+struct Edges { double l[3]; };
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");

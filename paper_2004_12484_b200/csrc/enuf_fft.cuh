@@ -507,6 +507,17 @@ struct ScaleTables {
     const void* iphi;   // [kcut+1]   1/Phi(k)
     const void* wf;     // [kcut^2+1] f^2 w, entry 0 unused (= 0)
 };
+// Orthorhombic plans (kBox; R26): the weight is not a function of the integer |n|^2, so it is evaluated
+// in place, in fp64, from s = |h|^2 Lmax^2 = nx^2 (Lmax/Lx)^2 + ny^2 (Lmax/Ly)^2 + nz^2 (Lmax/Lz)^2 (each product and
+// sum rounded once, in this order: membership s <= k_cut^2 is decided on this number):
+//   w = f^2 exp(-pi^2 |h|^2/alpha^2)/|h|^2,  f^2 = (1 + pi^2 lambda^2 |h|^2)^-4,  |h|^2 = s/Lmax^2    (length^2)
+// rounded once to T like the tables.  ik variant: b^_d = -i h_d psi^, h_d = n_d / L_d.
+struct BoxScale {
+    double a[3];        // (Lmax/L_d)^2
+    double l[3];        // L_d
+    double lm2;         // Lmax^2
+    double alpha, lambda;
+};
 
 // Step a7 inside the Z pass: every CTA publishes its fp64 energy partial (thread 0's `mine`); the CTA that
 // finishes last sums all partials in a fixed order (strided per thread, then a tree: the same order whichever
@@ -536,12 +547,12 @@ __device__ __forceinline__ void z_pass_energy_finish(double mine, double* __rest
     if (threadIdx.x == 0) { *e_out = e_scale * fin[0]; *done_count = 0u; }
 }
 
-template <typename T, int N, int NOUT>
+template <typename T, int N, int NOUT, bool kBox = false>
 __global__ void __launch_bounds__(kFftThreads)
 fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __restrict__ out2, FftGeom fg,
                    const Cx<T>* __restrict__ tw, ScaleTables st, double* __restrict__ e_partial,
                    Cx<T>* __restrict__ spectrum, unsigned* __restrict__ done_count, double e_scale,
-                   double* __restrict__ e_out) {
+                   double* __restrict__ e_out, const BoxScale bs) {
     pdl_prologue();
     using SF = FftShape<N, -1>;
     using SI = FftShape<N, +1>;
@@ -560,7 +571,8 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
     const int ky = kyp <= fg.kcut ? kyp : kyp - fg.Ky;
     const int kc2 = fg.kcut * fg.kcut;
     const int kxy2 = kx * kx + ky * ky;
-    const bool inside = live && kx <= fg.kcut && kxy2 <= kc2;
+    const double sxy = kBox ? __dadd_rn(__dmul_rn((double)(kx * kx), bs.a[0]), __dmul_rn((double)(ky * ky), bs.a[1])) : 0.0;
+    const bool inside = live && kx <= fg.kcut && (kBox ? sxy <= (double)kc2 : kxy2 <= kc2);
     const unsigned zstride = (unsigned)fg.Ky * (unsigned)fg.Kxp;   // all offsets fit 32 bits (<= 2^23 elements)
     Cx<T>* base = A2 + (size_t)kyp * fg.Kxp + kx;
     const Cx<T> zero = cx_make<T>((T)0, (T)0);
@@ -603,9 +615,27 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
             kzs[r] = kz;
             const int akz = kz < 0 ? -kz : kz;
             const int s = kxy2 + kz * kz;
-            if (inside && akz <= fg.kcut && s <= kc2 && s > 0) {
+            bool in_k = inside && akz <= fg.kcut && s > 0;
+            T w = (T)0;
+            if constexpr (kBox) {
+                const double sb = __dadd_rn(sxy, __dmul_rn((double)(kz * kz), bs.a[2]));
+                in_k = in_k && sb <= (double)kc2;
+                if (in_k) {
+                    constexpr double PI = 3.14159265358979323846264338327950288;
+                    const double h2 = sb / bs.lm2;
+                    double wd = exp(-PI * PI * h2 / (bs.alpha * bs.alpha)) / h2;
+                    if (bs.lambda != 0.0) {
+                        const double gq = 1.0 + PI * PI * bs.lambda * bs.lambda * h2;
+                        wd /= (gq * gq) * (gq * gq);
+                    }
+                    w = (T)wd;
+                }
+            } else {
+                in_k = in_k && s <= kc2;
+                if (in_k) w = wf[s];
+            }
+            if (in_k) {
                 const T ip3 = ipxy * iphi[akz];
-                const T w = wf[s];
                 Cx<T> S = cx_make<T>(v[r].x * ip3, v[r].y * ip3);
                 e_acc += mult * (double)w * ((double)S.x * (double)S.x + (double)S.y * (double)S.y);
                 if (spectrum) {
@@ -631,7 +661,8 @@ fft_z_fused_kernel(Cx<T>* __restrict__ A2, Cx<T>* __restrict__ out1, Cx<T>* __re
             // b^_d = -i n_d psi^ :  -i (x + i y) = y - i x
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
-                const T nd = (T)(d == 0 ? kx : (d == 1 ? ky : kzs[r]));
+                const int ni = d == 0 ? kx : (d == 1 ? ky : kzs[r]);
+                const T nd = kBox ? (T)((double)ni / bs.l[d]) : (T)ni;
                 v[r] = cx_make<T>(nd * keep[r].y, -nd * keep[r].x);
             }
             if (d > 0) __syncthreads();

@@ -87,7 +87,7 @@ template <typename T, int M_, bool kIk, bool kTrim = false>
 __global__ void __launch_bounds__(GatherCfg<M_, kTrim>::NT)
 gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
-              const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F) {
+              const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F, T ry, T rz) {
     pdl_prologue();
     using C = GatherCfg<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
@@ -345,7 +345,8 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
                         T kk = (b2 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, b2 ? k0 : k1, 4);
                         kk += __shfl_xor_sync(0xffffffffu, kk, 2);
                         kk += __shfl_xor_sync(0xffffffffu, kk, 1);
-                        if (act && (l16 & 3) == 0 && l16 < 12) F[3 * jp + (l16 >> 2)] = sc * kk;
+                        // (ry, rz: the y and z prefactors of an orthorhombic box relative to x; 1 otherwise)
+                        if (act && (l16 & 3) == 0 && l16 < 12) F[3 * jp + (l16 >> 2)] = sc * kk * (l16 < 4 ? (T)1 : (l16 < 8 ? ry : rz));
                     }
                 }
                 __syncwarp();                        // the batch's weight rows are rewritten next
@@ -527,7 +528,7 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
                 k += __shfl_xor_sync(0xffffffffu, k, 4);
                 k += __shfl_xor_sync(0xffffffffu, k, 2);
                 k += __shfl_xor_sync(0xffffffffu, k, 1);
-                if ((lane & 7) == 0 && lane < 24) F[3 * j + (lane >> 3)] = (T)((A)sc * k);
+                if ((lane & 7) == 0 && lane < 24) F[3 * j + (lane >> 3)] = (T)((A)sc * k) * (lane < 8 ? (T)1 : (lane < 16 ? ry : rz));
             }
         }
         __syncwarp();

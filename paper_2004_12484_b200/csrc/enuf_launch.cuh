@@ -129,7 +129,8 @@ int configure_kernels(enuf_plan* p) {
                   && set_smem(fft_x_forward_tma_kernel<T, N_>, fft_xf_tma_smem_bytes<T, N_>())
                   && set_smem(fft_x_inverse_tma_kernel<T, N_>, fft_xi_tma_smem_bytes<T, N_>(p->Kxp))
                   && set_smem(fft_y_forward_kernel<T, N_>, sb) && set_smem(fft_y_inverse_kernel<T, N_>, sb)
-                  && set_smem(fft_z_fused_kernel<T, N_, 1>, sb) && set_smem(fft_z_fused_kernel<T, N_, 3>, sb);
+                  && set_smem(fft_z_fused_kernel<T, N_, 1>, sb) && set_smem(fft_z_fused_kernel<T, N_, 3>, sb)
+                  && set_smem(fft_z_fused_kernel<T, N_, 1, true>, sb) && set_smem(fft_z_fused_kernel<T, N_, 3, true>, sb);
         return ok ? 0 : -1;
     });
 }
@@ -145,7 +146,7 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     const unsigned blocks = (unsigned)((N + 255) / 256);
     const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
     pdl_launch(p, bin_count_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q),
-                                               static_cast<T*>(F), N, p->L, p->tg, p->bin_count, p->scan_epoch, p->binrank);
+                                               static_cast<T*>(F), N, Edges{{p->Lb[0], p->Lb[1], p->Lb[2]}}, p->tg, p->bin_count, p->scan_epoch, p->binrank);
     int nlaunch = 4;
     if ((int)sblocks <= kScanMaxResident && (int)sblocks <= p->num_sms) {
         // every scan CTA is resident at once: one launch, chunk totals exchanged through scan_desc
@@ -157,8 +158,8 @@ int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
         pdl_launch(p, bin_scan_apply_kernel, sblocks, kScanThreads, 0, s, p->bin_count, nbins, p->scan_total, p->bin_offset,
                                                               p->bin_cursor);
     }
-    pdl_launch(p, bin_scatter_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q), N, p->L,
-                                                 p->tg, p->bin_offset, p->binrank, static_cast<PSlot<T>*>(p->rec));
+    pdl_launch(p, bin_scatter_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q), N,
+                                                 Edges{{p->Lb[0], p->Lb[1], p->Lb[2]}}, p->tg, p->bin_offset, p->binrank, static_cast<PSlot<T>*>(p->rec));
     // window rows of the sorted particles (read by the spreading kernel); N bounds the number of charged particles
     const unsigned rblocks = (unsigned)((N + 31) / 32);
     const int rc = dispatch_m(p, [&](auto mc) -> int {
@@ -266,16 +267,31 @@ int launch_fft_backward(enuf_plan* p) {
         const unsigned bz = (unsigned)(((size_t)p->Ky * p->Kxp + LPC - 1) / LPC);
         if ((int)bz > p->n_partial) return -1;
         Cx<T>* spec = p->keep_spectrum ? static_cast<Cx<T>*>(p->spectrum) : nullptr;
-        const double e_scale = 1.0 / (2.0 * 3.14159265358979323846 * p->L);   // Eq. 38: C/(2 pi L), C = 1
-        if (nout == 1)
-            pdl_launch(p, fft_z_fused_kernel<T, N_, 1>, bz, kFftThreads, sb, s, static_cast<Cx<T>*>(p->A2[0]), nullptr, nullptr,
-                                                                    fg, tw, st, p->e_partial, spec, p->fft_done,
-                                                                    e_scale, p->e_dev);
+        // Eq. 38: C/(2 pi L), C = 1; a box (weights in length^2, fft_z_fused_kernel): 1/(2 pi V)
+        const double PI = 3.14159265358979323846;
+        const double e_scale = p->box ? 1.0 / (2.0 * PI * p->Lb[0] * p->Lb[1] * p->Lb[2]) : 1.0 / (2.0 * PI * p->L);
+        BoxScale bs{};
+        {
+            double lm = p->Lb[0] > p->Lb[1] ? p->Lb[0] : p->Lb[1];
+            lm = lm > p->Lb[2] ? lm : p->Lb[2];
+            for (int d = 0; d < 3; ++d) { bs.a[d] = (lm / p->Lb[d]) * (lm / p->Lb[d]); bs.l[d] = p->Lb[d]; }
+            bs.lm2 = lm * lm; bs.alpha = p->alpha; bs.lambda = p->lambda;
+        }
+        Cx<T>* a0 = static_cast<Cx<T>*>(p->A2[0]);
+        Cx<T>* a1 = nout == 3 ? static_cast<Cx<T>*>(p->A2[1]) : nullptr;
+        Cx<T>* a2 = nout == 3 ? static_cast<Cx<T>*>(p->A2[2]) : nullptr;
+        if (nout == 1 && !p->box)
+            pdl_launch(p, fft_z_fused_kernel<T, N_, 1>, bz, kFftThreads, sb, s, a0, a1, a2, fg, tw, st, p->e_partial, spec,
+                       p->fft_done, e_scale, p->e_dev, bs);
+        else if (nout == 1)
+            pdl_launch(p, fft_z_fused_kernel<T, N_, 1, true>, bz, kFftThreads, sb, s, a0, a1, a2, fg, tw, st, p->e_partial, spec,
+                       p->fft_done, e_scale, p->e_dev, bs);
+        else if (!p->box)
+            pdl_launch(p, fft_z_fused_kernel<T, N_, 3>, bz, kFftThreads, sb, s, a0, a1, a2, fg, tw, st, p->e_partial, spec,
+                       p->fft_done, e_scale, p->e_dev, bs);
         else
-            pdl_launch(p, fft_z_fused_kernel<T, N_, 3>, bz, kFftThreads, sb, s, static_cast<Cx<T>*>(p->A2[0]),
-                                                                    static_cast<Cx<T>*>(p->A2[1]),
-                                                                    static_cast<Cx<T>*>(p->A2[2]), fg, tw, st,
-                                                                    p->e_partial, spec, p->fft_done, e_scale, p->e_dev);
+            pdl_launch(p, fft_z_fused_kernel<T, N_, 3, true>, bz, kFftThreads, sb, s, a0, a1, a2, fg, tw, st, p->e_partial, spec,
+                       p->fft_done, e_scale, p->e_dev, bs);
         launches = 1;
         for (int d = 0; d < nout; ++d) {
             pdl_launch(p, fft_y_inverse_kernel<T, N_>, by, kFftThreads, sb, s, static_cast<const Cx<T>*>(p->A2[d]),
@@ -317,17 +333,21 @@ int launch_gather(enuf_plan* p, void* F) {
             using C = GatherCfg<M_, kTrim>;
             const size_t sb = gather_smem_bytes<T, M_, kTrim>();
             if (p->variant == ENUF_FORCE_ANALYTIC) {
-                const T pre = (T)(-(double)p->n / (PI * p->L * p->L));
+                // cubic: -n/(pi L^2); box: -n/(pi V L_d), as the x value and the ratios L_x/L_y, L_x/L_z (1 when cubic)
+                const double vol = p->Lb[0] * p->Lb[1] * p->Lb[2];
+                const T pre = p->box ? (T)(-(double)p->n / (PI * vol * p->Lb[0])) : (T)(-(double)p->n / (PI * p->L * p->L));
+                const T ry = p->box ? (T)(p->Lb[0] / p->Lb[1]) : (T)1, rz = p->box ? (T)(p->Lb[0] / p->Lb[2]) : (T)1;
                 pdl_launch(p, gather_kernel<T, M_, false, kTrim>, ntiles, C::NT, sb, s, 
                     static_cast<const T*>(p->grid[0]), static_cast<const PSlot<T>*>(p->rec),
-                    p->bin_offset, p->tg, p->wp, pa, pre, 0, static_cast<T*>(F));
+                    p->bin_offset, p->tg, p->wp, pa, pre, 0, static_cast<T*>(F), ry, rz);
                 return 1;
             }
-            const T pre = (T)(2.0 / (p->L * p->L));
+            // Eq. 42: 2/L^2 with b^_d = -i n_d ..; box: 2/V with b^_d = -i h_d .. (fft_z_fused_kernel)
+            const T pre = p->box ? (T)(2.0 / (p->Lb[0] * p->Lb[1] * p->Lb[2])) : (T)(2.0 / (p->L * p->L));
             for (int d = 0; d < 3; ++d)
                 pdl_launch(p, gather_kernel<T, M_, true, kTrim>, ntiles, C::NT, sb, s, 
                     static_cast<const T*>(p->grid[d]), static_cast<const PSlot<T>*>(p->rec),
-                    p->bin_offset, p->tg, p->wp, pa, pre, d, static_cast<T*>(F));
+                    p->bin_offset, p->tg, p->wp, pa, pre, d, static_cast<T*>(F), (T)1, (T)1);
             return 3;
         };
         if constexpr (M_ >= 5 && sizeof(T) == 4) {

@@ -9,7 +9,9 @@
 struct enuf_plan {
     // problem
     int64_t N_cap = 0, N = 0;
-    double L = 0, alpha = 0, sigma = 0;
+    double L = 0, alpha = 0, sigma = 0;   // L = Lb[0]
+    double Lb[3] = {0, 0, 0};             // box edges (enuf_plan_create: three times L)
+    bool box = false;                     // edges differ: orthorhombic plan (enuf_plan_create_box, R26)
     int k_cut = 0, M = 0, n = 0, m = 0;
     // options
     int precision = ENUF_F32, window = ENUF_WINDOW_KAISER_BESSEL, variant = ENUF_FORCE_ANALYTIC;

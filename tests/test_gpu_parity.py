@@ -92,6 +92,82 @@ def test_spread_grid_matches_oracle(enuf, torch_cuda, oracle, name):
     plan.close()
 
 
+# ------------------------------------------------------------------ orthorhombic boxes (DESIGN R26)
+
+def _box_inputs(N, Lb, seed, npdt):
+    rng = np.random.default_rng(seed)
+    r = (rng.uniform(-0.5, 1.5, size=(N, 3)) * np.asarray(Lb)).astype(npdt)      # also outside the box
+    q = (np.where(np.arange(N) % 2 == 0, 1.0, -1.0) * (1.0 + 0.25 * rng.uniform(size=N))).astype(npdt)
+    q[::11] = 0                                                                  # neutral particles: F = 0
+    return r, q
+
+
+@pytest.mark.parametrize("n,m,window,dtype,Lb", [
+    (32, 3, "gaussian", "f64", (5.0, 6.5, 8.0)), (64, 6, "kaiser_bessel", "f64", (9.0, 4.0, 6.0)),
+    (64, 4, "kaiser_bessel", "f32", (5.0, 7.5, 6.25)), (128, 6, "kaiser_bessel", "f32", (12.0, 12.0, 7.0)),
+    (128, 2, "bspline", "f64", (3.0, 9.0, 4.5)), (256, 5, "kaiser_bessel", "f32", (20.0, 30.0, 25.0)),
+])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_box_matches_oracle(enuf, torch_cuda, oracle, n, m, window, dtype, Lb, variant):
+    """enuf_plan_create_box against Oracle B for boxes (oracle.enuf_box): energy, forces, spread grid and S~(n)
+    over the box's cutoff set K (a sphere of wave vectors, an ellipsoid of indices)."""
+    torch = torch_cuda
+    N = 1531
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = _box_inputs(N, Lb, 500 + n + m, npdt)
+    M = n // 2
+    k_cut = M // 2
+    alpha = 0.9 * math.pi * k_cut / (max(Lb) * 3.0)
+    lam = 0.05 * min(Lb) if m == 4 else 0.0
+    ref = oracle.enuf_box(r, q, Lb, alpha, k_cut, n, m, window, 2.0, variant=variant, slater_lambda=lam,
+                          want_S=True, want_grid=True)
+    plan = enuf.Plan(N, Lb, alpha, k_cut, M, sigma=2.0, m=m, window=window, variant=variant, slater_lambda=lam,
+                     dtype=torch.float64 if dtype == "f64" else torch.float32, keep_spectrum=True)
+    rt, qt = torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda()
+    E, F = plan.energy_forces(rt, qt)
+    tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+    ml = oracle.modes_box(k_cut, Lb)
+    assert 0 < len(ml) < len(oracle.modes(k_cut))
+    S = plan.structure_factor(ml)
+    assert np.abs(S - ref["S"]).max() <= (1e-12 if dtype == "f64" else 5e-6) * np.abs(ref["S"]).max()
+    # a mode of the cubic sphere that lies outside the box's K is refused
+    inside = set(map(tuple, ml))
+    outside = next(tuple(v) for v in oracle.modes(k_cut) if tuple(v) not in inside)
+    with pytest.raises(enuf.EnufError):
+        plan.structure_factor(np.array([outside], dtype=np.int32))
+    g = plan.spread_only(rt, qt).numpy()
+    assert np.abs(g - ref["grid"]).max() <= (1e-13 if dtype == "f64" else 2e-6) * np.abs(ref["grid"]).max()
+    plan.close()
+
+
+def test_box_with_equal_edges_is_the_cubic_plan(enuf, torch_cuda):
+    torch = torch_cuda
+    w = make_workload("cfg3")
+    rt, qt = torch.from_numpy(w.r).cuda(), torch.from_numpy(w.q).cuda()
+    out = []
+    for L in (w.L, (w.L, w.L, w.L)):
+        plan = enuf.Plan(w.N, L, w.alpha, w.k_cut, w.M, sigma=w.sigma, m=w.m, window=w.window,
+                         slater_lambda=w.slater_lambda, dtype=torch.float32)
+        E, F = plan.energy_forces(rt, qt)
+        out.append((E, F.cpu().numpy()))
+        plan.close()
+    # same kernels, same tables; the order of particles inside a bin, hence the fp32 rounding of the spread sums,
+    # changes from run to run, so equality holds to rounding only
+    assert abs(out[0][0] - out[1][0]) <= 1e-7 * abs(out[0][0])
+    assert rel_rms(out[1][1], out[0][1]) <= 1e-6
+
+
+def test_box_rejects_real_space(enuf, torch_cuda):
+    torch = torch_cuda
+    plan = enuf.Plan(10, (4.0, 5.0, 6.0), 1.0, 8, 32, dtype=torch.float64)
+    r = torch.rand(10, 3, dtype=torch.float64, device="cuda"); q = torch.ones(10, dtype=torch.float64, device="cuda")
+    with pytest.raises(enuf.EnufError):
+        plan.real_space(r, q, 1.0)
+    plan.close()
+
+
 @pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
 def test_structure_factor_matches_oracle(enuf, torch_cuda, oracle, name):
     w = make_workload(name)
