@@ -258,6 +258,25 @@ enum { ENUF_GET_ALPHA = 1, ENUF_GET_K_CUT = 2, ENUF_GET_M = 3, ENUF_GET_GRID = 4
 int enuf_plan_create_auto(enuf_plan **out, int64_t N, double L, double delta, double r_c, double sigma, int m);
 int enuf_plan_get(const enuf_plan *plan, int key, double *value);
 
+/*
+ * Allocation-free entry point, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): the self term of the Ewald sum,
+ *     *E_self = (alpha / sqrt(pi)) sum_i q_i^2            (Eq. 24; subtracted in Eq. 25, :223)
+ * -- the value enuf_real_space returns as *E_self -- from N charges q (DEVICE pointer, fp32 or fp64 as `precision`
+ * = ENUF_F32 / ENUF_F64 says) into E_self (DEVICE pointer to one double), on `cuda_stream` (NULL = legacy default
+ * stream).  Asynchronous: the value is there when the stream reaches that point.  The sum is formed in fp64 in a
+ * fixed order, so the result is reproducible bit by bit.  No plan is needed and nothing is allocated or freed: the
+ * scratch of the reduction (per-CTA partial sums and a counter, 128.25 KiB) is a static device array inside the
+ * library, held by every GPU that loads it until the process exits.  Hence:
+ *   - N <= ENUF_SELF_STATIC_MAX_N (2^24); larger N returns ENUF_EINVAL and launches nothing (use enuf_real_space);
+ *   - every call shares that array: calls that can overlap on the GPU (different streams, or several host threads)
+ *     race with one another; successive calls on one stream are safe.
+ * ENUF_EINVAL for a NULL E_self, NULL q with N > 0, N < 0, a bad precision or alpha; ENUF_ECUDA for CUDA errors.
+ */
+#define ENUF_SELF_STATIC_MAX_N 16777216
+int enuf_self_energy_static(const void *q, int64_t N, int precision, double alpha, void *cuda_stream,
+                            double *E_self);
+
 #ifdef __cplusplus
 }
 #endif

@@ -38,8 +38,9 @@ SYMBOLS = (
     "enuf_plan_copy_field", "enuf_plan_structure_factor", "enuf_spread_only",
     "enuf_plan_workspace_bytes", "enuf_plan_destroy", "enuf_last_error",
     "enuf_ncut", "enuf_alpha_from_rc", "enuf_rc_from_ncut",
-    "enuf_plan_create_auto", "enuf_plan_get", "enuf_plan_create_box",
+    "enuf_plan_create_auto", "enuf_plan_get", "enuf_plan_create_box", "enuf_self_energy_static",
 )
+SELF_STATIC_MAX_N = 1 << 24
 GET_ALPHA, GET_K_CUT, GET_M, GET_GRID, GET_SUPPORT = 1, 2, 3, 4, 5
 
 
@@ -96,6 +97,8 @@ def lib():
         L.enuf_plan_create_auto.restype = i
         L.enuf_plan_create_auto.argtypes = [C.POINTER(vp), i64, d, d, d, d, i]
         L.enuf_plan_get.restype = i; L.enuf_plan_get.argtypes = [vp, i, C.POINTER(d)]
+        L.enuf_self_energy_static.restype = i
+        L.enuf_self_energy_static.argtypes = [vp, i64, i, d, vp, vp]
         _lib = L
     return _lib
 
@@ -378,6 +381,27 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+def self_energy_static(q, alpha, out):
+    """enuf_self_energy_static: E_self = (alpha / sqrt(pi)) sum q_i^2 of the CUDA tensor q (fp32 or fp64, contiguous)
+    into the one-element fp64 CUDA tensor `out`, on torch's current stream, asynchronously.  Allocates nothing (the
+    scratch is a static device array in the library): N <= SELF_STATIC_MAX_N, and calls that overlap on the GPU race."""
+    import torch
+    if not torch.cuda.is_available():
+        raise EnufError(ECUDA, "no CUDA device available; this library has no CPU fallback")
+    if not (isinstance(q, torch.Tensor) and q.is_cuda and q.is_contiguous() and q.dim() == 1
+            and q.dtype in (torch.float32, torch.float64)):
+        raise TypeError("q must be a contiguous 1-D CUDA tensor of float32 or float64")
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.numel() == 1
+            and out.device == q.device):
+        raise TypeError("out must be a one-element float64 CUDA tensor on q's device")
+    with torch.cuda.device(q.device):
+        _check(lib().enuf_self_energy_static(C.c_void_p(q.data_ptr()), int(q.shape[0]),
+                                             F32 if q.dtype == torch.float32 else F64, float(alpha),
+                                             C.c_void_p(torch.cuda.current_stream().cuda_stream),
+                                             C.c_void_p(out.data_ptr())))
+    return out
 
 
 def energy_forces(r, q, L, alpha, k_cut, M, sigma=2.0, m=6, **kw):

@@ -1009,3 +1009,111 @@ double enuf_rc_from_ncut(int n_c, double alpha, double L) {
 }
 
 }  // extern "C"
+
+// ====================================================================== allocation-free entry point
+// enuf_self_energy_static (include/enuf.h): E_self = (alpha / sqrt(pi)) sum_i q_i^2 (Eq. 24), the
+// quantity enuf_real_space returns as *E_self, for callers that must not allocate (CUDA graph capture, serving
+// loops).  It is the two-level fp64 reduction of the real-space path (per-CTA partial sums, then one fixed-order
+// final sum; enuf_real.cuh) with its scratch -- the partial sums and the count of finished CTAs -- in a file-scope
+// device array instead of plan workspace.  Every GPU that loads the library holds the array (128.25 KiB) until exit.
+// Every call shares it: calls that overlap on the GPU (two streams, two host threads) race; calls on one stream do not.
+namespace {
+
+constexpr int kSelfThreads = 256, kSelfPerCta = 4 * kSelfThreads;      // 1024 charges per CTA
+constexpr int64_t kSelfMaxN = (int64_t)1 << 24;                        // ENUF_SELF_STATIC_MAX_N
+constexpr int kSelfMaxCtas = (int)(kSelfMaxN / kSelfPerCta);           // 16384 partial sums
+constexpr size_t kSelfCountOffset = sizeof(double) * kSelfMaxCtas;     // the finished-CTA counter follows the partials
+static_assert(kSelfMaxN == ENUF_SELF_STATIC_MAX_N, "header and kernel limits differ");
+
+static __device__ __align__(256) unsigned char g_self_scratch[kSelfCountOffset + 256];
+
+// partial[b] = sum of q_i^2 over the CTA's 1024 charges (fp64; fp32 charges are promoted exactly).  The CTA that
+// finishes last adds the partials in a fixed order (strided per thread, then a tree: the same whichever CTA it is)
+// and writes out[0] = scale * sum.  *done must be 0 at launch (the host clears it on the stream before every launch).
+template <typename T>
+__global__ void __launch_bounds__(kSelfThreads)
+self_energy_static_kernel(const T* __restrict__ q, int64_t N, double scale, double* __restrict__ partial,
+                          unsigned* __restrict__ done, double* __restrict__ out) {
+    __shared__ double red[kSelfThreads];
+    __shared__ bool is_last;
+    const int64_t base = (int64_t)blockIdx.x * kSelfPerCta;
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < kSelfPerCta / kSelfThreads; ++k) {
+        const int64_t i = base + (int64_t)k * kSelfThreads + threadIdx.x;
+        if (i < N) { const double v = (double)q[i]; s += v * v; }
+    }
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = kSelfThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x] = red[0];
+        __threadfence();
+        is_last = atomicAdd(done, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    double t = 0.0;
+    for (unsigned i = threadIdx.x; i < gridDim.x; i += kSelfThreads) t += __ldcg(&partial[i]);
+    red[threadIdx.x] = t;
+    __syncthreads();
+    for (int o = kSelfThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[0] = scale * red[0];
+}
+
+// Device address of g_self_scratch on the current device.  In host code the array's name is only a handle:
+// the address comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int kSelfMaxDevices = 64;
+void* g_self_addr[kSelfMaxDevices] = {nullptr};
+int self_scratch_address(void** out) {
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (dev >= 0 && dev < kSelfMaxDevices) {
+        void* cached = __atomic_load_n(&g_self_addr[dev], __ATOMIC_ACQUIRE);
+        if (cached) { *out = cached; return ENUF_OK; }
+    }
+    void* ptr = nullptr;
+    CU(cudaGetSymbolAddress(&ptr, g_self_scratch));
+    if (!ptr) return fail(ENUF_ECUDA, "cudaGetSymbolAddress returned a null address");
+    if (dev >= 0 && dev < kSelfMaxDevices) __atomic_store_n(&g_self_addr[dev], ptr, __ATOMIC_RELEASE);
+    *out = ptr;
+    return ENUF_OK;
+}
+
+}  // namespace
+
+extern "C" int enuf_self_energy_static(const void* q, int64_t N, int precision, double alpha, void* cuda_stream,
+                                       double* E_self) {
+    g_err[0] = 0;
+    if (!E_self) return fail(ENUF_EINVAL, "E_self is NULL");
+    if (precision != ENUF_F32 && precision != ENUF_F64) return fail(ENUF_EINVAL, "precision must be ENUF_F32 or ENUF_F64");
+    if (!(alpha > 0) || !std::isfinite(alpha)) return fail(ENUF_EINVAL, "alpha must be positive and finite");
+    if (N < 0) return fail(ENUF_EINVAL, "N = %lld is negative", (long long)N);
+    if (N > kSelfMaxN)
+        return fail(ENUF_EINVAL, "N = %lld exceeds ENUF_SELF_STATIC_MAX_N = %lld, the size the static scratch array was "
+                    "built for; use enuf_real_space", (long long)N, (long long)kSelfMaxN);
+    if (N > 0 && !q) return fail(ENUF_EINVAL, "q must be non-NULL when N > 0");
+    void* scratch = nullptr;
+    int rc = self_scratch_address(&scratch);
+    if (rc) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    double* partial = static_cast<double*>(scratch);
+    unsigned* done = reinterpret_cast<unsigned*>(static_cast<unsigned char*>(scratch) + kSelfCountOffset);
+    const unsigned ctas = N > 0 ? (unsigned)((N + kSelfPerCta - 1) / kSelfPerCta) : 1u;
+    const double scale = alpha * 0.56418958354775628694807945156077;     // alpha / sqrt(pi)
+    // the array keeps what the last call left: the counter must start at zero (the partials are overwritten)
+    CU(cudaMemsetAsync(done, 0, sizeof(unsigned), s));
+    if (precision == ENUF_F32)
+        self_energy_static_kernel<float><<<ctas, kSelfThreads, 0, s>>>(static_cast<const float*>(q), N, scale, partial, done, E_self);
+    else
+        self_energy_static_kernel<double><<<ctas, kSelfThreads, 0, s>>>(static_cast<const double*>(q), N, scale, partial, done, E_self);
+    CU(cudaGetLastError());
+    return ENUF_OK;
+}
