@@ -318,7 +318,11 @@ def run_ours(args):
                 evaluate(pos_dev[s_], q_dev, F=F_dev, want_energy=False)
             torch.cuda.synchronize()
         sampler.wait_first(keep_busy)
-    plan.set(enuf.OPT_PROFILE, 1)                                  # per-stage events from here on
+    # Two passes over the same K steps.  The first is the timed region (`value`, `ms_per_step`): the library as a
+    # user runs it, no event between the kernels of an evaluation (each kernel is launched as a programmatic
+    # dependent of its predecessor, ENUF_OPT_PDL).  The second records the library's per-stage events
+    # (ENUF_OPT_PROFILE; an event between two kernels orders them fully) and gives `stages` and the roofline
+    # kernel's duration; its own step time is reported as `ms_per_step_profiled`.
     torch.cuda.synchronize()
     barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -332,8 +336,19 @@ def run_ours(args):
     torch.cuda.synchronize()
     barrier()
     ms_total = max_over_ranks(ev0.elapsed_time(ev1))
-    clocks = sampler.stop() if sampler else None
     E_last = plan.energy()
+    plan.set(enuf.OPT_PROFILE, 1)
+    torch.cuda.synchronize()
+    barrier()
+    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev2.record()
+    for s in range(K):
+        evaluate(pos_dev[W + s], q_dev, F=F_dev, want_energy=False)
+    ev3.record()
+    torch.cuda.synchronize()
+    barrier()
+    ms_step_profiled = max_over_ranks(ev2.elapsed_time(ev3)) / K
+    clocks = sampler.stop() if sampler else None
     stage_ms, n_prof = plan.stage_ms_mean()
     ms_step = ms_total / K
     value = N_sys / (ms_step * 1e-3) if sharded else whole_job_value(w.N, world, ms_step)
@@ -534,7 +549,7 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
+        "ms_per_step": ms_step, "ms_per_step_profiled": ms_step_profiled, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
         "config": {"workload": args.workload, "N": int(w.N), "L": w.L, "alpha": w.alpha, "k_cut": w.k_cut,
                    "M": w.M, "sigma": w.sigma, "n": w.n, "m": w.m, "window": w.window, "variant": args.variant,
