@@ -27,7 +27,8 @@
  * derivative by differences, DFT == radix-2 FFT == numpy.fft, additivity Eq. 61,
  * S~(n) vs S(n) mode by mode, error falls with m; B-spline window: m = 1 hat
  * function in closed form, partition of unity, transform by quadrature, derivative by differences,
- * brute force against Oracle A.
+ * brute force against Oracle A; sinc-power window (:266): transform by quadrature over the real line,
+ * m = 1 transform = the textbook triangle, derivative by differences (both branches), brute force against Oracle A.
  * Parity unpinned against the paper: the Slater form factor in k-space (R19) -- it is
  * BASELINE.json's variant, pinned only against quadrature of Eq. 51 and Oracle A.
  *
@@ -45,7 +46,7 @@
 
 #define ORC_PI 3.14159265358979323846264338327950288
 
-enum { ORC_WIN_GAUSSIAN = 0, ORC_WIN_KAISER_BESSEL = 1, ORC_WIN_BSPLINE = 2 };
+enum { ORC_WIN_GAUSSIAN = 0, ORC_WIN_KAISER_BESSEL = 1, ORC_WIN_BSPLINE = 2, ORC_WIN_SINC_POWER = 3 };
 enum { ORC_FORCE_ANALYTIC = 0, ORC_FORCE_IK = 1 };
 
 int orc_num_threads(void)
@@ -92,9 +93,25 @@ static double bspline_rec(int p, double x)
     return ((x + 0.5 * p) * bspline_rec(p - 1, x + 0.5) + (0.5 * p - x) * bspline_rec(p - 1, x - 0.5)) / (p - 1);
 }
 
+/* Sinc-power window (PAPER.md:266 names "sinc power functions" among the NFFT windows without a formula; the NFFT
+ * literature it cites has phi(x) ~ sinc^{2m}(pi N x (2 sigma - 1)/(2m)), whose transform is a B-spline of order 2m).
+ * With x = d/n, n = sigma N, and phi(0) = 1 (R7):
+ *     phi(d) = sinc(pi c d)^{2m},  c = (2 - 1/sigma)/(2m),  sinc(t) = sin(t)/t;
+ * sinc(pi c d) is the transform of a box of width c and height 1/c, so phi is the transform of the 2m-fold
+ * convolution of that box:  Phi(k) = (1/c) B_2m(k/(n c)),  B_2m the centred cardinal B-spline of order 2m.
+ * The window is not compactly supported; the stencil cuts it (R8), as it cuts the Gaussian. */
+static double sincpow_c(int m, double sigma)
+{
+    return (2.0 - 1.0 / sigma) / (2.0 * m);
+}
+
 double orc_phi(int window, int m, double sigma, double d)
 {
-    if (window == ORC_WIN_BSPLINE) {
+    if (window == ORC_WIN_SINC_POWER) {
+        double t = ORC_PI * sincpow_c(m, sigma) * d;
+        double sc = t == 0.0 ? 1.0 : sin(t) / t;
+        return pow(sc, 2 * m);
+    } else if (window == ORC_WIN_BSPLINE) {
         return bspline_rec(2 * m, d) / bspline_rec(2 * m, 0.0);
     } else if (window == ORC_WIN_GAUSSIAN) {
         return exp(-d * d / gauss_b(m, sigma));
@@ -114,7 +131,21 @@ double orc_phi(int window, int m, double sigma, double d)
 /* d phi / d d (used by the analytic-derivative force variant). */
 double orc_dphi(int window, int m, double sigma, double d)
 {
-    if (window == ORC_WIN_BSPLINE) {
+    if (window == ORC_WIN_SINC_POWER) {
+        /* d/dd sinc(t)^{2m} = 2m sinc^{2m-1} pi c (t cos t - sin t)/t^2, t = pi c d;
+         * (t cos t - sin t)/t^2 = sum_{k>=1} (-1)^k 2k/(2k+1)! t^(2k-1) without the cancellation for small t */
+        double pc = ORC_PI * sincpow_c(m, sigma), t = pc * d, g, sc;
+        if (fabs(t) < 0.5) {
+            double t2 = t * t;
+            g = -t * (1.0 / 3.0 - t2 * (1.0 / 30.0 - t2 * (1.0 / 840.0 - t2 * (1.0 / 45360.0
+                - t2 * (1.0 / 3991680.0 - t2 * (1.0 / 518918400.0 - t2 / 93405312000.0))))));
+            sc = t == 0.0 ? 1.0 : sin(t) / t;
+        } else {
+            g = (t * cos(t) - sin(t)) / (t * t);
+            sc = sin(t) / t;
+        }
+        return 2.0 * m * pow(sc, 2 * m - 1) * pc * g;
+    } else if (window == ORC_WIN_BSPLINE) {
         /* B_p' (x) = B_{p-1}(x + 1/2) - B_{p-1}(x - 1/2) */
         return (bspline_rec(2 * m - 1, d + 0.5) - bspline_rec(2 * m - 1, d - 0.5)) / bspline_rec(2 * m, 0.0);
     } else if (window == ORC_WIN_GAUSSIAN) {
@@ -154,7 +185,10 @@ static double bessel_i0(double x)
  * Phi(k) = int phi(d) exp(-2 pi i k d / n) dd.                                   */
 double orc_Phi(int window, int m, double sigma, int n, int k)
 {
-    if (window == ORC_WIN_BSPLINE) {
+    if (window == ORC_WIN_SINC_POWER) {
+        double c = sincpow_c(m, sigma);
+        return bspline_rec(2 * m, (double)k / (n * c)) / c;
+    } else if (window == ORC_WIN_BSPLINE) {
         /* B_p is the p-fold convolution of the unit box, whose transform at frequency k/n is sinc(pi k/n) */
         double t = ORC_PI * k / n, sc = k == 0 ? 1.0 : sin(t) / t;
         return pow(sc, 2 * m) / bspline_rec(2 * m, 0.0);

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "enuf_oracle.c")
 _LIB = os.path.join(_HERE, "libenuf_oracle.so")
 
-WINDOWS = {"gaussian": 0, "kaiser_bessel": 1, "bspline": 2}
+WINDOWS = {"gaussian": 0, "kaiser_bessel": 1, "bspline": 2, "sinc_power": 3}
 VARIANTS = {"analytic": 0, "ik": 1}
 
 _lib = None

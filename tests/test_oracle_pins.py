@@ -191,6 +191,80 @@ def test_bspline_enuf_against_direct_ewald(oracle, variant, bound):
             assert abs(b["F"][i, d] + (ep - em) / (2 * h)) < 1e-7 * np.abs(b["F"]).max()
 
 
+# ----------------------------------------------------------------- sinc-power window
+
+def test_sinc_power_m1_transform_is_the_hat_function(oracle):
+    """m = 1: phi = sinc^2(pi c d), c = (2 - 1/sigma)/2.  Its transform is the textbook triangle of half-width c and
+    height 1/c (int sinc^2(pi c d) dd = 1/c); at the grid frequency k/n: (1/c) max(0, 1 - |k|/(n c))."""
+    for sigma, n in ((2.0, 64), (1.5, 48)):
+        c = (2.0 - 1.0 / sigma) / 2.0
+        for k in (0, 1, 7, 20, int(n * c), int(n * c) + 3):
+            want = max(0.0, 1.0 - k / (n * c)) / c
+            assert abs(oracle.Phi("sinc_power", 1, sigma, n, k) - want) < 1e-14
+    # the window itself at a few points, written out
+    for d in (0.25, 1.0, 1.5):
+        t = math.pi * 0.75 * d
+        assert abs(oracle.phi("sinc_power", 1, 2.0, d) - (math.sin(t) / t) ** 2) < 1e-15
+    assert oracle.phi("sinc_power", 1, 2.0, 4.0 / 3.0) < 1e-30           # first zero of sinc(pi c d): d = 1/c
+
+
+@pytest.mark.parametrize("m", [2, 3, 4, 6])
+def test_sinc_power_transform_by_quadrature(oracle, m):
+    """Phi(k) = int phi(d) cos(2 pi k d/n) dd over the real line (the window is not compactly supported: the integral
+    is taken over |d| <= D and the tail bounded by 2 int_D^inf (pi c d)^(-2m) dd)."""
+    n, sigma, D = 64, 2.0, 300.0
+    c = (2.0 - 1.0 / sigma) / (2.0 * m)
+    tail = 2.0 * (math.pi * c) ** (-2 * m) * D ** (1 - 2 * m) / (2 * m - 1)
+    assert tail < 2e-8
+    for k in (0, 1, 5, 16, 30):
+        f = lambda d: oracle.phi("sinc_power", m, sigma, d) * math.cos(2 * math.pi * k * d / n)
+        val, _ = integrate.quad(f, -D, D, limit=20000, epsabs=1e-13, epsrel=1e-13)
+        assert abs(val - oracle.Phi("sinc_power", m, sigma, n, k)) < tail + 1e-11, (k, val)
+    assert abs(oracle.phi("sinc_power", m, sigma, 0.0) - 1.0) < 1e-15     # R7
+
+
+@pytest.mark.parametrize("m", [1, 2, 4, 6])
+def test_sinc_power_derivative_by_differences(oracle, m):
+    """phi' against central differences of phi on both branches of its evaluation (series for |pi c d| < 1/2, closed form
+    beyond), continuity at the switch, oddness."""
+    c = (2.0 - 0.5) / (2.0 * m)
+    h = 1e-5
+    for d in (-m - 0.4, -1.7, -0.3, -1e-3, 0.0, 1e-4, 0.05, 0.37, 1.0, 2.6, m - 0.5, m + 0.45):
+        fd = (oracle.phi("sinc_power", m, 2.0, d + h) - oracle.phi("sinc_power", m, 2.0, d - h)) / (2 * h)
+        an = oracle.dphi("sinc_power", m, 2.0, d)
+        assert abs(fd - an) < 2e-9, (d, fd, an)
+        assert oracle.dphi("sinc_power", m, 2.0, -d) == -an
+    ds = 0.5 / (math.pi * c)                                              # the switch between the branches
+    a, b = oracle.dphi("sinc_power", m, 2.0, ds * (1 - 1e-9)), oracle.dphi("sinc_power", m, 2.0, ds * (1 + 1e-9))
+    assert abs(a - b) < 1e-8 * abs(a)
+
+
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_sinc_power_enuf_against_direct_ewald(oracle, variant):
+    """Brute force: Oracle B with the sinc-power window against Oracle A on 64 particles; the error falls with m
+    (the stencil cuts the window at sinc(3 pi/4 (1 + 1/2m))^(2m), 3e-7 of the peak at m = 6)."""
+    L, alpha, kc, n = 6.0, 1.0, 8, 32
+    r, q = random_neutral_gas(64, L, seed=22)
+    Ea, Fa = oracle.direct(r, q, L, alpha, kc)
+    errs = []
+    for m in (2, 4, 6):
+        b = oracle.enuf(r, q, L, alpha, kc, n, m, "sinc_power", variant=variant)
+        errs.append(math.sqrt(((b["F"] - Fa) ** 2).sum() / (Fa ** 2).sum()))
+        if m == 6:
+            assert abs(b["E"] - Ea) < 1e-4 * abs(Ea)
+    assert errs[0] > 3 * errs[1] > 9 * errs[2], errs
+    assert errs[2] < (2e-3 if variant == "analytic" else 2e-4), errs
+    if variant == "analytic":       # exact gradient of the ENUF energy (R17)
+        h, m = 1e-5, 4
+        b = oracle.enuf(r, q, L, alpha, kc, n, m, "sinc_power", variant=variant)
+        for i, d in ((5, 1), (33, 0)):
+            rp = r.copy(); rp[i, d] += h
+            rm = r.copy(); rm[i, d] -= h
+            ep = oracle.enuf(rp, q, L, alpha, kc, n, m, "sinc_power", forces=False)["E"]
+            em = oracle.enuf(rm, q, L, alpha, kc, n, m, "sinc_power", forces=False)["E"]
+            assert abs(b["F"][i, d] + (ep - em) / (2 * h)) < 1e-7 * np.abs(b["F"]).max()
+
+
 @pytest.mark.parametrize("window,m", [("kaiser_bessel", 4), ("kaiser_bessel", 6), ("gaussian", 4)])
 def test_window_normalisation_symmetry_support(oracle, window, m):
     assert abs(oracle.phi(window, m, 2.0, 0.0) - 1.0) < 1e-15           # R7
