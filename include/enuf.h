@@ -49,7 +49,8 @@ enum enuf_status {
 enum enuf_option {
     ENUF_OPT_PRECISION = 1,      /* ENUF_F32 (default) | ENUF_F64; only before the first evaluation */
     ENUF_OPT_WINDOW = 2,         /* ENUF_WINDOW_KAISER_BESSEL (default) | ENUF_WINDOW_GAUSSIAN (R6) |
-                                    ENUF_WINDOW_BSPLINE: centred cardinal B-spline of order 2m (:266)  */
+                                    ENUF_WINDOW_BSPLINE: centred cardinal B-spline of order 2m (:266) |
+                                    ENUF_WINDOW_SINC_POWER: sinc(pi c d)^2m, c = (2 - 1/sigma)/(2m) (:266) */
     ENUF_OPT_FORCE_VARIANT = 3,  /* ENUF_FORCE_ANALYTIC (default) | ENUF_FORCE_IK (paper, Eq. 41)   */
     ENUF_OPT_SLATER_LAMBDA = 4,  /* decay length of the Slater density Eq. 51 (:407); 0 = point (R19) */
     ENUF_OPT_NUM_PARTICLES = 5,  /* lower N for the next calls, 0 <= N <= planned capacity          */
@@ -72,7 +73,7 @@ enum enuf_option {
 };
 
 enum { ENUF_F32 = 0, ENUF_F64 = 1 };
-enum { ENUF_WINDOW_GAUSSIAN = 0, ENUF_WINDOW_KAISER_BESSEL = 1, ENUF_WINDOW_BSPLINE = 2 };
+enum { ENUF_WINDOW_GAUSSIAN = 0, ENUF_WINDOW_KAISER_BESSEL = 1, ENUF_WINDOW_BSPLINE = 2, ENUF_WINDOW_SINC_POWER = 3 };
 enum { ENUF_FORCE_ANALYTIC = 0, ENUF_FORCE_IK = 1 };
 
 /* stage indices of enuf_plan_stage_ms() */

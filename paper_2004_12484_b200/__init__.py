@@ -24,7 +24,7 @@ OPT_PDL = 10
 OPT_SPREAD_SPARSE = 11
 OPT_CUDA_GRAPH = 9
 F32, F64 = 0, 1
-WINDOWS = {"gaussian": 0, "kaiser_bessel": 1, "bspline": 2}
+WINDOWS = {"gaussian": 0, "kaiser_bessel": 1, "bspline": 2, "sinc_power": 3}
 VARIANTS = {"analytic": 0, "ik": 1}
 STAGES = ("bin", "spread", "fft", "gather", "energy")
 

@@ -79,6 +79,11 @@ double bspline_deriv_host(int p, int i, double x) {
 // Window transform Phi(k) = int phi(d) exp(-2 pi i k d/n) dd for the phi(0)=1 windows (R6, R7)
 double window_transform(const enuf_plan* p, int k) {
     const double m = p->m, sg = p->sigma, n = p->n;
+    if (p->window == ENUF_WINDOW_SINC_POWER) {
+        // sinc(pi c d) is the transform of a box of width c and height 1/c; its 2m-th power that of their 2m-fold convolution
+        const double c = (2.0 - 1.0 / sg) / (2.0 * m);
+        return bspline_host(2 * p->m, k / (n * c)) / c;
+    }
     if (p->window == ENUF_WINDOW_BSPLINE) {
         // the order-2m B-spline is the 2m-fold convolution of the unit box: sinc(pi k/n)^(2m), over B_2m(0)
         const double t = kPi * k / n, sc = k == 0 ? 1.0 : std::sin(t) / t;
@@ -99,7 +104,10 @@ void fill_window_params(enuf_plan* p) {
     enuf::WindowParams& w = p->wp;
     w.kind = p->window;
     w.m = p->m;
-    if (p->window == ENUF_WINDOW_BSPLINE) {
+    if (p->window == ENUF_WINDOW_SINC_POWER) {
+        w.b = kPi * (2.0 - 1.0 / p->sigma) / (2.0 * p->m);   // phi = sinc(b d)^2m
+        w.inv_b = w.bm = w.inv1m = w.A = 0.0;
+    } else if (p->window == ENUF_WINDOW_BSPLINE) {
         w.b = w.inv_b = w.bm = w.inv1m = 0.0;
         w.A = 1.0 / bspline_host(2 * p->m, 0.0);       // phi = A B_2m
     } else if (p->window == ENUF_WINDOW_GAUSSIAN) {
@@ -122,6 +130,10 @@ void fill_window_params(enuf_plan* p) {
 // Only used to fit the polynomial table: the kernels cut the support themselves.
 double window_smooth(const enuf_plan* p, double d) {
     const double m = p->m, sg = p->sigma;
+    if (p->window == ENUF_WINDOW_SINC_POWER) {
+        const double t = kPi * (2.0 - 1.0 / sg) / (2.0 * m) * d;
+        return std::pow(t == 0.0 ? 1.0 : std::sin(t) / t, 2 * p->m);
+    }
     if (p->window == ENUF_WINDOW_GAUSSIAN) {
         const double b = 2.0 * sg * m / ((2.0 * sg - 1.0) * kPi);
         return std::exp(-d * d / b);
@@ -563,7 +575,8 @@ int enuf_plan_set(enuf_plan* p, int key, double value) {
             p->precision = iv;
             return ENUF_OK;
         case ENUF_OPT_WINDOW:
-            if (iv != ENUF_WINDOW_GAUSSIAN && iv != ENUF_WINDOW_KAISER_BESSEL && iv != ENUF_WINDOW_BSPLINE)
+            if (iv != ENUF_WINDOW_GAUSSIAN && iv != ENUF_WINDOW_KAISER_BESSEL && iv != ENUF_WINDOW_BSPLINE &&
+                iv != ENUF_WINDOW_SINC_POWER)
                 return fail(ENUF_EINVAL, "unknown window");
             p->window = iv; p->tables_dirty = true; fill_window_params(p);
             p->trim = p->precision == ENUF_F32 && p->window == ENUF_WINDOW_KAISER_BESSEL && p->m >= 5;

@@ -29,7 +29,7 @@ template <> struct Vec4<double> { using type = double4; };
 struct WindowParams {
     int kind;          // ENUF_WINDOW_*
     int m;
-    double b;          // Gaussian: 2 sigma m/((2 sigma-1) pi); Kaiser-Bessel: pi (2 - 1/sigma)
+    double b;          // Gaussian: 2 sigma m/((2 sigma-1) pi); Kaiser-Bessel: pi (2 - 1/sigma); sinc-power: pi (2 - 1/sigma)/(2m)
     double inv_b;      // 1/b (Gaussian)
     double bm;         // b*m
     double inv1m;      // 1/(1 - exp(-2 b m))      (Kaiser-Bessel)
@@ -178,6 +178,8 @@ __device__ __forceinline__ float r_exp(float x) { return expf(x); }
 __device__ __forceinline__ double r_exp(double x) { return exp(x); }
 __device__ __forceinline__ float r_expm1(float x) { return expm1f(x); }
 __device__ __forceinline__ double r_expm1(double x) { return expm1(x); }
+__device__ __forceinline__ void r_sincos(float x, float* s, float* c) { sincosf(x, s, c); }
+__device__ __forceinline__ void r_sincos(double x, double* s, double* c) { sincos(x, s, c); }
 __device__ __forceinline__ float r_sqrt(float x) { return sqrtf(x); }
 __device__ __forceinline__ double r_sqrt(double x) { return sqrt(x); }
 
@@ -185,6 +187,8 @@ __device__ __forceinline__ double r_sqrt(double x) { return sqrt(x); }
 //   Gaussian:       phi = exp(-d^2/b)
 //   Kaiser-Bessel:  phi = [sinh(b s)/s] * m/sinh(b m), s = sqrt(m^2 - d^2), 0 for |d| > m,
 //                   evaluated overflow-free as (m/s) e^{b(s-m)} (1-e^{-2bs})/(1-e^{-2bm}).
+//   sinc-power:     phi = sinc(t)^{2m}, t = b d, b = pi (2 - 1/sigma)/(2m);
+//                   phi' = 2m sinc^{2m-1} b (t cos t - sin t)/t^2, the bracket by its series for |t| < 1/2.
 //
 // The stencil point is passed as (d0, j) with d = d0 - j, d0 = u - c in [-1/2, 1/2] and j the
 // integer stencil offset.  d^2 is formed as j^2 + d0 (d0 - 2j) and the Kaiser-Bessel exponent
@@ -217,7 +221,27 @@ __device__ __forceinline__ void window_eval(const WindowParams& wp, T d0, int j,
     const T jf = (T)j;
     const T d = d0 - jf;
     const T d2 = d0 * (d0 - (T)2 * jf) + jf * jf;
-    if (wp.kind == ENUF_WINDOW_BSPLINE) {
+    if (wp.kind == ENUF_WINDOW_SINC_POWER) {
+        if constexpr (M_ > 0) {
+            const T pc = (T)wp.b, t = pc * d, t2 = t * t;
+            T sn, cs;
+            r_sincos(t, &sn, &cs);
+            const T sc = t == (T)0 ? (T)1 : sn / t;
+            T pw = sc;                               // sinc^(2m-1)
+#pragma unroll
+            for (int i = 1; i < 2 * M_ - 1; ++i) pw *= sc;
+            phi = pw * sc;
+            if (kDeriv) {
+                T g;                                 // (t cos t - sin t)/t^2 = -t/3 + t^3/30 - t^5/840 + ..
+                if (t2 < (T)0.25)
+                    g = -t * ((T)(1.0 / 3.0) - t2 * ((T)(1.0 / 30.0) - t2 * ((T)(1.0 / 840.0) - t2 * ((T)(1.0 / 45360.0)
+                        - t2 * ((T)(1.0 / 3991680.0) - t2 * ((T)(1.0 / 518918400.0) - t2 * (T)(1.0 / 93405312000.0)))))));
+                else
+                    g = (t * cs - sn) / t2;
+                dphi = (T)(2 * M_) * pw * pc * g;
+            }
+        }
+    } else if (wp.kind == ENUF_WINDOW_BSPLINE) {
         if constexpr (M_ > 0) {
             T v, dv;
             bspline_eval<T, 2 * M_>(d, v, dv);

@@ -397,6 +397,58 @@ def test_bspline_window_matches_oracle(enuf, torch_cuda, oracle, n, m, dtype, va
     plan.close()
 
 
+@pytest.mark.parametrize("n,m,dtype", [(32, 1, "f64"), (32, 3, "f64"), (64, 6, "f64"), (32, 2, "f32"), (64, 4, "f32"),
+                                       (128, 6, "f32")])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_sinc_power_window_matches_oracle(enuf, torch_cuda, oracle, n, m, dtype, variant):
+    """ENUF_WINDOW_SINC_POWER: phi = sinc(pi c d)^2m, Phi(k) = B_2m(k/(n c))/c.  fp64: the closed form on
+    the device (phi' through the series of (t cos t - sin t)/t^2 for small t); fp32: the polynomial table fitted to the
+    closed form.  Against Oracle B."""
+    torch = torch_cuda
+    N, L = 333, 7.5
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = random_neutral_gas(N, L, seed=700 + n + m, dtype=npdt)
+    r[:3] = np.array([[0.0, 0.0, 0.0], [L / n * 5, L / n * 7 + 1e-7, L / n * 11 - 1e-9], [L / 2, L / 4, L / 8]], dtype=npdt)
+    M = n // 2
+    k_cut = M // 2
+    alpha = 0.9 * math.pi * k_cut / (L * 3.0)
+    ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, "sinc_power", 2.0, variant=variant)
+    plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=2.0, m=m, window="sinc_power", variant=variant,
+                     dtype=torch.float64 if dtype == "f64" else torch.float32)
+    E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+    tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+    plan.close()
+
+
+@pytest.mark.parametrize("n,M,m,window,dtype", [
+    (64, 42, 4, "gaussian", "f64"), (32, 20, 3, "kaiser_bessel", "f64"), (64, 44, 5, "sinc_power", "f64"),
+    (128, 86, 6, "kaiser_bessel", "f32"), (256, 170, 6, "kaiser_bessel", "f32"), (128, 84, 4, "bspline", "f32"),
+    (64, 42, 6, "sinc_power", "f32")])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_oversampling_other_than_two(enuf, torch_cuda, oracle, n, M, m, window, dtype, variant):
+    """sigma_s = n/M need not be 2 (PAPER.md:348, :360 sweep sigma_s = 1.5 and 2): any even M with n = sigma M one of the
+    grid sizes, e.g. M = 170, n = 256 (sigma = 1.506), M = 42, n = 64 (1.524), M = 86, n = 128 (1.488).  The window
+    parameters follow sigma (R6); k_cut = M/2, the full band.  Against Oracle B with the same sigma."""
+    torch = torch_cuda
+    N = 2000 if n >= 128 else 400
+    L = 9.0
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = random_neutral_gas(N, L, seed=900 + n + M, dtype=npdt)
+    sigma = n / M
+    k_cut = M // 2
+    alpha = 0.9 * math.pi * k_cut / (L * 3.0)
+    ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, window, sigma, variant=variant)
+    plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=sigma, m=m, window=window, variant=variant,
+                     dtype=torch.float64 if dtype == "f64" else torch.float32)
+    E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+    tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+    plan.close()
+
+
 def test_plan_auto_runs_config3(enuf, torch_cuda, oracle):
     """Plan.auto (enuf_plan_create_auto): config 3 planned from (delta, r_c) evaluates like the literal plan."""
     torch = torch_cuda
