@@ -56,8 +56,10 @@ enum enuf_option {
     ENUF_OPT_NUM_PARTICLES = 5,  /* lower N for the next calls, 0 <= N <= planned capacity          */
     ENUF_OPT_PROFILE = 6,        /* 1: record per-stage CUDA-event times (enuf_plan_stage_ms)        */
     ENUF_OPT_KEEP_SPECTRUM = 7,  /* 1: also store S~(n) so enuf_plan_structure_factor() can read it  */
-    ENUF_OPT_SPREAD_ZCHUNK = 8,  /* tuning: grid planes per spreading CTA (integer, 1..n);
-                                    default fills the SMs several times over                         */
+    ENUF_OPT_SPREAD_ZCHUNK = 8,  /* tuning: the spreading CTAs take fixed pieces of that many grid planes of one
+                                    column (integer, 1..n) instead of the default, equal shares of all
+                                    (column, plane) slabs, one per resident CTA.  Pieces shorter than 2m planes
+                                    make the rounding order of the shared planes run-dependent (R22)        */
     ENUF_OPT_PDL = 10,           /* 1 (default): the kernels of an evaluation are launched with programmatic
                                     dependent launch -- each may be scheduled while its predecessor still runs
                                     and waits for it on the device (griddepcontrol), which hides the launch

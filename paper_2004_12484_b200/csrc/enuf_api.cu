@@ -324,17 +324,6 @@ int ensure_allocated(enuf_plan* p) {
     // b m / sinh(b m) (<= 2.7e-9 for m >= 5): the fp32 kernels then skip that point
     p->trim = p->precision == ENUF_F32 && p->window == ENUF_WINDOW_KAISER_BESSEL && p->m >= 5;
     p->tg.trim = p->trim ? 1 : 0;
-    if (!p->zchunk_user) {
-        // spread: columns x z-chunks, all CTAs resident at once (one wave): as many chunks as the device has
-        // room for, but chunks of >= 8 planes (every chunk walks 2m extra slabs)
-        const int per_sm = p->precision == ENUF_F32 ? enuf::spread_ctas_per_sm<float>(p->spread_npx)
-                                                    : enuf::spread_ctas_per_sm<double>(p->spread_npx);
-        const int ncol = (p->n / (8 * p->spread_npx)) * (p->n / 16);
-        int chunks = p->num_sms * per_sm / ncol;
-        if (chunks < 1) chunks = 1;
-        p->zchunk = (p->n + chunks - 1) / chunks;
-        if (p->zchunk < 8) p->zchunk = 8;
-    }
     const size_t es = p->esize, n = p->n, n3 = n * n * n, cap = (size_t)(p->N_cap > 0 ? p->N_cap : 1);
     const int nfield = p->variant == ENUF_FORCE_IK ? 3 : 1;
     int rc;
@@ -554,7 +543,7 @@ int enuf_plan_create_box(enuf_plan** out, int64_t N, const double* Lb, double al
     p->tg.nt = n / enuf::kTile;
     p->tg.nbins = p->tg.nt * p->tg.nt * n;
     p->spread_npx = n >= 128 ? 4 : 2;
-    p->zchunk = n;                 // derived in ensure_allocated (depends on the precision and the SM count)
+    p->zchunk = n;                 // only used when set through ENUF_OPT_SPREAD_ZCHUNK
     p->Kxp = ((k_cut + 1 + enuf::kLinesPerGroup - 1) / enuf::kLinesPerGroup) * enuf::kLinesPerGroup;
     p->Ky = 2 * k_cut + 1;
     fill_window_params(p);

@@ -52,9 +52,12 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const T* __restrict__ r, const T* __restrict__ q, T* __restrict__ F, int64_t N,
                  Edges L, TileGeom g, uint32_t* __restrict__ count, uint32_t* __restrict__ scan_epoch,
-                 uint2* __restrict__ binrank) {
+                 uint2* __restrict__ binrank, unsigned zblocks, SpreadZero<T> zr) {
     pdl_prologue();
-    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // the first zblocks blocks clear the grid planes that two spreading pieces add into (enuf_spread.cuh); the first
+    // kernel of the evaluation does it because the previous evaluation's gather is the grid's last reader
+    if (blockIdx.x < zblocks) { spread_zero_block(zr, (int)blockIdx.x); return; }
+    int64_t j = (int64_t)(blockIdx.x - zblocks) * blockDim.x + threadIdx.x;
     if (j >= N) return;
     if (j == 0) scan_epoch[0] += 1u;    // the epoch of this evaluation's scan: kept on the device so that a
                                         // replayed CUDA graph (ENUF_OPT_CUDA_GRAPH) advances it as well

@@ -59,6 +59,34 @@ struct TileGeom {
                   //    bin_z - m + 1 .. bin_z + m)
 };
 
+// Work decomposition of the spreading kernel (enuf_spread.cuh, header comment).  T = ncol * n slabs in column-major linear order
+// (lin = column * n + bin plane); CTA c owns [lo, hi):
+//   chunk > 0: fixed pieces of `chunk` planes, G = ncol * ceil(n / chunk) CTAs (ENUF_OPT_SPREAD_ZCHUNK),
+//   chunk = 0: G equal ranges, boundaries floor(c T / G); a boundary closer than `minlen` to a column start is moved
+//              onto it, so that no piece is shorter than minlen = WZ - 1 planes: every grid plane then receives from
+//              at most two pieces and the sum of the two reductions does not depend on their order.
+struct SpreadSplit {
+    int G, n, ncol, chunk, minlen;
+};
+__host__ __device__ inline int spread_boundary(const SpreadSplit& sp, int c) {
+    int b = (int)(((long long)c * sp.ncol * sp.n) / sp.G);
+    const int z = b % sp.n;
+    if (z != 0) {
+        if (z < sp.minlen) b -= z;
+        else if (sp.n - z < sp.minlen) b += sp.n - z;
+    }
+    return b;
+}
+__host__ __device__ inline void spread_range(const SpreadSplit& sp, int c, int& lo, int& hi) {
+    if (sp.chunk > 0) {
+        const int cpc = (sp.n + sp.chunk - 1) / sp.chunk, col = c / cpc, z0 = (c - col * cpc) * sp.chunk;
+        lo = col * sp.n + z0;
+        hi = col * sp.n + (z0 + sp.chunk < sp.n ? z0 + sp.chunk : sp.n);
+    } else {
+        lo = spread_boundary(sp, c);
+        hi = spread_boundary(sp, c + 1);
+    }
+}
 // Piecewise-polynomial window table for the fp32 path (step a0).  For every stencil offset
 // j in [0, m] the weight phi(d0 - j), d0 in [-1/2, 1/2], is a polynomial p_j of degree
 // poly_degree(m) in d0 (Chebyshev interpolant of the window's analytic continuation, fitted

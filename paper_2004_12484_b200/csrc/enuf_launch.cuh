@@ -135,18 +135,50 @@ int configure_kernels(enuf_plan* p) {
     });
 }
 
+// Work decomposition of the spreading kernel for this evaluation (SpreadSplit, enuf_common.cuh): equal ranges of slabs,
+// as many as the device holds spreading CTAs at once, but none shorter than the planes two pieces share (WZ - 1) + 1;
+// ENUF_OPT_SPREAD_ZCHUNK asks for fixed pieces instead.
+template <typename T>
+static inline SpreadSplit make_spread_split(const enuf_plan* p) {
+    SpreadSplit sp{};
+    sp.n = p->n;
+    sp.ncol = (p->n / (8 * p->spread_npx)) * (p->n / 16);
+    sp.minlen = 2 * p->m - (p->trim ? 1 : 0);
+    if (p->zchunk_user) {
+        sp.chunk = p->zchunk;
+        sp.G = sp.ncol * ((p->n + p->zchunk - 1) / p->zchunk);
+    } else {
+        sp.chunk = 0;
+        const long long slabs = (long long)sp.ncol * sp.n;
+        long long G = (long long)p->num_sms * spread_ctas_per_sm<T>(p->spread_npx);
+        const long long gmax = slabs / (sp.minlen + 1);
+        if (G > gmax) G = gmax;
+        sp.G = (int)(G < 1 ? 1 : G);
+    }
+    return sp;
+}
+
 template <typename T>
 int launch_bin(enuf_plan* p, const void* r, const void* q, void* F) {
     cudaStream_t s = p->stream;
     const int64_t N = p->N;
     const int nbins = p->tg.nbins;
+    p->split = make_spread_split<T>(p);
+    SpreadZero<T> zr{};
+    zr.grid = static_cast<T*>(p->grid[0]);
+    zr.sp = p->split;
+    zr.cx = 8 * p->spread_npx; zr.cy = 16;
+    zr.shi = p->trim ? p->m - 1 : p->m;
+    zr.nzp = p->split.minlen;
+    const unsigned zblocks = (unsigned)(p->split.G + p->split.ncol);
     // the scan clears the histogram behind itself: a memset is needed only when that did not happen
     if (!p->bin_count_clean && cudaMemsetAsync(p->bin_count, 0, sizeof(uint32_t) * nbins, s) != cudaSuccess) return -1;
     p->bin_count_clean = false;
     const unsigned blocks = (unsigned)((N + 255) / 256);
     const unsigned sblocks = (unsigned)((nbins + kScanChunk - 1) / kScanChunk);
-    pdl_launch(p, bin_count_kernel<T>, blocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q),
-                                               static_cast<T*>(F), N, Edges{{p->Lb[0], p->Lb[1], p->Lb[2]}}, p->tg, p->bin_count, p->scan_epoch, p->binrank);
+    pdl_launch(p, bin_count_kernel<T>, blocks + zblocks, 256, 0, s, static_cast<const T*>(r), static_cast<const T*>(q),
+                                               static_cast<T*>(F), N, Edges{{p->Lb[0], p->Lb[1], p->Lb[2]}}, p->tg, p->bin_count, p->scan_epoch, p->binrank,
+                                               zblocks, zr);
     int nlaunch = 4;
     if ((int)sblocks <= kScanMaxResident && (int)sblocks <= p->num_sms) {
         // every scan CTA is resident at once: one launch, chunk totals exchanged through scan_desc
@@ -192,19 +224,19 @@ int launch_spread(enuf_plan* p) {
             auto run = [&](auto trim_c) -> int {
                 constexpr bool kTrim = decltype(trim_c)::value != 0;
                 using C = SpreadCfg<T, M_, kTrim, NPX>;
-                const dim3 grid((unsigned)((p->n / C::CX) * (p->n / C::CY)), (unsigned)((p->n + p->zchunk - 1) / p->zchunk));
+                const dim3 grid((unsigned)p->split.G);          // set by launch_bin, whose extra blocks cleared the shared planes
                 if constexpr (sizeof(T) == 4) {
                     if (p->spread_sparse) {      // few particles per slab: 8 stages of 32 slots (SpreadCfg)
                         pdl_launch(p, spread_kernel<T, M_, kTrim, NPX, true>, grid, C::NT,
                                    spread_smem_bytes<T, M_, kTrim, NPX, true>(), s,
                                    static_cast<const PSlot<T>*>(p->rec), static_cast<const T*>(p->rows), p->bin_offset, p->tg,
-                                   p->zchunk, static_cast<T*>(p->grid[0]));
+                                   p->split, static_cast<T*>(p->grid[0]));
                         return 0;
                     }
                 }
                 pdl_launch(p, spread_kernel<T, M_, kTrim, NPX>, grid, C::NT, spread_smem_bytes<T, M_, kTrim, NPX>(), s, 
                     static_cast<const PSlot<T>*>(p->rec), static_cast<const T*>(p->rows), p->bin_offset, p->tg,
-                    p->zchunk, static_cast<T*>(p->grid[0]));
+                    p->split, static_cast<T*>(p->grid[0]));
                 return 0;
             };
             if constexpr (M_ >= 5 && sizeof(T) == 4) {

@@ -55,8 +55,9 @@ struct enuf_plan {
     float poly_d[enuf::kPolyMaxDeg][enuf::kMaxM + 1] = {};       // (fp32 path; packed into PolyArg<m> per launch)
     float bs_c[2 * enuf::kMaxM][2 * enuf::kMaxM + 1] = {};       // B-spline window: exact pieces on d0 in [0, 1/2] (PolyArg::bc, bd)
     float bs_d[2 * enuf::kMaxM][2 * enuf::kMaxM + 1] = {};
-    int zchunk = 0;                   // grid planes per spread CTA
-    bool zchunk_user = false;         // set through ENUF_OPT_SPREAD_ZCHUNK: not re-derived
+    int zchunk = 0;                   // ENUF_OPT_SPREAD_ZCHUNK: fixed pieces of that many planes per spreading CTA (else equal ranges)
+    bool zchunk_user = false;
+    enuf::SpreadSplit split{};        // work decomposition of the spreading kernel, set per evaluation by launch_bin
     int spread_npx = 4;               // spread column = 8 spread_npx x 16 cells (4 for n >= 128, 2 below)
     int spread_sparse_user = -1;      // ENUF_OPT_SPREAD_SPARSE: -1 auto, 0 / 1 forced
     bool spread_sparse = false;       // fp32: eight-stage ring of 32-slot rounds (few particles per slab and column)

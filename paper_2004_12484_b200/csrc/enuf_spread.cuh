@@ -1,14 +1,21 @@
 // Step a2 -- spreading (adjoint NFFT, part 1):
 //   g[l] = sum_j q_j phi(u_jx - l_x) phi(u_jy - l_y) phi(u_jz - l_z), l periodic.
 //
-// Output-stationary, sliding z-window, warp-specialised.  A CTA owns a column of CX x 16 grid cells in
-// (x, y) (CX = 32, or 16 on small grids) and a chunk [z0, z1) of grid planes.  It has
+// Output-stationary, sliding z-window, warp-specialised.  The work is the set of SLABS (column, bin plane): a column
+// is CX x 16 grid cells in (x, y) (CX = 32, or 16 on small grids), slab s of a column holds the particles binned to
+// plane s, whose stencils reach the planes s - SHI .. s + SLO.  The ncol * n slabs, in column-major order, are cut into
+// one contiguous range per CTA (SpreadSplit: equal ranges, as many as the device holds CTAs at once); a range is one or
+// two PIECES (column, [z0, z1)).  A CTA stages every slab of its pieces exactly once -- there is no halo in z: the
+// WZ - 1 planes at either end of a piece, which also receive from the neighbouring piece, are added into the grid
+// with red.global.add (those planes of the column are zeroed beforehand by spread_zero_block, run as extra blocks of
+// the first kernel of the evaluation; each such value is 0 + a + b with a, b the two pieces' sums, so the result does
+// not depend on the order), all other planes are complete and written with one plain store.  A CTA has
 //   - NCONS = CX/8 x 2 CONSUMER warps, each owning an 8 x 8 patch of the column: every lane owns two
 //     x-adjacent cells and keeps, in registers, their partial sums on the WZ consecutive planes that the
 //     particles of slab s (bin plane s) can reach.  Per (warp, particle) visit the work is WZ packed FMAs
 //     acc[k] += (a0, a1) * (q wz[k]) with (a0, a1) = wx[cells] * wy[cell].  After slab s the lowest plane
-//     of the window is complete: one coalesced store, and the window slides.  Every grid value is written
-//     exactly once -- no atomics, no clearing of the grid, no shared-memory read-modify-write;
+//     of the window has everything this piece sends to it: one coalesced store (or reduction, see above), and the
+//     window slides.  No shared-memory read-modify-write, no clearing of the whole grid;
 //   - four PRODUCER warps taking the slabs in turn (slab i of the chunk goes to stage i % 3 of a three-stage ring):
 //     a producer culls the particles of the neighbouring bins against the column's halo, copies the three
 //     window rows of the accepted ones (evaluated ONCE per particle by window_rows_kernel, enuf_bin.cuh --
@@ -155,6 +162,51 @@ __device__ __forceinline__ void write_window_row(const WindowParams& wp, const P
     }
 }
 
+// The grid planes that two pieces share are zeroed before the spreading kernel adds into them: block i < G clears the
+// `nzp` = WZ - 1 planes from z0 - shi on (mod n) of the column where CTA i's range starts, block G + col those at the
+// start of column col (where a piece of that column always starts).  Run as extra blocks of bin_count_kernel.
+template <typename T>
+struct SpreadZero {
+    T* grid;            // nullptr: nothing to do
+    SpreadSplit sp;
+    int cx, cy;         // column footprint
+    int shi, nzp;       // planes z0 - shi .. z0 - shi + nzp - 1
+};
+template <typename T>
+__device__ __forceinline__ void spread_zero_block(const SpreadZero<T>& zr, int i) {
+    const SpreadSplit& sp = zr.sp;
+    int b;
+    if (i < sp.G) {
+        int lo, hi;
+        spread_range(sp, i, lo, hi);
+        if (lo >= hi) return;
+        b = lo;
+    } else {
+        b = (i - sp.G) * sp.n;
+    }
+    const int col = b / sp.n, z0 = b - col * sp.n;
+    const int ncolx = sp.n / zr.cx, Tx = col % ncolx, Ty = col / ncolx;
+    constexpr int VE = 16 / (int)sizeof(T);                 // elements per 16-byte store
+    const int vx = zr.cx / VE, per_plane = zr.cy * vx;
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+    for (int e = threadIdx.x; e < zr.nzp * per_plane; e += blockDim.x) {
+        const int k = e / per_plane, rem = e - k * per_plane, y = rem / vx, xv = rem - y * vx;
+        int pz = z0 - zr.shi + k;
+        pz += pz < 0 ? sp.n : 0; pz -= pz >= sp.n ? sp.n : 0;
+        T* dst = zr.grid + ((size_t)pz * sp.n + (size_t)(Ty * zr.cy + y)) * sp.n + Tx * zr.cx + xv * VE;
+        *reinterpret_cast<uint4*>(dst) = zero;
+    }
+}
+
+// grid[addr] += v for a pair of x-adjacent cells, without a return value (L2 reduction)
+__device__ __forceinline__ void red_pair(float2* addr, const float2 v) {
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void red_pair(double2* addr, const double2 v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(v.x) : "memory");
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(reinterpret_cast<double*>(addr) + 1), "d"(v.y) : "memory");
+}
+
 // explicit shared-space loads (32-bit shared addresses: no generic-to-shared conversion inside the visit loop)
 template <typename T> __device__ __forceinline__ typename Pair2<T>::type lds_pair(uint32_t a);
 template <> __device__ __forceinline__ float2 lds_pair<float>(uint32_t a) {
@@ -202,8 +254,11 @@ __device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar) {
 template <typename T, int M_, bool kTrim, int NPX, bool kSparse = false>
 __global__ void __launch_bounds__((SpreadCfg<T, M_, kTrim, NPX, kSparse>::NT), (SpreadCfg<T, M_, kTrim, NPX, kSparse>::CTAS_PER_SM))
 spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
-              const uint32_t* __restrict__ offset, TileGeom g, int zchunk, T* __restrict__ grid) {
+              const uint32_t* __restrict__ offset, TileGeom g, SpreadSplit sp, T* __restrict__ grid) {
     pdl_prologue();
+    int lo, hi;
+    spread_range(sp, (int)blockIdx.x, lo, hi);              // this CTA's slabs [lo, hi), lin = column * n + bin plane
+    if (lo >= hi) return;
     using C = SpreadCfg<T, M_, kTrim, NPX, kSparse>;
     using R = WindowRows<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
@@ -233,9 +288,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ncolx = g.n / CX;
-    const int Tx = blockIdx.x % ncolx, Ty = blockIdx.x / ncolx;
-    const int z0 = blockIdx.y * zchunk, z1 = min(g.n, z0 + zchunk);
-    const int s_begin = z0 - C::SLO, s_end = z1 + C::SHI;
 
     // the zero padding of every slot (and the all-zero slot CAP) is written once; rows are rewritten per round
     for (int i = tid; i < (int)(C::STAGE_BYTES * NSTAGE / 16); i += C::NT)
@@ -254,33 +306,16 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
 
     if (warp >= NCONS) {
         // =========================================================== producers
-        // producer k stages the slabs s_begin + k, s_begin + k + 4, ..; slab i of the chunk goes to stage i % 3
+        // the slabs of the CTA's pieces are numbered gi = 0, 1, .. in the order they are worked through; producer k stages
+        // the slabs gi = k, k + 4, ..; slab gi goes to stage gi % NSTAGE
         const int k = warp - NCONS;
         const int half = lane >> 4, l16 = lane & 15;
         const unsigned below = (1u << lane) - 1u;
-        // The halo of the column touches NBY rows of NBX bin columns; in bin order (TileGeom) the NBX bins of one
-        // row and plane are adjacent, so a slab is NBY ranges of the sorted array, each split in two where the
-        // row of columns wraps around the box (segments 2 jy, 2 jy + 1).  Lane sg < NSEG: (first bin of plane 0,
-        // number of bins) of segment sg.  Rows / columns the periodic box holds only once are taken once.
-        int seg_bin0 = 0, seg_nb = 0;
-        if (lane < NSEG) {
-            const int jy = lane >> 1, second = lane & 1;
-            const int nrow = C::NBY < g.nt ? C::NBY : g.nt, nbx = C::NBX < g.nt ? C::NBX : g.nt;
-            int ty = Ty * (CY / kTile) - 1 + jy;
-            ty += ty < 0 ? g.nt : 0; ty -= ty >= g.nt ? g.nt : 0;
-            int txlo = Tx * (CX / kTile) - 1;
-            txlo += txlo < 0 ? g.nt : 0;
-            if (nbx == g.nt) txlo = 0;
-            const int na = min(nbx, g.nt - txlo);        // bins before the wrap
-            const int tx = second ? 0 : txlo;
-            seg_nb = jy < nrow ? (second ? nbx - na : na) : 0;
-            seg_bin0 = bin_index(g, tx, ty, 0);
-        }
-        // first stencil point in column coordinates from the packed cell: the periodic image that can overlap the column
-        const int offx = -M_ - CX * Tx + (WZ - 1), offy = -M_ - CY * Ty + (WZ - 1), nmask = g.n - 1;
+        const int nmask = g.n - 1;
         const uint4* tb = reinterpret_cast<const uint4*>(segtab[k]);
         unsigned pe = 0, pa = 0;                 // parities of the next phase of empty_bar[(k - NSTAGE) & 3] / again_bar[k] to wait for
-        int blk0 = s_begin + k - C::NPROD * kBlk;
+        // per piece (set in the loop over pieces below): the halo's segments, the cull offsets, the block of loaded ranges
+        int seg_bin0 = 0, seg_nb = 0, offx = 0, offy = 0, blk0 = 0;
         // candidates of a slab, 32 per step, in packed numbering (segtab): a sparse slab is ONE step however its
         // particles are spread over the segments.  The cell words of up to kSteps steps are loaded together (one
         // global-load latency per slab, not one per step), then examined in order; those of the producer's NEXT slab
@@ -313,7 +348,35 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             }
             ebase += 32u * kSteps;
         };
-        for (int s = s_begin + k; s < s_end; s += C::NPROD) {
+        int gs = 0;                              // number of the piece's first slab
+        for (int lin = lo; lin < hi; ) {
+        const int col = lin / g.n, z0 = lin - col * g.n, z1 = min(g.n, z0 + (hi - lin));
+        const int Tx = col % ncolx, Ty = col / ncolx;
+        // The halo of the column touches NBY rows of NBX bin columns; in bin order (TileGeom) the NBX bins of one
+        // row and plane are adjacent, so a slab is NBY ranges of the sorted array, each split in two where the
+        // row of columns wraps around the box (segments 2 jy, 2 jy + 1).  Lane sg < NSEG: (first bin of plane 0,
+        // number of bins) of segment sg.  Rows / columns the periodic box holds only once are taken once.
+        seg_bin0 = 0; seg_nb = 0;
+        if (lane < NSEG) {
+            const int jy = lane >> 1, second = lane & 1;
+            const int nrow = C::NBY < g.nt ? C::NBY : g.nt, nbx = C::NBX < g.nt ? C::NBX : g.nt;
+            int ty = Ty * (CY / kTile) - 1 + jy;
+            ty += ty < 0 ? g.nt : 0; ty -= ty >= g.nt ? g.nt : 0;
+            int txlo = Tx * (CX / kTile) - 1;
+            txlo += txlo < 0 ? g.nt : 0;
+            if (nbx == g.nt) txlo = 0;
+            const int na = min(nbx, g.nt - txlo);        // bins before the wrap
+            const int tx = second ? 0 : txlo;
+            seg_nb = jy < nrow ? (second ? nbx - na : na) : 0;
+            seg_bin0 = bin_index(g, tx, ty, 0);
+        }
+        // first stencil point in column coordinates from the packed cell: the periodic image that can overlap the column
+        offx = -M_ - CX * Tx + (WZ - 1); offy = -M_ - CY * Ty + (WZ - 1);
+        const int s_first = z0 + ((k - gs) & 3);  // this producer's first slab of the piece
+        blk0 = s_first - C::NPROD * kBlk;
+        preloaded = false;
+        for (int s = s_first; s < z1; s += C::NPROD) {
+            const int gi = gs + (s - z0);
             if (s - blk0 >= C::NPROD * kBlk) {
                 // ranges of this producer's next kBlk slabs: lane & 15 = slab, lanes 0..15 load the starts, 16..31 the ends
                 blk0 = s;
@@ -343,7 +406,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 __syncwarp();
             }
             const int js = (s - blk0) / C::NPROD;
-            const int stage = (s - s_begin) % NSTAGE;
+            const int stage = gi % NSTAGE;
             unsigned char* sbase = smem_raw + (size_t)stage * C::STAGE_BYTES;
             const uint32_t sl32 = smem_u32(sbase);
             uint2* lists = reinterpret_cast<uint2*>(sbase + C::SLOT_BYTES);
@@ -392,7 +455,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     if (ebase >= total) { slab_done = true; break; }   // the ranges are exhausted
                     load_steps(js);                                    // a long slab: the next kSteps steps
                 }
-                if (slab_done && s + C::NPROD < s_end && js + 1 < kBlk) {
+                if (slab_done && s + C::NPROD < z1 && js + 1 < kBlk) {
                     ebase = 0u;
                     load_steps(js + 1);                                // the next slab of this producer (same block of ranges)
                     preloaded = true;
@@ -429,9 +492,9 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 }
                 if (first_round) {
                     // the slab that held the stage before (s - NSTAGE, staged by producer (k - NSTAGE) & 3) must be finished
-                    if (s - NSTAGE >= s_begin) {
+                    if (gi >= NSTAGE) {
                         if constexpr (C::kStageBars) {
-                            mbar_wait_backoff(&empty_bar[stage], (unsigned)(((s - s_begin) / NSTAGE - 1) & 1));
+                            mbar_wait_backoff(&empty_bar[stage], (unsigned)((gi / NSTAGE - 1) & 1));
                         } else {
                             mbar_wait_backoff(&empty_bar[(k - NSTAGE) & 3], pe); pe ^= 1u;
                         }
@@ -484,13 +547,15 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 if (lane == 0) mbar_arrive(fb);
             }
         }
+        gs += z1 - z0;
+        lin += z1 - z0;
+        }
         return;
     }
 
     // =============================================================== consumers
     const int px0 = 8 * (warp % NPX), py0 = 8 * (warp / NPX);
     const int lxl = (lane & 3) * 2, lyl = lane >> 2;              // this lane's two cells (lxl, lyl), (lxl + 1, lyl) of the patch
-    T* gout = grid + ((size_t)(Ty * CY + py0 + lyl)) * g.n + Tx * CX + px0 + lxl;
     const size_t plane = (size_t)g.n * g.n;
     constexpr int NV = (WZ + 3) / 4;
 
@@ -518,8 +583,13 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     const uint32_t cl32 = smem_u32(cl_s) + (uint32_t)warp * 4u;
     const uint32_t lpw = (uint32_t)C::SLOT_BYTES + (uint32_t)(warp * LCAP * sizeof(uint2));
     int stage = 0, prod = 0;
-    gout += (ptrdiff_t)(s_begin - C::SHI) * (ptrdiff_t)plane;     // plane s - SHI; first dereferenced at plane z0
-    for (int s = s_begin; s < s_end; ++s) {
+    for (int lin = lo; lin < hi; ) {
+    const int col = lin / g.n, z0 = lin - col * g.n, z1 = min(g.n, z0 + (hi - lin));
+    const int Tx = col % ncolx, Ty = col / ncolx;
+    T* gcol = grid + ((size_t)(Ty * CY + py0 + lyl)) * g.n + Tx * CX + px0 + lxl;     // this lane's cells on plane 0
+    int pz = z0 - C::SHI;                                       // plane the next slab completes (mod n)
+    pz += pz < 0 ? g.n : 0;
+    for (int s = z0; s < z1; ++s) {
         const int bar = C::kStageBars ? stage : prod;
         const uint32_t sbz = smem32 + (uint32_t)stage * (uint32_t)C::STAGE_BYTES;
         const uint32_t sbx = sbz + lxl * ES, sby = sbz + lyl * ES;
@@ -558,14 +628,28 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             __syncwarp();
             if (lane == 0) mbar_arrive((cl >> 16) ? eb32 + 8u * (uint32_t)bar : ab32 + 8u * (uint32_t)prod);
         } while (!(cl >> 16));
-        // the lowest plane of the window (s - SHI) is complete: store it, slide
-        if (s >= z0 + C::SHI) *reinterpret_cast<P2*>(gout) = acc[0];
-        gout += plane;
+        // the lowest plane of the window, s - SHI, has received everything this piece sends to it.  It is complete
+        // (plain store) unless it is one of the piece's first WZ - 1 planes, which the piece below also adds to
+        {
+            P2* out = reinterpret_cast<P2*>(gcol + (size_t)pz * plane);
+            if (s - z0 >= WZ - 1) *out = acc[0];
+            else red_pair(out, acc[0]);
+        }
+        pz = pz + 1 == g.n ? 0 : pz + 1;
 #pragma unroll
         for (int kk = 0; kk + 1 < WZ; ++kk) acc[kk] = acc[kk + 1];
         acc[WZ - 1].x = (T)0; acc[WZ - 1].y = (T)0;
         stage = stage + 1 == NSTAGE ? 0 : stage + 1;
         prod = (prod + 1) & 3;
+    }
+    // the WZ - 1 planes above the piece's last complete one, shared with the piece above
+#pragma unroll
+    for (int kk = 0; kk + 1 < WZ; ++kk) {
+        red_pair(reinterpret_cast<P2*>(gcol + (size_t)pz * plane), acc[kk]);
+        pz = pz + 1 == g.n ? 0 : pz + 1;
+        acc[kk].x = (T)0; acc[kk].y = (T)0;
+    }
+    lin += z1 - z0;
     }
 }
 
