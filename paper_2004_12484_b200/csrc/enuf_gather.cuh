@@ -84,7 +84,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // kIk = true : one component d of the paper's ik variant, F[.,d] = pre*q * sum B_d[l] phi phi phi
 //              with pre = 2/L^2 (Eq. 42).
 template <typename T, int M_, bool kIk, bool kTrim = false>
-__global__ void __launch_bounds__(GatherCfg<M_, kTrim>::NT)
+__global__ void __launch_bounds__((GatherCfg<M_, kTrim>::NT), (sizeof(T) == 4 ? 2 : 1))
 gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
               const uint32_t* __restrict__ offset, TileGeom g, WindowParams wp,
               const __grid_constant__ PolyArg<M_> pa, T pre, int component, T* __restrict__ F, T ry, T rz) {
@@ -287,14 +287,8 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
                     const int base = base_s[slot];
                     const T* origin = tile_s + base + rowbase;
                     T fx = (T)0, fy = (T)0, fz = (T)0;
-                    auto finish_row = [&](int i, int j, const T (&v)[WE]) {
-                        P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
-#pragma unroll
-                        for (int k = 0; k < WE; ++k) {
-                            if (k & 1) fma_pair(sb2, wx[k], v[k]);
-                            else fma_pair(sa, wx[k], v[k]);
-                        }
-                        const P2 s2 = pair_add(sa, sb2);                   // (sum Psi phi_x, sum Psi phi_x')
+                    // (sum Psi phi_x, sum Psi phi_x') of one row -> the three force sums with the row's y, z weights
+                    auto finish_sums = [&](int i, int j, const P2 s2) {
                         if (kIk) {
                             fx += s2.x * (wy[i].x * wz[j].x);
                         } else {
@@ -310,24 +304,38 @@ gather_kernel(const T* __restrict__ field, const PSlot<T>* __restrict__ slots,
 #pragma unroll
                             for (int i = 0; i < NR; ++i) {
                                 const P2* row = reinterpret_cast<const P2*>(origin + 4 * i * SX + 4 * j * SPL);
-                                T v[WE];
+                                P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
 #pragma unroll
-                                for (int k = 0; k < WE / 2; ++k) { const P2 t2 = row[k]; v[2 * k] = t2.x; v[2 * k + 1] = t2.y; }
-                                finish_row(i, j, v);
+                                for (int k = 0; k < WE / 2; ++k) {
+                                    const P2 t2 = row[k];
+                                    fma_pair(sa, wx[2 * k], t2.x);
+                                    fma_pair(sb2, wx[2 * k + 1], t2.y);
+                                }
+                                finish_sums(i, j, pair_add(sa, sb2));
                             }
                     } else {
+                        // the row starts on an odd column: first and last element by single-word loads, the rest as
+                        // aligned pairs.  A single-word load serves both halves in one wavefront only if they hit
+                        // different banks: the 16 first elements of a half sit in the 16 odd banks, the 16 last ones
+                        // in the 16 even banks, so half 0 loads (first, last) and half 1 (last, first)
+                        const P2 wa = half ? wx[WE - 1] : wx[0], wb = half ? wx[0] : wx[WE - 1];
+                        const int oa = half ? WE - 1 : 0, ob = half ? 0 : WE - 1;
 #pragma unroll
                         for (int j = 0; j < NR; ++j)
 #pragma unroll
                             for (int i = 0; i < NR; ++i) {
                                 const T* rowf = origin + 4 * i * SX + 4 * j * SPL;
                                 const P2* row = reinterpret_cast<const P2*>(rowf + 1);
-                                T v[WE];
-                                v[0] = rowf[0];
+                                P2 sa, sb2; sa.x = (T)0; sa.y = (T)0; sb2.x = (T)0; sb2.y = (T)0;
+                                fma_pair(sa, wa, rowf[oa]);
 #pragma unroll
-                                for (int k = 0; k < WE / 2 - 1; ++k) { const P2 t2 = row[k]; v[2 * k + 1] = t2.x; v[2 * k + 2] = t2.y; }
-                                v[WE - 1] = rowf[WE - 1];
-                                finish_row(i, j, v);
+                                for (int k = 0; k < WE / 2 - 1; ++k) {
+                                    const P2 t2 = row[k];
+                                    fma_pair(sb2, wx[2 * k + 1], t2.x);
+                                    fma_pair(sa, wx[2 * k + 2], t2.y);
+                                }
+                                fma_pair(sb2, wb, rowf[ob]);
+                                finish_sums(i, j, pair_add(sa, sb2));
                             }
                     }
                     const size_t jp = (size_t)(uint32_t)idx_s[slot];
