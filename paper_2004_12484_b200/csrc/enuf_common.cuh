@@ -59,33 +59,82 @@ struct TileGeom {
                   //    bin_z - m + 1 .. bin_z + m)
 };
 
-// Work decomposition of the spreading kernel (enuf_spread.cuh, header comment).  T = ncol * n slabs in column-major linear order
-// (lin = column * n + bin plane); CTA c owns [lo, hi):
-//   chunk > 0: fixed pieces of `chunk` planes, G = ncol * ceil(n / chunk) CTAs (ENUF_OPT_SPREAD_ZCHUNK),
-//   chunk = 0: G equal ranges, boundaries floor(c T / G); a boundary closer than `minlen` to a column start is moved
-//              onto it, so that no piece is shorter than minlen = WZ - 1 planes: every grid plane then receives from
-//              at most two pieces and the sum of the two reductions does not depend on their order.
+// Work decomposition of the spreading kernel (enuf_spread.cuh, header comment).  The ncol * n slabs (column, bin plane)
+// are cut into PIECES (column, [z0, z1)) and every CTA gets about S / G slabs:
+//   chunk > 0: fixed pieces of `chunk` planes, one per CTA, G = ncol * ceil(n / chunk) (ENUF_OPT_SPREAD_ZCHUNK);
+//   chunk = 0: every column is cut at the SAME planes into q full pieces [cut(j), cut(j+1)), cut(j) = j zr0 / q, of about
+//              S / G planes each -- CTA c < q ncol takes piece j = c / ncol of column c % ncol, so that these CTAs sweep
+//              their columns in step and a particle in the halo of several columns is fetched by all of them at about
+//              the same time (it is still in L2 for the later ones) -- and the remainders [zr0, n) of the columns, laid
+//              end to end, are shared equally among the other G - q ncol CTAs (a range of them is a few pieces of
+//              neighbouring columns).  q = 0 (fewer CTAs than columns): zr0 = 0, everything is "remainder".
+//              A range boundary closer than `minlen` to the start of a column's remainder is moved onto it, so that no
+//              piece is shorter than minlen = WZ - 1 planes: every grid plane then receives from at most two pieces and
+//              the sum of the two reductions does not depend on their order.
 struct SpreadSplit {
     int G, n, ncol, chunk, minlen;
+    int q, zr0;
 };
-__host__ __device__ inline int spread_boundary(const SpreadSplit& sp, int c) {
-    int b = (int)(((long long)c * sp.ncol * sp.n) / sp.G);
-    const int z = b % sp.n;
+struct SpreadPiece { int col, z0, z1; };
+// boundary b (0..Grem) of the remainder space: columns of rlen = n - zr0 planes laid end to end
+__host__ __device__ inline int spread_rem_boundary(const SpreadSplit& sp, int b) {
+    const int rlen = sp.n - sp.zr0, grem = sp.G - sp.q * sp.ncol;
+    int u = (int)(((long long)b * sp.ncol * rlen) / grem);
+    const int z = u % rlen;
     if (z != 0) {
-        if (z < sp.minlen) b -= z;
-        else if (sp.n - z < sp.minlen) b += sp.n - z;
+        if (z < sp.minlen) u -= z;
+        else if (rlen - z < sp.minlen) u += rlen - z;
     }
-    return b;
+    return u;
 }
-__host__ __device__ inline void spread_range(const SpreadSplit& sp, int c, int& lo, int& hi) {
+// the i-th piece of CTA c; false when the CTA has fewer pieces
+__host__ __device__ inline bool spread_piece(const SpreadSplit& sp, int c, int i, SpreadPiece& pc) {
     if (sp.chunk > 0) {
-        const int cpc = (sp.n + sp.chunk - 1) / sp.chunk, col = c / cpc, z0 = (c - col * cpc) * sp.chunk;
-        lo = col * sp.n + z0;
-        hi = col * sp.n + (z0 + sp.chunk < sp.n ? z0 + sp.chunk : sp.n);
-    } else {
-        lo = spread_boundary(sp, c);
-        hi = spread_boundary(sp, c + 1);
+        if (i > 0) return false;
+        const int cpc = (sp.n + sp.chunk - 1) / sp.chunk;
+        pc.col = c / cpc;
+        pc.z0 = (c - pc.col * cpc) * sp.chunk;
+        pc.z1 = pc.z0 + sp.chunk < sp.n ? pc.z0 + sp.chunk : sp.n;
+        return true;
     }
+    if (c < sp.q * sp.ncol) {
+        if (i > 0) return false;
+        const int j = c / sp.ncol;
+        pc.col = c - j * sp.ncol;
+        pc.z0 = (int)(((long long)j * sp.zr0) / sp.q);
+        pc.z1 = (int)(((long long)(j + 1) * sp.zr0) / sp.q);
+        return true;
+    }
+    const int rlen = sp.n - sp.zr0, cr = c - sp.q * sp.ncol;
+    const int ulo = spread_rem_boundary(sp, cr), uhi = spread_rem_boundary(sp, cr + 1);
+    const int u = i == 0 ? ulo : (ulo / rlen + i) * rlen;      // later pieces start with their column's remainder
+    if (u >= uhi) return false;
+    pc.col = u / rlen;
+    pc.z0 = sp.zr0 + (u - pc.col * rlen);
+    pc.z1 = pc.z0 + (uhi - u) < sp.n ? pc.z0 + (uhi - u) : sp.n;
+    return true;
+}
+// Where pieces start = where two pieces share planes (a piece ends where another starts, or at the top of its column,
+// which wraps onto the column's first piece): start number i of the G + ncol that spread_zero_block clears.
+//   i < q ncol: full piece i;  then ncol: the remainders' starts (col, zr0);  then G - q ncol: the remainder CTAs' first pieces.
+__host__ __device__ inline bool spread_piece_start(const SpreadSplit& sp, int i, int& col, int& z0) {
+    if (sp.chunk > 0) {
+        if (i >= sp.G) return false;
+        SpreadPiece pc;
+        spread_piece(sp, i, 0, pc);
+        col = pc.col; z0 = pc.z0;
+        return true;
+    }
+    SpreadPiece pc;
+    if (i < sp.q * sp.ncol) { spread_piece(sp, i, 0, pc); col = pc.col; z0 = pc.z0; return true; }
+    i -= sp.q * sp.ncol;
+    if (sp.zr0 >= sp.n) return false;                            // no remainders
+    if (i < sp.ncol) { col = i; z0 = sp.zr0; return true; }
+    i -= sp.ncol;
+    if (i >= sp.G - sp.q * sp.ncol) return false;
+    if (!spread_piece(sp, sp.q * sp.ncol + i, 0, pc)) return false;
+    col = pc.col; z0 = pc.z0;
+    return true;
 }
 // Piecewise-polynomial window table for the fp32 path (step a0).  For every stencil offset
 // j in [0, m] the weight phi(d0 - j), d0 in [-1/2, 1/2], is a polynomial p_j of degree

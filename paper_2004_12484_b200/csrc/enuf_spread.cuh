@@ -3,9 +3,10 @@
 //
 // Output-stationary, sliding z-window, warp-specialised.  The work is the set of SLABS (column, bin plane): a column
 // is CX x 16 grid cells in (x, y) (CX = 32, or 16 on small grids), slab s of a column holds the particles binned to
-// plane s, whose stencils reach the planes s - SHI .. s + SLO.  The ncol * n slabs, in column-major order, are cut into
-// one contiguous range per CTA (SpreadSplit: equal ranges, as many as the device holds CTAs at once); a range is one or
-// two PIECES (column, [z0, z1)).  A CTA stages every slab of its pieces exactly once -- there is no halo in z: the
+// plane s, whose stencils reach the planes s - SHI .. s + SLO.  The ncol * n slabs are cut into PIECES (column, [z0, z1))
+// and shared equally among as many CTAs as the device holds at once (SpreadSplit, enuf_common.cuh: most CTAs get one
+// piece, cut at the same planes in every column; the rest share the columns' remainders).  A CTA stages every slab of
+// its pieces exactly once -- there is no halo in z: the
 // WZ - 1 planes at either end of a piece, which also receive from the neighbouring piece, are added into the grid
 // with red.global.add (those planes of the column are zeroed beforehand by spread_zero_block, run as extra blocks of
 // the first kernel of the evaluation; each such value is 0 + a + b with a, b the two pieces' sums, so the result does
@@ -162,9 +163,9 @@ __device__ __forceinline__ void write_window_row(const WindowParams& wp, const P
     }
 }
 
-// The grid planes that two pieces share are zeroed before the spreading kernel adds into them: block i < G clears the
-// `nzp` = WZ - 1 planes from z0 - shi on (mod n) of the column where CTA i's range starts, block G + col those at the
-// start of column col (where a piece of that column always starts).  Run as extra blocks of bin_count_kernel.
+// The grid planes that two pieces share are zeroed before the spreading kernel adds into them: block i of G + ncol clears
+// the `nzp` = WZ - 1 planes from z0 - shi on (mod n) of the column where piece start i lies (spread_piece_start,
+// enuf_common.cuh).  Run as extra blocks of bin_count_kernel.
 template <typename T>
 struct SpreadZero {
     T* grid;            // nullptr: nothing to do
@@ -175,16 +176,8 @@ struct SpreadZero {
 template <typename T>
 __device__ __forceinline__ void spread_zero_block(const SpreadZero<T>& zr, int i) {
     const SpreadSplit& sp = zr.sp;
-    int b;
-    if (i < sp.G) {
-        int lo, hi;
-        spread_range(sp, i, lo, hi);
-        if (lo >= hi) return;
-        b = lo;
-    } else {
-        b = (i - sp.G) * sp.n;
-    }
-    const int col = b / sp.n, z0 = b - col * sp.n;
+    int col, z0;
+    if (!spread_piece_start(sp, i, col, z0)) return;
     const int ncolx = sp.n / zr.cx, Tx = col % ncolx, Ty = col / ncolx;
     constexpr int VE = 16 / (int)sizeof(T);                 // elements per 16-byte store
     const int vx = zr.cx / VE, per_plane = zr.cy * vx;
@@ -256,9 +249,8 @@ __global__ void __launch_bounds__((SpreadCfg<T, M_, kTrim, NPX, kSparse>::NT), (
 spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
               const uint32_t* __restrict__ offset, TileGeom g, SpreadSplit sp, T* __restrict__ grid) {
     pdl_prologue();
-    int lo, hi;
-    spread_range(sp, (int)blockIdx.x, lo, hi);              // this CTA's slabs [lo, hi), lin = column * n + bin plane
-    if (lo >= hi) return;
+    SpreadPiece pc;
+    if (!spread_piece(sp, (int)blockIdx.x, 0, pc)) return;  // (an empty range: its boundaries were moved onto each other)
     using C = SpreadCfg<T, M_, kTrim, NPX, kSparse>;
     using R = WindowRows<M_, kTrim>;
     using P2 = typename Pair2<T>::type;
@@ -349,9 +341,9 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             ebase += 32u * kSteps;
         };
         int gs = 0;                              // number of the piece's first slab
-        for (int lin = lo; lin < hi; ) {
-        const int col = lin / g.n, z0 = lin - col * g.n, z1 = min(g.n, z0 + (hi - lin));
-        const int Tx = col % ncolx, Ty = col / ncolx;
+        for (int pi = 0; spread_piece(sp, (int)blockIdx.x, pi, pc); ++pi) {
+        const int z0 = pc.z0, z1 = pc.z1;
+        const int Tx = pc.col % ncolx, Ty = pc.col / ncolx;
         // The halo of the column touches NBY rows of NBX bin columns; in bin order (TileGeom) the NBX bins of one
         // row and plane are adjacent, so a slab is NBY ranges of the sorted array, each split in two where the
         // row of columns wraps around the box (segments 2 jy, 2 jy + 1).  Lane sg < NSEG: (first bin of plane 0,
@@ -548,7 +540,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
             }
         }
         gs += z1 - z0;
-        lin += z1 - z0;
         }
         return;
     }
@@ -583,9 +574,9 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
     const uint32_t cl32 = smem_u32(cl_s) + (uint32_t)warp * 4u;
     const uint32_t lpw = (uint32_t)C::SLOT_BYTES + (uint32_t)(warp * LCAP * sizeof(uint2));
     int stage = 0, prod = 0;
-    for (int lin = lo; lin < hi; ) {
-    const int col = lin / g.n, z0 = lin - col * g.n, z1 = min(g.n, z0 + (hi - lin));
-    const int Tx = col % ncolx, Ty = col / ncolx;
+    for (int pi = 0; spread_piece(sp, (int)blockIdx.x, pi, pc); ++pi) {
+    const int z0 = pc.z0, z1 = pc.z1;
+    const int Tx = pc.col % ncolx, Ty = pc.col / ncolx;
     T* gcol = grid + ((size_t)(Ty * CY + py0 + lyl)) * g.n + Tx * CX + px0 + lxl;     // this lane's cells on plane 0
     int pz = z0 - C::SHI;                                       // plane the next slab completes (mod n)
     pz += pz < 0 ? g.n : 0;
@@ -649,7 +640,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
         pz = pz + 1 == g.n ? 0 : pz + 1;
         acc[kk].x = (T)0; acc[kk].y = (T)0;
     }
-    lin += z1 - z0;
     }
 }
 
