@@ -279,4 +279,74 @@ window_rows_kernel(const PSlot<T>* __restrict__ slots, const uint32_t* __restric
     }
 }
 
+// Scatter and window rows in one pass over the particles in CALLER order, for systems of at most kBinFusedMaxN particles
+// (launch_bin, enuf_launch.cuh; larger ones run the two kernels above): a CTA of three warps takes 32 consecutive particles, warp d locates dimension d of
+// particle `lane` (cell index and offset, fp64 as in locate()), the three meet in shared memory, warp 0 writes the
+// sorted-array slot at offset[bin] + rank and warp d evaluates the particle's window row of dimension d; the rows leave
+// as 16-byte stores, RP / 4 consecutive threads per particle (one particle's rows are contiguous, the particles of a
+// CTA land wherever their bins are).  Against bin_scatter + window_rows this saves the second pass over the slots
+// and one launch; the scattered 160-byte row blocks cost more than that once N reaches ~1e6.
+constexpr int64_t kBinFusedMaxN = 262144;
+template <typename T, int M_, bool kTrim>
+__global__ void __launch_bounds__(kRowsThreads)
+bin_place_kernel(const T* __restrict__ r, const T* __restrict__ q, int64_t N, Edges L, TileGeom g,
+                 const uint32_t* __restrict__ offset, const uint2* __restrict__ binrank, PSlot<T>* __restrict__ slots,
+                 WindowParams wp, const __grid_constant__ PolyArg<M_> pa, T* __restrict__ rows) {
+    pdl_prologue();
+    using R = WindowRows<M_, kTrim>;
+    using V4 = typename Vec4<T>::type;
+    constexpr int SP = R::RP + 4;                                  // 44 / 52 elements: conflict-free 16-byte accesses
+    __shared__ __align__(16) T tile[32 * SP];
+    __shared__ T d0_s[3][32];
+    __shared__ int c_s[3][32];
+    __shared__ uint32_t pos_s[32];
+    const int lane = threadIdx.x & 31, dim = threadIdx.x >> 5;
+    const int64_t j = (int64_t)blockIdx.x * 32 + lane;
+    uint2 br = make_uint2(kNoBin, 0u);
+    if (j < N) br = binrank[j];
+    const bool live = br.x != kNoBin;
+    T d0 = (T)0, qj = (T)0;
+    int ci = 0;
+    if (live) {
+        // one dimension of locate(): x = r/L; x -= floor(x); u = n x; c = floor(u + 1/2); d0 = u - c
+        double x = __ddiv_rn((double)r[3 * j + dim], L.l[dim]);
+        x -= floor(x);
+        if (x >= 1.0) x = 0.0;
+        const double u = __dmul_rn((double)g.n, x);
+        const double c = floor(__dadd_rn(u, 0.5));
+        d0 = (T)(u - c);
+        ci = (int)c;
+        ci = ci >= g.n ? ci - g.n : ci;
+        qj = q[j];
+        d0_s[dim][lane] = d0;
+        c_s[dim][lane] = ci;
+        if (dim == 0) pos_s[lane] = offset[br.x] + br.y;
+    } else if (dim == 0) {
+        pos_s[lane] = 0xffffffffu;
+    }
+    __syncthreads();
+    if (live) {
+        const int ksx = (kTrim && d0_s[0][lane] > (T)0) ? 1 : 0;
+        if (dim == 0) {
+            PSlot<T> o;
+            o.rec.dx = d0_s[0][lane]; o.rec.dy = d0_s[1][lane]; o.rec.dz = d0_s[2][lane]; o.rec.q = qj;
+            const uint32_t ksy = (kTrim && o.rec.dy > (T)0) ? 1u : 0u;
+            o.cell = pack_cell(c_s[0][lane], c_s[1][lane], c_s[2][lane]) | ((uint32_t)ksx << 30) | (ksy << 31);
+            o.idx = (uint32_t)j;
+            slots[pos_s[lane]] = o;
+        }
+        // parity of the first x stencil point (grid index c_x - m + ks_x; n is even, so wrapping keeps it)
+        const int parx = (c_s[0][lane] + M_ + ksx) & 1;
+        write_window_row<T, M_, kTrim>(wp, pa, dim, d0, qj, parx, tile + lane * SP);
+    }
+    __syncthreads();
+    constexpr int CH = R::RP / 4;                                  // 16-byte (fp32) / 32-byte (fp64) chunks per particle
+    for (int c = threadIdx.x; c < 32 * CH; c += kRowsThreads) {
+        const int pp = c / CH, cc = c - pp * CH;
+        const uint32_t pos = pos_s[pp];
+        if (pos != 0xffffffffu)
+            reinterpret_cast<V4*>(rows + (size_t)pos * R::RP)[cc] = reinterpret_cast<const V4*>(tile + pp * SP)[cc];
+    }
+}
+
 }  // namespace enuf

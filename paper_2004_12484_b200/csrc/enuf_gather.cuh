@@ -57,7 +57,8 @@ struct GatherCfg {
     static constexpr bool kPairWarp = kPair && WE % 4 == 0;
     static constexpr int PBW = kPairWarp ? 4 : 5;               // particles per warp batch (3 lanes per particle compute weights); shared memory: 2 CTAs per SM
     static constexpr int ITER = (WE * WE + 31) / 32;            // stencil rows per lane
-    static constexpr int WP = kPairWarp ? WE : 14;              // pitch of a (phi, phi') weight row: >= WE, 16-byte aligned
+    static constexpr int WP = 14;                               // pitch of a (phi, phi') weight row: >= WE, 16-byte aligned; 28 words: the
+                                                                //   12 lanes that store a batch's rows 16 bytes at a time collide two-way, not three-way
     static constexpr int PERM = 64;                             // kPairWarp: particles a warp sorts by row parity at a time
 };
 
