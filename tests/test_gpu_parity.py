@@ -92,6 +92,32 @@ def test_spread_grid_matches_oracle(enuf, torch_cuda, oracle, name):
     plan.close()
 
 
+@pytest.mark.parametrize("n,m,window,dtype", [(32, 4, "gaussian", "f64"), (64, 6, "kaiser_bessel", "f32"),
+                                              (128, 6, "kaiser_bessel", "f32"), (128, 2, "bspline", "f64")])
+@pytest.mark.parametrize("zchunk", [0, 1, 5, 13, 32, 1000])
+def test_spread_pieces_any_cut(enuf, torch_cuda, oracle, n, m, window, dtype, zchunk):
+    """The spreading kernel's decomposition (every (column, plane) slab staged once, pieces that share
+    2m planes with their neighbours through red.global.add on planes zeroed by bin_count's first blocks): the grid must be
+    the oracle's whatever the cuts are -- the plan's own equal shares (zchunk = 0), pieces of one plane (every plane gets
+    2m + 1 contributors), pieces shorter and longer than the shared planes, one piece per column (zchunk >= n: the piece's
+    top wraps onto its own bottom).  Two evaluations in a row: the shared planes are zeroed again each time."""
+    torch = torch_cuda
+    N, L = 3000, 11.0
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = random_neutral_gas(N, L, seed=4100 + n + m, dtype=npdt)
+    M = n // 2
+    plan = enuf.Plan(N, L, 0.8, M // 2, M, sigma=2.0, m=m, window=window, dtype=torch.float64 if dtype == "f64" else torch.float32)
+    if zchunk:
+        plan.set(enuf.OPT_SPREAD_ZCHUNK, min(zchunk, n))
+    ref = oracle.spread(r, q, L, n, m, window, 2.0)
+    tol = 1e-13 if dtype == "f64" else 2e-6
+    rd, qd = torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda()
+    for _ in range(2):
+        g = plan.spread_only(rd, qd).numpy()
+        assert np.abs(g - ref).max() <= tol * np.abs(ref).max()
+    plan.close()
+
+
 # ------------------------------------------------------------------ orthorhombic boxes (SURVEY 8(f).4, DESIGN R26)
 
 def _box_inputs(N, Lb, seed, npdt):
