@@ -126,12 +126,22 @@ real_force_kernel(const typename Vec4<T>::type* __restrict__ pos, const uint32_t
         auto pair = [&](const V4& pj, T dx, T dy, T dz, bool other) {
             const T d2 = dx * dx + dy * dy + dz * dz;
             if (d2 <= r_cut2 && other) {
-                const T d = r_sqrt(d2), inv_d = (T)1 / d;
+                T d, inv_d;
+                if (sizeof(T) == 4) {
+                    // 1/d by the reciprocal-square-root unit and one Newton step (relative error ~1e-7), d = d2 / d:
+                    // no IEEE square root and division (each a MUFU plus a fix-up sequence with a slow path)
+                    const float d2f = (float)d2;
+                    float y = rsqrtf(d2f);
+                    y = y * fmaf(-0.5f * d2f, y * y, 1.5f);
+                    inv_d = (T)y; d = (T)(d2f * y);
+                } else {
+                    d = r_sqrt(d2); inv_d = (T)1 / d;
+                }
                 const T ad = alpha * d;
                 const T ex = r_exp(-ad * ad);
                 T ec;
                 if (sizeof(T) == 4) {
-                    const float t = __frcp_rn(fmaf(0.5f, (float)ad, 1.0f)), u = fmaf(t, ef.ua, ef.ub);
+                    const float t = __fdividef(1.0f, fmaf(0.5f, (float)ad, 1.0f)), u = fmaf(t, ef.ua, ef.ub);
                     float P = ef.c[kErfcDeg];
 #pragma unroll
                     for (int k = kErfcDeg - 1; k >= 0; --k) P = fmaf(P, u, ef.c[k]);
