@@ -661,7 +661,8 @@ int orc_enuf(int64_t N, const double *r, const double *q, double L, double alpha
              double *E, double *F, int64_t nsample, const int64_t *sample,
              double *grid_out, double *S_out_re, double *S_out_im)
 {
-    if (n < 2 * m + 1 || (n & (n - 1)) || k_cut < 1 || 2 * k_cut > n || m < 1 || m > 20) return -2;
+    /* the radix-2 line transform needs a power of two; the plain DFT (use_dft) is the definition for any n */
+    if (n < 2 * m + 1 || ((n & (n - 1)) && !use_dft) || k_cut < 1 || 2 * k_cut > n || m < 1 || m > 20) return -2;
     size_t n3 = (size_t)n * n * n;
     double *g_re = (double *)calloc(n3, sizeof(double));
     double *g_im = (double *)calloc(n3, sizeof(double));
@@ -930,7 +931,8 @@ int orc_enuf_box(int64_t N, const double *r, const double *q, const double *Lb, 
                  double *E, double *F, int64_t nsample, const int64_t *sample,
                  double *grid_out, double *S_out_re, double *S_out_im)
 {
-    if (n < 2 * m + 1 || (n & (n - 1)) || k_cut < 1 || 2 * k_cut > n || m < 1 || m > 20) return -2;
+    /* the radix-2 line transform needs a power of two; the plain DFT (use_dft) is the definition for any n */
+    if (n < 2 * m + 1 || ((n & (n - 1)) && !use_dft) || k_cut < 1 || 2 * k_cut > n || m < 1 || m > 20) return -2;
     size_t n3 = (size_t)n * n * n;
     double *g_re = (double *)calloc(n3, sizeof(double));
     double *g_im = (double *)calloc(n3, sizeof(double));

@@ -191,6 +191,47 @@ def test_bspline_enuf_against_direct_ewald(oracle, variant, bound):
             assert abs(b["F"][i, d] + (ep - em) / (2 * h)) < 1e-7 * np.abs(b["F"]).max()
 
 
+# ----------------------------------------------------------------- oversampling 1.5: grids that are not powers of two
+
+@pytest.mark.parametrize("n", [12, 24, 48])
+def test_dft_line_any_length_equals_numpy(oracle, n):
+    """The oracle's plain DFT line transform (the definition, Eq. 34-35 convention R11) for lengths 3 * 2^k, the grids
+    of sigma_s = 1.5, against numpy.fft in both directions; and a 3-D transform with the axis order."""
+    rng = np.random.default_rng(n)
+    x = rng.normal(size=n) + 1j * rng.normal(size=n)
+    assert np.abs(oracle.fft_line(x, -1, True) - np.fft.fft(x)).max() < 1e-12
+    assert np.abs(oracle.fft_line(x, +1, True) - np.fft.ifft(x) * n).max() < 1e-12
+    if n <= 24:
+        a = rng.normal(size=(n, n, n)) + 1j * rng.normal(size=(n, n, n))
+        assert np.abs(oracle.fft3d(a, -1, True) - np.fft.fftn(a)).max() < 1e-10
+
+
+@pytest.mark.parametrize("window", ["kaiser_bessel", "gaussian"])
+def test_enuf_oversampling_one_and_a_half_against_direct_ewald(oracle, window):
+    """sigma_s = 1.5 (M = 16, n = 24; the paper sweeps 1.5 and 2, Fig. 1): Oracle B with the DFT on the 24^3 grid against
+    Oracle A.  The error falls with m and is larger than at sigma_s = 2 with the same m; the analytic forces are the
+    exact gradient of the ENUF energy at any sigma (R17)."""
+    L, alpha, kc, M = 6.0, 1.0, 8, 16
+    r, q = random_neutral_gas(64, L, seed=21)
+    Ea, Fa = oracle.direct(r, q, L, alpha, kc)
+    err = {}
+    for sigma in (1.5, 2.0):
+        for m in (2, 4):
+            b = oracle.enuf(r, q, L, alpha, kc, int(sigma * M), m, window, sigma, variant="ik", use_dft=True)
+            err[sigma, m] = math.sqrt(((b["F"] - Fa) ** 2).sum() / (Fa ** 2).sum())
+            assert abs(b["E"] - Ea) < (3e-3 if m == 2 else 5e-5) * abs(Ea)
+    assert err[1.5, 4] < 0.05 * err[1.5, 2] and err[2.0, 4] < 0.05 * err[2.0, 2], err
+    assert err[1.5, 4] > 2 * err[2.0, 4], err
+    n, m, h = 24, 4, 1e-5
+    b = oracle.enuf(r, q, L, alpha, kc, n, m, window, 1.5, variant="analytic", use_dft=True)
+    for i, d in ((7, 2), (50, 0)):
+        rp = r.copy(); rp[i, d] += h
+        rm = r.copy(); rm[i, d] -= h
+        ep = oracle.enuf(rp, q, L, alpha, kc, n, m, window, 1.5, forces=False, use_dft=True)["E"]
+        em = oracle.enuf(rm, q, L, alpha, kc, n, m, window, 1.5, forces=False, use_dft=True)["E"]
+        assert abs(b["F"][i, d] + (ep - em) / (2 * h)) < 1e-7 * np.abs(b["F"]).max()
+
+
 # ----------------------------------------------------------------- sinc-power window (PAPER.md:266)
 
 def test_sinc_power_m1_transform_is_the_hat_function(oracle):
