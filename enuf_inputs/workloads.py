@@ -145,13 +145,13 @@ def _cfg4():
                    window="kaiser_bessel", seed=seed, meta={"delta": 1e-5})
 
 
-def _cfg5(N: int = 1_000_000):
+def _cfg5(N: int = 1_000_000, sigma: float = 2.0, name: str = "cfg5"):
     L, seed = 215.0, 5005
     r = uniform01(seed, np.arange(3 * N)).reshape(N, 3) * L
     q = np.where(np.arange(N) % 2 == 0, 1.0, -1.0)
     r_c, delta = 10.0, 1e-4
     alpha = math.sqrt(-math.log(delta)) / r_c          # 0.30348542587702925
-    return _finish("cfg5", r, q, "f32", L=L, alpha=alpha, k_cut=64, M=128, sigma=2.0, m=6,
+    return _finish(name, r, q, "f32", L=L, alpha=alpha, k_cut=64, M=128, sigma=sigma, m=6,
                    window="kaiser_bessel", seed=seed,
                    meta={"delta": delta, "r_c": r_c, "step_displacement": 0.05})
 
@@ -171,6 +171,8 @@ def make_workload(name: str) -> Workload:
         return _cfg4()
     if name == "cfg5":
         return _cfg5()
+    if name == "cfg5_sigma15":      # config 5 on the 192^3 grid of sigma_s = 1.5; same inputs
+        return _cfg5(sigma=1.5, name=name)
     raise KeyError(name)
 
 

@@ -97,9 +97,9 @@ enum enuf_stage {
  *   k_cut  reciprocal cutoff n_c in integer wavevectors: modes 0 < |n|^2 <= k_cut^2 (R4);
  *          1 <= k_cut <= M/2 (R5)
  *   M      NFFT bandwidth per dimension (Eq. 33, :272), any integer >= 2 k_cut
- *   sigma  oversampling factor sigma_s > 1 (:348, :360); n = sigma*M must be 32, 64, 128 or 256 (to 1e-9).  sigma = 2
- *          with M a power of two is the usual choice; any other M works with sigma = n/M (M = 170, n = 256:
- *          sigma = 1.506); sigma = 1.5 exactly would need n = 1.5 * 2^k, which the FFT does not have
+ *   sigma  oversampling factor sigma_s > 1 (:348, :360); n = sigma*M (to 1e-9) must be 32, 64, 128 or 256 -- the fused,
+ *          pruned FFT: sigma = 2 with M a power of two, or any other M with sigma = n/M (M = 170, n = 256: 1.506) --
+ *          or 48, 96, 192, 384: sigma = 1.5 with M = 32 ... 256, cubic boxes only, on a plain (slower) FFT path
  *   m      window cut-off: stencil of 2m+1 grid points per dimension (:268, R8), 1 <= m <= 6
  * Defaults: fp32, Kaiser-Bessel window, analytic-derivative forces, point charges,
  * the legacy default stream.  *out is set to NULL on failure.

@@ -210,7 +210,11 @@ int build_tables(enuf_plan* p) {
     // twiddles of the four-step FFT, one table per direction, laid out [k1][a] (enuf_fft.cuh):
     // forward (RA, RB) = (16, n/16), inverse (n/16, 16); entry = exp(-2 pi i a k1 / n)
     std::vector<double> tw(4 * (size_t)n), iphi((size_t)kc + 1), wf((size_t)kc * kc + 1);
-    for (int dir = 0; dir < 2; ++dir) {
+    if (p->mixed) {
+        // plain table exp(-2 pi i j / n), j < n (enuf_fft_mixed.cuh)
+        for (int j = 0; j < n; ++j) { tw[2 * j] = std::cos(2.0 * kPi * j / n); tw[2 * j + 1] = -std::sin(2.0 * kPi * j / n); }
+    }
+    for (int dir = 0; dir < 2 && !p->mixed; ++dir) {
         const int RA = dir == 0 ? 16 : n / 16, RB = n / RA;
         for (int k1 = 0; k1 < RA; ++k1)
             for (int a = 0; a < RB; ++a) {
@@ -339,15 +343,16 @@ int ensure_allocated(enuf_plan* p) {
     ALLOC(p->scan_epoch, 4);
     for (int d = 0; d < nfield; ++d) {
         ALLOC(p->grid[d], es * n3);
-        ALLOC(p->A1[d], 2 * es * n * n * p->Kxp);
-        ALLOC(p->A2[d], 2 * es * n * p->Ky * p->Kxp);
+        // (mixed-radix grids: A1 is the full complex n^3 spectrum, A2 is not used)
+        ALLOC(p->A1[d], p->mixed ? 2 * es * n3 : 2 * es * n * n * p->Kxp);
+        ALLOC(p->A2[d], p->mixed ? 16 : 2 * es * n * p->Ky * p->Kxp);
     }
     if (p->keep_spectrum) ALLOC(p->spectrum, 2 * es * (size_t)p->Ky * p->Ky * p->Kxp);
     ALLOC(p->tw, 4 * es * n);
     ALLOC(p->iphi, es * ((size_t)p->k_cut + 1));
     ALLOC(p->wf, es * ((size_t)p->k_cut * p->k_cut + 1));
-    const int lpc = 256 / (p->n / 16);
-    p->n_partial = (int)(((size_t)p->Ky * p->Kxp + lpc - 1) / lpc);
+    const int lpc = 256 / (p->n / 16 > 0 ? p->n / 16 : 1);
+    p->n_partial = p->mixed ? enuf_plan::kMixedScaleCtas : (int)(((size_t)p->Ky * p->Kxp + lpc - 1) / lpc);
     ALLOC(p->e_partial, 8 * (size_t)p->n_partial);
     ALLOC(p->e_dev, 8);
     ALLOC(p->fft_done, 4);
@@ -367,8 +372,8 @@ int ensure_allocated(enuf_plan* p) {
     p->events_valid = true;
     // pad columns of A1/A2 (kx in (k_cut, Kxp)) must hold finite values
     for (int d = 0; d < nfield; ++d) {
-        cudaMemsetAsync(p->A1[d], 0, 2 * es * n * n * p->Kxp, p->stream);
-        cudaMemsetAsync(p->A2[d], 0, 2 * es * n * p->Ky * p->Kxp, p->stream);
+        cudaMemsetAsync(p->A1[d], 0, p->mixed ? 2 * es * n3 : 2 * es * n * n * p->Kxp, p->stream);
+        cudaMemsetAsync(p->A2[d], 0, p->mixed ? 16 : 2 * es * n * p->Ky * p->Kxp, p->stream);
     }
     if (p->spectrum) cudaMemsetAsync(p->spectrum, 0, 2 * es * (size_t)p->Ky * p->Ky * p->Kxp, p->stream);
     cudaMemsetAsync(p->e_dev, 0, 8, p->stream);
@@ -529,14 +534,18 @@ int enuf_plan_create_box(enuf_plan** out, int64_t N, const double* Lb, double al
     if (!(sigma > 1.0) || !std::isfinite(sigma)) return fail(ENUF_EINVAL, "sigma must be > 1");
     const double nd = sigma * M;
     const int n = (int)std::lround(nd);
-    if (std::fabs(nd - n) > 1e-9 || (n != 32 && n != 64 && n != 128 && n != 256))
-        return fail(ENUF_EINVAL, "sigma*M = %g must be one of 32, 64, 128, 256", nd);
+    const bool pow2 = n == 32 || n == 64 || n == 128 || n == 256, mixed = n == 48 || n == 96 || n == 192 || n == 384;
+    if (std::fabs(nd - n) > 1e-9 || !(pow2 || mixed))
+        return fail(ENUF_EINVAL, "sigma*M = %g must be one of 32, 64, 128, 256 or 48, 96, 192, 384", nd);
+    if (mixed && !(Lb[0] == Lb[1] && Lb[1] == Lb[2]))
+        return fail(ENUF_EINVAL, "grids of 3 * 2^k points (sigma*M = %d) are for cubic boxes only", n);
     if (k_cut < 1 || 2 * k_cut > M) return fail(ENUF_EINVAL, "k_cut = %d must satisfy 1 <= k_cut <= M/2 = %d", k_cut, M / 2);
     if (m < 1 || m > enuf::kMaxM) return fail(ENUF_EINVAL, "m = %d must satisfy 1 <= m <= %d", m, enuf::kMaxM);
     enuf_plan* p = new (std::nothrow) enuf_plan();
     if (!p) return fail(ENUF_ENOMEM, "out of host memory");
     p->N_cap = p->N = N;
     p->L = L; p->alpha = alpha; p->sigma = sigma; p->k_cut = k_cut; p->M = M; p->n = n; p->m = m;
+    p->mixed = mixed;
     for (int d = 0; d < 3; ++d) p->Lb[d] = Lb[d];
     p->box = !(Lb[0] == Lb[1] && Lb[1] == Lb[2]);
     p->tg.n = n;
@@ -679,7 +688,8 @@ int enuf_spectrum_partial(enuf_plan* p, const void* r, const void* q, void* F) {
     }
     if (p->N == 0) {
         // no particles on this rank: its partial spectrum is zero
-        CU(cudaMemsetAsync(p->A2[0], 0, 2 * p->esize * (size_t)p->n * p->Ky * p->Kxp, p->stream));
+        if (p->mixed) CU(cudaMemsetAsync(p->A1[0], 0, 2 * p->esize * (size_t)p->n * p->n * p->n, p->stream));
+        else CU(cudaMemsetAsync(p->A2[0], 0, 2 * p->esize * (size_t)p->n * p->Ky * p->Kxp, p->stream));
         if (p->profile) for (int i = 0; i <= 2; ++i) cudaEventRecord(p->ev[i], p->stream);
     } else {
         rc = p->precision == ENUF_F32 ? run_partial<float>(p, r, q, F) : run_partial<double>(p, r, q, F);
@@ -694,8 +704,9 @@ int enuf_plan_spectrum_buffer(enuf_plan* p, void** dev_ptr, size_t* count) {
     if (!p || !dev_ptr || !count) return fail(ENUF_EINVAL, "plan, dev_ptr or count is NULL");
     int rc = prepare(p);
     if (rc) return rc;
-    *dev_ptr = p->A2[0];
-    *count = 2 * (size_t)p->n * p->Ky * p->Kxp;
+    // (grids of 3 * 2^k points: the full complex n^3 spectrum after the three forward passes)
+    *dev_ptr = p->mixed ? p->A1[0] : p->A2[0];
+    *count = p->mixed ? 2 * (size_t)p->n * p->n * p->n : 2 * (size_t)p->n * p->Ky * p->Kxp;
     return ENUF_OK;
 }
 

@@ -5,6 +5,7 @@
 
 #include "enuf_bin.cuh"
 #include "enuf_fft.cuh"
+#include "enuf_fft_mixed.cuh"
 #include "enuf_gather.cuh"
 #include "enuf_plan.h"
 #include "enuf_real.cuh"
@@ -122,6 +123,12 @@ int configure_kernels(enuf_plan* p) {
         return ok ? 0 : -1;
     });
     if (rc) return rc;
+    if (p->mixed) {
+        const size_t sb = fft_mixed_smem_bytes<T>(p->n);
+        const bool ok = set_smem(fft_mixed_kernel<T, true, false, true>, sb) && set_smem(fft_mixed_kernel<T, false, false, false>, sb)
+                        && set_smem(fft_mixed_kernel<T, false, true, true>, sb);
+        return ok ? 0 : -1;
+    }
     return dispatch_n(p->n, [&](auto nc) -> int {
         constexpr int N_ = decltype(nc)::value;
         const size_t sb = fft_smem_bytes<T, N_>();
@@ -284,8 +291,30 @@ int launch_spread(enuf_plan* p) {
 // Forward half of the FFT stage (a3): X real-to-complex and Y passes; leaves the partial spectrum
 // [z][ky'][kx] of this plan's particles in A2[0].  Linear in the charges, so partial spectra of
 // particle subsets add (Eq. 61): the multi-GPU path all-reduces A2[0] here.
+// Grids of 3 * 2^k points (enuf_fft_mixed.cuh): three line-transform launches per 3-D FFT on the full complex grid A1.
+template <typename T>
+static inline void launch_mixed_pass(enuf_plan* p, int dir, int sign, const void* in, void* out) {
+    const size_t n = (size_t)p->n, sb = fft_mixed_smem_bytes<T>(p->n);
+    const unsigned blocks = (unsigned)(n * n / mix_lines<T>());
+    const Cx<T>* tw = static_cast<const Cx<T>*>(p->tw);
+    if (dir == 0 && sign < 0)        // X forward: real grid in
+        pdl_launch(p, fft_mixed_kernel<T, true, false, true>, blocks, kFftThreads, sb, p->stream, in, out, p->n, n * n, n, (size_t)1, sign, tw);
+    else if (dir == 0)               // X inverse: real grid out
+        pdl_launch(p, fft_mixed_kernel<T, false, true, true>, blocks, kFftThreads, sb, p->stream, in, out, p->n, n * n, n, (size_t)1, sign, tw);
+    else if (dir == 1)
+        pdl_launch(p, fft_mixed_kernel<T, false, false, false>, blocks, kFftThreads, sb, p->stream, in, out, p->n, n * n, (size_t)1, n, sign, tw);
+    else
+        pdl_launch(p, fft_mixed_kernel<T, false, false, false>, blocks, kFftThreads, sb, p->stream, in, out, p->n, n, (size_t)1, n * n, sign, tw);
+}
+
 template <typename T>
 int launch_fft_forward(enuf_plan* p) {
+    if (p->mixed) {
+        launch_mixed_pass<T>(p, 0, -1, p->grid[0], p->A1[0]);
+        launch_mixed_pass<T>(p, 1, -1, p->A1[0], p->A1[0]);
+        launch_mixed_pass<T>(p, 2, -1, p->A1[0], p->A1[0]);
+        return launch_ok(p) ? 3 : -1;
+    }
     cudaStream_t s = p->stream;
     FftGeom fg{p->n, p->k_cut, p->Kxp, p->Ky};
     const Cx<T>* tw = static_cast<const Cx<T>*>(p->tw);
@@ -316,6 +345,26 @@ int launch_fft_forward(enuf_plan* p) {
 // variant writes A2[0..2]), Y and X inverse passes into the real field(s), energy reduction.
 template <typename T>
 int launch_fft_backward(enuf_plan* p) {
+    if (p->mixed) {
+        const int nout = p->variant == ENUF_FORCE_IK ? 3 : 1;
+        const double PI = 3.14159265358979323846;
+        ScaleTables st{p->iphi, p->wf};
+        Cx<T>* spec = p->keep_spectrum ? static_cast<Cx<T>*>(p->spectrum) : nullptr;
+        Cx<T>* c0 = static_cast<Cx<T>*>(p->A1[0]);
+        if (nout == 1)
+            pdl_launch(p, mixed_scale_kernel<T, 1>, enuf_plan::kMixedScaleCtas, kFftThreads, 0, p->stream, c0, (Cx<T>*)nullptr,
+                       (Cx<T>*)nullptr, p->n, p->k_cut, p->Kxp, p->Ky, st, p->e_partial, spec, p->fft_done, 1.0 / (2.0 * PI * p->L), p->e_dev);
+        else
+            pdl_launch(p, mixed_scale_kernel<T, 3>, enuf_plan::kMixedScaleCtas, kFftThreads, 0, p->stream, c0,
+                       static_cast<Cx<T>*>(p->A1[1]), static_cast<Cx<T>*>(p->A1[2]), p->n, p->k_cut, p->Kxp, p->Ky, st, p->e_partial, spec,
+                       p->fft_done, 1.0 / (2.0 * PI * p->L), p->e_dev);
+        for (int d = 0; d < nout; ++d) {
+            launch_mixed_pass<T>(p, 2, +1, p->A1[d], p->A1[d]);
+            launch_mixed_pass<T>(p, 1, +1, p->A1[d], p->A1[d]);
+            launch_mixed_pass<T>(p, 0, +1, p->A1[d], p->grid[d]);
+        }
+        return launch_ok(p) ? 1 + 3 * nout : -1;
+    }
     cudaStream_t s = p->stream;
     FftGeom fg{p->n, p->k_cut, p->Kxp, p->Ky};
     const Cx<T>* tw = static_cast<const Cx<T>*>(p->tw);

@@ -13,6 +13,7 @@ struct enuf_plan {
     double Lb[3] = {0, 0, 0};             // box edges (enuf_plan_create: three times L)
     bool box = false;                     // edges differ: orthorhombic plan (enuf_plan_create_box, R26)
     int k_cut = 0, M = 0, n = 0, m = 0;
+    bool mixed = false;                   // n = 3 * 2^k (sigma_s = 1.5): the plain mixed-radix FFT path (enuf_fft_mixed.cuh)
     // options
     int precision = ENUF_F32, window = ENUF_WINDOW_KAISER_BESSEL, variant = ENUF_FORCE_ANALYTIC;
     double lambda = 0.0;
@@ -92,6 +93,7 @@ struct enuf_plan {
     void* q_stage = nullptr;
     void* F_stage = nullptr;
     // profiling: ring of kProfRing evaluations x (ENUF_NUM_STAGES + 1) events
+    static constexpr int kMixedScaleCtas = 1024;   // CTAs (= energy partials) of the mixed-radix path's scaling kernel
     static constexpr int kProfRing = 128;
     static constexpr int kProfEv = ENUF_NUM_STAGES + 1;
     cudaEvent_t* ev_ring = nullptr;     // [kProfRing * kProfEv]

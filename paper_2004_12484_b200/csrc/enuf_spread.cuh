@@ -303,7 +303,6 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
         const int k = warp - NCONS;
         const int half = lane >> 4, l16 = lane & 15;
         const unsigned below = (1u << lane) - 1u;
-        const int nmask = g.n - 1;
         const uint4* tb = reinterpret_cast<const uint4*>(segtab[k]);
         unsigned pe = 0, pa = 0;                 // parities of the next phase of empty_bar[(k - NSTAGE) & 3] / again_bar[k] to wait for
         // per piece (set in the loop over pieces below): the halo's segments, the cull offsets, the block of loaded ranges
@@ -373,7 +372,7 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                 // ranges of this producer's next kBlk slabs: lane & 15 = slab, lanes 0..15 load the starts, 16..31 the ends
                 blk0 = s;
                 __syncwarp();
-                const int cz = (blk0 + C::NPROD * l16) & nmask;
+                const int cz = (blk0 + C::NPROD * l16) % g.n;              // (slabs past the piece's end are loaded but not used)
                 uint32_t pend[8], pdel[8], run = 0u;
 #pragma unroll
                 for (int sg = 0; sg < 8; ++sg) { pend[sg] = 0u; pdel[sg] = 0u; }
@@ -418,8 +417,12 @@ spread_kernel(const PSlot<T>* __restrict__ slots, const T* __restrict__ rows,
                     for (int j = 0; j < kSteps; ++j) {
                         if (j < nst) {                                  // (uniform)
                             const uint32_t cwj = cw[j];
-                            const int X0 = (((int)(cwj & 1023u) + (int)((cwj >> 30) & 1u) + offx) & nmask) - (WZ - 1);
-                            const int Y0 = (((int)((cwj >> 10) & 1023u) + (int)(cwj >> 31) + offy) & nmask) - (WZ - 1);
+                            // (c + ks + off lies in (-n, 2n): wrapped into [0, n) without assuming a power of two)
+                            int vx = (int)(cwj & 1023u) + (int)((cwj >> 30) & 1u) + offx;
+                            int vy = (int)((cwj >> 10) & 1023u) + (int)(cwj >> 31) + offy;
+                            vx += vx < 0 ? g.n : 0; vx -= vx >= g.n ? g.n : 0;
+                            vy += vy < 0 ? g.n : 0; vy -= vy >= g.n ? g.n : 0;
+                            const int X0 = vx - (WZ - 1), Y0 = vy - (WZ - 1);
                             const bool ok = cwj != 0xffffffffu && X0 <= CX - 1 && Y0 <= CY - 1;
                             bal[j] = __ballot_sync(FULL, ok);
                             pkv[j] = ok ? ((X0 + 32) | ((Y0 + 32) << 8)) : -1;

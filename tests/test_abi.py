@@ -120,6 +120,15 @@ def test_plan_create_auto_reproduces_the_config_literals(lib):
     assert abs(get(h, enuf.GET_ALPHA) - 0.30348542587702925) < 1e-15 and get(h, enuf.GET_K_CUT) == 64
     assert get(h, enuf.GET_M) == 128 and get(h, enuf.GET_GRID) == 256
     lib.enuf_plan_destroy(h)
+    # the same rule at sigma_s = 1.5: M = 128 on the 192^3 grid (the mixed-radix FFT path)
+    h = C.c_void_p()
+    assert lib.enuf_plan_create_auto(C.byref(h), 1000000, 215.0, 1e-4, 10.0, 1.5, 6) == enuf.OK
+    assert get(h, enuf.GET_M) == 128 and get(h, enuf.GET_GRID) == 192
+    lib.enuf_plan_destroy(h)
+    # a grid of 3 * 2^k points is for cubic boxes only
+    h = C.c_void_p()
+    Lb = (C.c_double * 3)(10.0, 12.0, 10.0)
+    assert lib.enuf_plan_create_box(C.byref(h), 10, Lb, 1.0, 8, 32, 1.5, 4) == enuf.EINVAL
     # bad arguments, and a grid the library does not have (sigma M = 512)
     h = C.c_void_p()
     assert lib.enuf_plan_create_auto(C.byref(h), 10, 215.0, 1.5, 10.0, 2.0, 6) == enuf.EINVAL

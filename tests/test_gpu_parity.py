@@ -475,6 +475,55 @@ def test_oversampling_other_than_two(enuf, torch_cuda, oracle, n, M, m, window, 
     plan.close()
 
 
+@pytest.mark.parametrize("n,m,window,dtype", [(48, 4, "gaussian", "f64"), (48, 6, "kaiser_bessel", "f64"), (96, 3, "bspline", "f64"),
+                                              (96, 6, "kaiser_bessel", "f32"), (48, 4, "sinc_power", "f32"),
+                                              (96, 2, "gaussian", "f32")])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_oversampling_one_and_a_half(enuf, torch_cuda, oracle, n, m, window, dtype, variant):
+    """sigma_s = 1.5 exactly: M = 32 / 64 on grids of 48 / 96 points, which take the mixed-radix
+    FFT path (enuf_fft_mixed.cuh: one radix-3 step, then radix-2 steps, full complex spectrum, pointwise scaling).
+    Against Oracle B with the plain DFT on the same grid: E, F, and the structure factor on sampled modes."""
+    torch = torch_cuda
+    N, L = 1500, 9.0
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = random_neutral_gas(N, L, seed=1500 + n + m, dtype=npdt)
+    M = int(round(n / 1.5))
+    k_cut = M // 2
+    alpha = 0.9 * math.pi * k_cut / (L * 3.0)
+    ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, window, 1.5, variant=variant, use_dft=True, want_S=True)
+    plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=1.5, m=m, window=window, variant=variant, keep_spectrum=True,
+                     dtype=torch.float64 if dtype == "f64" else torch.float32)
+    E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+    tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+    modes = oracle.modes(k_cut)
+    pick = modes[:: max(1, len(modes) // 500)]
+    S = plan.structure_factor(pick)
+    idx = np.arange(len(modes))[:: max(1, len(modes) // 500)]
+    assert np.abs(S - ref["S"][idx]).max() <= (1e-11 if dtype == "f64" else 5e-6) * np.abs(ref["S"]).max()
+    plan.close()
+
+
+@pytest.mark.parametrize("n", [192, 384])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_large_mixed_grids_against_direct_ewald(enuf, torch_cuda, oracle, n, variant):
+    """The two large grids of sigma_s = 1.5 (M = 128, 256), where Oracle B's plain DFT is too slow for a test: fp64 plans
+    against Oracle A (the direct Ewald sum over the same mode set), which they must match to the NFFT error of a
+    Kaiser-Bessel m = 6 window at sigma = 1.5 (~1e-8; any mistake in the radix steps or twiddles is O(1))."""
+    torch = torch_cuda
+    N, L, k_cut = 400, 9.0, 14
+    r, q = random_neutral_gas(N, L, seed=1900 + n)
+    M = int(round(n / 1.5))
+    alpha = 1.1
+    Ea, Fa = oracle.direct(r, q, L, alpha, k_cut)
+    plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=1.5, m=6, window="kaiser_bessel", variant=variant, dtype=torch.float64)
+    E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+    assert abs(E - Ea) <= 1e-7 * abs(Ea)
+    assert rel_rms(F.cpu().numpy(), Fa) <= 1e-6
+    plan.close()
+
+
 def test_plan_auto_runs_config3(enuf, torch_cuda, oracle):
     """Plan.auto (enuf_plan_create_auto): config 3 planned from (delta, r_c) evaluates like the literal plan."""
     torch = torch_cuda
