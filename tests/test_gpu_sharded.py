@@ -80,6 +80,22 @@ def test_sharded_fp64_matches_oracle_b(enuf, torch_cuda, oracle, name, variant, 
     assert rel_rms(F, ref["F"]) <= 1e-11
 
 
+@pytest.mark.parametrize("variant,world", [("analytic", 2), ("ik", 3)])
+def test_sharded_on_a_grid_of_three_times_a_power_of_two(enuf, torch_cuda, oracle, variant, world):
+    """sigma_s = 1.5 (M = 32 on the 48^3 grid, the mixed-radix FFT path): the buffer the ranks exchange is the full complex
+    spectrum after the three forward passes; Eq. 61 holds for it just the same."""
+    torch = torch_cuda
+    N, L, n, M, m = 1200, 8.0, 48, 32, 4
+    r, q = random_neutral_gas(N, L, seed=48)
+    k_cut, alpha = M // 2, 1.2
+    ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, "kaiser_bessel", 1.5, variant=variant, use_dft=True)
+    Es, F = sharded_eval(enuf, torch, r, q, world,
+                         lambda cnt: enuf.Plan(cnt, L, alpha, k_cut, M, sigma=1.5, m=m, dtype=torch.float64, variant=variant))
+    assert all(E == Es[0] for E in Es)
+    assert abs(Es[0] - ref["E"]) <= 1e-12 * abs(ref["E"])
+    assert rel_rms(F, ref["F"]) <= 1e-11
+
+
 def test_sharded_fp32_with_an_empty_rank(enuf, torch_cuda, oracle):
     """20k-particle fp32 Kaiser-Bessel m = 6 gas over 3 ranks, the last of which owns no particle."""
     torch = torch_cuda
