@@ -76,16 +76,15 @@ fft_mixed_kernel(const void* __restrict__ in, void* __restrict__ out, int n, siz
     const int pitch = n + 1;
     Cx<T>* s0 = reinterpret_cast<Cx<T>*>(smem_raw);
     Cx<T>* s1 = s0 + (size_t)kMixLines * pitch;
-    const int id0 = blockIdx.x * kMixLines;
-    auto locate = [&](int e, int& l, int& i) {
-        if (kAlongX) { l = e / n; i = e - l * n; }
-        else { i = e / kMixLines; l = e - i * kMixLines; }
-    };
-    for (int e = threadIdx.x; e < kMixLines * n; e += blockDim.x) {
-        int l, i;
-        locate(e, l, i);
-        const int id = id0 + l;
-        const size_t off = (size_t)(id / n) * A + (size_t)(id % n) * B + (size_t)i * stride;
+    // a thread stays with one line: along x the tpl threads of a line run along it, otherwise consecutive threads take
+    // consecutive lines (= consecutive x) of the same element index
+    constexpr int tpl = kFftThreads / kMixLines;
+    const int l = kAlongX ? threadIdx.x / tpl : threadIdx.x % kMixLines;
+    const int i0 = kAlongX ? threadIdx.x % tpl : threadIdx.x / kMixLines;
+    const int id = blockIdx.x * kMixLines + l;
+    const size_t base = (size_t)(id / n) * A + (size_t)(id % n) * B;
+    for (int i = i0; i < n; i += tpl) {
+        const size_t off = base + (size_t)i * stride;
         Cx<T> v;
         if (kRealIn) { v.x = static_cast<const T*>(in)[off]; v.y = (T)0; }
         else v = static_cast<const Cx<T>*>(in)[off];
@@ -102,11 +101,8 @@ fft_mixed_kernel(const void* __restrict__ in, void* __restrict__ out, int n, siz
         __syncthreads();
         Cx<T>* t = src; src = dst; dst = t;
     }
-    for (int e = threadIdx.x; e < kMixLines * n; e += blockDim.x) {
-        int l, i;
-        locate(e, l, i);
-        const int id = id0 + l;
-        const size_t off = (size_t)(id / n) * A + (size_t)(id % n) * B + (size_t)i * stride;
+    for (int i = i0; i < n; i += tpl) {
+        const size_t off = base + (size_t)i * stride;
         const Cx<T> v = src[(size_t)l * pitch + i];
         if (kRealOut) static_cast<T*>(out)[off] = v.x;
         else static_cast<Cx<T>*>(out)[off] = v;
