@@ -282,6 +282,19 @@ int enuf_plan_get(const enuf_plan *plan, int key, double *value);
 int enuf_self_energy_static(const void *q, int64_t N, int precision, double alpha, void *cuda_stream,
                             double *E_self);
 
+/*
+ * Host only, no CUDA call: checks the work decomposition the spreading kernel would use (step a2)
+ * on a grid of n points (a multiple of 16; columns of 32 x 16 cells for n >= 128, 16 x 16 below), window cut-off m
+ * (trimmed != 0: the 2m-plane stencils of fp32 Kaiser-Bessel, m >= 5), precision ENUF_F32 / ENUF_F64, a device of
+ * num_sms multiprocessors, and zchunk as ENUF_OPT_SPREAD_ZCHUNK (0 = the default, equal shares): every (column,
+ * plane) slab must lie in exactly one piece, no piece may be shorter than the planes it shares with its neighbour
+ * (zchunk = 0), and every piece start must be among the starts whose shared planes are zeroed.  ENUF_OK, or
+ * ENUF_EINVAL with the first violation in enuf_last_error.  *G_out: CTAs; *min / *max_slabs_out: slabs of the
+ * least and the most loaded CTA (any of the three may be NULL).  A test tap.
+ */
+int enuf_spread_split_check(int n, int m, int precision, int trimmed, int num_sms, int zchunk, int *G_out,
+                            int *min_slabs_out, int *max_slabs_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -39,6 +39,7 @@ SYMBOLS = (
     "enuf_plan_workspace_bytes", "enuf_plan_destroy", "enuf_last_error",
     "enuf_ncut", "enuf_alpha_from_rc", "enuf_rc_from_ncut",
     "enuf_plan_create_auto", "enuf_plan_get", "enuf_plan_create_box", "enuf_self_energy_static",
+    "enuf_spread_split_check",
 )
 SELF_STATIC_MAX_N = 1 << 24
 GET_ALPHA, GET_K_CUT, GET_M, GET_GRID, GET_SUPPORT = 1, 2, 3, 4, 5
@@ -97,6 +98,8 @@ def lib():
         L.enuf_plan_create_auto.restype = i
         L.enuf_plan_create_auto.argtypes = [C.POINTER(vp), i64, d, d, d, d, i]
         L.enuf_plan_get.restype = i; L.enuf_plan_get.argtypes = [vp, i, C.POINTER(d)]
+        L.enuf_spread_split_check.restype = i
+        L.enuf_spread_split_check.argtypes = [i, i, i, i, i, i, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.enuf_self_energy_static.restype = i
         L.enuf_self_energy_static.argtypes = [vp, i64, i, d, vp, vp]
         _lib = L

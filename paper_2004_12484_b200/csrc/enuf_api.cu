@@ -1130,3 +1130,51 @@ extern "C" int enuf_self_energy_static(const void* q, int64_t N, int precision, 
     CU(cudaGetLastError());
     return ENUF_OK;
 }
+
+// Host-only check of the spreading kernel's work decomposition (enuf_common.cuh: spread_split_make, spread_piece,
+// spread_piece_start) for a grid, window and device size: every (column, plane) slab in exactly one piece, no piece
+// shorter than the planes it shares with its neighbour, every piece start among the starts that are zeroed.
+extern "C" int enuf_spread_split_check(int n, int m, int precision, int trimmed, int num_sms, int zchunk, int* G_out,
+                                       int* min_slabs_out, int* max_slabs_out) {
+    g_err[0] = 0;
+    if (n < 32 || n > 1024 || n % 16 != 0) return fail(ENUF_EINVAL, "n = %d must be a multiple of 16 in [32, 1024]", n);
+    if (m < 1 || m > enuf::kMaxM || num_sms < 1 || zchunk < 0 || zchunk > n) return fail(ENUF_EINVAL, "bad m, num_sms or zchunk");
+    const int npx = n >= 128 ? 4 : 2;
+    if (n % (8 * npx) != 0) return fail(ENUF_EINVAL, "n = %d is not a multiple of the column width %d", n, 8 * npx);
+    const int per_sm = precision == ENUF_F32 ? enuf::spread_ctas_per_sm<float>(npx) : enuf::spread_ctas_per_sm<double>(npx);
+    const enuf::SpreadSplit sp = enuf::spread_split_make(n, npx, m, trimmed != 0, (long long)num_sms * per_sm, zchunk);
+    std::vector<unsigned char> cover((size_t)sp.ncol * n, 0);
+    std::vector<unsigned char> zeroed((size_t)sp.ncol * n, 0);
+    for (int i = 0; i < sp.G + sp.ncol; ++i) {
+        int col, z0;
+        if (enuf::spread_piece_start(sp, i, col, z0)) {
+            if (col < 0 || col >= sp.ncol || z0 < 0 || z0 >= n) return fail(ENUF_EINVAL, "piece start %d out of range", i);
+            zeroed[(size_t)col * n + z0] = 1;
+        }
+    }
+    int lo = 1 << 30, hi = 0;
+    for (int c = 0; c < sp.G; ++c) {
+        int tot = 0;
+        enuf::SpreadPiece pc;
+        for (int i = 0; enuf::spread_piece(sp, c, i, pc); ++i) {
+            if (pc.col < 0 || pc.col >= sp.ncol || pc.z0 < 0 || pc.z1 > n || pc.z0 >= pc.z1)
+                return fail(ENUF_EINVAL, "CTA %d piece %d = (col %d, [%d, %d)) out of range", c, i, pc.col, pc.z0, pc.z1);
+            if (zchunk == 0 && pc.z1 - pc.z0 < sp.minlen && pc.z1 - pc.z0 < n)
+                return fail(ENUF_EINVAL, "CTA %d piece %d has %d planes, fewer than the %d it shares", c, i, pc.z1 - pc.z0, sp.minlen);
+            if (!zeroed[(size_t)pc.col * n + pc.z0])
+                return fail(ENUF_EINVAL, "start of CTA %d piece %d (col %d, z %d) is not zeroed", c, i, pc.col, pc.z0);
+            for (int z = pc.z0; z < pc.z1; ++z)
+                if (cover[(size_t)pc.col * n + z]++) return fail(ENUF_EINVAL, "slab (col %d, z %d) is in two pieces", pc.col, z);
+            tot += pc.z1 - pc.z0;
+        }
+        if (tot > 0) { lo = tot < lo ? tot : lo; hi = tot > hi ? tot : hi; }
+    }
+    for (size_t i = 0; i < cover.size(); ++i)
+        if (!cover[i]) return fail(ENUF_EINVAL, "slab (col %d, z %d) is in no piece", (int)(i / n), (int)(i % n));
+    for (int col = 0; col < sp.ncol; ++col)     // a column's top wraps onto its first piece
+        if (!zeroed[(size_t)col * n]) return fail(ENUF_EINVAL, "start of column %d is not zeroed", col);
+    if (G_out) *G_out = sp.G;
+    if (min_slabs_out) *min_slabs_out = lo;
+    if (max_slabs_out) *max_slabs_out = hi;
+    return ENUF_OK;
+}

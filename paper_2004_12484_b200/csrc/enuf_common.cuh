@@ -136,6 +136,47 @@ __host__ __device__ inline bool spread_piece_start(const SpreadSplit& sp, int i,
     col = pc.col; z0 = pc.z0;
     return true;
 }
+// The decomposition for a grid of n points, columns of 8 npx x 16 cells, window cut-off m (trimmed stencils: 2m planes)
+// on a device that holds `slots` spreading CTAs at once; zchunk > 0 asks for fixed pieces instead (host only).
+// q full pieces per column, cut at the same planes in all columns; the other CTAs share the remainders [zr0, n), the
+// remainders of k whole columns each (k the smallest divisor of ncol that the resident CTAs allow): with L slabs per
+// CTA, q L + L / k = n, i.e. L = k n / (1 + k q) and G = q ncol + ncol / k.
+inline SpreadSplit spread_split_make(int n, int npx, int m, bool trim, long long slots, int zchunk) {
+    SpreadSplit sp{};
+    sp.n = n;
+    sp.ncol = (n / (8 * npx)) * (n / 16);
+    sp.minlen = 2 * m - (trim ? 1 : 0);
+    sp.q = 0; sp.zr0 = 0;
+    if (zchunk > 0) {
+        sp.chunk = zchunk;
+        sp.G = sp.ncol * ((n + zchunk - 1) / zchunk);
+        return sp;
+    }
+    sp.chunk = 0;
+    const long long slabs = (long long)sp.ncol * n;
+    long long G = slots;
+    const long long gmax = slabs / (sp.minlen + 1);
+    if (G > gmax) G = gmax;
+    if (G < 1) G = 1;
+    const double len = (double)slabs / (double)G;                 // slabs per CTA if G divided them exactly
+    sp.q = (int)((double)n / len + 1e-9);
+    if (sp.q > 0) {
+        const double spare = (double)G / sp.ncol - sp.q;          // CTAs per column beyond the q full pieces
+        int k = spare > 1e-9 ? (int)(1.0 / spare - 1e-9) + 1 : sp.ncol + 1;
+        while (k <= sp.ncol && sp.ncol % k != 0) ++k;
+        if (k <= sp.ncol) {
+            const double L = (double)k * n / (1.0 + (double)k * sp.q);
+            sp.zr0 = (int)(sp.q * L + 0.5);
+            G = (long long)sp.q * sp.ncol + sp.ncol / k;
+        }
+        if (k > sp.ncol || sp.zr0 > n - sp.minlen) {              // no remainder worth a piece: q equal pieces per column
+            sp.zr0 = n;
+            G = (long long)sp.q * sp.ncol;
+        }
+    }
+    sp.G = (int)G;
+    return sp;
+}
 // Piecewise-polynomial window table for the fp32 path (step a0).  For every stencil offset
 // j in [0, m] the weight phi(d0 - j), d0 in [-1/2, 1/2], is a polynomial p_j of degree
 // poly_degree(m) in d0 (Chebyshev interpolant of the window's analytic continuation, fitted

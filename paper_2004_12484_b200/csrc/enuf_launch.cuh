@@ -147,43 +147,8 @@ int configure_kernels(enuf_plan* p) {
 // ENUF_OPT_SPREAD_ZCHUNK asks for fixed pieces instead.
 template <typename T>
 static inline SpreadSplit make_spread_split(const enuf_plan* p) {
-    SpreadSplit sp{};
-    sp.n = p->n;
-    sp.ncol = (p->n / (8 * p->spread_npx)) * (p->n / 16);
-    sp.minlen = 2 * p->m - (p->trim ? 1 : 0);
-    sp.q = 0; sp.zr0 = 0;
-    if (p->zchunk_user) {
-        sp.chunk = p->zchunk;
-        sp.G = sp.ncol * ((p->n + p->zchunk - 1) / p->zchunk);
-    } else {
-        sp.chunk = 0;
-        const long long slabs = (long long)sp.ncol * sp.n;
-        long long G = (long long)p->num_sms * spread_ctas_per_sm<T>(p->spread_npx);
-        const long long gmax = slabs / (sp.minlen + 1);
-        if (G > gmax) G = gmax;
-        if (G < 1) G = 1;
-        // q full pieces per column, cut at the same planes in all columns; the other CTAs share the remainders [zr0, n),
-        // the remainders of k whole columns each (k the smallest divisor of ncol that the resident CTAs allow): with
-        // L slabs per CTA, q L + L / k = n, i.e. L = k n / (1 + k q) and G = q ncol + ncol / k
-        const double len = (double)slabs / (double)G;                 // slabs per CTA if G divided them exactly
-        sp.q = (int)((double)sp.n / len + 1e-9);
-        if (sp.q > 0) {
-            const double spare = (double)G / sp.ncol - sp.q;          // CTAs per column beyond the q full pieces
-            int k = spare > 1e-9 ? (int)(1.0 / spare - 1e-9) + 1 : sp.ncol + 1;
-            while (k <= sp.ncol && sp.ncol % k != 0) ++k;
-            if (k <= sp.ncol) {
-                const double L = (double)k * sp.n / (1.0 + (double)k * sp.q);
-                sp.zr0 = (int)(sp.q * L + 0.5);
-                G = (long long)sp.q * sp.ncol + sp.ncol / k;
-            }
-            if (k > sp.ncol || sp.zr0 > sp.n - sp.minlen) {            // no remainder worth a piece: q equal pieces per column
-                sp.zr0 = sp.n;
-                G = (long long)sp.q * sp.ncol;
-            }
-        }
-        sp.G = (int)G;
-    }
-    return sp;
+    return spread_split_make(p->n, p->spread_npx, p->m, p->trim, (long long)p->num_sms * spread_ctas_per_sm<T>(p->spread_npx),
+                             p->zchunk_user ? p->zchunk : 0);
 }
 
 template <typename T>

@@ -136,3 +136,31 @@ def test_plan_create_auto_reproduces_the_config_literals(lib):
     assert lib.enuf_plan_create_auto(C.byref(h), 10, 430.0, 1e-4, 10.0, 2.0, 6) == enuf.EINVAL
     assert b"sigma*M" in lib.enuf_last_error()
     assert lib.enuf_plan_get(None, enuf.GET_ALPHA, C.byref(v)) == enuf.EINVAL
+
+
+def test_spread_decomposition_covers_every_slab_once():
+    """The spreading kernel's pieces, checked on the host for every grid size, window, precision,
+    device sizes from 1 to 200 SMs and several ENUF_OPT_SPREAD_ZCHUNK values: every (column, plane) slab in exactly one
+    piece, no piece shorter than the planes it shares, every piece start zeroed; the default shares are balanced."""
+    import ctypes as C
+    import paper_2004_12484_b200 as enuf
+    lib = enuf.lib()
+    G, lo, hi = C.c_int(), C.c_int(), C.c_int()
+    for n in (32, 48, 64, 96, 128, 192, 256, 384):
+        for m in (1, 2, 4, 6):
+            for prec in (enuf.F32, enuf.F64):
+                trim = 1 if (prec == enuf.F32 and m >= 5) else 0
+                for sms in (1, 7, 20, 108, 132, 148, 200):
+                    rc = lib.enuf_spread_split_check(n, m, prec, trim, sms, 0, C.byref(G), C.byref(lo), C.byref(hi))
+                    assert rc == enuf.OK, (n, m, prec, sms, lib.enuf_last_error())
+                    ncol = (n // (32 if n >= 128 else 16)) * (n // 16)
+                    assert 1 <= G.value <= max(ncol * n // (2 * m - trim + 1), 1)
+                    # balanced: the most loaded CTA is within a piece's minimum length (or 15 %) of the least loaded one
+                    assert hi.value - lo.value <= max(2 * m, 0.15 * hi.value) or G.value <= ncol, (n, m, sms, G.value, lo.value, hi.value)
+                for z in (1, 5, 16, n):
+                    rc = lib.enuf_spread_split_check(n, m, prec, trim, 148, z, C.byref(G), None, None)
+                    assert rc == enuf.OK, (n, m, prec, z, lib.enuf_last_error())
+    # the headline configuration: 288 CTAs of 112 .. 114 slabs on a 148-SM device
+    assert lib.enuf_spread_split_check(256, 6, enuf.F32, 1, 148, 0, C.byref(G), C.byref(lo), C.byref(hi)) == enuf.OK
+    assert (G.value, lo.value, hi.value) == (288, 112, 114)
+    assert lib.enuf_spread_split_check(40, 6, enuf.F32, 1, 148, 0, None, None, None) == enuf.EINVAL
