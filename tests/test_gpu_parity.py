@@ -524,6 +524,32 @@ def test_large_mixed_grids_against_direct_ewald(enuf, torch_cuda, oracle, n, var
     plan.close()
 
 
+@pytest.mark.parametrize("N", [2, 31, 33, 262144, 262145])
+def test_particle_counts_around_the_block_sizes_and_the_bin_threshold(enuf, torch_cuda, oracle, N):
+    """Ragged particle counts: fewer than a warp, one more than a warp (the 32-particle blocks of bin_place), and the two
+    sides of the threshold between the one-pass scatter + rows (N <= 262 144) and the two-kernel form.  A handful of
+    particles is compared in fp64 (in fp32 their forces are small against each particle's own field, whose rounding sets
+    the absolute error: 4e-6 relative for two particles -- that case gets ten times the bar)."""
+    torch = torch_cuda
+    L, n, M, m = 12.0, 64, 32, 6
+    alpha, k_cut = 0.9, 16
+    for dt, npdt in ((torch.float32, np.float32),) + (((torch.float64, np.float64),) if N < 1000 else ()):
+        r, q = random_neutral_gas(N, L, seed=77, dtype=npdt)
+        sample = None if N < 1000 else list(range(0, N, max(1, N // 3000)))
+        ref = oracle.enuf(r, q, L, alpha, k_cut, n, m, "kaiser_bessel", 2.0, sample=sample)
+        plan = enuf.Plan(N, L, alpha, k_cut, M, m=m, dtype=dt)
+        E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+        Fh = F.cpu().numpy()
+        Fh = Fh if sample is None else Fh[sample]
+        if dt == torch.float64:
+            te, tf = F64_E, F64_F
+        else:
+            te, tf = F32_E, (F32_F if N >= 1000 else 10 * F32_F)
+        assert abs(E - ref["E"]) <= te * abs(ref["E"])
+        assert rel_rms(Fh, ref["F"]) <= tf
+        plan.close()
+
+
 def test_plan_auto_runs_config3(enuf, torch_cuda, oracle):
     """Plan.auto (enuf_plan_create_auto): config 3 planned from (delta, r_c) evaluates like the literal plan."""
     torch = torch_cuda
