@@ -80,7 +80,8 @@ enum { ENUF_FORCE_ANALYTIC = 0, ENUF_FORCE_IK = 1 };
 
 /* stage indices of enuf_plan_stage_ms() */
 enum enuf_stage {
-    ENUF_STAGE_BIN = 0,     /* a1: histogram, scan, scatter, window rows of the sorted particles */
+    ENUF_STAGE_BIN = 0,     /* a1: histogram (+ zeroing of the grid planes that two spreading pieces share), scan,
+                               scatter, window rows of the sorted particles */
     ENUF_STAGE_SPREAD = 1,  /* a2: grid values are stored once; only the planes two pieces of a column share are reduced */
     ENUF_STAGE_FFT = 2,     /* a3 + a4 + a5 */
     ENUF_STAGE_GATHER = 3,  /* a6 */
