@@ -5,7 +5,7 @@
 //   X forward  G (real) -> C (complex n^3),  Y, Z forward in place,
 //   scale      S~ = g^/D, E partials (fp64), psi^ = f^2 w S~/D  (or the three b^_d of the ik variant), pointwise,
 //   Z, Y inverse in place, X inverse C -> G (real part),
-// every line transform a Stockham autosort FFT in shared memory (one radix-3 step, then radix-2 steps; the
+// every line transform a Stockham autosort FFT in shared memory (one radix-3 step, then radix-4 steps and at most one radix-2 step; the
 // twiddles exp(-2 pi i j/n) come from a table made in fp64 on the host).  Same conventions as the oracle (R11:
 // forward e^-, inverse e^+, both unnormalised; R4, R12 for the mode set).  Cubic boxes only.
 #pragma once
@@ -22,7 +22,7 @@ template <typename T> constexpr int mix_lines() { return sizeof(T) == 4 ? 16 : 8
 template <typename T> size_t fft_mixed_smem_bytes(int n) { return 2 * sizeof(Cx<T>) * (size_t)mix_lines<T>() * (n + 1); }
 
 // One Stockham step of radix R on the lines of a CTA (length n, kFftThreads / nl threads per line): src -> dst.
-// Ns = product of the radices already done = 1 (the radix-3 step) or 3 * 2^sh (the radix-2 steps).
+// Ns = product of the radices already done = 1 (the radix-3 step) or 3 * 2^sh (the radix-4 and radix-2 steps).
 // Item j in [0, n/R): v[r] = src[j + r n/R] w^(r (j mod Ns) n/(Ns R)), DFT_R, dst[(j / Ns) Ns R + (j mod Ns) + r Ns] = v[r]
 // (r (j mod Ns) n/(Ns R) < n: the table index needs no reduction; j / Ns = (j >> sh) / 3: no division by a run-time value).
 template <typename T, int R>
@@ -49,6 +49,14 @@ __device__ __forceinline__ void mix_step(const Cx<T>* __restrict__ src, Cx<T>* _
         if (R == 2) {
             d[0] = cx_add(v[0], v[1]);
             d[Ns] = cx_sub(v[0], v[1]);
+        } else if (R == 4) {
+            // DFT_4: X1 = (a - c) + w (b - d), X3 = (a - c) - w (b - d), w = exp(sign 2 pi i/4) = sign i
+            const Cx<T> s02 = cx_add(v[0], v[2]), d02 = cx_sub(v[0], v[2]), s13 = cx_add(v[1], v[3]), d13 = cx_sub(v[1], v[3]);
+            const Cx<T> rot = sign < 0 ? cx_make<T>(d13.y, -d13.x) : cx_make<T>(-d13.y, d13.x);
+            d[0] = cx_add(s02, s13);
+            d[Ns] = cx_add(d02, rot);
+            d[2 * Ns] = cx_sub(s02, s13);
+            d[3 * Ns] = cx_sub(d02, rot);
         } else {
             // DFT_3: X1 = a + b w + c w^2, X2 = a + b w^2 + c w, w = exp(sign 2 pi i/3) = (-1/2, sign sqrt(3)/2)
             const T h = (T)0.86602540378443864676 * (T)(sign < 0 ? -1 : 1);
@@ -96,7 +104,13 @@ fft_mixed_kernel(const void* __restrict__ in, void* __restrict__ out, int n, siz
     mix_step<T, 3>(src, dst, n, kMixLines, 0, sign, tw);
     __syncthreads();
     { Cx<T>* t = src; src = dst; dst = t; }
-    for (int sh = 0; (3 << sh) < n; ++sh) {
+    int sh = 0;
+    for (; (12 << sh) <= n; sh += 2) {                       // radix-4 steps while a factor 4 is left ..
+        mix_step<T, 4>(src, dst, n, kMixLines, sh, sign, tw);
+        __syncthreads();
+        Cx<T>* t = src; src = dst; dst = t;
+    }
+    if ((3 << sh) < n) {                                     // .. and one radix-2 step for an odd power of two
         mix_step<T, 2>(src, dst, n, kMixLines, sh, sign, tw);
         __syncthreads();
         Cx<T>* t = src; src = dst; dst = t;
