@@ -100,7 +100,7 @@ enum enuf_stage {
  *   M      NFFT bandwidth per dimension (Eq. 33, :272), any integer >= 2 k_cut
  *   sigma  oversampling factor sigma_s > 1 (:348, :360); n = sigma*M (to 1e-9) must be 32, 64, 128 or 256 -- the fused,
  *          pruned FFT: sigma = 2 with M a power of two, or any other M with sigma = n/M (M = 170, n = 256: 1.506) --
- *          or 48, 96, 192, 384: sigma = 1.5 with M = 32 ... 256, cubic boxes only, on a plain (slower) FFT path
+ *          or 48, 96, 192, 384: sigma = 1.5 with M = 32 ... 256, on a plain (slower) FFT path
  *   m      window cut-off: stencil of 2m+1 grid points per dimension (:268, R8), 1 <= m <= 6
  * Defaults: fp32, Kaiser-Bessel window, analytic-derivative forces, point charges,
  * the legacy default stream.  *out is set to NULL on failure.

@@ -537,8 +537,6 @@ int enuf_plan_create_box(enuf_plan** out, int64_t N, const double* Lb, double al
     const bool pow2 = n == 32 || n == 64 || n == 128 || n == 256, mixed = n == 48 || n == 96 || n == 192 || n == 384;
     if (std::fabs(nd - n) > 1e-9 || !(pow2 || mixed))
         return fail(ENUF_EINVAL, "sigma*M = %g must be one of 32, 64, 128, 256 or 48, 96, 192, 384", nd);
-    if (mixed && !(Lb[0] == Lb[1] && Lb[1] == Lb[2]))
-        return fail(ENUF_EINVAL, "grids of 3 * 2^k points (sigma*M = %d) are for cubic boxes only", n);
     if (k_cut < 1 || 2 * k_cut > M) return fail(ENUF_EINVAL, "k_cut = %d must satisfy 1 <= k_cut <= M/2 = %d", k_cut, M / 2);
     if (m < 1 || m > enuf::kMaxM) return fail(ENUF_EINVAL, "m = %d must satisfy 1 <= m <= %d", m, enuf::kMaxM);
     enuf_plan* p = new (std::nothrow) enuf_plan();

@@ -7,7 +7,7 @@
 //   Z, Y inverse in place, X inverse C -> G (real part),
 // every line transform a Stockham autosort FFT in shared memory (one radix-3 step, then radix-4 steps and at most one radix-2 step; the
 // twiddles exp(-2 pi i j/n) come from a table made in fp64 on the host).  Same conventions as the oracle (R11:
-// forward e^-, inverse e^+, both unnormalised; R4, R12 for the mode set).  Cubic boxes only.
+// forward e^-, inverse e^+, both unnormalised; R4, R12 for the mode set; R26 for orthorhombic boxes).
 #pragma once
 
 #include "enuf_common.cuh"
@@ -128,11 +128,13 @@ fft_mixed_kernel(const void* __restrict__ in, void* __restrict__ out, int n, siz
 //   S~ = g^ iphi[|kx|] iphi[|ky|] iphi[|kz|],  E += wf[|k|^2] |S~|^2  (every mode of the full space once),
 //   psi^ = wf S~ iphi iphi iphi  (NOUT = 1)  or  b^_d = -i n_d psi^ into C0, C1, C2  (NOUT = 3); zero elsewhere.
 // The energy partials are summed by the last CTA in a fixed order (z_pass_energy_finish).
-template <typename T, int NOUT>
+// kBox (orthorhombic plans, R26): membership and weight from s = |h|^2 Lmax^2 formed in fp64 in the same order
+// as the fused Z pass (fft_z_fused_kernel), b^_d = -i h_d psi^ with h_d = n_d / L_d.
+template <typename T, int NOUT, bool kBox = false>
 __global__ void __launch_bounds__(kFftThreads)
 mixed_scale_kernel(Cx<T>* __restrict__ C0, Cx<T>* __restrict__ C1, Cx<T>* __restrict__ C2, int n, int kcut, int Kxp, int Ky,
                    ScaleTables st, double* __restrict__ e_partial, Cx<T>* __restrict__ spectrum,
-                   unsigned* __restrict__ done_count, double e_scale, double* __restrict__ e_out) {
+                   unsigned* __restrict__ done_count, double e_scale, double* __restrict__ e_out, const BoxScale bs) {
     pdl_prologue();
     __shared__ double red[kFftThreads / 32];
     const T* iphi = static_cast<const T*>(st.iphi);
@@ -146,9 +148,28 @@ mixed_scale_kernel(Cx<T>* __restrict__ C0, Cx<T>* __restrict__ C1, Cx<T>* __rest
         const int ax = kx < 0 ? -kx : kx, ay = ky < 0 ? -ky : ky, az = kz < 0 ? -kz : kz;
         const int s = kx * kx + ky * ky + kz * kz;
         Cx<T> o = cx_make<T>((T)0, (T)0);
-        if (ax <= kcut && ay <= kcut && az <= kcut && s > 0 && s <= kc2) {
+        bool in_k = ax <= kcut && ay <= kcut && az <= kcut && s > 0;
+        T w = (T)0;
+        if constexpr (kBox) {
+            const double sxy = __dadd_rn(__dmul_rn((double)(kx * kx), bs.a[0]), __dmul_rn((double)(ky * ky), bs.a[1]));
+            const double sb = __dadd_rn(sxy, __dmul_rn((double)(kz * kz), bs.a[2]));
+            in_k = in_k && sxy <= (double)kc2 && sb <= (double)kc2;
+            if (in_k) {
+                constexpr double PI = 3.14159265358979323846264338327950288;
+                const double h2 = sb / bs.lm2;
+                double wd = exp(-PI * PI * h2 / (bs.alpha * bs.alpha)) / h2;
+                if (bs.lambda != 0.0) {
+                    const double gq = 1.0 + PI * PI * bs.lambda * bs.lambda * h2;
+                    wd /= (gq * gq) * (gq * gq);
+                }
+                w = (T)wd;
+            }
+        } else {
+            in_k = in_k && s <= kc2;
+            if (in_k) w = wf[s];
+        }
+        if (in_k) {
             const T ip3 = iphi[ax] * iphi[ay] * iphi[az];
-            const T w = wf[s];
             const Cx<T> g = C0[idx];
             const Cx<T> S = cx_make<T>(g.x * ip3, g.y * ip3);
             e_acc += (double)w * ((double)S.x * (double)S.x + (double)S.y * (double)S.y);
@@ -163,9 +184,11 @@ mixed_scale_kernel(Cx<T>* __restrict__ C0, Cx<T>* __restrict__ C1, Cx<T>* __rest
             C0[idx] = o;
         } else {
             // b^_d = -i n_d psi^ :  -i (x + i y) = y - i x
-            C0[idx] = cx_make<T>((T)kx * o.y, -(T)kx * o.x);
-            C1[idx] = cx_make<T>((T)ky * o.y, -(T)ky * o.x);
-            C2[idx] = cx_make<T>((T)kz * o.y, -(T)kz * o.x);
+            const T hx = kBox ? (T)((double)kx / bs.l[0]) : (T)kx, hy = kBox ? (T)((double)ky / bs.l[1]) : (T)ky,
+                    hz = kBox ? (T)((double)kz / bs.l[2]) : (T)kz;
+            C0[idx] = cx_make<T>(hx * o.y, -hx * o.x);
+            C1[idx] = cx_make<T>(hy * o.y, -hy * o.x);
+            C2[idx] = cx_make<T>(hz * o.y, -hz * o.x);
         }
     }
 #pragma unroll

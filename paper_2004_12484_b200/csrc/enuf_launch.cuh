@@ -316,13 +316,30 @@ int launch_fft_backward(enuf_plan* p) {
         ScaleTables st{p->iphi, p->wf};
         Cx<T>* spec = p->keep_spectrum ? static_cast<Cx<T>*>(p->spectrum) : nullptr;
         Cx<T>* c0 = static_cast<Cx<T>*>(p->A1[0]);
-        if (nout == 1)
-            pdl_launch(p, mixed_scale_kernel<T, 1>, enuf_plan::kMixedScaleCtas, kFftThreads, 0, p->stream, c0, (Cx<T>*)nullptr,
-                       (Cx<T>*)nullptr, p->n, p->k_cut, p->Kxp, p->Ky, st, p->e_partial, spec, p->fft_done, 1.0 / (2.0 * PI * p->L), p->e_dev);
+        Cx<T>* c1 = nout == 3 ? static_cast<Cx<T>*>(p->A1[1]) : nullptr;
+        Cx<T>* c2 = nout == 3 ? static_cast<Cx<T>*>(p->A1[2]) : nullptr;
+        // Eq. 38: C/(2 pi L), C = 1; a box (weights in length^2): 1/(2 pi V)
+        const double e_scale = p->box ? 1.0 / (2.0 * PI * p->Lb[0] * p->Lb[1] * p->Lb[2]) : 1.0 / (2.0 * PI * p->L);
+        BoxScale bs{};
+        {
+            double lm = p->Lb[0] > p->Lb[1] ? p->Lb[0] : p->Lb[1];
+            lm = lm > p->Lb[2] ? lm : p->Lb[2];
+            for (int d = 0; d < 3; ++d) { bs.a[d] = (lm / p->Lb[d]) * (lm / p->Lb[d]); bs.l[d] = p->Lb[d]; }
+            bs.lm2 = lm * lm; bs.alpha = p->alpha; bs.lambda = p->lambda;
+        }
+        const unsigned ctas = enuf_plan::kMixedScaleCtas;
+        if (nout == 1 && !p->box)
+            pdl_launch(p, mixed_scale_kernel<T, 1, false>, ctas, kFftThreads, 0, p->stream, c0, c1, c2, p->n, p->k_cut, p->Kxp,
+                       p->Ky, st, p->e_partial, spec, p->fft_done, e_scale, p->e_dev, bs);
+        else if (nout == 1)
+            pdl_launch(p, mixed_scale_kernel<T, 1, true>, ctas, kFftThreads, 0, p->stream, c0, c1, c2, p->n, p->k_cut, p->Kxp,
+                       p->Ky, st, p->e_partial, spec, p->fft_done, e_scale, p->e_dev, bs);
+        else if (!p->box)
+            pdl_launch(p, mixed_scale_kernel<T, 3, false>, ctas, kFftThreads, 0, p->stream, c0, c1, c2, p->n, p->k_cut, p->Kxp,
+                       p->Ky, st, p->e_partial, spec, p->fft_done, e_scale, p->e_dev, bs);
         else
-            pdl_launch(p, mixed_scale_kernel<T, 3>, enuf_plan::kMixedScaleCtas, kFftThreads, 0, p->stream, c0,
-                       static_cast<Cx<T>*>(p->A1[1]), static_cast<Cx<T>*>(p->A1[2]), p->n, p->k_cut, p->Kxp, p->Ky, st, p->e_partial, spec,
-                       p->fft_done, 1.0 / (2.0 * PI * p->L), p->e_dev);
+            pdl_launch(p, mixed_scale_kernel<T, 3, true>, ctas, kFftThreads, 0, p->stream, c0, c1, c2, p->n, p->k_cut, p->Kxp,
+                       p->Ky, st, p->e_partial, spec, p->fft_done, e_scale, p->e_dev, bs);
         for (int d = 0; d < nout; ++d) {
             launch_mixed_pass<T>(p, 2, +1, p->A1[d], p->A1[d]);
             launch_mixed_pass<T>(p, 1, +1, p->A1[d], p->A1[d]);

@@ -125,10 +125,11 @@ def test_plan_create_auto_reproduces_the_config_literals(lib):
     assert lib.enuf_plan_create_auto(C.byref(h), 1000000, 215.0, 1e-4, 10.0, 1.5, 6) == enuf.OK
     assert get(h, enuf.GET_M) == 128 and get(h, enuf.GET_GRID) == 192
     lib.enuf_plan_destroy(h)
-    # a grid of 3 * 2^k points is for cubic boxes only
+    # ... and for an orthorhombic box
     h = C.c_void_p()
     Lb = (C.c_double * 3)(10.0, 12.0, 10.0)
-    assert lib.enuf_plan_create_box(C.byref(h), 10, Lb, 1.0, 8, 32, 1.5, 4) == enuf.EINVAL
+    assert lib.enuf_plan_create_box(C.byref(h), 10, Lb, 1.0, 8, 32, 1.5, 4) == enuf.OK
+    lib.enuf_plan_destroy(h)
     # bad arguments, and a grid the library does not have (sigma M = 512)
     h = C.c_void_p()
     assert lib.enuf_plan_create_auto(C.byref(h), 10, 215.0, 1.5, 10.0, 2.0, 6) == enuf.EINVAL

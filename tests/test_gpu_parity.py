@@ -168,6 +168,34 @@ def test_box_matches_oracle(enuf, torch_cuda, oracle, n, m, window, dtype, Lb, v
     plan.close()
 
 
+@pytest.mark.parametrize("n,m,window,dtype,Lb", [(48, 4, "kaiser_bessel", "f64", (5.0, 6.5, 8.0)),
+                                                 (96, 6, "kaiser_bessel", "f32", (9.0, 7.0, 12.0))])
+@pytest.mark.parametrize("variant", ["analytic", "ik"])
+def test_box_at_oversampling_one_and_a_half(enuf, torch_cuda, oracle, n, m, window, dtype, Lb, variant):
+    """Orthorhombic box on a grid of 3 * 2^k points: the mixed-radix path's pointwise kernel decides membership and
+    evaluates the weight as the fused Z pass does for boxes.  Against the box oracle with the plain DFT."""
+    torch = torch_cuda
+    N = 1200
+    npdt = np.float64 if dtype == "f64" else np.float32
+    r, q = _box_inputs(N, Lb, 900 + n + m, npdt)
+    M = int(round(n / 1.5))
+    k_cut = M // 2
+    alpha = 0.9 * math.pi * k_cut / (max(Lb) * 3.0)
+    lam = 0.05 * min(Lb) if m == 4 else 0.0
+    ref = oracle.enuf_box(r, q, Lb, alpha, k_cut, n, m, window, 1.5, variant=variant, slater_lambda=lam, use_dft=True,
+                          want_S=True)
+    plan = enuf.Plan(N, Lb, alpha, k_cut, M, sigma=1.5, m=m, window=window, variant=variant, slater_lambda=lam,
+                     dtype=torch.float64 if dtype == "f64" else torch.float32, keep_spectrum=True)
+    E, F = plan.energy_forces(torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda())
+    tf, te = (F64_F, F64_E) if dtype == "f64" else (F32_F, F32_E)
+    assert abs(E - ref["E"]) <= te * abs(ref["E"])
+    assert rel_rms(F.cpu().numpy(), ref["F"]) <= tf
+    ml = oracle.modes_box(k_cut, Lb)
+    S = plan.structure_factor(ml)
+    assert np.abs(S - ref["S"]).max() <= (1e-11 if dtype == "f64" else 5e-6) * np.abs(ref["S"]).max()
+    plan.close()
+
+
 def test_box_with_equal_edges_is_the_cubic_plan(enuf, torch_cuda):
     torch = torch_cuda
     w = make_workload("cfg3")
