@@ -185,8 +185,9 @@ def sub_box_sample(w, scale: int):
 
 def oracle_step(O, w, r, q, L, k_cut, n, variant):
     t = time.perf_counter()
+    # (grids of 3 * 2^k points, sigma = 1.5: the oracle's radix-2 transform does not apply, its plain DFT does)
     out = O.enuf(r, q, L, w.alpha, k_cut, n, w.m, w.window, w.sigma, variant=variant,
-                 slater_lambda=w.slater_lambda)
+                 slater_lambda=w.slater_lambda, use_dft=(n & (n - 1)) != 0)
     return time.perf_counter() - t, out
 
 
