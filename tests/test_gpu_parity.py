@@ -822,3 +822,28 @@ def test_mixed_grid_graph_replay_and_host_call(enuf, torch_cuda, oracle):
     Fh = Fh.numpy() if hasattr(Fh, "numpy") else np.asarray(Fh)
     assert abs(Eh - ref["E"]) <= F32_E * abs(ref["E"]) and rel_rms(Fh, ref["F"]) <= F32_F
     plan.close()
+
+
+@pytest.mark.parametrize("window", ["kaiser_bessel", "gaussian", "bspline"])
+def test_error_against_direct_ewald_falls_with_m_for_both_oversampling_factors(enuf, torch_cuda, oracle, window):
+    """The paper's Fig. 1 statement: for sigma_s = 1.5 and 2.0 the error of ENUF against the Ewald
+    sum falls sharply with the window cut-off m.  fp64 plans with M = 32 (grids of 48 and 64 points), the paper's ik
+    forces, against Oracle A over the same mode set: the error shrinks by at least 3x per step of m up to the fp64
+    floor, and at equal m the larger oversampling factor is the more accurate one."""
+    torch = torch_cuda
+    N, L, M, k_cut, alpha = 300, 7.0, 32, 16, 1.3
+    r, q = random_neutral_gas(N, L, seed=360)
+    Ea, Fa = oracle.direct(r, q, L, alpha, k_cut)
+    rt, qt = torch.from_numpy(r).cuda(), torch.from_numpy(q).cuda()
+    err = {}
+    for sigma in (1.5, 2.0):
+        for m in range(1, 7):
+            plan = enuf.Plan(N, L, alpha, k_cut, M, sigma=sigma, m=m, window=window, variant="ik", dtype=torch.float64)
+            E, F = plan.energy_forces(rt, qt)
+            err[sigma, m] = rel_rms(F.cpu().numpy(), Fa)
+            plan.close()
+        for m in range(2, 7):
+            assert err[sigma, m] < err[sigma, m - 1] / 3 or err[sigma, m] < 1e-11, (sigma, m, err)
+    for m in range(2, 7):
+        assert err[2.0, m] < err[1.5, m] or err[1.5, m] < 1e-11, (m, err)
+    assert err[2.0, 6] < (1e-8 if window == "kaiser_bessel" else 1e-4)
